@@ -1,0 +1,162 @@
+"""Pins for oracle.transformer / oracle.attention against library routines, closed forms and invariants."""
+import numpy as np
+import torch
+import torch.nn.functional as F
+
+from oracle import attention, transformer as tr
+from paper_2605_30859_b200 import workloads as wl
+
+
+def tiny_cfg(**kw):
+    cfg = dict(n_layers=2, d_model=32, n_q_heads=4, n_kv_heads=2, head_dim=8, ffn=48, vocab=40,
+               n_experts=0, top_k=0, expert_ffn=0, qk_norm=False, rope_theta=1.0e4, rms_eps=1e-6, dtype="f32")
+    cfg.update(kw)
+    return cfg
+
+
+def tiny_model(seed=0, std=0.3, **kw):
+    return wl.host_model(wl.make_model(tiny_cfg(**kw), seed=seed, std=std))
+
+
+def test_softmax_rows_sum_to_one_and_shift_invariant():
+    z = np.random.default_rng(0).normal(size=(5, 17)) * 30
+    p = tr.softmax(z)
+    assert np.allclose(p.sum(-1), 1.0, atol=1e-14)
+    assert np.allclose(p, tr.softmax(z + 1234.5), atol=1e-13)
+
+
+def test_rmsnorm_against_torch_and_invariants():
+    rng = np.random.default_rng(1)
+    x, w = rng.normal(size=(3, 16)), rng.normal(size=16)
+    ref = F.rms_norm(torch.from_numpy(x), (16,), torch.from_numpy(w), eps=1e-6).numpy()
+    assert np.allclose(tr.rmsnorm(x, w, 1e-6), ref, atol=1e-14)
+    y = tr.rmsnorm(x, np.ones(16), 0.0)
+    assert np.allclose(np.sqrt(np.mean(y * y, -1)), 1.0)
+    assert np.allclose(tr.rmsnorm(7.0 * x, w, 0.0), tr.rmsnorm(x, w, 0.0))
+
+
+def test_rope_closed_forms():
+    # hd = 2: a plain 2-D rotation by angle pos (theta^0 = 1)
+    x = np.array([[[1.0, 0.0]]])                                  # [T=1, H=1, hd=2]
+    y = tr.rope(x, np.array([3]), 100.0)
+    assert np.allclose(y[0, 0], [np.cos(3.0), np.sin(3.0)])
+    # hd = 4: pairs are (0,2) at frequency 1 and (1,3) at frequency theta^(-1/2)
+    x = np.array([[[1.0, 0.0, 0.0, 0.0]], [[0.0, 1.0, 0.0, 0.0]]])
+    y = tr.rope(x, np.array([2, 5]), 100.0)
+    assert np.allclose(y[0, 0], [np.cos(2.0), 0, np.sin(2.0), 0])
+    assert np.allclose(y[1, 0], [0, np.cos(0.5), 0, np.sin(0.5)])
+    # norm preserving
+    z = np.random.default_rng(0).normal(size=(4, 3, 8))
+    assert np.allclose(np.linalg.norm(tr.rope(z, np.arange(4), 1e4), axis=-1), np.linalg.norm(z, axis=-1))
+
+
+def test_rope_scores_depend_on_relative_position_only():
+    rng = np.random.default_rng(2)
+    q, k = rng.normal(size=(1, 1, 16)), rng.normal(size=(1, 1, 16))
+    def score(pq, pk):
+        return float(np.sum(tr.rope(q, np.array([pq]), 1e6) * tr.rope(k, np.array([pk]), 1e6)))
+    assert abs(score(10, 3) - score(1010, 1003)) < 1e-9
+    assert abs(score(10, 3) - score(11, 3)) > 1e-6
+
+
+def test_attention_against_torch_sdpa_with_gqa_mapping():
+    rng = np.random.default_rng(3)
+    T, Hq, Hkv, hd = 9, 4, 2, 8
+    q, K, V = rng.normal(size=(Hq, hd)), rng.normal(size=(T, Hkv, hd)), rng.normal(size=(T, Hkv, hd))
+    out = tr.attention_one(q, K, V, Hkv)
+    tq = torch.from_numpy(q)[None, :, None, :]                                   # [1,Hq,1,hd]
+    tk = torch.from_numpy(K).permute(1, 0, 2).repeat_interleave(Hq // Hkv, 0)[None]   # kv head h//rep
+    tv = torch.from_numpy(V).permute(1, 0, 2).repeat_interleave(Hq // Hkv, 0)[None]
+    ref = F.scaled_dot_product_attention(tq, tk, tv)[0, :, 0, :].numpy()
+    assert np.allclose(out, ref, atol=1e-13)
+
+
+def test_prefix_shared_equals_unshared_and_split_kv_merge_equals_unsplit():
+    rng = np.random.default_rng(4)
+    P, t, Hq, Hkv, hd = 13, 7, 4, 2, 8
+    Kp_, Vp = rng.normal(size=(P, Hkv, hd)), rng.normal(size=(P, Hkv, hd))
+    Ks, Vs = rng.normal(size=(t, Hkv, hd)), rng.normal(size=(t, Hkv, hd))
+    q = rng.normal(size=(Hq, hd)) * 3
+    whole = attention.attention_row(q, Kp_, Vp, Ks, Vs)
+    K, V = np.concatenate([Kp_, Ks]), np.concatenate([Vp, Vs])
+    for cuts in ([P], [5, P, P + 3], [1, 2, 3, 19]):
+        edges = [0] + cuts + [P + t]
+        for h in range(Hq):
+            g = h // (Hq // Hkv)
+            parts = [attention.partial(q[h], K[a:b, g], V[a:b, g]) for a, b in zip(edges[:-1], edges[1:])]
+            assert np.allclose(attention.merge_partials(parts), whole[h], atol=1e-13)
+
+
+def torch_forward(model, tokens):
+    """The same decoder built from torch library routines (rms_norm, SDPA, silu, linear); RoPE has no
+    library routine and is pinned separately above, so the oracle's own rope is applied here."""
+    cfg = model["cfg"]
+    t64 = lambda a: torch.from_numpy(np.asarray(a, dtype=np.float64))
+    Hq, Hkv, hd, d = cfg["n_q_heads"], cfg["n_kv_heads"], cfg["head_dim"], cfg["d_model"]
+    T = len(tokens)
+    h = F.embedding(torch.as_tensor(tokens, dtype=torch.long), t64(model["embed"]))
+    for L in model["layers"]:
+        a = F.rms_norm(h, (d,), t64(L["attn_norm"]), eps=cfg["rms_eps"])
+        qkv = F.linear(a, t64(L["wqkv"]))
+        q, k, v = qkv.split([Hq * hd, Hkv * hd, Hkv * hd], dim=-1)
+        q = t64(tr.rope(q.reshape(T, Hq, hd).numpy(), np.arange(T), cfg["rope_theta"])).permute(1, 0, 2)[None]
+        k = t64(tr.rope(k.reshape(T, Hkv, hd).numpy(), np.arange(T), cfg["rope_theta"])).permute(1, 0, 2)[None]
+        v = v.reshape(T, Hkv, hd).permute(1, 0, 2)[None]
+        o = F.scaled_dot_product_attention(q, k, v, is_causal=True, enable_gqa=True)[0].permute(1, 0, 2).reshape(T, -1)
+        h = h + F.linear(o, t64(L["wo"]))
+        b = F.rms_norm(h, (d,), t64(L["mlp_norm"]), eps=cfg["rms_eps"])
+        g, u = F.linear(b, t64(L["wgu"])).chunk(2, dim=-1)
+        h = h + F.linear(F.silu(g) * u, t64(L["wd"]))
+    return F.linear(F.rms_norm(h, (d,), t64(model["final_norm"]), eps=cfg["rms_eps"]), t64(model["lm_head"])).numpy()
+
+
+def test_forward_full_against_torch_library_decoder():
+    model = tiny_model(seed=5)
+    tokens = np.array([3, 17, 0, 39, 22, 8, 8, 1, 30, 11])
+    assert np.allclose(tr.forward_full(model, tokens), torch_forward(model, tokens), atol=1e-11)
+
+
+def test_incremental_decode_equals_full_causal_forward():
+    for kw in (dict(), dict(qk_norm=True), dict(n_experts=4, top_k=2, expert_ffn=24, ffn=0)):
+        model = tiny_model(seed=6, **kw)
+        tokens = np.array([5, 1, 9, 33, 2, 2, 18, 7, 25, 12, 0, 3])
+        P = 5
+        full = tr.forward_full(model, tokens)
+        z0, kv0 = tr.prefill(model, tokens[:P])
+        assert np.allclose(z0, full[P - 1], atol=1e-11)
+        kv = [(a.copy(), b.copy()) for a, b in kv0]
+        for t in range(P, len(tokens)):
+            z = tr.decode_one(model, kv, tokens[t], t)
+            assert np.allclose(z, full[t], atol=1e-10), (kw, t)
+
+
+def test_zero_weights_give_uniform_logits():
+    model = tiny_model(seed=7)
+    model["lm_head"] = np.zeros((40, 32))
+    z = tr.forward_full(model, np.array([1, 2, 3]))
+    assert np.all(z == 0.0)
+    assert np.allclose(tr.softmax(z), 1.0 / 40)
+
+
+def test_moe_single_expert_equals_dense_and_gates_sum_to_one():
+    dense = tiny_model(seed=8)
+    moe = tiny_model(seed=8, n_experts=1, top_k=1, expert_ffn=48, ffn=0)
+    for Ld, Lm in zip(dense["layers"], moe["layers"]):
+        Lm["wqkv"], Lm["wo"] = Ld["wqkv"], Ld["wo"]
+        Lm["wgu_e"], Lm["wd_e"] = np.asarray(Ld["wgu"], dtype=np.float64)[None], np.asarray(Ld["wd"], dtype=np.float64)[None]
+    moe["embed"], moe["lm_head"] = dense["embed"], dense["lm_head"]
+    tokens = np.array([4, 4, 31, 7])
+    assert np.allclose(tr.forward_full(moe, tokens), tr.forward_full(dense, tokens), atol=1e-12)
+    m4 = tiny_model(seed=9, n_experts=6, top_k=3, expert_ffn=16, ffn=0)
+    b = np.random.default_rng(0).normal(size=32)
+    ids, w = tr.moe_route(m4["layers"][0], m4["cfg"], b)
+    assert len(set(ids.tolist())) == 3 and abs(np.sum(w) - 1.0) < 1e-14 and np.all(np.diff(w) <= 0)
+    p = tr.softmax(np.asarray(m4["layers"][0]["wr"], dtype=np.float64) @ b)
+    assert set(ids.tolist()) == set(np.argsort(p)[-3:].tolist())
+
+
+def test_moe_route_tie_prefers_lower_expert_id():
+    cfg = dict(top_k=2)
+    layer = dict(wr=np.zeros((5, 3)))                       # all logits equal -> experts 0,1
+    ids, w = tr.moe_route(layer, cfg, np.ones(3))
+    assert ids.tolist() == [0, 1] and np.allclose(w, 0.5)
