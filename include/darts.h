@@ -1,0 +1,210 @@
+/*
+ * darts.h — C-ABI of the B200-native DARTS group-rollout decoder (arxiv/paper_2605_30859).
+ *
+ * What the library computes (citations: PAPER.md:<line>, section):
+ *   For each prompt q_i of a rollout batch, M'_i = Kp[i] redundant trajectories are decoded
+ *   autoregressively ("intra-prompt redundant rollout", §4.1.1) over ONE shared,
+ *   paged prompt KV cache; after every lock-step decode step the distribution-aware rule of
+ *   Alg. 2 (PAPER.md:465-477, prose :426-432, :479) is applied per prompt on the device:
+ *     - M'_i <  M_up : dual-end length sampling — wait for the whole pool, keep the S = K - L_long
+ *       shortest and the L_long longest trajectories, the longest drawn only from trajectories that
+ *       did not hit the length limit (§4.1.2);
+ *     - M'_i >= M_up : shortest-only sampling with proactive early stop — as soon as K valid
+ *       trajectories exist the other M'_i - K are halted (§4.3.1).
+ *   Finished / pruned rows are compacted out of the batch on the device.
+ *   Notation: the paper's M is `K` here, M'_i is `Kp[i]`, the paper's K (short count) is K - L_long.
+ *
+ * Conventions
+ *   - Every function returns a darts_status (0 = DARTS_OK).  No exceptions, no exit(), no stdout.
+ *     darts_last_error(ctx) returns a ctx-owned, NUL-terminated description of the last failure.
+ *   - "device" pointers are CUDA device pointers allocated by the caller (e.g. with torch); "host"
+ *     pointers are ordinary host memory.  The library never frees caller memory.  Weights are
+ *     BORROWED: the pointers in darts_weights must stay valid until darts_destroy.
+ *   - The library allocates no device memory of its own: everything it needs (KV page pool, page
+ *     tables, row state, activations) is carved out of the caller's workspace, whose size
+ *     darts_workspace_bytes reports.  It owns a few bytes of pinned host memory for counters.
+ *   - All work is enqueued on runtime_desc.stream (a cudaStream_t passed as void*).  Only
+ *     darts_rollout, darts_get_results, darts_get_counters and darts_debug_* synchronise.
+ *   - One ctx = one GPU = one stream; a ctx is not thread-safe.
+ *   - There is no CPU fallback and no other backend: on a device that is not sm_100 every entry
+ *     point that needs the GPU returns DARTS_ERR_UNSUPPORTED.
+ *
+ * Layouts
+ *   - Projections are [out_features, in_features] row-major in the model dtype (F32 or BF16).
+ *     wqkv rows: n_q_heads q-heads, then n_kv_heads k-heads, then n_kv_heads v-heads (head_dim rows each).
+ *     wgu rows:  ffn gate rows, then ffn up rows.  MoE: wgu_e [E][2*expert_ffn][d], wd_e [E][d][expert_ffn],
+ *     router wr [E][d] always F32.
+ *   - Rows (trajectories) are numbered group-major: row = sum_{i'<i} Kp[i'] + j.
+ *   - KV cache (library-owned, inside the workspace): pages of page_size tokens,
+ *     [layer][page][K|V][kv_head][token][head_dim]; a row's page table is
+ *     [its prompt's shared prefix pages || its own suffix pages]; the suffix starts on a fresh page,
+ *     so the K' samples of a prompt share the prefix pages without any copy.
+ */
+#ifndef DARTS_H_
+#define DARTS_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef int32_t darts_status;
+enum {
+  DARTS_OK = 0,
+  DARTS_ERR_INVALID_ARG = 1,       /* NULLs, K > Kp[i], Kp[i] > 32, L_long >= K, G > max_prompts, ... */
+  DARTS_ERR_UNSUPPORTED = 2,       /* head_dim / page_size / dtype combination, non-sm_100 device */
+  DARTS_ERR_KV_POOL_EXHAUSTED = 3, /* page pool ran dry; the rollout is stopped, nothing is corrupted */
+  DARTS_ERR_WORKSPACE_TOO_SMALL = 4,
+  DARTS_ERR_CUDA = 5,              /* sticky; darts_last_error carries cudaGetErrorString */
+  DARTS_ERR_BAD_STATE = 6          /* e.g. darts_decode_step before darts_prefill */
+};
+
+enum { DARTS_F32 = 0, DARTS_BF16 = 1 };
+
+/* Row status (rows "reaching the system length limit" are incomplete/invalid = TRUNC;
+ * rows halted by the early-stop signal = PRUNED). */
+enum { DARTS_ROW_ACTIVE = 0, DARTS_ROW_VALID = 1, DARTS_ROW_TRUNC = 2, DARTS_ROW_PRUNED = 3 };
+
+/* Selection mode.  AUTO is the paper's rule: shortest-only + early stop iff Kp[i] >= M_up. */
+enum { DARTS_MODE_AUTO = 0, DARTS_MODE_DUAL_END = 1, DARTS_MODE_SHORTEST_EARLY_STOP = 2 };
+
+enum {
+  DARTS_FLAG_DUMP_LOGITS = 1,       /* keep fp32 logits of every row of the last step for darts_debug_logits */
+  DARTS_FLAG_NO_PREFIX_SHARING = 2  /* A/B switch: attention re-reads the prefix once per row, not per group */
+};
+
+typedef struct {
+  int32_t n_layers, d_model, n_q_heads, n_kv_heads, head_dim;
+  int32_t ffn;                         /* dense SwiGLU width (0 for MoE / attention-only) */
+  int32_t vocab;                       /* 0: attention-only context (config 2), no model weights needed */
+  int32_t n_experts, top_k, expert_ffn;/* 0 => dense */
+  int32_t dtype;                       /* DARTS_F32 | DARTS_BF16: weights, activations fed to GEMMs, KV cache */
+  int32_t qk_norm;                     /* 1: per-head RMSNorm of q and k before RoPE */
+  float rope_theta, rms_eps;
+  int32_t eos_id;                      /* -1 disables natural EOS */
+} darts_model_desc;
+
+/* Device pointers; per-layer members are HOST arrays of n_layers device pointers. */
+typedef struct {
+  const void *embed, *final_norm, *lm_head;
+  const void *const *attn_norm, *const *wqkv, *const *q_norm, *const *k_norm, *const *wo;
+  const void *const *mlp_norm, *const *wgu, *const *wd;
+  const void *const *wr, *const *wgu_e, *const *wd_e;
+} darts_weights;
+
+typedef struct {
+  int32_t page_size;                   /* tokens per KV page (64 for the tuned bf16 path) */
+  int32_t n_pages;                     /* pages in the pool (shared by all layers' slabs) */
+  int32_t max_rows;                    /* >= sum Kp[i] */
+  int32_t max_prompts, max_prompt_len, max_new;
+  int32_t prefill_chunk;               /* max prompt tokens per prefill pass (>= max_prompt_len); 0 = default */
+  uint32_t flags;
+  void *workspace;                     /* device; >= darts_workspace_bytes() */
+  size_t workspace_bytes;
+  void *stream;                        /* cudaStream_t */
+} darts_runtime_desc;
+
+/* Per-prompt rule parameters (Alg. 2 inputs "Target Size M, Dual-End Short Size K"). */
+typedef struct {
+  int32_t K;                           /* keep count (paper's M) */
+  int32_t L_long;                      /* dual-end long count (paper's L; 1 in all main experiments) */
+  int32_t M_up;                        /* saturation threshold (paper: 2M); 0 => 2*K */
+  int32_t mode;                        /* DARTS_MODE_* */
+} darts_policy;
+
+/* Caller buffers (HOST unless a member says device) filled by darts_get_results; any may be NULL. */
+typedef struct {
+  int32_t *tokens;                     /* [n_rows][max_new], -1 beyond len */
+  int32_t *len;                        /* [n_rows] generated tokens incl. the terminal EOS */
+  uint8_t *status;                     /* [n_rows] DARTS_ROW_* */
+  float *margin;                       /* [n_rows][max_new] Gumbel-max top1-top2 margin per sampled token */
+  int32_t *sel;                        /* [G][K] selected sample indices j, rule order */
+  uint32_t *sel_mask;                  /* [G] bitset of sel */
+  int32_t *close_step;                 /* [G] step index at which the group closed */
+  float *len_mean, *len_var;           /* [G] mean / population variance of the pool's lengths (sigma_L^2) */
+} darts_results;
+
+typedef struct {
+  int64_t n_steps;                     /* lock-step decode iterations incl. step 0 (first token from prefill) */
+  int64_t n_generated_tokens;          /* all sampled tokens, incl. rows later pruned */
+  int64_t n_kept_tokens;               /* tokens of the K selected trajectories of every prompt */
+  int64_t n_near_ties;                 /* sampled tokens whose margin < 1e-3 */
+  int64_t n_row_steps;                 /* sum over steps of active rows (= n_generated_tokens) */
+  int64_t peak_pages;                  /* high-water mark of pages in use */
+  int64_t kernel_launches;             /* kernels this ctx launched since darts_create */
+} darts_counters;
+
+typedef struct darts_ctx darts_ctx;
+
+/* Host-only sizing of the workspace for (model, runtime). */
+darts_status darts_workspace_bytes(const darts_model_desc *m, const darts_runtime_desc *rt, size_t *out);
+
+/* Carve the workspace, record borrowed weight pointers.  `w` may be NULL only if m->vocab == 0. */
+darts_status darts_create(const darts_model_desc *m, const darts_weights *w, const darts_runtime_desc *rt,
+                          darts_ctx **out);
+darts_status darts_destroy(darts_ctx *ctx);
+const char *darts_last_error(const darts_ctx *ctx);
+
+/* SURVEY §8(a) rows 1-2 + the first token (step 0):  one causal forward per PROMPT (not per sample)
+ * writes the shared prefix pages; the last-position logits are sampled Kp[i] times with Philox keys
+ * (seed, i, j, 0).  prompt_tokens / prompt_offsets (G+1) / Kp (G) / forced_len ([G][Kp_max] row-major,
+ * Kp_max = max Kp, or NULL) are DEVICE pointers; Kp_host mirrors Kp on the host (needed for sizing).
+ * forced_len[i][j] == len forces token len of trajectory (i,j) to eos_id (BASELINE.json workloads). */
+darts_status darts_prefill(darts_ctx *ctx, const int32_t *prompt_tokens, const int32_t *prompt_offsets_host,
+                           int32_t G, const int32_t *Kp_host, const int32_t *forced_len,
+                           const darts_policy *policy, float temperature, uint64_t seed);
+
+/* SURVEY §8(a) rows 3-8 for all active rows: embed, L x [RMSNorm, QKV, RoPE + KV append,
+ * prefix-shared split-KV attention, O-proj, RMSNorm, SwiGLU MLP or MoE], final norm, LM head fused
+ * with temperature + Philox Gumbel-max, EOS / forced-stop / length update.  No-op when nothing is active. */
+darts_status darts_decode_step(darts_ctx *ctx);
+
+/* per-prompt rule (Alg. 2), pruning, page release, stable compaction of the
+ * active row list.  n_active_out: device or pinned host int32, may be NULL. */
+darts_status darts_select_and_compact(darts_ctx *ctx, int32_t *n_active_out);
+
+/* north_star signature: prefill + loop until every prompt has closed; synchronises before returning.
+ * prompts: DEVICE [G][prompt_len] int32 (equal-length prompts); Kp_scalar = K' for every prompt.
+ * L_long = 1, M_up = 2K, mode AUTO (use darts_prefill + the step calls for anything else). */
+darts_status darts_rollout(darts_ctx *ctx, const int32_t *prompts, int32_t prompt_len, int32_t G,
+                           int32_t Kp_scalar, int32_t K, int32_t max_len, float temperature, uint64_t seed,
+                           const int32_t *forced_len, darts_results *out);
+
+/* Same loop after a caller-issued darts_prefill (ragged prompts, per-prompt Kp, explicit policy). */
+darts_status darts_run_to_completion(darts_ctx *ctx, darts_results *out);
+
+/* End-to-end convenience with HOST inputs (bench `e2e`): copies prompts / forced_len host->device,
+ * runs the rollout, copies results device->host. */
+darts_status darts_rollout_host(darts_ctx *ctx, const int32_t *prompts_host, int32_t prompt_len, int32_t G,
+                                const int32_t *Kp_host, const int32_t *forced_len_host, const darts_policy *policy,
+                                int32_t max_len, float temperature, uint64_t seed, darts_results *out);
+
+darts_status darts_get_results(darts_ctx *ctx, darts_results *out);
+darts_status darts_get_counters(darts_ctx *ctx, darts_counters *out);
+darts_status darts_n_active(darts_ctx *ctx, int32_t *out_host);      /* synchronises */
+
+/* Parity hooks (valid with DARTS_FLAG_DUMP_LOGITS): fp32 logits of global row `row` from the most
+ * recent step that row took part in (step 0: the prompt's prefill logits).  out: HOST [vocab]. */
+darts_status darts_debug_logits(darts_ctx *ctx, int32_t row, float *out_host);
+
+/* Teacher forcing for parity at bf16 (R12): overwrite the token the next decode step feeds
+ * for global row `row`.  tokens: HOST [n_rows] (-1 = leave). */
+darts_status darts_debug_set_last_tokens(darts_ctx *ctx, const int32_t *tokens_host, int32_t n_rows);
+
+/* ---- Attention-only entry points (BASELINE.json config 2) -------------------
+ * Build G groups of Kp rows whose KV is given explicitly, then time darts_attention alone.
+ * k_prefix/v_prefix: DEVICE [G][P][n_kv_heads][head_dim]; suffix_len: HOST [R]; k_suffix/v_suffix:
+ * DEVICE packed [sum suffix_len][n_kv_heads][head_dim] in row order.  Loads layer 0 of the cache. */
+darts_status darts_attn_load(darts_ctx *ctx, int32_t G, int32_t P, int32_t Kp, const void *k_prefix,
+                             const void *v_prefix, const int32_t *suffix_len_host, const void *k_suffix,
+                             const void *v_suffix);
+/* q: DEVICE [R][n_q_heads][head_dim] (model dtype); out: DEVICE same shape.  One decode-step attention
+ * over all R rows on layer `layer`; asynchronous on the ctx stream. */
+darts_status darts_attention(darts_ctx *ctx, int32_t layer, const void *q, void *out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DARTS_H_ */

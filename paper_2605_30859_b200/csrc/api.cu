@@ -1,0 +1,529 @@
+// C-ABI entry points (include/darts.h): workspace carving, prefill, decode step, selection/compaction,
+// the rollout loop and result read-back.  Host logic only; every step of the path runs in the kernels.
+#include <algorithm>
+#include <new>
+#include <vector>
+
+#include "internal.cuh"
+
+namespace {
+
+struct Carver {
+  char *base;
+  size_t off = 0;
+  explicit Carver(void *b) : base((char *)b) {}
+  template <typename T> T *take(size_t n) {
+    off = (off + 255) & ~(size_t)255;
+    T *p = base ? (T *)(base + off) : nullptr;
+    off += n * sizeof(T);
+    return p;
+  }
+};
+
+int ceil_div(int a, int b) { return (a + b - 1) / b; }
+
+int default_chunk(const darts_runtime_desc *rt) {
+  int c = rt->prefill_chunk > 0 ? rt->prefill_chunk : 4096;
+  return std::max(c, rt->max_prompt_len);
+}
+
+// One routine lays the workspace out for both sizing (c->... pointers NULL) and creation.
+size_t carve(darts_ctx *c, void *base) {
+  const darts_model_desc &m = c->m;
+  const darts_runtime_desc &rt = c->rt;
+  Carver k(base);
+  bool model = m.vocab > 0;
+  c->elt = m.dtype == DARTS_F32 ? 4 : 2;
+  c->n_qkv = (m.n_q_heads + 2 * m.n_kv_heads) * m.head_dim;
+  c->max_suffix_pages = ceil_div(rt.max_new, rt.page_size) + 1;
+  c->max_prefix_pages = std::max(1, ceil_div(rt.max_prompt_len, rt.page_size));
+  c->act_rows = model ? std::max(rt.max_rows, default_chunk(&rt)) : rt.max_rows;
+  c->kv_tile_elems = (size_t)rt.page_size * m.head_dim;
+  c->kv_page_elems = 2 * (size_t)m.n_kv_heads * c->kv_tile_elems;
+  c->kv_layer_elems = (size_t)rt.n_pages * c->kv_page_elems;
+  size_t R = rt.max_rows, G = rt.max_prompts, A = c->act_rows;
+  c->kv_pool = k.take<char>((size_t)m.n_layers * c->kv_layer_elems * c->elt);
+  c->st = k.take<DevState>(1);
+  c->free_pages = k.take<int32_t>(rt.n_pages);
+  c->row_list = k.take<int32_t>(R);
+  c->row_list_tmp = k.take<int32_t>(R);
+  c->row_prompt = k.take<int32_t>(R);
+  c->row_sample = k.take<int32_t>(R);
+  c->row_len = k.take<int32_t>(R);
+  c->row_forced = k.take<int32_t>(R);
+  c->row_last_tok = k.take<int32_t>(R);
+  c->row_slot = k.take<int32_t>(R);
+  c->row_slot_step = k.take<int32_t>(R);
+  c->row_pages = k.take<int32_t>(R * c->max_suffix_pages);
+  c->row_status = k.take<uint8_t>(R);
+  c->g_off = k.take<int32_t>(G + 1);
+  c->g_Kp = k.take<int32_t>(G);
+  c->g_plen = k.take<int32_t>(G);
+  c->g_closed = k.take<int32_t>(G);
+  c->g_sel = k.take<int32_t>(G * DARTS_MAX_KP);
+  c->g_close_step = k.take<int32_t>(G);
+  c->g_prefix_pages = k.take<int32_t>(G * c->max_prefix_pages);
+  c->g_tok_off = k.take<int32_t>(G + 1);
+  c->g_mask = k.take<uint32_t>(G);
+  c->g_len_mean = k.take<float>(G);
+  c->g_len_var = k.take<float>(G);
+  c->slot_row = k.take<int32_t>(A);
+  c->slot_tok = k.take<int32_t>(A);
+  c->slot_pos = k.take<int32_t>(A);
+  c->slot_dst_page = k.take<int32_t>(A);
+  c->slot_dst_off = k.take<int32_t>(A);
+  c->slot_prompt = k.take<int32_t>(A);
+  c->slot_npre = k.take<int32_t>(A);
+  c->slot_nsuf = k.take<int32_t>(A);
+  c->forced_stage = k.take<int32_t>(G * DARTS_MAX_KP);
+  if (model) {
+    size_t F = m.n_experts ? (size_t)m.top_k * m.expert_ffn : (size_t)m.ffn;
+    c->tokens_out = k.take<int32_t>(R * rt.max_new);
+    c->margin_out = k.take<float>(R * rt.max_new);
+    c->prompt_tokens = k.take<int32_t>(G * rt.max_prompt_len);
+    c->slot_cs = k.take<float2>(A * (m.head_dim / 2));
+    c->h = k.take<float>(A * m.d_model);
+    c->qkv32 = k.take<float>(A * c->n_qkv);
+    c->gu32 = k.take<float>(A * 2 * F);
+    c->logits = k.take<float>(R * m.vocab);
+    c->z0 = k.take<float>(G * m.vocab);
+    c->hlast = k.take<float>(G * m.d_model);
+    c->xn = k.take<char>(A * m.d_model * c->elt);
+    c->q = k.take<char>(A * m.n_q_heads * m.head_dim * c->elt);
+    c->ao = k.take<char>(A * m.n_q_heads * m.head_dim * c->elt);
+    c->act = k.take<char>(A * F * c->elt);
+  }
+  return (k.off + 255) & ~(size_t)255;
+}
+
+darts_status validate(const darts_model_desc *m, const darts_runtime_desc *rt, char *err, size_t n) {
+  if (!m || !rt) { snprintf(err, n, "NULL descriptor"); return DARTS_ERR_INVALID_ARG; }
+  if (m->n_layers <= 0 || m->n_q_heads <= 0 || m->n_kv_heads <= 0 || m->head_dim <= 0 || m->n_q_heads % m->n_kv_heads) {
+    snprintf(err, n, "bad head geometry"); return DARTS_ERR_INVALID_ARG;
+  }
+  if (m->dtype != DARTS_F32 && m->dtype != DARTS_BF16) { snprintf(err, n, "dtype must be F32 or BF16"); return DARTS_ERR_UNSUPPORTED; }
+  if (m->head_dim % 32 || m->head_dim > 256 || (m->head_dim / 32 != 1 && m->head_dim / 32 != 2 && m->head_dim / 32 != 4 && m->head_dim / 32 != 8)) {
+    snprintf(err, n, "head_dim %d not in {32,64,128,256}", m->head_dim); return DARTS_ERR_UNSUPPORTED;
+  }
+  if (m->n_q_heads / m->n_kv_heads > 32) { snprintf(err, n, "GQA ratio > 32"); return DARTS_ERR_UNSUPPORTED; }
+  if (rt->page_size <= 0 || rt->n_pages <= 0 || rt->max_rows <= 0 || rt->max_prompts <= 0 || rt->max_new <= 0 || rt->max_prompt_len <= 0) {
+    snprintf(err, n, "runtime sizes must be positive"); return DARTS_ERR_INVALID_ARG;
+  }
+  if (m->vocab > 0 && m->n_experts == 0 && m->ffn <= 0) { snprintf(err, n, "dense model needs ffn > 0"); return DARTS_ERR_INVALID_ARG; }
+  return DARTS_OK;
+}
+
+darts_status check_device(darts_ctx *c) {
+  int dev = 0;
+  cudaDeviceProp p;
+  CUDA_TRY(c, cudaGetDevice(&dev));
+  CUDA_TRY(c, cudaGetDeviceProperties(&p, dev));
+  if (p.major != 10) FAIL(c, DARTS_ERR_UNSUPPORTED, "device is sm_%d%d; this library is sm_100a only (no fallback)", p.major, p.minor);
+  return DARTS_OK;
+}
+
+const void **dup_ptrs(const void *const *src, int n) {
+  if (!src) return nullptr;
+  const void **d = new const void *[n];
+  for (int i = 0; i < n; ++i) d[i] = src[i];
+  return d;
+}
+
+#define TRY(x) do { darts_status s__ = (x); if (s__ != DARTS_OK) return s__; } while (0)
+
+// One transformer pass over `rows` slots whose plan (slot_*) is already on the device.
+darts_status forward_layers(darts_ctx *c, int rows_ub, const int32_t *n_rows_dev) {
+  const darts_model_desc &m = c->m;
+  TRY(launch_embed(c, c->slot_tok, 0, rows_ub, n_rows_dev));
+  TRY(launch_rope_table(c, rows_ub, n_rows_dev));
+  int qd = m.n_q_heads * m.head_dim;
+  for (int l = 0; l < m.n_layers; ++l) {
+    TRY(launch_rmsnorm(c, c->h, c->attn_norm[l], c->xn, rows_ub, n_rows_dev));
+    TRY(launch_gemm(c, c->xn, c->wqkv[l], c->qkv32, c->n_qkv, m.d_model, rows_ub, n_rows_dev, false));
+    TRY(launch_rope_append(c, l, rows_ub, n_rows_dev));
+    TRY(launch_attention(c, l, c->q, c->ao, rows_ub, n_rows_dev));
+    TRY(launch_gemm(c, c->ao, c->wo[l], c->h, m.d_model, qd, rows_ub, n_rows_dev, true));
+    TRY(launch_rmsnorm(c, c->h, c->mlp_norm[l], c->xn, rows_ub, n_rows_dev));
+    if (m.n_experts == 0) {
+      TRY(launch_gemm(c, c->xn, c->wgu[l], c->gu32, 2 * m.ffn, m.d_model, rows_ub, n_rows_dev, false));
+      TRY(launch_silu_mul(c, rows_ub, n_rows_dev));
+      TRY(launch_gemm(c, c->act, c->wd[l], c->h, m.d_model, m.ffn, rows_ub, n_rows_dev, true));
+    } else {
+      TRY(launch_moe(c, l, rows_ub, n_rows_dev));
+    }
+  }
+  return DARTS_OK;
+}
+
+void refresh_ub(darts_ctx *c) {
+  long long v = *(volatile long long *)c->pinned;          // {n_active, generation} written in one store
+  if ((uint32_t)(v >> 32) == c->gen) c->host_active_ub = std::min(c->host_active_ub, (int32_t)(v & 0xffffffff));
+}
+
+darts_status prefill_impl(darts_ctx *c, const int32_t *prompt_tokens_dev, bool tokens_in_place, const int32_t *offs, int32_t G,
+                          const int32_t *Kp, const int32_t *forced_len_dev, const darts_policy *pol, float temperature, uint64_t seed) {
+  if (c->sticky) return c->sticky;
+  if (!c->has_weights) FAIL(c, DARTS_ERR_BAD_STATE, "context was created without weights (attention-only)");
+  if (!offs || !Kp || !pol || G <= 0 || (!tokens_in_place && !prompt_tokens_dev)) FAIL(c, DARTS_ERR_INVALID_ARG, "NULL argument or G <= 0");
+  if (G > c->rt.max_prompts) FAIL(c, DARTS_ERR_INVALID_ARG, "G=%d > max_prompts=%d", G, c->rt.max_prompts);
+  darts_policy p = *pol;
+  if (p.M_up <= 0) p.M_up = 2 * p.K;                                            // PAPER.md:204 (M_up = 2M)
+  if (p.K <= 0 || p.K > DARTS_MAX_KP || p.L_long < 0 || p.L_long >= p.K)
+    FAIL(c, DARTS_ERR_INVALID_ARG, "need 0 < K <= 32 and 0 <= L_long < K (K=%d, L_long=%d)", p.K, p.L_long);
+  if (p.mode < DARTS_MODE_AUTO || p.mode > DARTS_MODE_SHORTEST_EARLY_STOP) FAIL(c, DARTS_ERR_INVALID_ARG, "bad mode %d", p.mode);
+  std::vector<int32_t> g_off(G + 1), plen(G), tok_off(G + 1), pre_pages((size_t)G * c->max_prefix_pages, -1);
+  int R = 0, Kp_max = 0, n_prefix_pages = 0;
+  for (int i = 0; i < G; ++i) {
+    if (Kp[i] < p.K || Kp[i] > DARTS_MAX_KP) FAIL(c, DARTS_ERR_INVALID_ARG, "need K <= Kp[i] <= 32 (Kp[%d]=%d, K=%d)", i, Kp[i], p.K);
+    int P = offs[i + 1] - offs[i];
+    if (P <= 0 || P > c->rt.max_prompt_len) FAIL(c, DARTS_ERR_INVALID_ARG, "prompt %d has length %d (max %d)", i, P, c->rt.max_prompt_len);
+    g_off[i] = R; plen[i] = P; tok_off[i] = offs[i] - offs[0];
+    R += Kp[i]; Kp_max = std::max(Kp_max, Kp[i]);
+    for (int q = 0; q < ceil_div(P, c->rt.page_size); ++q) pre_pages[(size_t)i * c->max_prefix_pages + q] = n_prefix_pages++;
+  }
+  g_off[G] = R; tok_off[G] = offs[G] - offs[0];
+  if (R > c->rt.max_rows) FAIL(c, DARTS_ERR_INVALID_ARG, "sum Kp = %d > max_rows = %d", R, c->rt.max_rows);
+  if (n_prefix_pages > c->rt.n_pages) FAIL(c, DARTS_ERR_KV_POOL_EXHAUSTED, "prefix needs %d pages, pool has %d", n_prefix_pages, c->rt.n_pages);
+  c->pol = p; c->temperature = temperature; c->seed = seed; c->G = G; c->R = R; c->Kp_max = Kp_max;
+  if (c->max_len <= 0 || c->max_len > c->rt.max_new) c->max_len = c->rt.max_new;
+  c->gen += 1; c->host_active_ub = R; c->steps_issued = 0; c->prefilled = false;
+  cudaStream_t s = c->stream;
+  int total_tok = tok_off[G];
+  if (!tokens_in_place)
+    CUDA_TRY(c, cudaMemcpyAsync(c->prompt_tokens, prompt_tokens_dev + offs[0], (size_t)total_tok * 4, cudaMemcpyDeviceToDevice, s));
+  CUDA_TRY(c, cudaMemcpyAsync(c->g_off, g_off.data(), (G + 1) * 4, cudaMemcpyHostToDevice, s));
+  CUDA_TRY(c, cudaMemcpyAsync(c->g_Kp, Kp, G * 4, cudaMemcpyHostToDevice, s));
+  CUDA_TRY(c, cudaMemcpyAsync(c->g_plen, plen.data(), G * 4, cudaMemcpyHostToDevice, s));
+  CUDA_TRY(c, cudaMemcpyAsync(c->g_tok_off, tok_off.data(), (G + 1) * 4, cudaMemcpyHostToDevice, s));
+  CUDA_TRY(c, cudaMemcpyAsync(c->g_prefix_pages, pre_pages.data(), pre_pages.size() * 4, cudaMemcpyHostToDevice, s));
+  CUDA_TRY(c, cudaMemsetAsync(c->tokens_out, 0xFF, (size_t)R * c->rt.max_new * 4, s));
+  CUDA_TRY(c, cudaMemsetAsync(c->margin_out, 0, (size_t)R * c->rt.max_new * 4, s));
+  CUDA_TRY(c, cudaMemsetAsync(c->g_sel, 0xFF, (size_t)G * DARTS_MAX_KP * 4, s));
+  TRY(launch_init_rows(c, forced_len_dev, n_prefix_pages));
+  // one causal pass per PROMPT, in chunks of whole prompts
+  int chunk = default_chunk(&c->rt);
+  for (int g0 = 0; g0 < G;) {
+    int g1 = g0, ntok = 0;
+    while (g1 < G && ntok + plen[g1] <= chunk) ntok += plen[g1++];
+    int tb = tok_off[g0];
+    TRY(launch_plan_prefill(c, tb, ntok, g0, g1));
+    TRY(forward_layers(c, ntok, nullptr));
+    TRY(launch_gather_last(c, tb, ntok, g0, g1));
+    TRY(launch_rmsnorm(c, c->hlast, c->final_norm, c->xn, g1 - g0, nullptr));
+    TRY(launch_gemm(c, c->xn, c->lm_head, c->z0 + (size_t)g0 * c->m.vocab, c->m.vocab, c->m.d_model, g1 - g0, nullptr, false));
+    g0 = g1;
+  }
+  TRY(launch_sample(c, c->z0, 1, R));                                            // step 0: Kp[i] draws from the shared z0[i]
+  c->prefilled = true;
+  return DARTS_OK;
+}
+
+}  // namespace
+
+// dispatchers: the tuned sm_100a kernels take the shapes they support, the generic kernels the rest
+darts_status launch_gemm_tc(darts_ctx *c, const void *X, const void *W, float *C, int N, int K, int rows_ub,
+                            const int32_t *n_rows_dev, bool accumulate, bool *taken);
+darts_status launch_attention_sm100(darts_ctx *c, int layer, const void *q, void *out, int rows_ub, const int32_t *n_rows_dev, bool *taken);
+
+darts_status launch_gemm(darts_ctx *c, const void *X, const void *W, float *C, int N, int K, int rows_ub, const int32_t *n_rows_dev,
+                         bool accumulate, bool w_is_f32) {
+  if (rows_ub <= 0) return DARTS_OK;
+  if (c->m.dtype == DARTS_BF16 && !w_is_f32) {
+    bool taken = false;
+    darts_status s = launch_gemm_tc(c, X, W, C, N, K, rows_ub, n_rows_dev, accumulate, &taken);
+    if (s != DARTS_OK || taken) return s;
+  }
+  return launch_gemm_simt(c, X, W, C, N, K, rows_ub, n_rows_dev, accumulate, w_is_f32);
+}
+
+darts_status launch_attention(darts_ctx *c, int layer, const void *q, void *out, int rows_ub, const int32_t *n_rows_dev) {
+  if (rows_ub <= 0) return DARTS_OK;
+  bool taken = false;
+  darts_status s = launch_attention_sm100(c, layer, q, out, rows_ub, n_rows_dev, &taken);
+  if (s != DARTS_OK || taken) return s;
+  return launch_attention_ref(c, layer, q, out, rows_ub, n_rows_dev);
+}
+
+extern "C" {
+
+darts_status darts_workspace_bytes(const darts_model_desc *m, const darts_runtime_desc *rt, size_t *out) {
+  char err[128];
+  if (!out) return DARTS_ERR_INVALID_ARG;
+  darts_status s = validate(m, rt, err, sizeof(err));
+  if (s != DARTS_OK) return s;
+  darts_ctx tmp{};
+  tmp.m = *m; tmp.rt = *rt;
+  *out = carve(&tmp, nullptr);
+  return DARTS_OK;
+}
+
+darts_status darts_create(const darts_model_desc *m, const darts_weights *w, const darts_runtime_desc *rt, darts_ctx **out) {
+  if (!out) return DARTS_ERR_INVALID_ARG;
+  *out = nullptr;
+  char err[128];
+  darts_status s = validate(m, rt, err, sizeof(err));
+  if (s != DARTS_OK) return s;
+  if (m->vocab > 0 && !w) return DARTS_ERR_INVALID_ARG;
+  if (!rt->workspace) return DARTS_ERR_INVALID_ARG;
+  darts_ctx *c = new (std::nothrow) darts_ctx{};
+  if (!c) return DARTS_ERR_INVALID_ARG;
+  c->m = *m; c->rt = *rt; c->stream = (cudaStream_t)rt->stream;
+  *out = c;                                    // returned even on failure so darts_last_error can be read
+  if ((s = check_device(c)) != DARTS_OK) return s;
+  size_t need = carve(c, rt->workspace);
+  if (need > rt->workspace_bytes) FAIL(c, DARTS_ERR_WORKSPACE_TOO_SMALL, "workspace %zu < %zu bytes", rt->workspace_bytes, need);
+  if (((uintptr_t)rt->workspace & 255) != 0) FAIL(c, DARTS_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
+  c->has_weights = m->vocab > 0;
+  if (c->has_weights) {
+    int L = m->n_layers;
+    c->embed = w->embed; c->final_norm = w->final_norm; c->lm_head = w->lm_head;
+    c->attn_norm = dup_ptrs(w->attn_norm, L); c->wqkv = dup_ptrs(w->wqkv, L); c->wo = dup_ptrs(w->wo, L);
+    c->q_norm = dup_ptrs(w->q_norm, L); c->k_norm = dup_ptrs(w->k_norm, L);
+    c->mlp_norm = dup_ptrs(w->mlp_norm, L); c->wgu = dup_ptrs(w->wgu, L); c->wd = dup_ptrs(w->wd, L);
+    c->wr = dup_ptrs(w->wr, L); c->wgu_e = dup_ptrs(w->wgu_e, L); c->wd_e = dup_ptrs(w->wd_e, L);
+    bool ok = c->embed && c->final_norm && c->lm_head && c->attn_norm && c->wqkv && c->wo && c->mlp_norm &&
+              (m->n_experts ? (c->wr && c->wgu_e && c->wd_e) : (c->wgu && c->wd)) && (!m->qk_norm || (c->q_norm && c->k_norm));
+    if (!ok) FAIL(c, DARTS_ERR_INVALID_ARG, "missing weight pointers");
+  }
+  void *pin = nullptr;
+  CUDA_TRY(c, cudaHostAlloc(&pin, 64, cudaHostAllocMapped));
+  memset(pin, 0, 64);
+  c->pinned = (volatile int32_t *)pin;
+  void *pd = nullptr;
+  CUDA_TRY(c, cudaHostGetDevicePointer(&pd, pin, 0));
+  c->pinned_dev = (int32_t *)pd;
+  CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev[0], cudaEventDisableTiming));
+  CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev[1], cudaEventDisableTiming));
+  CUDA_TRY(c, cudaMemsetAsync(c->st, 0, sizeof(DevState), c->stream));
+  return DARTS_OK;
+}
+
+darts_status darts_destroy(darts_ctx *c) {
+  if (!c) return DARTS_OK;
+  if (c->stream || c->pinned) cudaStreamSynchronize(c->stream);
+  if (c->pinned) cudaFreeHost((void *)c->pinned);
+  if (c->ev[0]) cudaEventDestroy(c->ev[0]);
+  if (c->ev[1]) cudaEventDestroy(c->ev[1]);
+  const void **arrs[] = {c->attn_norm, c->wqkv, c->q_norm, c->k_norm, c->wo, c->mlp_norm, c->wgu, c->wd, c->wr, c->wgu_e, c->wd_e};
+  for (auto a : arrs) delete[] a;
+  delete c;
+  return DARTS_OK;
+}
+
+const char *darts_last_error(const darts_ctx *c) { return c ? c->err : "NULL context"; }
+
+darts_status darts_prefill(darts_ctx *c, const int32_t *prompt_tokens, const int32_t *prompt_offsets_host, int32_t G,
+                           const int32_t *Kp_host, const int32_t *forced_len, const darts_policy *policy, float temperature, uint64_t seed) {
+  if (!c) return DARTS_ERR_INVALID_ARG;
+  return prefill_impl(c, prompt_tokens, false, prompt_offsets_host, G, Kp_host, forced_len, policy, temperature, seed);
+}
+
+darts_status darts_decode_step(darts_ctx *c) {
+  if (!c) return DARTS_ERR_INVALID_ARG;
+  if (c->sticky) return c->sticky;
+  if (!c->prefilled) FAIL(c, DARTS_ERR_BAD_STATE, "darts_decode_step before darts_prefill");
+  refresh_ub(c);
+  int ub = c->host_active_ub;
+  if (ub <= 0) return DARTS_OK;
+  const int32_t *n = &c->st->n_active;
+  TRY(launch_plan_decode(c, ub));
+  TRY(forward_layers(c, ub, n));
+  TRY(launch_rmsnorm(c, c->h, c->final_norm, c->xn, ub, n));
+  TRY(launch_gemm(c, c->xn, c->lm_head, c->logits, c->m.vocab, c->m.d_model, ub, n, false));
+  TRY(launch_sample(c, c->logits, 0, ub));
+  c->steps_issued++;
+  return DARTS_OK;
+}
+
+darts_status darts_select_and_compact(darts_ctx *c, int32_t *n_active_out) {
+  if (!c) return DARTS_ERR_INVALID_ARG;
+  if (c->sticky) return c->sticky;
+  if (!c->prefilled) FAIL(c, DARTS_ERR_BAD_STATE, "darts_select_and_compact before darts_prefill");
+  TRY(launch_select(c));
+  return launch_compact(c, n_active_out);
+}
+
+darts_status darts_n_active(darts_ctx *c, int32_t *out_host) {
+  if (!c || !out_host) return DARTS_ERR_INVALID_ARG;
+  DevState st;
+  CUDA_TRY(c, cudaMemcpyAsync(&st, c->st, sizeof(st), cudaMemcpyDeviceToHost, c->stream));
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  *out_host = st.n_active;
+  c->host_active_ub = std::min(c->host_active_ub, st.n_active);
+  if (st.err) { c->sticky = st.err; FAIL(c, st.err, "KV page pool exhausted"); }
+  return DARTS_OK;
+}
+
+darts_status darts_get_results(darts_ctx *c, darts_results *o) {
+  if (!c || !o) return DARTS_ERR_INVALID_ARG;
+  if (!c->prefilled) FAIL(c, DARTS_ERR_BAD_STATE, "no rollout to read");
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  size_t R = c->R, G = c->G, mn = c->rt.max_new;
+  if (o->tokens) CUDA_TRY(c, cudaMemcpy(o->tokens, c->tokens_out, R * mn * 4, cudaMemcpyDeviceToHost));
+  if (o->margin) CUDA_TRY(c, cudaMemcpy(o->margin, c->margin_out, R * mn * 4, cudaMemcpyDeviceToHost));
+  if (o->len) CUDA_TRY(c, cudaMemcpy(o->len, c->row_len, R * 4, cudaMemcpyDeviceToHost));
+  if (o->status) CUDA_TRY(c, cudaMemcpy(o->status, c->row_status, R, cudaMemcpyDeviceToHost));
+  if (o->sel) CUDA_TRY(c, cudaMemcpy(o->sel, c->g_sel, G * c->pol.K * 4, cudaMemcpyDeviceToHost));
+  if (o->sel_mask) CUDA_TRY(c, cudaMemcpy(o->sel_mask, c->g_mask, G * 4, cudaMemcpyDeviceToHost));
+  if (o->close_step) CUDA_TRY(c, cudaMemcpy(o->close_step, c->g_close_step, G * 4, cudaMemcpyDeviceToHost));
+  if (o->len_mean) CUDA_TRY(c, cudaMemcpy(o->len_mean, c->g_len_mean, G * 4, cudaMemcpyDeviceToHost));
+  if (o->len_var) CUDA_TRY(c, cudaMemcpy(o->len_var, c->g_len_var, G * 4, cudaMemcpyDeviceToHost));
+  return DARTS_OK;
+}
+
+darts_status darts_get_counters(darts_ctx *c, darts_counters *o) {
+  if (!c || !o) return DARTS_ERR_INVALID_ARG;
+  DevState st;
+  CUDA_TRY(c, cudaMemcpyAsync(&st, c->st, sizeof(st), cudaMemcpyDeviceToHost, c->stream));
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  o->n_steps = st.step; o->n_generated_tokens = (int64_t)st.n_generated; o->n_kept_tokens = (int64_t)st.n_kept;
+  o->n_near_ties = (int64_t)st.n_near_ties; o->n_row_steps = (int64_t)st.n_row_steps; o->peak_pages = st.peak_used;
+  o->kernel_launches = c->launches;
+  return DARTS_OK;
+}
+
+darts_status darts_run_to_completion(darts_ctx *c, darts_results *out) {
+  if (!c) return DARTS_ERR_INVALID_ARG;
+  if (c->sticky) return c->sticky;
+  if (!c->prefilled) FAIL(c, DARTS_ERR_BAD_STATE, "darts_run_to_completion before darts_prefill");
+  TRY(darts_select_and_compact(c, nullptr));
+  // The host never waits for a step's result: it sizes grids from a stale (monotone, hence safe) upper
+  // bound of n_active mirrored in pinned memory and stays at most two iterations ahead of the device.
+  for (int it = 0; it <= c->max_len + 4; ++it) {
+    refresh_ub(c);
+    if (c->host_active_ub <= 0) break;
+    TRY(darts_decode_step(c));
+    TRY(darts_select_and_compact(c, nullptr));
+    CUDA_TRY(c, cudaEventRecord(c->ev[it & 1], c->stream));
+    if (it >= 1) CUDA_TRY(c, cudaEventSynchronize(c->ev[(it + 1) & 1]));
+  }
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  int32_t na = 0;
+  TRY(darts_n_active(c, &na));
+  if (na != 0) FAIL(c, DARTS_ERR_BAD_STATE, "rollout loop ended with %d active rows", na);
+  return out ? darts_get_results(c, out) : DARTS_OK;
+}
+
+static darts_status rollout_common(darts_ctx *c, const int32_t *prompts_dev, bool in_place, int32_t prompt_len, int32_t G,
+                                   const int32_t *Kp, const int32_t *forced_dev, const darts_policy *pol, int32_t max_len,
+                                   float temperature, uint64_t seed, darts_results *out) {
+  if (prompt_len <= 0 || G <= 0) FAIL(c, DARTS_ERR_INVALID_ARG, "prompt_len and G must be positive");
+  if (max_len <= 0 || max_len > c->rt.max_new) FAIL(c, DARTS_ERR_INVALID_ARG, "max_len %d outside (0, max_new=%d]", max_len, c->rt.max_new);
+  std::vector<int32_t> offs(G + 1);
+  for (int i = 0; i <= G; ++i) offs[i] = i * prompt_len;
+  c->max_len = max_len;
+  TRY(prefill_impl(c, prompts_dev, in_place, offs.data(), G, Kp, forced_dev, pol, temperature, seed));
+  return darts_run_to_completion(c, out);
+}
+
+darts_status darts_rollout(darts_ctx *c, const int32_t *prompts, int32_t prompt_len, int32_t G, int32_t Kp_scalar, int32_t K,
+                           int32_t max_len, float temperature, uint64_t seed, const int32_t *forced_len, darts_results *out) {
+  if (!c) return DARTS_ERR_INVALID_ARG;
+  if (!prompts) FAIL(c, DARTS_ERR_INVALID_ARG, "prompts is NULL");
+  std::vector<int32_t> Kp(std::max(G, 1), Kp_scalar);
+  darts_policy pol{K, K > 1 ? 1 : 0, 2 * K, DARTS_MODE_AUTO};                    // L=1, M_up=2M (:204)
+  return rollout_common(c, prompts, false, prompt_len, G, Kp.data(), forced_len, &pol, max_len, temperature, seed, out);
+}
+
+darts_status darts_rollout_host(darts_ctx *c, const int32_t *prompts_host, int32_t prompt_len, int32_t G, const int32_t *Kp_host,
+                                const int32_t *forced_len_host, const darts_policy *policy, int32_t max_len, float temperature,
+                                uint64_t seed, darts_results *out) {
+  if (!c) return DARTS_ERR_INVALID_ARG;
+  if (!prompts_host || !Kp_host || !policy) FAIL(c, DARTS_ERR_INVALID_ARG, "NULL argument");
+  if (G <= 0 || G > c->rt.max_prompts || prompt_len <= 0 || prompt_len > c->rt.max_prompt_len) FAIL(c, DARTS_ERR_INVALID_ARG, "bad G / prompt_len");
+  if (!c->has_weights) FAIL(c, DARTS_ERR_BAD_STATE, "attention-only context");
+  CUDA_TRY(c, cudaMemcpyAsync(c->prompt_tokens, prompts_host, (size_t)G * prompt_len * 4, cudaMemcpyHostToDevice, c->stream));
+  const int32_t *forced_dev = nullptr;
+  if (forced_len_host) {
+    int Kp_max = 0;
+    for (int i = 0; i < G; ++i) Kp_max = std::max(Kp_max, Kp_host[i]);
+    if (Kp_max > DARTS_MAX_KP) FAIL(c, DARTS_ERR_INVALID_ARG, "Kp > 32");
+    CUDA_TRY(c, cudaMemcpyAsync(c->forced_stage, forced_len_host, (size_t)G * Kp_max * 4, cudaMemcpyHostToDevice, c->stream));
+    forced_dev = c->forced_stage;
+  }
+  return rollout_common(c, nullptr, true, prompt_len, G, Kp_host, forced_dev, policy, max_len, temperature, seed, out);
+}
+
+darts_status darts_debug_logits(darts_ctx *c, int32_t row, float *out_host) {
+  if (!c || !out_host) return DARTS_ERR_INVALID_ARG;
+  if (!c->prefilled || row < 0 || row >= c->R) FAIL(c, DARTS_ERR_INVALID_ARG, "bad row %d", row);
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  int32_t slot, sstep, prompt;
+  DevState st;
+  CUDA_TRY(c, cudaMemcpy(&slot, c->row_slot + row, 4, cudaMemcpyDeviceToHost));
+  CUDA_TRY(c, cudaMemcpy(&sstep, c->row_slot_step + row, 4, cudaMemcpyDeviceToHost));
+  CUDA_TRY(c, cudaMemcpy(&prompt, c->row_prompt + row, 4, cudaMemcpyDeviceToHost));
+  CUDA_TRY(c, cudaMemcpy(&st, c->st, sizeof(st), cudaMemcpyDeviceToHost));
+  const float *src;
+  if (sstep == 0) src = c->z0 + (size_t)prompt * c->m.vocab;
+  else {
+    // valid only for the most recent decode step (the logits buffer is overwritten every step)
+    if (sstep != c->steps_issued) FAIL(c, DARTS_ERR_BAD_STATE, "row %d last decoded at step %d, buffer holds step %d", row, sstep, c->steps_issued);
+    src = c->logits + (size_t)slot * c->m.vocab;
+  }
+  CUDA_TRY(c, cudaMemcpy(out_host, src, (size_t)c->m.vocab * 4, cudaMemcpyDeviceToHost));
+  return DARTS_OK;
+}
+
+darts_status darts_debug_set_last_tokens(darts_ctx *c, const int32_t *tokens_host, int32_t n_rows) {
+  if (!c || !tokens_host) return DARTS_ERR_INVALID_ARG;
+  if (!c->prefilled || n_rows != c->R) FAIL(c, DARTS_ERR_INVALID_ARG, "n_rows must equal the rollout's row count");
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  std::vector<int32_t> cur(n_rows);
+  CUDA_TRY(c, cudaMemcpy(cur.data(), c->row_last_tok, (size_t)n_rows * 4, cudaMemcpyDeviceToHost));
+  for (int r = 0; r < n_rows; ++r) if (tokens_host[r] >= 0) cur[r] = tokens_host[r];
+  CUDA_TRY(c, cudaMemcpy(c->row_last_tok, cur.data(), (size_t)n_rows * 4, cudaMemcpyHostToDevice));
+  return DARTS_OK;
+}
+
+darts_status darts_attn_load(darts_ctx *c, int32_t G, int32_t P, int32_t Kp, const void *k_prefix, const void *v_prefix,
+                             const int32_t *suffix_len_host, const void *k_suffix, const void *v_suffix) {
+  if (!c) return DARTS_ERR_INVALID_ARG;
+  if (c->sticky) return c->sticky;
+  if (!k_prefix || !v_prefix || !suffix_len_host || !k_suffix || !v_suffix || G <= 0 || P <= 0 || Kp <= 0) FAIL(c, DARTS_ERR_INVALID_ARG, "NULL / non-positive argument");
+  int R = G * Kp, page = c->rt.page_size;
+  if (G > c->rt.max_prompts || R > c->rt.max_rows || P > c->rt.max_prompt_len) FAIL(c, DARTS_ERR_INVALID_ARG, "G, G*Kp or P exceed the runtime sizes");
+  int npp = ceil_div(P, page);
+  std::vector<int32_t> pre((size_t)G * c->max_prefix_pages, -1), rowp((size_t)R * c->max_suffix_pages, -1);
+  std::vector<int32_t> sprompt(R), snpre(R, P), snsuf(R), srow(R), rlist(R);
+  std::vector<int64_t> soffs(R + 1, 0);
+  int next = 0;
+  for (int g = 0; g < G; ++g) for (int q = 0; q < npp; ++q) pre[(size_t)g * c->max_prefix_pages + q] = next++;
+  for (int r = 0; r < R; ++r) {
+    int t = suffix_len_host[r];
+    if (t < 0 || ceil_div(t, page) > c->max_suffix_pages) FAIL(c, DARTS_ERR_INVALID_ARG, "suffix_len[%d]=%d exceeds max_new", r, t);
+    for (int q = 0; q < ceil_div(t, page); ++q) rowp[(size_t)r * c->max_suffix_pages + q] = next++;
+    sprompt[r] = r / Kp; snsuf[r] = t; srow[r] = r; rlist[r] = r; soffs[r + 1] = soffs[r] + t;
+  }
+  if (next > c->rt.n_pages) FAIL(c, DARTS_ERR_KV_POOL_EXHAUSTED, "need %d pages, pool has %d", next, c->rt.n_pages);
+  cudaStream_t s = c->stream;
+  // suffix offsets (int64) and lengths are staged in the (otherwise unused here) free_pages / row_len arrays
+  if ((size_t)c->rt.n_pages * 4 < (size_t)(R + 1) * 8) FAIL(c, DARTS_ERR_WORKSPACE_TOO_SMALL, "n_pages too small to stage offsets");
+  int64_t *soffs_dev = (int64_t *)c->free_pages;
+  CUDA_TRY(c, cudaMemcpyAsync(soffs_dev, soffs.data(), (size_t)(R + 1) * 8, cudaMemcpyHostToDevice, s));
+  CUDA_TRY(c, cudaMemcpyAsync(c->row_len, suffix_len_host, (size_t)R * 4, cudaMemcpyHostToDevice, s));
+  CUDA_TRY(c, cudaMemcpyAsync(c->g_prefix_pages, pre.data(), pre.size() * 4, cudaMemcpyHostToDevice, s));
+  CUDA_TRY(c, cudaMemcpyAsync(c->row_pages, rowp.data(), rowp.size() * 4, cudaMemcpyHostToDevice, s));
+  CUDA_TRY(c, cudaMemcpyAsync(c->slot_prompt, sprompt.data(), (size_t)R * 4, cudaMemcpyHostToDevice, s));
+  CUDA_TRY(c, cudaMemcpyAsync(c->slot_npre, snpre.data(), (size_t)R * 4, cudaMemcpyHostToDevice, s));
+  CUDA_TRY(c, cudaMemcpyAsync(c->slot_nsuf, snsuf.data(), (size_t)R * 4, cudaMemcpyHostToDevice, s));
+  CUDA_TRY(c, cudaMemcpyAsync(c->slot_row, srow.data(), (size_t)R * 4, cudaMemcpyHostToDevice, s));
+  CUDA_TRY(c, cudaMemcpyAsync(c->row_list, rlist.data(), (size_t)R * 4, cudaMemcpyHostToDevice, s));
+  DevState st{};
+  st.n_active = R; st.n_rows = R; st.n_groups = G; st.free_top = 0;
+  CUDA_TRY(c, cudaMemcpyAsync(c->st, &st, sizeof(st), cudaMemcpyHostToDevice, s));
+  darts_status rs = launch_attn_load(c, G, P, Kp, k_prefix, v_prefix, c->row_len, soffs_dev, k_suffix, v_suffix, soffs[R]);
+  if (rs != DARTS_OK) return rs;
+  c->attn_rows = R; c->G = G; c->R = R; c->Kp_max = Kp;
+  return DARTS_OK;
+}
+
+darts_status darts_attention(darts_ctx *c, int32_t layer, const void *q, void *out) {
+  if (!c) return DARTS_ERR_INVALID_ARG;
+  if (c->sticky) return c->sticky;
+  if (!q || !out || layer < 0 || layer >= c->m.n_layers) FAIL(c, DARTS_ERR_INVALID_ARG, "bad q / out / layer");
+  if (c->attn_rows <= 0) FAIL(c, DARTS_ERR_BAD_STATE, "darts_attention before darts_attn_load");
+  return launch_attention(c, layer, q, out, c->attn_rows, &c->st->n_active);
+}
+
+}  // extern "C"

@@ -1,0 +1,150 @@
+// Internal declarations shared by the translation units of libdarts.so (not part of the C-ABI).
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+
+#include "darts.h"
+
+#define DARTS_MAX_KP 32          // a group's pool is ranked by one warp (include/darts.h: Kp[i] <= 32)
+#define NEAR_TIE_MARGIN 1e-3f    // north_star: "bit-exact wherever the Gumbel-max margin exceeds 1e-3"
+
+// Device-resident scalar state of a rollout (one instance per ctx).
+struct DevState {
+  int32_t n_active;              // rows still decoding (== length of row_list)
+  int32_t n_rows;                // sum Kp
+  int32_t n_groups;
+  int32_t free_top;              // number of pages on the free stack
+  int32_t err;                   // sticky device-side error (DARTS_ERR_KV_POOL_EXHAUSTED)
+  int32_t step;                  // index of the NEXT lock-step iteration (0 = first token)
+  int32_t peak_used;
+  int32_t n_open_groups;
+  unsigned long long n_generated, n_near_ties, n_kept, n_row_steps;
+};
+
+struct darts_ctx {
+  darts_model_desc m;
+  darts_runtime_desc rt;
+  cudaStream_t stream;
+  bool has_weights;
+  // borrowed weights (host-side copies of the per-layer pointer arrays)
+  const void *embed, *final_norm, *lm_head;
+  const void **attn_norm, **wqkv, **q_norm, **k_norm, **wo, **mlp_norm, **wgu, **wd, **wr, **wgu_e, **wd_e;
+
+  // geometry
+  int elt;                       // sizeof model dtype
+  int n_qkv;                     // (Hq + 2 Hkv) * hd
+  int max_suffix_pages, max_prefix_pages;
+  int act_rows;                  // rows the activation buffers hold: max(max_rows, prefill_chunk)
+  size_t kv_tile_elems;          // page_size * head_dim                      (one (page, K|V, head) tile)
+  size_t kv_page_elems;          // 2 * Hkv * kv_tile_elems                   (one page of one layer)
+  size_t kv_layer_elems;         // n_pages * kv_page_elems
+
+  // carve-outs (device)
+  void *kv_pool;
+  DevState *st;
+  int32_t *free_pages;
+  int32_t *row_list, *row_list_tmp;
+  int32_t *row_prompt, *row_sample, *row_len, *row_forced, *row_last_tok, *row_pages, *row_slot, *row_slot_step;
+  uint8_t *row_status;
+  int32_t *tokens_out;
+  float *margin_out;
+  int32_t *g_off, *g_Kp, *g_plen, *g_closed, *g_sel, *g_close_step, *g_prefix_pages, *g_tok_off;
+  uint32_t *g_mask;
+  float *g_len_mean, *g_len_var;
+  int32_t *prompt_tokens;        // private copy of the prompt tokens [sum P]
+  // per-slot plan of the current pass
+  int32_t *slot_row, *slot_tok, *slot_pos, *slot_dst_page, *slot_dst_off, *slot_prompt, *slot_npre, *slot_nsuf;
+  float2 *slot_cs;               // [act_rows][hd/2] (cos, sin)
+  // activations
+  float *h, *qkv32, *gu32, *logits, *z0, *hlast, *attn_part;
+  void *xn, *q, *ao, *act;
+  // attention-only mode (config 2)
+  int32_t attn_rows;
+
+  // policy / sampling
+  darts_policy pol;
+  float temperature;
+  uint64_t seed;
+  int32_t G, R, Kp_max, max_len;
+  int32_t *forced_stage;       // device staging for host-provided forced_len
+  uint32_t gen;                  // rollout generation (tags the pinned mirror)
+  cudaEvent_t ev[2];
+  bool prefilled;
+  int32_t host_active_ub;        // stale-but-safe upper bound of n_active known to the host
+  int32_t steps_issued;
+
+  // pinned host mirror written by the compaction kernel
+  volatile int32_t *pinned;      // host view: [0] n_active + [1] generation (one 64-bit store), [2] err
+  int32_t *pinned_dev;           // device view of the same mapped allocation
+  int64_t launches;
+  char err[512];
+  darts_status sticky;
+};
+
+#define CUDA_TRY(ctx, expr)                                                                   \
+  do {                                                                                        \
+    cudaError_t e__ = (expr);                                                                 \
+    if (e__ != cudaSuccess) {                                                                 \
+      snprintf((ctx)->err, sizeof((ctx)->err), "%s:%d: %s: %s", __FILE__, __LINE__, #expr,    \
+               cudaGetErrorString(e__));                                                      \
+      (ctx)->sticky = DARTS_ERR_CUDA;                                                         \
+      return DARTS_ERR_CUDA;                                                                  \
+    }                                                                                         \
+  } while (0)
+
+#define FAIL(ctx, code, ...)                                  \
+  do {                                                        \
+    snprintf((ctx)->err, sizeof((ctx)->err), __VA_ARGS__);    \
+    return (code);                                            \
+  } while (0)
+
+template <typename T> __device__ __forceinline__ float to_f(T x);
+template <> __device__ __forceinline__ float to_f<float>(float x) { return x; }
+template <> __device__ __forceinline__ float to_f<__nv_bfloat16>(__nv_bfloat16 x) { return __bfloat162float(x); }
+template <typename T> __device__ __forceinline__ T from_f(float x);
+template <> __device__ __forceinline__ float from_f<float>(float x) { return x; }
+template <> __device__ __forceinline__ __nv_bfloat16 from_f<__nv_bfloat16>(float x) { return __float2bfloat16_rn(x); }
+
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ float warp_max(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+
+// Element offset of (layer, page, kv, head) tile in the pool; tiles are page_size x head_dim.
+__host__ __device__ __forceinline__ size_t kv_tile_offset(size_t layer_elems, size_t page_elems, size_t tile_elems,
+                                                          int n_kv_heads, int layer, int page, int kv, int head) {
+  return (size_t)layer * layer_elems + (size_t)page * page_elems + ((size_t)kv * n_kv_heads + head) * tile_elems;
+}
+
+// ---- launchers implemented across the .cu files (all asynchronous on ctx->stream) ----------------
+// n_rows_dev: device pointer to the live row count (kernels ignore slots >= *n_rows_dev); rows_ub: host upper bound.
+darts_status launch_embed(darts_ctx *c, const int32_t *tok_of_slot_src, int mode, int rows_ub, const int32_t *n_rows_dev);
+darts_status launch_rmsnorm(darts_ctx *c, const float *h, const void *w, void *out, int rows_ub, const int32_t *n_rows_dev);
+darts_status launch_gemm(darts_ctx *c, const void *X, const void *W, float *C, int N, int K, int rows_ub,
+                         const int32_t *n_rows_dev, bool accumulate, bool w_is_f32 = false);
+darts_status launch_rope_table(darts_ctx *c, int rows_ub, const int32_t *n_rows_dev);
+darts_status launch_rope_append(darts_ctx *c, int layer, int rows_ub, const int32_t *n_rows_dev);
+darts_status launch_attention(darts_ctx *c, int layer, const void *q, void *out, int rows_ub, const int32_t *n_rows_dev);
+darts_status launch_silu_mul(darts_ctx *c, int rows_ub, const int32_t *n_rows_dev);
+darts_status launch_moe(darts_ctx *c, int layer, int rows_ub, const int32_t *n_rows_dev);
+darts_status launch_sample(darts_ctx *c, const float *logits, int step0, int rows_ub);
+darts_status launch_plan_decode(darts_ctx *c, int rows_ub);
+darts_status launch_plan_prefill(darts_ctx *c, int tok_begin, int n_tok, int g_begin, int g_end);
+darts_status launch_gather_last(darts_ctx *c, int tok_begin, int n_tok, int g_begin, int g_end);
+darts_status launch_select(darts_ctx *c);
+darts_status launch_compact(darts_ctx *c, int32_t *n_active_out);
+darts_status launch_init_rows(darts_ctx *c, const int32_t *forced_len, int n_prefix_pages_total);
+darts_status launch_attn_load(darts_ctx *c, int G, int P, int Kp, const void *kp, const void *vp, const int32_t *suffix_len_dev,
+                              const int64_t *suffix_offs_dev, const void *ks, const void *vs, long long n_suffix_tok);
+darts_status launch_gemm_simt(darts_ctx *c, const void *X, const void *W, float *C, int N, int K, int rows_ub,
+                              const int32_t *n_rows_dev, bool accumulate, bool w_is_f32);
+darts_status launch_attention_ref(darts_ctx *c, int layer, const void *q, void *out, int rows_ub, const int32_t *n_rows_dev);
