@@ -41,6 +41,7 @@ size_t carve(darts_ctx *c, void *base) {
   c->kv_tile_elems = (size_t)rt.page_size * m.head_dim;
   c->kv_page_elems = 2 * (size_t)m.n_kv_heads * c->kv_tile_elems;
   c->kv_layer_elems = (size_t)rt.n_pages * c->kv_page_elems;
+  c->kv_swz = (c->elt == 2 && m.head_dim == 128) ? 1 : 0;
   size_t R = rt.max_rows, G = rt.max_prompts, A = c->act_rows;
   c->kv_pool = k.take<char>((size_t)m.n_layers * c->kv_layer_elems * c->elt);
   c->st = k.take<DevState>(1);
@@ -76,6 +77,17 @@ size_t carve(darts_ctx *c, void *base) {
   c->slot_npre = k.take<int32_t>(A);
   c->slot_nsuf = k.take<int32_t>(A);
   c->forced_stage = k.take<int32_t>(G * DARTS_MAX_KP);
+  if (attention_sm100_supported(c)) {
+    size_t max_parts = R * ((size_t)ceil_div(rt.max_prompt_len, 512) + 2) + (size_t)rt.n_pages / 8 + 16;
+    c->attn_max_items = (int)max_parts;
+    c->attn_items_pre = k.take<int32_t>(max_parts * 6);
+    c->attn_items_suf = k.take<int32_t>(max_parts * 6);
+    c->attn_nitems = k.take<int32_t>(4);
+    c->part_base = k.take<int32_t>(R);
+    c->part_cnt = k.take<int32_t>(R);
+    c->part_ml = k.take<float>(max_parts * m.n_q_heads * 2);
+    c->part_acc = k.take<float>(max_parts * m.n_q_heads * m.head_dim);
+  }
   if (model) {
     size_t F = m.n_experts ? (size_t)m.top_k * m.expert_ffn : (size_t)m.ffn;
     c->tokens_out = k.take<int32_t>(R * rt.max_new);
@@ -119,6 +131,7 @@ darts_status check_device(darts_ctx *c) {
   CUDA_TRY(c, cudaGetDevice(&dev));
   CUDA_TRY(c, cudaGetDeviceProperties(&p, dev));
   if (p.major != 10) FAIL(c, DARTS_ERR_UNSUPPORTED, "device is sm_%d%d; this library is sm_100a only (no fallback)", p.major, p.minor);
+  c->n_sms = p.multiProcessorCount;
   return DARTS_OK;
 }
 
@@ -206,6 +219,7 @@ darts_status prefill_impl(darts_ctx *c, const int32_t *prompt_tokens_dev, bool t
     int g1 = g0, ntok = 0;
     while (g1 < G && ntok + plen[g1] <= chunk) ntok += plen[g1++];
     int tb = tok_off[g0];
+    c->attn_plan_valid = false;                      // prefill is causal per token: generic kernel
     TRY(launch_plan_prefill(c, tb, ntok, g0, g1));
     TRY(forward_layers(c, ntok, nullptr));
     TRY(launch_gather_last(c, tb, ntok, g0, g1));
@@ -295,6 +309,8 @@ darts_status darts_create(const darts_model_desc *m, const darts_weights *w, con
   CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev[0], cudaEventDisableTiming));
   CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev[1], cudaEventDisableTiming));
   CUDA_TRY(c, cudaMemsetAsync(c->st, 0, sizeof(DevState), c->stream));
+  // The pool must hold finite values everywhere: a partially filled page is multiplied by zero probabilities.
+  CUDA_TRY(c, cudaMemsetAsync(c->kv_pool, 0, (size_t)m->n_layers * c->kv_layer_elems * c->elt, c->stream));
   return DARTS_OK;
 }
 
@@ -327,6 +343,8 @@ darts_status darts_decode_step(darts_ctx *c) {
   if (ub <= 0) return DARTS_OK;
   const int32_t *n = &c->st->n_active;
   TRY(launch_plan_decode(c, ub));
+  c->attn_plan_valid = attention_sm100_supported(c);
+  if (c->attn_plan_valid) TRY(launch_attention_plan_sm100(c, ub, n));
   TRY(forward_layers(c, ub, n));
   TRY(launch_rmsnorm(c, c->h, c->final_norm, c->xn, ub, n));
   TRY(launch_gemm(c, c->xn, c->lm_head, c->logits, c->m.vocab, c->m.d_model, ub, n, false));
@@ -515,6 +533,8 @@ darts_status darts_attn_load(darts_ctx *c, int32_t G, int32_t P, int32_t Kp, con
   darts_status rs = launch_attn_load(c, G, P, Kp, k_prefix, v_prefix, c->row_len, soffs_dev, k_suffix, v_suffix, soffs[R]);
   if (rs != DARTS_OK) return rs;
   c->attn_rows = R; c->G = G; c->R = R; c->Kp_max = Kp;
+  c->attn_plan_valid = attention_sm100_supported(c);
+  if (c->attn_plan_valid) TRY(launch_attention_plan_sm100(c, R, &c->st->n_active));
   return DARTS_OK;
 }
 

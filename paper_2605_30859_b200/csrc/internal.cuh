@@ -24,6 +24,19 @@ struct DevState {
   unsigned long long n_generated, n_near_ties, n_kept, n_row_steps;
 };
 
+// KV cache geometry.  One layer slab = [page][kv_head][K|V][token][head_dim]; the (K,V) tiles of one
+// (page, head) are adjacent so the tuned attention kernel fetches both with ONE bulk copy.  With swz set
+// (bf16, head_dim 128) the 16-byte chunks of a token row are XOR-permuted by (token & 7): the layout in HBM is
+// already the bank-conflict-free layout ldmatrix wants in shared memory, so a plain linear copy stages it.
+struct KvGeom {
+  size_t page_elems, tile_elems;
+  int hd, swz;
+};
+__device__ __forceinline__ size_t kv_elem(const KvGeom &g, int page, int head, int kv, int tok, int d) {
+  int dd = g.swz ? ((((d >> 3) ^ (tok & 7)) << 3) | (d & 7)) : d;
+  return (size_t)page * g.page_elems + ((size_t)head * 2 + kv) * g.tile_elems + (size_t)tok * g.hd + dd;
+}
+
 struct darts_ctx {
   darts_model_desc m;
   darts_runtime_desc rt;
@@ -41,6 +54,8 @@ struct darts_ctx {
   size_t kv_tile_elems;          // page_size * head_dim                      (one (page, K|V, head) tile)
   size_t kv_page_elems;          // 2 * Hkv * kv_tile_elems                   (one page of one layer)
   size_t kv_layer_elems;         // n_pages * kv_page_elems
+  int kv_swz;                    // 1: swizzled token rows (bf16, head_dim 128)
+  KvGeom geom() const { return KvGeom{kv_page_elems, kv_tile_elems, m.head_dim, kv_swz}; }
 
   // carve-outs (device)
   void *kv_pool;
@@ -63,6 +78,12 @@ struct darts_ctx {
   void *xn, *q, *ao, *act;
   // attention-only mode (config 2)
   int32_t attn_rows;
+  // tuned attention (kernels_attn_sm100.cu): per-step work list and split-KV partials
+  int32_t *attn_items_pre, *attn_items_suf, *attn_nitems, *part_base, *part_cnt;
+  float *part_ml, *part_acc;
+  int attn_max_items;
+  bool attn_plan_valid;
+  int n_sms;
 
   // policy / sampling
   darts_policy pol;
@@ -119,12 +140,6 @@ __device__ __forceinline__ float warp_max(float v) {
   return v;
 }
 
-// Element offset of (layer, page, kv, head) tile in the pool; tiles are page_size x head_dim.
-__host__ __device__ __forceinline__ size_t kv_tile_offset(size_t layer_elems, size_t page_elems, size_t tile_elems,
-                                                          int n_kv_heads, int layer, int page, int kv, int head) {
-  return (size_t)layer * layer_elems + (size_t)page * page_elems + ((size_t)kv * n_kv_heads + head) * tile_elems;
-}
-
 // ---- launchers implemented across the .cu files (all asynchronous on ctx->stream) ----------------
 // n_rows_dev: device pointer to the live row count (kernels ignore slots >= *n_rows_dev); rows_ub: host upper bound.
 darts_status launch_embed(darts_ctx *c, const int32_t *tok_of_slot_src, int mode, int rows_ub, const int32_t *n_rows_dev);
@@ -147,4 +162,6 @@ darts_status launch_attn_load(darts_ctx *c, int G, int P, int Kp, const void *kp
                               const int64_t *suffix_offs_dev, const void *ks, const void *vs, long long n_suffix_tok);
 darts_status launch_gemm_simt(darts_ctx *c, const void *X, const void *W, float *C, int N, int K, int rows_ub,
                               const int32_t *n_rows_dev, bool accumulate, bool w_is_f32);
+darts_status launch_attention_plan_sm100(darts_ctx *c, int rows_ub, const int32_t *n_rows_dev);
+bool attention_sm100_supported(const darts_ctx *c);
 darts_status launch_attention_ref(darts_ctx *c, int layer, const void *q, void *out, int rows_ub, const int32_t *n_rows_dev);

@@ -11,7 +11,7 @@ __global__ void attn_ref_k(const T *__restrict__ q, T *__restrict__ out, const T
                            const int32_t *__restrict__ slot_prompt, const int32_t *__restrict__ slot_npre,
                            const int32_t *__restrict__ slot_nsuf, const int32_t *__restrict__ slot_row,
                            const int32_t *__restrict__ g_prefix_pages, const int32_t *__restrict__ row_pages, int mpp, int msp,
-                           int Hq, int Hkv, int page, size_t page_elems, size_t tile_elems, float scale,
+                           int Hq, int Hkv, int page, KvGeom geo, float scale,
                            const int32_t *n_rows_dev, int rows_ub) {
   constexpr int hd = DPL * 32;
   int slot = blockIdx.y;
@@ -32,8 +32,8 @@ __global__ void attn_ref_k(const T *__restrict__ q, T *__restrict__ out, const T
     const int32_t *pages = seg == 0 ? g_prefix_pages + (size_t)slot_prompt[slot] * mpp : row_pages + (size_t)slot_row[slot] * msp;
     for (int n = 0; n < count; ++n) {
       int pg = pages[n / page], off = n % page;
-      const T *kp = kv_layer + (size_t)pg * page_elems + (size_t)kvh * tile_elems + (size_t)off * hd + lane * DPL;
-      const T *vp = kp + (size_t)Hkv * tile_elems;
+      const T *kp = kv_layer + kv_elem(geo, pg, kvh, 0, off, lane * DPL);   // DPL <= 8 dims stay inside one 16-byte chunk
+      const T *vp = kv_layer + kv_elem(geo, pg, kvh, 1, off, lane * DPL);
       float s = 0.f;
 #pragma unroll
       for (int k = 0; k < DPL; ++k) s = fmaf(qr[k], to_f<T>(kp[k]), s);
@@ -59,8 +59,8 @@ darts_status run(darts_ctx *c, int layer, const void *q, void *out, int rows_ub,
   const T *kv = (const T *)c->kv_pool + (size_t)layer * c->kv_layer_elems;
   float scale = 1.0f / sqrtf((float)m.head_dim);
 #define ARGS (const T *)q, (T *)out, kv, c->slot_prompt, c->slot_npre, c->slot_nsuf, c->slot_row, c->g_prefix_pages, c->row_pages, \
-             c->max_prefix_pages, c->max_suffix_pages, m.n_q_heads, m.n_kv_heads, c->rt.page_size, c->kv_page_elems,              \
-             c->kv_tile_elems, scale, n_rows_dev, rows_ub
+             c->max_prefix_pages, c->max_suffix_pages, m.n_q_heads, m.n_kv_heads, c->rt.page_size, c->geom(),                     \
+             scale, n_rows_dev, rows_ub
   switch (m.head_dim / 32) {
     case 1: attn_ref_k<T, 1><<<grid, block, 0, c->stream>>>(ARGS); break;
     case 2: attn_ref_k<T, 2><<<grid, block, 0, c->stream>>>(ARGS); break;

@@ -1,6 +1,476 @@
-// Prefix-shared split-KV attention for bf16 / head_dim 128 / page 64 (placeholder: declines every shape).
+// Prefix-shared split-KV GQA decode attention for the bf16 path (head_dim 128, page 64).   SURVEY.md §8(a) row 5.
+//
+// Work is cut into ITEMS of at most CH_PAGES pages (512 tokens) of ONE page table:
+//   prefix item  = (group of active rows of one prompt, chunk of the prompt's shared prefix pages):
+//                  every page is fetched ONCE for all the group's rows ("reads each prompt-prefix page once per
+//                  group", north_star); query rows = rows x (Hq/Hkv) heads, up to 64 per item;
+//   suffix item  = (one row, chunk of its own pages).
+// Items x kv-heads are strided over a persistent grid (2 CTAs per SM).  Inside a CTA one producer warp streams
+// the (page, head) K+V tile pairs — 32 KB, contiguous in HBM by construction of the cache layout — into a
+// 3-stage shared-memory ring with cp.async.bulk (the TMA bulk-copy engine) + mbarrier transaction counts, and
+// four consumer warps run QK^T / PV on tensor cores (mma.sync m16n8k16 bf16, fp32 accumulate) with an online
+// softmax in fp32.  The cache is stored pre-swizzled (internal.cuh: kv_elem), so the linear copy lands in the
+// bank-conflict-free layout ldmatrix needs.  Every item writes one un-normalised partial (m, l, acc) per query
+// row; attn_merge_k combines a row's partials by log-sum-exp in chunk order.  The split depends only on a row's
+// own lengths (fixed 512-token chunks), so a row's arithmetic does not depend on which other rows are active,
+// apart from which row block of its group it falls in.
 #include "internal.cuh"
-darts_status launch_attention_sm100(darts_ctx *, int, const void *, void *, int, const int32_t *, bool *taken) {
+
+namespace {
+
+constexpr int CH_PAGES = 8;                 // pages per item
+constexpr int PAGE = 64, HD = 128;
+constexpr int CH_TOK = CH_PAGES * PAGE;
+constexpr int STAGES = 3;
+constexpr int STAGE_BYTES = 2 * PAGE * HD * 2;   // K tile + V tile of one (page, head)
+constexpr int N_CONS = 4;                   // consumer warps
+constexpr int THREADS = (N_CONS + 1) * 32;
+constexpr int ITEM_INTS = 6;                // first_slot, n_slots, page_begin, n_tokens, chunk_k, is_prefix
+
+struct Smem {
+  alignas(128) unsigned char stage[STAGES][STAGE_BYTES];
+  float scratch[N_CONS][4][HD];             // cross-warp merge of TOKSPLIT items, 4 query rows per round
+  float ml[N_CONS][16][2];
+  unsigned long long full[STAGES], empty[STAGES];
+};
+
+// ------------------------------------------------------------------------------------------------ PTX helpers
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(void *bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(void *bar, int bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(void *bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(void *bar, int parity) {
+  asm volatile(
+      "{\n.reg .pred p;\nWAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\nbra WAIT_%=;\nDONE_%=:\n}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, int bytes, void *bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+               "l"(src), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+__device__ __forceinline__ void ldsm4(uint32_t addr, uint32_t &r0, uint32_t &r1, uint32_t &r2, uint32_t &r3) {
+  asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];" : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3) : "r"(addr));
+}
+__device__ __forceinline__ void ldsm4t(uint32_t addr, uint32_t &r0, uint32_t &r1, uint32_t &r2, uint32_t &r3) {
+  asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];" : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3) : "r"(addr));
+}
+__device__ __forceinline__ void mma16816(float (&c)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0, uint32_t b1) {
+  asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+               : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+               : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+}
+__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
+  __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
+  return *reinterpret_cast<uint32_t *>(&v);
+}
+__device__ __forceinline__ void cons_bar() { asm volatile("bar.sync 1, %0;" ::"n"(N_CONS * 32) : "memory"); }
+
+struct Params {
+  const __nv_bfloat16 *q;                   // [slot][Hq][128]
+  const __nv_bfloat16 *kv_layer;
+  const int32_t *items_pre, *items_suf, *n_items;   // n_items[0] = prefix items, [1] = suffix items
+  const int32_t *slot_prompt, *slot_row, *g_prefix_pages, *row_pages, *part_base;
+  float *part_ml, *part_acc;
+  int mpp, msp, Hq, Hkv, rep;
+  size_t page_elems, tile_elems;
+  float c;                                  // softmax scale * log2(e)
+};
+
+// Online-softmax update of NT score n-tiles (two row sets: g and g+8).  Emits P (bf16x2) and rescales O.
+template <int NT>
+__device__ __forceinline__ void softmax_update(float (&S)[NT][4], float (&m)[2], float (&l)[2], float (&O)[16][4],
+                                               uint32_t (&P)[NT][2], float c) {
+#pragma unroll
+  for (int rs = 0; rs < 2; ++rs) {
+    float mx = -INFINITY;
+#pragma unroll
+    for (int nt = 0; nt < NT; ++nt) mx = fmaxf(mx, fmaxf(S[nt][2 * rs], S[nt][2 * rs + 1]));
+    mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 1));
+    mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 2));
+    float mn = fmaxf(m[rs], mx);
+    float ms = mn == -INFINITY ? 0.f : mn;
+    float corr = exp2f((m[rs] - ms) * c);
+    float msc = ms * c, sum = 0.f;
+#pragma unroll
+    for (int nt = 0; nt < NT; ++nt) {
+      float p0 = exp2f(fmaf(S[nt][2 * rs], c, -msc)), p1 = exp2f(fmaf(S[nt][2 * rs + 1], c, -msc));
+      sum += p0 + p1;
+      P[nt][rs] = pack_bf16(p0, p1);
+    }
+    l[rs] = l[rs] * corr + sum;
+    m[rs] = mn;
+#pragma unroll
+    for (int nt = 0; nt < 16; ++nt) { O[nt][2 * rs] *= corr; O[nt][2 * rs + 1] *= corr; }
+  }
+}
+
+// scores of n-tile pair starting at token tok0 (16 tokens) for all 8 k-steps
+__device__ __forceinline__ void qk_16tok(uint32_t sK, int tok0, const uint32_t (&Qa)[8][4], float (&S0)[4], float (&S1)[4], int lane) {
+  int mat = lane >> 3, r = lane & 7;
+  int token = tok0 + (mat >> 1) * 8 + r;
+  uint32_t rowaddr = sK + token * (HD * 2);
+#pragma unroll
+  for (int ks = 0; ks < 8; ++ks) {
+    int chunk = 2 * ks + (mat & 1);
+    uint32_t b0, b1, b2, b3;
+    ldsm4(rowaddr + ((chunk ^ r) << 4), b0, b1, b2, b3);
+    mma16816(S0, Qa[ks][0], Qa[ks][1], Qa[ks][2], Qa[ks][3], b0, b1);
+    mma16816(S1, Qa[ks][0], Qa[ks][1], Qa[ks][2], Qa[ks][3], b2, b3);
+  }
+}
+
+// O += P(16 rows x 16 tokens starting at tokb) . V
+__device__ __forceinline__ void pv_16tok(uint32_t sV, int tokb, uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, float (&O)[16][4], int lane) {
+  int mat = lane >> 3, r = lane & 7;
+  int token = tokb + (mat & 1) * 8 + r;
+  uint32_t rowaddr = sV + token * (HD * 2);
+#pragma unroll
+  for (int np = 0; np < 8; ++np) {
+    int chunk = 2 * np + (mat >> 1);
+    uint32_t b0, b1, b2, b3;
+    ldsm4t(rowaddr + ((chunk ^ r) << 4), b0, b1, b2, b3);
+    mma16816(O[2 * np], a0, a1, a2, a3, b0, b1);
+    mma16816(O[2 * np + 1], a0, a1, a2, a3, b2, b3);
+  }
+}
+
+__global__ void __launch_bounds__(THREADS, 2) attn_main_k(Params p) {
+  extern __shared__ unsigned char smem_raw[];
+  Smem &sm = *reinterpret_cast<Smem *>(((uintptr_t)smem_raw + 127) & ~(uintptr_t)127);
+  int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < STAGES; ++s) { mbar_init(&sm.full[s], 1); mbar_init(&sm.empty[s], N_CONS); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  int n_pre = p.n_items[0], n_suf = p.n_items[1];
+  long long total = (long long)(n_pre + n_suf) * p.Hkv;
+  int stage = 0, phase = 0;
+
+  if (warp == N_CONS) {
+    // ------------------------------------------------------------------ producer: one lane streams the pages
+    if (lane == 0) {
+      for (long long w = blockIdx.x; w < total; w += gridDim.x) {
+        int item = (int)(w / p.Hkv), kvh = (int)(w % p.Hkv);
+        const int32_t *it = item < n_pre ? p.items_pre + (size_t)item * ITEM_INTS : p.items_suf + (size_t)(item - n_pre) * ITEM_INTS;
+        int first = it[0], page_begin = it[2], n_tok = it[3], is_pre = it[5];
+        const int32_t *table = is_pre ? p.g_prefix_pages + (size_t)p.slot_prompt[first] * p.mpp : p.row_pages + (size_t)p.slot_row[first] * p.msp;
+        int npg = (n_tok + PAGE - 1) / PAGE;
+        for (int pg = 0; pg < npg; ++pg) {
+          mbar_wait(&sm.empty[stage], phase ^ 1);
+          int page_id = table[page_begin + pg];
+          const __nv_bfloat16 *src = p.kv_layer + (size_t)page_id * p.page_elems + (size_t)kvh * 2 * p.tile_elems;
+          mbar_expect_tx(&sm.full[stage], STAGE_BYTES);
+          bulk_g2s(sm.stage[stage], src, STAGE_BYTES, &sm.full[stage]);
+          if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        }
+      }
+    }
+    return;
+  }
+
+  // -------------------------------------------------------------------- consumers
+  int g = lane >> 2, t = lane & 3;
+  for (long long w = blockIdx.x; w < total; w += gridDim.x) {
+    int item = (int)(w / p.Hkv), kvh = (int)(w % p.Hkv);
+    const int32_t *it = item < n_pre ? p.items_pre + (size_t)item * ITEM_INTS : p.items_suf + (size_t)(item - n_pre) * ITEM_INTS;
+    int first = it[0], n_slots = it[1], n_tok = it[3], chunk_k = it[4];
+    int n_rows = n_slots * p.rep;
+    bool rowsplit = n_rows > 16;
+    int mt = rowsplit ? warp : 0;                                  // m-tile this warp works on
+    bool warp_has_rows = mt * 16 < n_rows;
+    // Q fragments (A operand) of this warp's m-tile: rows r = 16 mt + g (+8)
+    uint32_t Qa[8][4];
+    {
+      int r0 = mt * 16 + g, r1 = r0 + 8;
+      const __nv_bfloat16 *q0 = r0 < n_rows ? p.q + ((size_t)(first + r0 / p.rep) * p.Hq + kvh * p.rep + r0 % p.rep) * HD : nullptr;
+      const __nv_bfloat16 *q1 = r1 < n_rows ? p.q + ((size_t)(first + r1 / p.rep) * p.Hq + kvh * p.rep + r1 % p.rep) * HD : nullptr;
+#pragma unroll
+      for (int ks = 0; ks < 8; ++ks) {
+        int d = 16 * ks + 2 * t;
+        Qa[ks][0] = q0 ? *reinterpret_cast<const uint32_t *>(q0 + d) : 0u;
+        Qa[ks][1] = q1 ? *reinterpret_cast<const uint32_t *>(q1 + d) : 0u;
+        Qa[ks][2] = q0 ? *reinterpret_cast<const uint32_t *>(q0 + d + 8) : 0u;
+        Qa[ks][3] = q1 ? *reinterpret_cast<const uint32_t *>(q1 + d + 8) : 0u;
+      }
+    }
+    float O[16][4];
+#pragma unroll
+    for (int nt = 0; nt < 16; ++nt) O[nt][0] = O[nt][1] = O[nt][2] = O[nt][3] = 0.f;
+    float m[2] = {-INFINITY, -INFINITY}, l[2] = {0.f, 0.f};
+    int npg = (n_tok + PAGE - 1) / PAGE;
+    for (int pg = 0; pg < npg; ++pg) {
+      mbar_wait(&sm.full[stage], phase);
+      uint32_t sK = smem_u32(sm.stage[stage]), sV = sK + PAGE * HD * 2;
+      int valid = min(PAGE, n_tok - pg * PAGE);
+      if (!rowsplit) {
+        int tok0 = warp * 16;                                      // this warp's 16 tokens of the page
+        if (tok0 < valid) {
+          float S[2][4] = {};
+          qk_16tok(sK, tok0, Qa, S[0], S[1], lane);
+#pragma unroll
+          for (int nt = 0; nt < 2; ++nt) {
+            int tk = tok0 + nt * 8 + 2 * t;
+            if (tk >= valid) { S[nt][0] = -INFINITY; S[nt][2] = -INFINITY; }
+            if (tk + 1 >= valid) { S[nt][1] = -INFINITY; S[nt][3] = -INFINITY; }
+          }
+          uint32_t P[2][2];
+          softmax_update<2>(S, m, l, O, P, p.c);
+          pv_16tok(sV, tok0, P[0][0], P[0][1], P[1][0], P[1][1], O, lane);
+        }
+      } else if (warp_has_rows) {
+        float S[8][4] = {};
+#pragma unroll
+        for (int np = 0; np < 4; ++np) qk_16tok(sK, np * 16, Qa, S[2 * np], S[2 * np + 1], lane);
+        if (valid < PAGE) {
+#pragma unroll
+          for (int nt = 0; nt < 8; ++nt) {
+            int tk = nt * 8 + 2 * t;
+            if (tk >= valid) { S[nt][0] = -INFINITY; S[nt][2] = -INFINITY; }
+            if (tk + 1 >= valid) { S[nt][1] = -INFINITY; S[nt][3] = -INFINITY; }
+          }
+        }
+        uint32_t P[8][2];
+        softmax_update<8>(S, m, l, O, P, p.c);
+#pragma unroll
+        for (int kt = 0; kt < 4; ++kt) pv_16tok(sV, kt * 16, P[2 * kt][0], P[2 * kt][1], P[2 * kt + 1][0], P[2 * kt + 1][1], O, lane);
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&sm.empty[stage]);
+      if (++stage == STAGES) { stage = 0; phase ^= 1; }
+    }
+    // row sums live in quads: reduce
+#pragma unroll
+    for (int rs = 0; rs < 2; ++rs) {
+      l[rs] += __shfl_xor_sync(0xffffffffu, l[rs], 1);
+      l[rs] += __shfl_xor_sync(0xffffffffu, l[rs], 2);
+    }
+    if (rowsplit) {
+      // each warp owns its rows: write the partial directly
+#pragma unroll
+      for (int rs = 0; rs < 2; ++rs) {
+        int r = mt * 16 + g + 8 * rs;
+        if (r < n_rows) {
+          int slot = first + r / p.rep, head = kvh * p.rep + r % p.rep;
+          size_t pi = (size_t)(p.part_base[slot] + chunk_k) * p.Hq + head;
+          if (t == 0) { p.part_ml[pi * 2] = m[rs]; p.part_ml[pi * 2 + 1] = l[rs]; }
+#pragma unroll
+          for (int nt = 0; nt < 16; ++nt)
+            *reinterpret_cast<float2 *>(p.part_acc + pi * HD + nt * 8 + 2 * t) = make_float2(O[nt][2 * rs], O[nt][2 * rs + 1]);
+        }
+      }
+    } else {
+      // the four warps hold partials over disjoint tokens of the same <= 16 rows: merge through shared memory
+      if (t == 0) {
+        sm.ml[warp][g][0] = m[0]; sm.ml[warp][g][1] = l[0];
+        sm.ml[warp][g + 8][0] = m[1]; sm.ml[warp][g + 8][1] = l[1];
+      }
+      int rounds = (n_rows + 3) >> 2;
+      for (int rb = 0; rb < rounds; ++rb) {
+        int rs = rb >> 1, glo = (rb & 1) * 4;
+        if (g >= glo && g < glo + 4) {
+#pragma unroll
+          for (int nt = 0; nt < 16; ++nt)
+            *reinterpret_cast<float2 *>(&sm.scratch[warp][g - glo][nt * 8 + 2 * t]) = rs == 0 ? make_float2(O[nt][0], O[nt][1]) : make_float2(O[nt][2], O[nt][3]);
+        }
+        cons_bar();
+        int rr = threadIdx.x >> 5, d4 = (threadIdx.x & 31) * 4;     // 128 consumer threads: row rr, dims d4..d4+3
+        int r = rb * 4 + rr;
+        if (r < n_rows) {
+          float M = -INFINITY;
+#pragma unroll
+          for (int wv = 0; wv < N_CONS; ++wv) M = fmaxf(M, sm.ml[wv][r][0]);
+          float L = 0.f, a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
+#pragma unroll
+          for (int wv = 0; wv < N_CONS; ++wv) {
+            float sc = exp2f((sm.ml[wv][r][0] - M) * p.c);
+            float4 v = *reinterpret_cast<const float4 *>(&sm.scratch[wv][rr][d4]);
+            L += sc * sm.ml[wv][r][1];
+            a0 += sc * v.x; a1 += sc * v.y; a2 += sc * v.z; a3 += sc * v.w;
+          }
+          int slot = first + r / p.rep, head = kvh * p.rep + r % p.rep;
+          size_t pi = (size_t)(p.part_base[slot] + chunk_k) * p.Hq + head;
+          if ((threadIdx.x & 31) == 0) { p.part_ml[pi * 2] = M; p.part_ml[pi * 2 + 1] = L; }
+          *reinterpret_cast<float4 *>(p.part_acc + pi * HD + d4) = make_float4(a0, a1, a2, a3);
+        }
+        cons_bar();
+      }
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------ merge
+// out[slot][h] = sum_k w_k acc_k / sum_k w_k l_k,  w_k = 2^((m_k - M) c), over the row's partials in chunk order.
+__global__ void attn_merge_k(const float *__restrict__ part_ml, const float *__restrict__ part_acc, const int32_t *__restrict__ part_base,
+                             const int32_t *__restrict__ part_cnt, __nv_bfloat16 *__restrict__ out, int Hq, float c,
+                             const int32_t *n_rows_dev, int rows_ub) {
+  int slot = blockIdx.x;
+  int R = n_rows_dev ? min(*n_rows_dev, rows_ub) : rows_ub;
+  if (slot >= R) return;
+  int lane = threadIdx.x & 31;
+  int base = part_base[slot], cnt = part_cnt[slot];
+  for (int h = threadIdx.x >> 5; h < Hq; h += blockDim.x >> 5) {
+    float M = -INFINITY;
+    for (int k = 0; k < cnt; ++k) M = fmaxf(M, part_ml[((size_t)(base + k) * Hq + h) * 2]);
+    float L = 0.f;
+    float4 a = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int k = 0; k < cnt; ++k) {
+      size_t pi = (size_t)(base + k) * Hq + h;
+      float sc = exp2f((part_ml[pi * 2] - M) * c);
+      L += sc * part_ml[pi * 2 + 1];
+      float4 v = *reinterpret_cast<const float4 *>(part_acc + pi * HD + lane * 4);
+      a.x += sc * v.x; a.y += sc * v.y; a.z += sc * v.z; a.w += sc * v.w;
+    }
+    float inv = 1.0f / L;
+    uint2 o;
+    o.x = pack_bf16(a.x * inv, a.y * inv);
+    o.y = pack_bf16(a.z * inv, a.w * inv);
+    *reinterpret_cast<uint2 *>(out + ((size_t)slot * Hq + h) * HD + lane * 4) = o;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------ plan (one CTA)
+__device__ __forceinline__ int scan1024(int v, int *total, int *smem) {
+  int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  int incl = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    int x = __shfl_up_sync(0xffffffffu, incl, o);
+    if (lane >= o) incl += x;
+  }
+  if (lane == 31) smem[warp] = incl;
+  __syncthreads();
+  if (warp == 0) {
+    int wv = lane < (int)(blockDim.x >> 5) ? smem[lane] : 0, wi = wv;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      int x = __shfl_up_sync(0xffffffffu, wi, o);
+      if (lane >= o) wi += x;
+    }
+    smem[lane] = wi - wv;
+    if (lane == 31) smem[32] = wi;
+  }
+  __syncthreads();
+  int res = smem[warp] + incl - v;
+  *total = smem[32];
+  __syncthreads();
+  return res;
+}
+
+__global__ void attn_plan_k(const int32_t *__restrict__ slot_prompt, const int32_t *__restrict__ slot_npre,
+                            const int32_t *__restrict__ slot_nsuf, int32_t *items_pre, int32_t *items_suf, int32_t *n_items,
+                            int32_t *part_base, int32_t *part_cnt, int rep, int no_share, int max_items, const int32_t *n_rows_dev,
+                            int rows_ub) {
+  __shared__ int sm[33];
+  __shared__ int b_part, b_pre, b_suf;
+  int n = n_rows_dev ? min(*n_rows_dev, rows_ub) : rows_ub;
+  if (threadIdx.x == 0) { b_part = 0; b_pre = 0; b_suf = 0; }
+  __syncthreads();
+  int RB = 64 / rep;                                   // slots per ROWSPLIT item (64 query rows)
+  for (int base = 0; base < n; base += blockDim.x) {
+    int slot = base + threadIdx.x;
+    int npc = 0, nsc = 0, gsize = 0, nblk = 0;
+    if (slot < n) {
+      npc = (slot_npre[slot] + CH_TOK - 1) / CH_TOK;
+      nsc = (slot_nsuf[slot] + CH_TOK - 1) / CH_TOK;
+      int pr = slot_prompt[slot];
+      bool leader = no_share || slot == 0 || slot_prompt[slot - 1] != pr;
+      if (leader) {
+        gsize = 1;
+        if (!no_share) while (slot + gsize < n && slot_prompt[slot + gsize] == pr) ++gsize;
+        nblk = gsize * rep <= 16 ? 1 : (gsize + RB - 1) / RB;
+      }
+    }
+    int tp, tq, ts;
+    int ep = scan1024(npc + nsc, &tp, sm);
+    int eq = scan1024(nblk * npc, &tq, sm);
+    int es = scan1024(nsc, &ts, sm);
+    int bp = b_part, bq = b_pre, bs = b_suf;
+    if (slot < n) {
+      part_base[slot] = bp + ep;
+      part_cnt[slot] = npc + nsc;
+      int idx = bq + eq;
+      int per = nblk <= 1 ? gsize : RB;
+      for (int b = 0; b < nblk; ++b)
+        for (int ck = 0; ck < npc; ++ck, ++idx) {
+          if (idx >= max_items) continue;
+          int32_t *it = items_pre + (size_t)idx * ITEM_INTS;
+          it[0] = slot + b * per;
+          it[1] = min(per, gsize - b * per);
+          it[2] = ck * CH_PAGES;
+          it[3] = min(CH_TOK, slot_npre[slot] - ck * CH_TOK);
+          it[4] = ck;
+          it[5] = 1;
+        }
+      idx = bs + es;
+      for (int ck = 0; ck < nsc; ++ck, ++idx) {
+        if (idx >= max_items) continue;
+        int32_t *it = items_suf + (size_t)idx * ITEM_INTS;
+        it[0] = slot; it[1] = 1; it[2] = ck * CH_PAGES;
+        it[3] = min(CH_TOK, slot_nsuf[slot] - ck * CH_TOK);
+        it[4] = npc + ck; it[5] = 0;
+      }
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) { b_part = bp + tp; b_pre = bq + tq; b_suf = bs + ts; }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) { n_items[0] = min(b_pre, max_items); n_items[1] = min(b_suf, max_items); n_items[2] = b_part; }
+}
+
+}  // namespace
+
+size_t attn_sm100_smem_bytes() { return sizeof(Smem) + 128; }
+
+// Plan once per decode step (the lengths are the same for every layer), then per layer: main + merge.
+darts_status launch_attention_plan_sm100(darts_ctx *c, int rows_ub, const int32_t *n_rows_dev) {
+  int rep = c->m.n_q_heads / c->m.n_kv_heads;
+  attn_plan_k<<<1, 1024, 0, c->stream>>>(c->slot_prompt, c->slot_npre, c->slot_nsuf, c->attn_items_pre, c->attn_items_suf, c->attn_nitems,
+                                         c->part_base, c->part_cnt, rep, (c->rt.flags & DARTS_FLAG_NO_PREFIX_SHARING) ? 1 : 0,
+                                         c->attn_max_items, n_rows_dev, rows_ub);
+  c->launches++;
+  if (cudaGetLastError() != cudaSuccess) FAIL(c, DARTS_ERR_CUDA, "launch attn_plan failed");
+  return DARTS_OK;
+}
+
+bool attention_sm100_supported(const darts_ctx *c) {
+  int rep = c->m.n_q_heads / c->m.n_kv_heads;
+  return c->m.dtype == DARTS_BF16 && c->m.head_dim == HD && c->rt.page_size == PAGE && (rep == 1 || rep == 2 || rep == 4 || rep == 8 || rep == 16);
+}
+
+darts_status launch_attention_sm100(darts_ctx *c, int layer, const void *q, void *out, int rows_ub, const int32_t *n_rows_dev, bool *taken) {
   *taken = false;
+  if (!attention_sm100_supported(c) || !c->attn_plan_valid) return DARTS_OK;
+  *taken = true;
+  static bool attr_set = false;
+  size_t smem = attn_sm100_smem_bytes();
+  if (!attr_set) {
+    CUDA_TRY(c, cudaFuncSetAttribute(attn_main_k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    attr_set = true;
+  }
+  Params p;
+  p.q = (const __nv_bfloat16 *)q;
+  p.kv_layer = (const __nv_bfloat16 *)c->kv_pool + (size_t)layer * c->kv_layer_elems;
+  p.items_pre = c->attn_items_pre; p.items_suf = c->attn_items_suf; p.n_items = c->attn_nitems;
+  p.slot_prompt = c->slot_prompt; p.slot_row = c->slot_row; p.g_prefix_pages = c->g_prefix_pages; p.row_pages = c->row_pages;
+  p.part_base = c->part_base; p.part_ml = c->part_ml; p.part_acc = c->part_acc;
+  p.mpp = c->max_prefix_pages; p.msp = c->max_suffix_pages; p.Hq = c->m.n_q_heads; p.Hkv = c->m.n_kv_heads; p.rep = p.Hq / p.Hkv;
+  p.page_elems = c->kv_page_elems; p.tile_elems = c->kv_tile_elems;
+  p.c = 1.4426950408889634f / sqrtf((float)HD);
+  int grid = c->n_sms * 2;
+  attn_main_k<<<grid, THREADS, smem, c->stream>>>(p);
+  c->launches++;
+  if (cudaGetLastError() != cudaSuccess) FAIL(c, DARTS_ERR_CUDA, "launch attn_main failed: %s", cudaGetErrorString(cudaGetLastError()));
+  attn_merge_k<<<rows_ub, 256, 0, c->stream>>>(c->part_ml, c->part_acc, c->part_base, c->part_cnt, (__nv_bfloat16 *)out, p.Hq, p.c, n_rows_dev, rows_ub);
+  c->launches++;
+  if (cudaGetLastError() != cudaSuccess) FAIL(c, DARTS_ERR_CUDA, "launch attn_merge failed");
   return DARTS_OK;
 }

@@ -111,7 +111,7 @@ template <typename T>
 __global__ void rope_append_k(const float *__restrict__ qkv, T *__restrict__ q_out, T *__restrict__ kv_layer,
                               const int32_t *__restrict__ slot_dst_page, const int32_t *__restrict__ slot_dst_off,
                               const float2 *__restrict__ cs, const T *__restrict__ q_norm, const T *__restrict__ k_norm,
-                              int Hq, int Hkv, int hd, float eps, size_t page_elems, size_t tile_elems,
+                              int Hq, int Hkv, int hd, float eps, KvGeom geo,
                               const int32_t *n_rows_dev, int rows_ub) {
   int slot = blockIdx.y;
   if (slot >= live_rows(n_rows_dev, rows_ub)) return;
@@ -123,8 +123,7 @@ __global__ void rope_append_k(const float *__restrict__ qkv, T *__restrict__ q_o
   int page = slot_dst_page[slot], off = slot_dst_off[slot];
   if (head >= Hq + Hkv) {  // v: plain copy
     if (page < 0) return;
-    T *dst = kv_layer + (size_t)page * page_elems + ((size_t)Hkv + (head - Hq - Hkv)) * tile_elems + (size_t)off * hd;
-    for (int k = lane; k < hd; k += 32) dst[k] = from_f<T>(src[k]);
+    for (int k = lane; k < hd; k += 32) kv_layer[kv_elem(geo, page, head - Hq - Hkv, 1, off, k)] = from_f<T>(src[k]);
     return;
   }
   bool is_q = head < Hq;
@@ -136,18 +135,18 @@ __global__ void rope_append_k(const float *__restrict__ qkv, T *__restrict__ q_o
     ss = warp_sum(ss);
     r = 1.0f / sqrtf(ss / hd + eps);
   }
-  T *dst;
-  if (is_q) dst = q_out + (size_t)slot * Hq * hd + (size_t)head * hd;
-  else {
-    if (page < 0) return;
-    dst = kv_layer + (size_t)page * page_elems + (size_t)(head - Hq) * tile_elems + (size_t)off * hd;
-  }
+  if (!is_q && page < 0) return;
+  T *qdst = q_out + (size_t)slot * Hq * hd + (size_t)head * hd;
   for (int p = lane; p < half; p += 32) {
     float x1 = src[p], x2 = src[p + half];
     if (nw) { x1 = x1 * r * to_f<T>(nw[p]); x2 = x2 * r * to_f<T>(nw[p + half]); }
     float2 t = cs[(size_t)slot * half + p];
-    dst[p] = from_f<T>(x1 * t.x - x2 * t.y);
-    dst[p + half] = from_f<T>(x2 * t.x + x1 * t.y);
+    T y1 = from_f<T>(x1 * t.x - x2 * t.y), y2 = from_f<T>(x2 * t.x + x1 * t.y);
+    if (is_q) { qdst[p] = y1; qdst[p + half] = y2; }
+    else {
+      kv_layer[kv_elem(geo, page, head - Hq, 0, off, p)] = y1;
+      kv_layer[kv_elem(geo, page, head - Hq, 0, off, p + half)] = y2;
+    }
   }
 }
 
@@ -159,7 +158,7 @@ darts_status launch_rope_append(darts_ctx *c, int layer, int rows_ub, const int3
                     c->qkv32, (T *)c->q, (T *)c->kv_pool + (size_t)layer * c->kv_layer_elems, c->slot_dst_page, c->slot_dst_off,
                     c->slot_cs, c->m.qk_norm ? (const T *)c->q_norm[layer] : nullptr,
                     c->m.qk_norm ? (const T *)c->k_norm[layer] : nullptr, c->m.n_q_heads, c->m.n_kv_heads, c->m.head_dim,
-                    c->m.rms_eps, c->kv_page_elems, c->kv_tile_elems, n_rows_dev, rows_ub));
+                    c->m.rms_eps, c->geom(), n_rows_dev, rows_ub));
   return post_launch(c, "rope_append");
 }
 

@@ -205,8 +205,7 @@ template <typename T>
 __global__ void attn_load_k(T *kv_layer, const T *__restrict__ kp, const T *__restrict__ vp, const T *__restrict__ ks,
                             const T *__restrict__ vs, const int32_t *__restrict__ suffix_len, const int64_t *__restrict__ suffix_offs,
                             const int32_t *__restrict__ g_prefix_pages, const int32_t *__restrict__ row_pages, int G, int P, int Kp,
-                            int Hkv, int hd, int page, int mpp, int msp, size_t page_elems, size_t tile_elems, long long n_prefix_tok,
-                            long long n_tok) {
+                            int Hkv, int hd, int page, int mpp, int msp, KvGeom geo, long long n_prefix_tok, long long n_tok) {
   long long tok = blockIdx.x;
   if (tok >= n_tok) return;
   const T *srck, *srcv;
@@ -228,9 +227,8 @@ __global__ void attn_load_k(T *kv_layer, const T *__restrict__ kp, const T *__re
   }
   for (int e = threadIdx.x; e < Hkv * hd; e += blockDim.x) {
     int h = e / hd, d = e % hd;
-    size_t o = (size_t)pg * page_elems + (size_t)h * tile_elems + (size_t)off * hd + d;
-    kv_layer[o] = srck[e];
-    kv_layer[o + (size_t)Hkv * tile_elems] = srcv[e];
+    kv_layer[kv_elem(geo, pg, h, 0, off, d)] = srck[e];
+    kv_layer[kv_elem(geo, pg, h, 1, off, d)] = srcv[e];
   }
 }
 
@@ -272,13 +270,12 @@ darts_status launch_attn_load(darts_ctx *c, int G, int P, int Kp, const void *kp
     attn_load_k<float><<<(unsigned)n_tok, 128, 0, c->stream>>>((float *)c->kv_pool, (const float *)kp, (const float *)vp, (const float *)ks,
                                                                (const float *)vs, suffix_len_dev, suffix_offs_dev, c->g_prefix_pages,
                                                                c->row_pages, G, P, Kp, c->m.n_kv_heads, c->m.head_dim, c->rt.page_size,
-                                                               c->max_prefix_pages, c->max_suffix_pages, c->kv_page_elems, c->kv_tile_elems,
-                                                               n_pre, n_tok);
+                                                               c->max_prefix_pages, c->max_suffix_pages, c->geom(), n_pre, n_tok);
   else
     attn_load_k<__nv_bfloat16><<<(unsigned)n_tok, 128, 0, c->stream>>>(
         (__nv_bfloat16 *)c->kv_pool, (const __nv_bfloat16 *)kp, (const __nv_bfloat16 *)vp, (const __nv_bfloat16 *)ks,
         (const __nv_bfloat16 *)vs, suffix_len_dev, suffix_offs_dev, c->g_prefix_pages, c->row_pages, G, P, Kp, c->m.n_kv_heads,
-        c->m.head_dim, c->rt.page_size, c->max_prefix_pages, c->max_suffix_pages, c->kv_page_elems, c->kv_tile_elems, n_pre, n_tok);
+        c->m.head_dim, c->rt.page_size, c->max_prefix_pages, c->max_suffix_pages, c->geom(), n_pre, n_tok);
   c->launches++;
   if (cudaGetLastError() != cudaSuccess) FAIL(c, DARTS_ERR_CUDA, "launch attn_load failed");
   return DARTS_OK;
