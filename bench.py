@@ -190,7 +190,7 @@ def main():
     ap.add_argument("--steps", type=int, default=2)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours")
-    ap.add_argument("--workload", default="c3")
+    ap.add_argument("--workload", default="c2")
     ap.add_argument("--max-new", type=int, default=None, help="debug only: shorten the rollout (INVALID as a bench number)")
     ap.add_argument("--G", type=int, default=None, help="debug only")
     ap.add_argument("--layers", type=int, default=None, help="debug only")
