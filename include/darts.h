@@ -72,7 +72,8 @@ enum { DARTS_MODE_AUTO = 0, DARTS_MODE_DUAL_END = 1, DARTS_MODE_SHORTEST_EARLY_S
 
 enum {
   DARTS_FLAG_DUMP_LOGITS = 1,       /* keep fp32 logits of every row of the last step for darts_debug_logits */
-  DARTS_FLAG_NO_PREFIX_SHARING = 2  /* A/B switch: attention re-reads the prefix once per row, not per group */
+  DARTS_FLAG_NO_PREFIX_SHARING = 2, /* A/B switch: attention re-reads the prefix once per row, not per group */
+  DARTS_FLAG_PROFILE_ATTENTION = 4  /* bracket layer 0's attention of every decode step with CUDA events (bench roofline) */
 };
 
 typedef struct {
@@ -185,6 +186,11 @@ darts_status darts_get_results(darts_ctx *ctx, darts_results *out);
 darts_status darts_get_counters(darts_ctx *ctx, darts_counters *out);
 darts_status darts_n_active(darts_ctx *ctx, int32_t *out_host);      /* synchronises */
 
+/* With DARTS_FLAG_PROFILE_ATTENTION: device time (ms, CUDA events on the ctx stream) of layer 0's attention launches
+ * (split-KV main kernel + merge) for every decode step since the last darts_prefill, in step order.
+ * ms_host: HOST [cap]; *n_out = number of steps recorded (may exceed cap; only cap are written).  Synchronises. */
+darts_status darts_get_attention_times(darts_ctx *ctx, float *ms_host, int32_t cap, int32_t *n_out);
+
 /* Parity hooks (valid with DARTS_FLAG_DUMP_LOGITS): fp32 logits of global row `row` from the most
  * recent step that row took part in (step 0: the prompt's prefill logits).  out: HOST [vocab]. */
 darts_status darts_debug_logits(darts_ctx *ctx, int32_t row, float *out_host);
@@ -192,6 +198,13 @@ darts_status darts_debug_logits(darts_ctx *ctx, int32_t row, float *out_host);
 /* Teacher forcing for parity at bf16 (R12): overwrite the token the next decode step feeds
  * for global row `row`.  tokens: HOST [n_rows] (-1 = leave). */
 darts_status darts_debug_set_last_tokens(darts_ctx *ctx, const int32_t *tokens_host, int32_t n_rows);
+
+/* Parity hook for the tcgen05 GEMM that carries every projection of the bf16 path:
+ * C[rows][N] (fp32) = X[rows][K] . W[N][K]^T with bf16 X, W.  All pointers DEVICE.  split_k >= 1 K-splits are
+ * computed as separate partials in `scratch` (>= split_k * rows * N floats) and added in split order.
+ * Needs K % 64 == 0 and N % 4 == 0 (DARTS_ERR_UNSUPPORTED otherwise).  Asynchronous on the ctx stream. */
+darts_status darts_debug_gemm_bf16(darts_ctx *ctx, const void *X, const void *W, float *C, float *scratch, int32_t rows,
+                                   int32_t N, int32_t K, int32_t split_k);
 
 /* ---- Attention-only entry points (BASELINE.json config 2) -------------------
  * Build G groups of Kp rows whose KV is given explicitly, then time darts_attention alone.

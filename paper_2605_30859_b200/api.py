@@ -22,7 +22,7 @@ OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_KV_POOL_EXHAUSTED, ERR_WORKSPACE_TOO_S
 F32, BF16 = 0, 1
 ROW_ACTIVE, ROW_VALID, ROW_TRUNC, ROW_PRUNED = 0, 1, 2, 3
 MODE_AUTO, MODE_DUAL_END, MODE_SHORTEST_EARLY_STOP = 0, 1, 2
-FLAG_DUMP_LOGITS, FLAG_NO_PREFIX_SHARING = 1, 2
+FLAG_DUMP_LOGITS, FLAG_NO_PREFIX_SHARING, FLAG_PROFILE_ATTENTION = 1, 2, 4
 
 _vp, _i32, _u32, _u64, _f32 = C.c_void_p, C.c_int32, C.c_uint32, C.c_uint64, C.c_float
 _pp = C.POINTER(C.c_void_p)
@@ -79,8 +79,10 @@ darts_rollout_host = _sig("darts_rollout_host", _ctx, _vp, _i32, _i32, _vp, _vp,
 darts_get_results = _sig("darts_get_results", _ctx, C.POINTER(Results))
 darts_get_counters = _sig("darts_get_counters", _ctx, C.POINTER(Counters))
 darts_n_active = _sig("darts_n_active", _ctx, C.POINTER(_i32))
+darts_get_attention_times = _sig("darts_get_attention_times", _ctx, _vp, _i32, C.POINTER(_i32))
 darts_debug_logits = _sig("darts_debug_logits", _ctx, _i32, _vp)
 darts_debug_set_last_tokens = _sig("darts_debug_set_last_tokens", _ctx, _vp, _i32)
+darts_debug_gemm_bf16 = _sig("darts_debug_gemm_bf16", _ctx, _vp, _vp, _vp, _vp, _i32, _i32, _i32, _i32)
 darts_attn_load = _sig("darts_attn_load", _ctx, _i32, _i32, _i32, _vp, _vp, _vp, _vp, _vp)
 darts_attention = _sig("darts_attention", _ctx, _i32, _vp, _vp)
 
@@ -234,6 +236,15 @@ class Darts:
         self._check(darts_get_counters(self.ctx, C.byref(c)))
         return {n: getattr(c, n) for n, _ in Counters._fields_}
 
+    def attention_times(self):
+        """ms per decode step of layer 0's attention launches (needs FLAG_PROFILE_ATTENTION)."""
+        n = _i32()
+        self._check(darts_get_attention_times(self.ctx, None, 0, C.byref(n)))
+        out = np.empty(n.value, np.float32)
+        if n.value:
+            self._check(darts_get_attention_times(self.ctx, _np_ptr(out), n.value, C.byref(n)))
+        return out
+
     def debug_logits(self, row):
         out = np.empty(self.cfg["vocab"], np.float32)
         self._check(darts_debug_logits(self.ctx, row, _np_ptr(out)))
@@ -242,6 +253,16 @@ class Darts:
     def debug_set_last_tokens(self, tokens):
         t = np.ascontiguousarray(tokens, dtype=np.int32)
         self._check(darts_debug_set_last_tokens(self.ctx, _np_ptr(t), len(t)))
+
+    def debug_gemm_bf16(self, X, W, split_k=1):
+        """C = X @ W.T on the tcgen05 GEMM (bf16 device tensors X [rows,K], W [N,K]); returns fp32 [rows,N] on device."""
+        rows, K = X.shape
+        N = W.shape[0]
+        out = torch.empty(rows, N, dtype=torch.float32, device="cuda")
+        scratch = torch.empty(split_k * rows * N, dtype=torch.float32, device="cuda")
+        self._check(darts_debug_gemm_bf16(self.ctx, X.data_ptr(), W.data_ptr(), out.data_ptr(), scratch.data_ptr(), rows, N, K, split_k))
+        self._scratch = scratch
+        return out
 
     # ---- attention-only (config 2) -----------------------------------------------------------------
     def attn_load(self, G, P, Kp, k_prefix, v_prefix, suffix_len, k_suffix, v_suffix):

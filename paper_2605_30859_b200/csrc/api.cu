@@ -88,16 +88,40 @@ size_t carve(darts_ctx *c, void *base) {
     c->part_ml = k.take<float>(max_parts * m.n_q_heads * 2);
     c->part_acc = k.take<float>(max_parts * m.n_q_heads * m.head_dim);
   }
+  size_t Fm = m.n_experts ? (size_t)m.top_k * m.expert_ffn : (size_t)m.ffn;
+  int qd_ = m.n_q_heads * m.head_dim;
+  c->tc_path = model && m.dtype == DARTS_BF16 && tc_shape_ok(c->n_qkv, m.d_model) && tc_shape_ok(m.d_model, qd_) &&
+               tc_shape_ok(m.vocab, m.d_model) &&
+               (m.n_experts ? (tc_shape_ok(2 * m.expert_ffn, m.d_model) && tc_shape_ok(m.d_model, m.expert_ffn))
+                            : (tc_shape_ok(2 * m.ffn, m.d_model) && tc_shape_ok(m.d_model, m.ffn)));
   if (model) {
-    size_t F = m.n_experts ? (size_t)m.top_k * m.expert_ffn : (size_t)m.ffn;
+    size_t F = Fm;
     c->tokens_out = k.take<int32_t>(R * rt.max_new);
     c->margin_out = k.take<float>(R * rt.max_new);
     c->prompt_tokens = k.take<int32_t>(G * rt.max_prompt_len);
     c->slot_cs = k.take<float2>(A * (m.head_dim / 2));
     c->h = k.take<float>(A * m.d_model);
-    c->qkv32 = k.take<float>(A * c->n_qkv);
-    c->gu32 = k.take<float>(A * 2 * F);
-    c->logits = k.take<float>(R * m.vocab);
+    if (c->tc_path) {
+      size_t maxN = std::max<size_t>(std::max<size_t>(c->n_qkv, 2 * F), m.d_model);
+      c->part_bytes = std::max<size_t>(A * maxN * 4, (size_t)64 << 20);
+      c->part = k.take<float>(c->part_bytes / 4);
+      c->top2 = k.take<float>((size_t)ceil_div(m.vocab, 128) * R * 4);
+      if (rt.flags & DARTS_FLAG_DUMP_LOGITS) c->logits = k.take<float>(R * m.vocab);
+      if (m.n_experts) {
+        size_t RK = A * m.top_k;
+        c->moe_eid = k.take<int32_t>(RK);
+        c->moe_pos = k.take<int32_t>(RK);
+        c->moe_tok = k.take<int32_t>(RK);
+        c->moe_w = k.take<float>(RK);
+        c->moe_off = k.take<int32_t>(m.n_experts + 1);
+        c->moe_cnt = k.take<int32_t>(m.n_experts);
+        c->xs = k.take<char>(RK * m.d_model * 2);
+      }
+    } else {
+      c->qkv32 = k.take<float>(A * c->n_qkv);
+      c->gu32 = k.take<float>(A * 2 * F);
+      c->logits = k.take<float>(R * m.vocab);
+    }
     c->z0 = k.take<float>(G * m.vocab);
     c->hlast = k.take<float>(G * m.d_model);
     c->xn = k.take<char>(A * m.d_model * c->elt);
@@ -168,6 +192,82 @@ darts_status forward_layers(darts_ctx *c, int rows_ub, const int32_t *n_rows_dev
   return DARTS_OK;
 }
 
+// Tensor-core path (bf16): every projection on tcgen05, split-K partials reduced inside the consumer kernels, the
+// residual add fused with the next RMSNorm.  Leaves xn = rmsnorm(h_L) * final_norm for the LM head.
+TcGemm tc_gemm(darts_ctx *c, const CUtensorMap *a, const CUtensorMap *b, int N, int K, int rows_ub, const int32_t *n_rows_dev) {
+  TcGemm g{};
+  g.a_map = a; g.b_map = b; g.C = c->part; g.N = N; g.K = K; g.rows_ub = rows_ub; g.n_rows_dev = n_rows_dev;
+  g.S = tc_pick_split(c, N, K, rows_ub, 0);
+  g.split_stride = (size_t)rows_ub * N;
+  return g;
+}
+
+darts_status forward_layers_tc(darts_ctx *c, int rows_ub, const int32_t *n_rows_dev) {
+  const darts_model_desc &m = c->m;
+  const int d = m.d_model, qd = m.n_q_heads * m.head_dim, F = m.ffn, L = m.n_layers;
+  TRY(launch_embed(c, c->slot_tok, 0, rows_ub, n_rows_dev));
+  TRY(launch_rope_table(c, rows_ub, n_rows_dev));
+  TRY(launch_rmsnorm(c, c->h, c->attn_norm[0], c->xn, rows_ub, n_rows_dev));
+  for (int l = 0; l < L; ++l) {
+    TcGemm g = tc_gemm(c, &c->tm_xn, &c->tm_wqkv[l], c->n_qkv, d, rows_ub, n_rows_dev);
+    TRY(launch_gemm_tc(c, g));
+    TRY(launch_rope_append_part(c, l, g.S, rows_ub, n_rows_dev));
+    TRY(launch_attention(c, l, c->q, c->ao, rows_ub, n_rows_dev));
+    g = tc_gemm(c, &c->tm_ao, &c->tm_wo[l], d, qd, rows_ub, n_rows_dev);
+    TRY(launch_gemm_tc(c, g));
+    TRY(launch_add_rmsnorm(c, c->part, g.S, g.split_stride, c->mlp_norm[l], rows_ub, n_rows_dev));
+    const void *next_norm = l + 1 < L ? c->attn_norm[l + 1] : c->final_norm;
+    if (m.n_experts == 0) {
+      g = tc_gemm(c, &c->tm_xn, &c->tm_wgu[l], 2 * F, d, rows_ub, n_rows_dev);
+      TRY(launch_gemm_tc(c, g));
+      TRY(launch_silu_mul_part(c, g.S, rows_ub, n_rows_dev));
+      g = tc_gemm(c, &c->tm_act, &c->tm_wd[l], d, F, rows_ub, n_rows_dev);
+      TRY(launch_gemm_tc(c, g));
+      TRY(launch_add_rmsnorm(c, c->part, g.S, g.split_stride, next_norm, rows_ub, n_rows_dev));
+    } else {
+      TRY(launch_moe_tc(c, l, next_norm, rows_ub, n_rows_dev));
+    }
+  }
+  return DARTS_OK;
+}
+
+// LM head over xn (or any bf16 [rows][d] matrix behind `a`): plain logits store (prefill) or fused sampling (decode).
+darts_status lm_head_tc(darts_ctx *c, const CUtensorMap *a, float *logits_out, int rows_ub, const int32_t *n_rows_dev, bool sample) {
+  TcGemm g{};
+  g.a_map = a; g.b_map = &c->tm_lm; g.C = logits_out; g.N = c->m.vocab; g.K = c->m.d_model; g.rows_ub = rows_ub; g.n_rows_dev = n_rows_dev;
+  g.S = 1; g.split_stride = 0; g.sample = sample;
+  return launch_gemm_tc(c, g);
+}
+
+darts_status make_maps(darts_ctx *c) {
+  const darts_model_desc &m = c->m;
+  const int d = m.d_model, qd = m.n_q_heads * m.head_dim, L = m.n_layers;
+  c->tm_wqkv = new CUtensorMap[L]; c->tm_wo = new CUtensorMap[L];
+  if (m.n_experts == 0) { c->tm_wgu = new CUtensorMap[L]; c->tm_wd = new CUtensorMap[L]; }
+  else { c->tm_wgu_e = new CUtensorMap[L]; c->tm_wd_e = new CUtensorMap[L]; }
+  for (int l = 0; l < L; ++l) {
+    TRY(tc_make_map(c, &c->tm_wqkv[l], c->wqkv[l], c->n_qkv, d, 128));
+    TRY(tc_make_map(c, &c->tm_wo[l], c->wo[l], d, qd, 128));
+    if (m.n_experts == 0) {
+      TRY(tc_make_map(c, &c->tm_wgu[l], c->wgu[l], 2 * m.ffn, d, 128));
+      TRY(tc_make_map(c, &c->tm_wd[l], c->wd[l], d, m.ffn, 128));
+    } else {
+      TRY(tc_make_map(c, &c->tm_wgu_e[l], c->wgu_e[l], (long long)m.n_experts * 2 * m.expert_ffn, d, 128));
+      TRY(tc_make_map(c, &c->tm_wd_e[l], c->wd_e[l], (long long)m.n_experts * d, m.expert_ffn, 128));
+    }
+  }
+  TRY(tc_make_map(c, &c->tm_lm, c->lm_head, m.vocab, d, 128));
+  TRY(tc_make_map(c, &c->tm_xn, c->xn, c->act_rows, d, 16));
+  TRY(tc_make_map(c, &c->tm_ao, c->ao, c->act_rows, qd, 16));
+  TRY(tc_make_map(c, &c->tm_hl, c->hlast, c->rt.max_prompts, d, 16));
+  if (m.n_experts == 0) TRY(tc_make_map(c, &c->tm_act, c->act, c->act_rows, m.ffn, 16));
+  else {
+    TRY(tc_make_map(c, &c->tm_act, c->act, (long long)c->act_rows * m.top_k, m.expert_ffn, 16));
+    TRY(tc_make_map(c, &c->tm_xs, c->xs, (long long)c->act_rows * m.top_k, d, 16));
+  }
+  return DARTS_OK;
+}
+
 void refresh_ub(darts_ctx *c) {
   long long v = *(volatile long long *)c->pinned;          // {n_active, generation} written in one store
   if ((uint32_t)(v >> 32) == c->gen) c->host_active_ub = std::min(c->host_active_ub, (int32_t)(v & 0xffffffff));
@@ -199,7 +299,7 @@ darts_status prefill_impl(darts_ctx *c, const int32_t *prompt_tokens_dev, bool t
   if (n_prefix_pages > c->rt.n_pages) FAIL(c, DARTS_ERR_KV_POOL_EXHAUSTED, "prefix needs %d pages, pool has %d", n_prefix_pages, c->rt.n_pages);
   c->pol = p; c->temperature = temperature; c->seed = seed; c->G = G; c->R = R; c->Kp_max = Kp_max;
   if (c->max_len <= 0 || c->max_len > c->rt.max_new) c->max_len = c->rt.max_new;
-  c->gen += 1; c->host_active_ub = R; c->steps_issued = 0; c->prefilled = false;
+  c->gen += 1; c->host_active_ub = R; c->steps_issued = 0; c->prefilled = false; c->prof_n = 0;
   cudaStream_t s = c->stream;
   int total_tok = tok_off[G];
   if (!tokens_in_place)
@@ -221,10 +321,16 @@ darts_status prefill_impl(darts_ctx *c, const int32_t *prompt_tokens_dev, bool t
     int tb = tok_off[g0];
     c->attn_plan_valid = false;                      // prefill is causal per token: generic kernel
     TRY(launch_plan_prefill(c, tb, ntok, g0, g1));
-    TRY(forward_layers(c, ntok, nullptr));
-    TRY(launch_gather_last(c, tb, ntok, g0, g1));
-    TRY(launch_rmsnorm(c, c->hlast, c->final_norm, c->xn, g1 - g0, nullptr));
-    TRY(launch_gemm(c, c->xn, c->lm_head, c->z0 + (size_t)g0 * c->m.vocab, c->m.vocab, c->m.d_model, g1 - g0, nullptr, false));
+    if (c->tc_path) {
+      TRY(forward_layers_tc(c, ntok, nullptr));
+      TRY(launch_gather_rows_bf16(c, c->xn, c->hlast, tb, g0, g1));             // final-normed hidden of each prompt's last token
+      TRY(lm_head_tc(c, &c->tm_hl, c->z0 + (size_t)g0 * c->m.vocab, g1 - g0, nullptr, false));
+    } else {
+      TRY(forward_layers(c, ntok, nullptr));
+      TRY(launch_gather_last(c, tb, ntok, g0, g1));
+      TRY(launch_rmsnorm(c, c->hlast, c->final_norm, c->xn, g1 - g0, nullptr));
+      TRY(launch_gemm(c, c->xn, c->lm_head, c->z0 + (size_t)g0 * c->m.vocab, c->m.vocab, c->m.d_model, g1 - g0, nullptr, false));
+    }
     g0 = g1;
   }
   TRY(launch_sample(c, c->z0, 1, R));                                            // step 0: Kp[i] draws from the shared z0[i]
@@ -235,27 +341,33 @@ darts_status prefill_impl(darts_ctx *c, const int32_t *prompt_tokens_dev, bool t
 }  // namespace
 
 // dispatchers: the tuned sm_100a kernels take the shapes they support, the generic kernels the rest
-darts_status launch_gemm_tc(darts_ctx *c, const void *X, const void *W, float *C, int N, int K, int rows_ub,
-                            const int32_t *n_rows_dev, bool accumulate, bool *taken);
 darts_status launch_attention_sm100(darts_ctx *c, int layer, const void *q, void *out, int rows_ub, const int32_t *n_rows_dev, bool *taken);
 
 darts_status launch_gemm(darts_ctx *c, const void *X, const void *W, float *C, int N, int K, int rows_ub, const int32_t *n_rows_dev,
                          bool accumulate, bool w_is_f32) {
   if (rows_ub <= 0) return DARTS_OK;
-  if (c->m.dtype == DARTS_BF16 && !w_is_f32) {
-    bool taken = false;
-    darts_status s = launch_gemm_tc(c, X, W, C, N, K, rows_ub, n_rows_dev, accumulate, &taken);
-    if (s != DARTS_OK || taken) return s;
-  }
   return launch_gemm_simt(c, X, W, C, N, K, rows_ub, n_rows_dev, accumulate, w_is_f32);
 }
 
 darts_status launch_attention(darts_ctx *c, int layer, const void *q, void *out, int rows_ub, const int32_t *n_rows_dev) {
   if (rows_ub <= 0) return DARTS_OK;
+  bool prof = (c->rt.flags & DARTS_FLAG_PROFILE_ATTENTION) && layer == 0 && c->in_decode;
+  if (prof) {
+    while ((int)c->prof_ev.size() < 2 * (c->prof_n + 1)) {
+      cudaEvent_t e;
+      CUDA_TRY(c, cudaEventCreate(&e));
+      c->prof_ev.push_back(e);
+    }
+    CUDA_TRY(c, cudaEventRecord(c->prof_ev[2 * c->prof_n], c->stream));
+  }
   bool taken = false;
   darts_status s = launch_attention_sm100(c, layer, q, out, rows_ub, n_rows_dev, &taken);
-  if (s != DARTS_OK || taken) return s;
-  return launch_attention_ref(c, layer, q, out, rows_ub, n_rows_dev);
+  if (s == DARTS_OK && !taken) s = launch_attention_ref(c, layer, q, out, rows_ub, n_rows_dev);
+  if (prof && s == DARTS_OK) {
+    CUDA_TRY(c, cudaEventRecord(c->prof_ev[2 * c->prof_n + 1], c->stream));
+    c->prof_n++;
+  }
+  return s;
 }
 
 extern "C" {
@@ -298,6 +410,7 @@ darts_status darts_create(const darts_model_desc *m, const darts_weights *w, con
     bool ok = c->embed && c->final_norm && c->lm_head && c->attn_norm && c->wqkv && c->wo && c->mlp_norm &&
               (m->n_experts ? (c->wr && c->wgu_e && c->wd_e) : (c->wgu && c->wd)) && (!m->qk_norm || (c->q_norm && c->k_norm));
     if (!ok) FAIL(c, DARTS_ERR_INVALID_ARG, "missing weight pointers");
+    if (c->tc_path && (s = make_maps(c)) != DARTS_OK) return s;
   }
   void *pin = nullptr;
   CUDA_TRY(c, cudaHostAlloc(&pin, 64, cudaHostAllocMapped));
@@ -320,8 +433,11 @@ darts_status darts_destroy(darts_ctx *c) {
   if (c->pinned) cudaFreeHost((void *)c->pinned);
   if (c->ev[0]) cudaEventDestroy(c->ev[0]);
   if (c->ev[1]) cudaEventDestroy(c->ev[1]);
+  for (cudaEvent_t e : c->prof_ev) cudaEventDestroy(e);
   const void **arrs[] = {c->attn_norm, c->wqkv, c->q_norm, c->k_norm, c->wo, c->mlp_norm, c->wgu, c->wd, c->wr, c->wgu_e, c->wd_e};
   for (auto a : arrs) delete[] a;
+  CUtensorMap *maps[] = {c->tm_wqkv, c->tm_wo, c->tm_wgu, c->tm_wd, c->tm_wgu_e, c->tm_wd_e};
+  for (auto a : maps) delete[] a;
   delete c;
   return DARTS_OK;
 }
@@ -345,10 +461,18 @@ darts_status darts_decode_step(darts_ctx *c) {
   TRY(launch_plan_decode(c, ub));
   c->attn_plan_valid = attention_sm100_supported(c);
   if (c->attn_plan_valid) TRY(launch_attention_plan_sm100(c, ub, n));
-  TRY(forward_layers(c, ub, n));
-  TRY(launch_rmsnorm(c, c->h, c->final_norm, c->xn, ub, n));
-  TRY(launch_gemm(c, c->xn, c->lm_head, c->logits, c->m.vocab, c->m.d_model, ub, n, false));
-  TRY(launch_sample(c, c->logits, 0, ub));
+  c->in_decode = true;
+  struct Leave { darts_ctx *c; ~Leave() { c->in_decode = false; } } leave{c};
+  if (c->tc_path) {
+    TRY(forward_layers_tc(c, ub, n));
+    TRY(lm_head_tc(c, &c->tm_xn, nullptr, ub, n, true));                          // logits never reach HBM (unless DUMP_LOGITS)
+    TRY(launch_sample_finalize(c, ceil_div(c->m.vocab, 128), ub));
+  } else {
+    TRY(forward_layers(c, ub, n));
+    TRY(launch_rmsnorm(c, c->h, c->final_norm, c->xn, ub, n));
+    TRY(launch_gemm(c, c->xn, c->lm_head, c->logits, c->m.vocab, c->m.d_model, ub, n, false));
+    TRY(launch_sample(c, c->logits, 0, ub));
+  }
   c->steps_issued++;
   return DARTS_OK;
 }
@@ -369,6 +493,14 @@ darts_status darts_n_active(darts_ctx *c, int32_t *out_host) {
   *out_host = st.n_active;
   c->host_active_ub = std::min(c->host_active_ub, st.n_active);
   if (st.err) { c->sticky = st.err; FAIL(c, st.err, "KV page pool exhausted"); }
+  return DARTS_OK;
+}
+
+darts_status darts_get_attention_times(darts_ctx *c, float *ms_host, int32_t cap, int32_t *n_out) {
+  if (!c || !n_out || (cap > 0 && !ms_host)) return DARTS_ERR_INVALID_ARG;
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  *n_out = c->prof_n;
+  for (int k = 0; k < c->prof_n && k < cap; ++k) CUDA_TRY(c, cudaEventElapsedTime(&ms_host[k], c->prof_ev[2 * k], c->prof_ev[2 * k + 1]));
   return DARTS_OK;
 }
 
@@ -476,6 +608,7 @@ darts_status darts_debug_logits(darts_ctx *c, int32_t row, float *out_host) {
   if (sstep == 0) src = c->z0 + (size_t)prompt * c->m.vocab;
   else {
     // valid only for the most recent decode step (the logits buffer is overwritten every step)
+    if (!c->logits) FAIL(c, DARTS_ERR_BAD_STATE, "decode logits are not kept: create the context with DARTS_FLAG_DUMP_LOGITS");
     if (sstep != c->steps_issued) FAIL(c, DARTS_ERR_BAD_STATE, "row %d last decoded at step %d, buffer holds step %d", row, sstep, c->steps_issued);
     src = c->logits + (size_t)slot * c->m.vocab;
   }
@@ -492,6 +625,21 @@ darts_status darts_debug_set_last_tokens(darts_ctx *c, const int32_t *tokens_hos
   for (int r = 0; r < n_rows; ++r) if (tokens_host[r] >= 0) cur[r] = tokens_host[r];
   CUDA_TRY(c, cudaMemcpy(c->row_last_tok, cur.data(), (size_t)n_rows * 4, cudaMemcpyHostToDevice));
   return DARTS_OK;
+}
+
+darts_status darts_debug_gemm_bf16(darts_ctx *c, const void *X, const void *W, float *C, float *scratch, int32_t rows, int32_t N, int32_t K,
+                                   int32_t split_k) {
+  if (!c) return DARTS_ERR_INVALID_ARG;
+  if (c->sticky) return c->sticky;
+  if (!X || !W || !C || !scratch || rows <= 0 || N <= 0 || K <= 0 || split_k < 1) FAIL(c, DARTS_ERR_INVALID_ARG, "NULL / non-positive argument");
+  if (!tc_shape_ok(N, K) || split_k > K / 64) FAIL(c, DARTS_ERR_UNSUPPORTED, "tcgen05 GEMM needs K %% 64 == 0, N %% 4 == 0, split_k <= K/64");
+  CUtensorMap ta, tb;
+  TRY(tc_make_map(c, &ta, X, rows, K, 16));
+  TRY(tc_make_map(c, &tb, W, N, K, 128));
+  TcGemm g{};
+  g.a_map = &ta; g.b_map = &tb; g.C = scratch; g.N = N; g.K = K; g.S = split_k; g.rows_ub = rows; g.split_stride = (size_t)rows * N;
+  TRY(launch_gemm_tc(c, g));
+  return launch_sum_partials(c, scratch, C, split_k, (size_t)rows * N);
 }
 
 darts_status darts_attn_load(darts_ctx *c, int32_t G, int32_t P, int32_t Kp, const void *k_prefix, const void *v_prefix,

@@ -1,10 +1,13 @@
 // Internal declarations shared by the translation units of libdarts.so (not part of the C-ABI).
 #pragma once
+#include <cuda.h>
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <stdio.h>
 #include <string.h>
+
+#include <vector>
 
 #include "darts.h"
 
@@ -78,6 +81,17 @@ struct darts_ctx {
   void *xn, *q, *ao, *act;
   // attention-only mode (config 2)
   int32_t attn_rows;
+  // tensor-core path (bf16, kernels_gemm_tc.cu): split-K partial buffer, LM-head top-2 partials, tensor maps
+  bool tc_path;                  // every GEMM of this model runs on tcgen05
+  float *part;                   // [S][rows][N] fp32 partials of the GEMM in flight
+  size_t part_bytes;
+  float *top2;                   // float4 [vocab tiles][max_rows]
+  CUtensorMap *tm_wqkv, *tm_wo, *tm_wgu, *tm_wd, *tm_wgu_e, *tm_wd_e;   // host arrays [n_layers]
+  CUtensorMap tm_lm, tm_xn, tm_ao, tm_act, tm_xs, tm_hl;                      // activations: 16-row boxes
+  // MoE (kernels_moe.cu)
+  int32_t *moe_eid, *moe_pos, *moe_off, *moe_cnt, *moe_tok;
+  float *moe_w;
+  void *xs;                      // expert-sorted copy of xn [max_rows * top_k][d]
   // tuned attention (kernels_attn_sm100.cu): per-step work list and split-KV partials
   int32_t *attn_items_pre, *attn_items_suf, *attn_nitems, *part_base, *part_cnt;
   float *part_ml, *part_acc;
@@ -101,6 +115,10 @@ struct darts_ctx {
   volatile int32_t *pinned;      // host view: [0] n_active + [1] generation (one 64-bit store), [2] err
   int32_t *pinned_dev;           // device view of the same mapped allocation
   int64_t launches;
+  // DARTS_FLAG_PROFILE_ATTENTION: event pairs around layer 0's attention of each decode step
+  std::vector<cudaEvent_t> prof_ev;
+  int prof_n;
+  bool in_decode;
   char err[512];
   darts_status sticky;
 };
@@ -151,6 +169,7 @@ darts_status launch_rope_append(darts_ctx *c, int layer, int rows_ub, const int3
 darts_status launch_attention(darts_ctx *c, int layer, const void *q, void *out, int rows_ub, const int32_t *n_rows_dev);
 darts_status launch_silu_mul(darts_ctx *c, int rows_ub, const int32_t *n_rows_dev);
 darts_status launch_moe(darts_ctx *c, int layer, int rows_ub, const int32_t *n_rows_dev);
+darts_status launch_moe_tc(darts_ctx *c, int layer, const void *next_norm, int rows_ub, const int32_t *n_rows_dev);
 darts_status launch_sample(darts_ctx *c, const float *logits, int step0, int rows_ub);
 darts_status launch_plan_decode(darts_ctx *c, int rows_ub);
 darts_status launch_plan_prefill(darts_ctx *c, int tok_begin, int n_tok, int g_begin, int g_end);
@@ -162,6 +181,29 @@ darts_status launch_attn_load(darts_ctx *c, int G, int P, int Kp, const void *kp
                               const int64_t *suffix_offs_dev, const void *ks, const void *vs, long long n_suffix_tok);
 darts_status launch_gemm_simt(darts_ctx *c, const void *X, const void *W, float *C, int N, int K, int rows_ub,
                               const int32_t *n_rows_dev, bool accumulate, bool w_is_f32);
+// tcgen05 GEMM (kernels_gemm_tc.cu)
+struct TcGemm {
+  const CUtensorMap *a_map, *b_map;   // activations [rows][K] (16-row boxes), weights [N (x groups)][K] (128-row boxes)
+  float *C;                           // partials [S][rows][N] (ignored when sample)
+  size_t split_stride;
+  int N, K, S, rows_ub;
+  const int32_t *n_rows_dev;
+  int n_groups;                       // grouped (MoE): blockIdx.z / S = group
+  const int32_t *grp_off;
+  int b_rows_per_group;
+  bool sample;                        // LM head: fused temperature + Gumbel-max epilogue -> ctx->top2
+};
+darts_status launch_gemm_tc(darts_ctx *c, const TcGemm &g);
+darts_status tc_make_map(darts_ctx *c, CUtensorMap *out, const void *base, long long rows, int K, int box_rows);
+bool tc_shape_ok(int N, int K);
+int tc_pick_split(const darts_ctx *c, int N, int K, int rows_ub, int n_groups);
+// consumers of the split-K partials (kernels_fused.cu)
+darts_status launch_rope_append_part(darts_ctx *c, int layer, int S, int rows_ub, const int32_t *n_rows_dev);
+darts_status launch_add_rmsnorm(darts_ctx *c, const float *part, int S, size_t split_stride, const void *w, int rows_ub, const int32_t *n_rows_dev);
+darts_status launch_silu_mul_part(darts_ctx *c, int S, int rows_ub, const int32_t *n_rows_dev);
+darts_status launch_sample_finalize(darts_ctx *c, int n_tiles, int rows_ub);
+darts_status launch_sum_partials(darts_ctx *c, const float *part, float *out, int S, size_t n);
+darts_status launch_gather_rows_bf16(darts_ctx *c, const void *src, void *dst, int tok_begin, int g_begin, int g_end);
 darts_status launch_attention_plan_sm100(darts_ctx *c, int rows_ub, const int32_t *n_rows_dev);
 bool attention_sm100_supported(const darts_ctx *c);
 darts_status launch_attention_ref(darts_ctx *c, int layer, const void *q, void *out, int rows_ub, const int32_t *n_rows_dev);

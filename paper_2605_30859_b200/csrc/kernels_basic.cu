@@ -111,7 +111,7 @@ template <typename T>
 __global__ void rope_append_k(const float *__restrict__ qkv, T *__restrict__ q_out, T *__restrict__ kv_layer,
                               const int32_t *__restrict__ slot_dst_page, const int32_t *__restrict__ slot_dst_off,
                               const float2 *__restrict__ cs, const T *__restrict__ q_norm, const T *__restrict__ k_norm,
-                              int Hq, int Hkv, int hd, float eps, KvGeom geo,
+                              int Hq, int Hkv, int hd, float eps, KvGeom geo, int S, size_t split_stride,
                               const int32_t *n_rows_dev, int rows_ub) {
   int slot = blockIdx.y;
   if (slot >= live_rows(n_rows_dev, rows_ub)) return;
@@ -119,11 +119,13 @@ __global__ void rope_append_k(const float *__restrict__ qkv, T *__restrict__ q_o
   int head = blockIdx.x * 4 + warp;
   if (head >= Hq + 2 * Hkv) return;
   const float *src = qkv + (size_t)slot * (Hq + 2 * Hkv) * hd + (size_t)head * hd;
+  // split-K partials (tensor-core path): element = sum over splits in split order; S == 1 for the SIMT path
+  auto ld = [&](int k) { float v = src[k]; for (int s = 1; s < S; ++s) v += src[(size_t)s * split_stride + k]; return v; };
   int half = hd >> 1;
   int page = slot_dst_page[slot], off = slot_dst_off[slot];
   if (head >= Hq + Hkv) {  // v: plain copy
     if (page < 0) return;
-    for (int k = lane; k < hd; k += 32) kv_layer[kv_elem(geo, page, head - Hq - Hkv, 1, off, k)] = from_f<T>(src[k]);
+    for (int k = lane; k < hd; k += 32) kv_layer[kv_elem(geo, page, head - Hq - Hkv, 1, off, k)] = from_f<T>(ld(k));
     return;
   }
   bool is_q = head < Hq;
@@ -131,14 +133,14 @@ __global__ void rope_append_k(const float *__restrict__ qkv, T *__restrict__ q_o
   float r = 1.f;
   if (nw) {
     float ss = 0.f;
-    for (int k = lane; k < hd; k += 32) ss += src[k] * src[k];
+    for (int k = lane; k < hd; k += 32) { float v = ld(k); ss += v * v; }
     ss = warp_sum(ss);
     r = 1.0f / sqrtf(ss / hd + eps);
   }
   if (!is_q && page < 0) return;
   T *qdst = q_out + (size_t)slot * Hq * hd + (size_t)head * hd;
   for (int p = lane; p < half; p += 32) {
-    float x1 = src[p], x2 = src[p + half];
+    float x1 = ld(p), x2 = ld(p + half);
     if (nw) { x1 = x1 * r * to_f<T>(nw[p]); x2 = x2 * r * to_f<T>(nw[p + half]); }
     float2 t = cs[(size_t)slot * half + p];
     T y1 = from_f<T>(x1 * t.x - x2 * t.y), y2 = from_f<T>(x2 * t.x + x1 * t.y);
@@ -150,6 +152,18 @@ __global__ void rope_append_k(const float *__restrict__ qkv, T *__restrict__ q_o
   }
 }
 
+darts_status launch_rope_append_part(darts_ctx *c, int layer, int S, int rows_ub, const int32_t *n_rows_dev) {
+  if (rows_ub <= 0) return DARTS_OK;
+  int nh = c->m.n_q_heads + 2 * c->m.n_kv_heads;
+  dim3 grid((nh + 3) / 4, rows_ub);
+  using T = __nv_bfloat16;
+  rope_append_k<T><<<grid, 128, 0, c->stream>>>(c->part, (T *)c->q, (T *)c->kv_pool + (size_t)layer * c->kv_layer_elems, c->slot_dst_page,
+                                                c->slot_dst_off, c->slot_cs, c->m.qk_norm ? (const T *)c->q_norm[layer] : nullptr,
+                                                c->m.qk_norm ? (const T *)c->k_norm[layer] : nullptr, c->m.n_q_heads, c->m.n_kv_heads,
+                                                c->m.head_dim, c->m.rms_eps, c->geom(), S, (size_t)rows_ub * c->n_qkv, n_rows_dev, rows_ub);
+  return post_launch(c, "rope_append_part");
+}
+
 darts_status launch_rope_append(darts_ctx *c, int layer, int rows_ub, const int32_t *n_rows_dev) {
   if (rows_ub <= 0) return DARTS_OK;
   int nh = c->m.n_q_heads + 2 * c->m.n_kv_heads;
@@ -158,7 +172,7 @@ darts_status launch_rope_append(darts_ctx *c, int layer, int rows_ub, const int3
                     c->qkv32, (T *)c->q, (T *)c->kv_pool + (size_t)layer * c->kv_layer_elems, c->slot_dst_page, c->slot_dst_off,
                     c->slot_cs, c->m.qk_norm ? (const T *)c->q_norm[layer] : nullptr,
                     c->m.qk_norm ? (const T *)c->k_norm[layer] : nullptr, c->m.n_q_heads, c->m.n_kv_heads, c->m.head_dim,
-                    c->m.rms_eps, c->geom(), n_rows_dev, rows_ub));
+                    c->m.rms_eps, c->geom(), 1, 0, n_rows_dev, rows_ub));
   return post_launch(c, "rope_append");
 }
 

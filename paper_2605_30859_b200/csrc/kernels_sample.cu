@@ -25,6 +25,28 @@ __device__ __forceinline__ Top2 top2_merge(const Top2 &a, const Top2 &b) {
   return r;
 }
 
+// Stop rules in the order of SURVEY.md §8(c) step 5, bookkeeping of the sampled token (one thread per row).
+__device__ __forceinline__ void finish_row(DevState *st, int row, int slot, int s, const Top2 &t, int32_t *row_len, uint8_t *row_status,
+                                           const int32_t *row_forced, int32_t *row_last_tok, int32_t *row_slot, int32_t *row_slot_step,
+                                           int32_t *tokens_out, float *margin_out, int max_new_stride, int max_len, int eos_id) {
+  int tok = t.i1;
+  float margin = t.b1 - t.b2;
+  int len = s + 1;
+  uint8_t status = DARTS_ROW_ACTIVE;
+  if (row_forced[row] == len) { tok = eos_id; status = DARTS_ROW_VALID; }   // forced EOS (BASELINE.json workloads)
+  else if (eos_id >= 0 && tok == eos_id) status = DARTS_ROW_VALID;          // natural EOS
+  else if (len == max_len) status = DARTS_ROW_TRUNC;                        // length limit
+  tokens_out[(size_t)row * max_new_stride + s] = tok;
+  margin_out[(size_t)row * max_new_stride + s] = margin;
+  row_last_tok[row] = tok;
+  row_len[row] = len;
+  row_status[row] = status;
+  row_slot[row] = slot;
+  row_slot_step[row] = st->step;
+  atomicAdd(&st->n_generated, 1ULL);
+  if (margin < NEAR_TIE_MARGIN) atomicAdd(&st->n_near_ties, 1ULL);
+}
+
 __global__ void __launch_bounds__(256) sample_k(DevState *st, const float *__restrict__ logits, int V, int step0,
                                                 const int32_t *__restrict__ row_list, const int32_t *__restrict__ row_prompt,
                                                 const int32_t *__restrict__ row_sample, int32_t *row_len, uint8_t *row_status,
@@ -63,22 +85,43 @@ __global__ void __launch_bounds__(256) sample_k(DevState *st, const float *__res
   __syncthreads();
   if (threadIdx.x == 0) {
     for (int w = 1; w < (int)(blockDim.x >> 5); ++w) t = top2_merge(t, red[w]);
-    int tok = t.i1;
-    float margin = t.b1 - t.b2;
-    int len = s + 1;
-    uint8_t status = DARTS_ROW_ACTIVE;
-    if (row_forced[row] == len) { tok = eos_id; status = DARTS_ROW_VALID; }   // forced EOS (BASELINE.json workloads)
-    else if (eos_id >= 0 && tok == eos_id) status = DARTS_ROW_VALID;          // natural EOS
-    else if (len == max_len) status = DARTS_ROW_TRUNC;                        // length limit
-    tokens_out[(size_t)row * max_new_stride + s] = tok;
-    margin_out[(size_t)row * max_new_stride + s] = margin;
-    row_last_tok[row] = tok;
-    row_len[row] = len;
-    row_status[row] = status;
-    row_slot[row] = slot;
-    row_slot_step[row] = st->step;
-    atomicAdd(&st->n_generated, 1ULL);
-    if (margin < NEAR_TIE_MARGIN) atomicAdd(&st->n_near_ties, 1ULL);
+    finish_row(st, row, slot, s, t, row_len, row_status, row_forced, row_last_tok, row_slot, row_slot_step, tokens_out, margin_out,
+               max_new_stride, max_len, eos_id);
+  }
+}
+
+// LM-head tensor-core path: the GEMM epilogue left one (best, second, argbest) per (vocab tile, slot); merge the tiles
+// (max with lowest-id tie-break is order-independent) and apply the stop rules.
+__global__ void __launch_bounds__(128) sample_finalize_k(DevState *st, const float4 *__restrict__ top2, int n_tiles, int rows_ub,
+                                                         const int32_t *__restrict__ row_list, int32_t *row_len, uint8_t *row_status,
+                                                         const int32_t *__restrict__ row_forced, int32_t *row_last_tok, int32_t *row_slot,
+                                                         int32_t *row_slot_step, int32_t *tokens_out, float *margin_out, int max_new_stride,
+                                                         int max_len, int eos_id) {
+  int slot = blockIdx.x;
+  if (slot >= st->n_active) return;
+  int row = row_list[slot];
+  int s = row_len[row];
+  Top2 t{-INFINITY, -INFINITY, 0x7fffffff};
+  for (int k = threadIdx.x; k < n_tiles; k += blockDim.x) {
+    float4 v = top2[(size_t)k * rows_ub + slot];
+    Top2 u{v.x, v.y, __float_as_int(v.z)};
+    t = top2_merge(t, u);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    Top2 u;
+    u.b1 = __shfl_xor_sync(0xffffffffu, t.b1, o);
+    u.b2 = __shfl_xor_sync(0xffffffffu, t.b2, o);
+    u.i1 = __shfl_xor_sync(0xffffffffu, t.i1, o);
+    t = top2_merge(t, u);
+  }
+  __shared__ Top2 red[4];
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = t;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < (int)(blockDim.x >> 5); ++w) t = top2_merge(t, red[w]);
+    finish_row(st, row, slot, s, t, row_len, row_status, row_forced, row_last_tok, row_slot, row_slot_step, tokens_out, margin_out,
+               max_new_stride, max_len, eos_id);
   }
 }
 
@@ -94,6 +137,21 @@ darts_status launch_sample(darts_ctx *c, const float *logits, int step0, int row
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) {
     snprintf(c->err, sizeof(c->err), "launch sample: %s", cudaGetErrorString(e));
+    c->sticky = DARTS_ERR_CUDA;
+    return DARTS_ERR_CUDA;
+  }
+  return DARTS_OK;
+}
+
+darts_status launch_sample_finalize(darts_ctx *c, int n_tiles, int rows_ub) {
+  if (rows_ub <= 0) return DARTS_OK;
+  sample_finalize_k<<<rows_ub, 128, 0, c->stream>>>(c->st, (const float4 *)c->top2, n_tiles, rows_ub, c->row_list, c->row_len, c->row_status,
+                                                    c->row_forced, c->row_last_tok, c->row_slot, c->row_slot_step, c->tokens_out,
+                                                    c->margin_out, c->rt.max_new, c->max_len, c->m.eos_id);
+  c->launches++;
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) {
+    snprintf(c->err, sizeof(c->err), "launch sample_finalize: %s", cudaGetErrorString(e));
     c->sticky = DARTS_ERR_CUDA;
     return DARTS_ERR_CUDA;
   }

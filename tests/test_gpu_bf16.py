@@ -1,0 +1,87 @@
+"""-m gpu parity of the bf16 tensor-core path (tcgen05 GEMMs, tuned attention, fused LM-head sampling) against the oracle,
+teacher-forced (R12): the oracle consumes the GPU's tokens, logits must agree within 2e-2 relative
+(north_star), tokens must agree wherever the oracle's margin exceeds twice the measured logit error."""
+import numpy as np
+import pytest
+
+from oracle import PRUNED, MODE_DUAL_END
+from oracle import rollout as ro
+from paper_2605_30859_b200 import workloads as wl
+from tests.gpu_util import make_ctx, rel_inf
+
+pytestmark = pytest.mark.gpu
+
+LOGIT_TOL_BF16 = 2e-2
+
+SMALL = dict(n_layers=2, d_model=256, n_q_heads=4, n_kv_heads=2, head_dim=128, ffn=512, vocab=1024, n_experts=0, top_k=0,
+             expert_ffn=0, qk_norm=False, rope_theta=1.0e6, rms_eps=1.0e-6, dtype="bf16")
+
+
+def run_stepwise(d, prompts, Kp, K, T, seed, forced, **kw):
+    """Drive the C-ABI step by step, keeping the fp32 logits of every (row, step)."""
+    d.prefill(prompts, Kp, K, temperature=T, seed=seed, forced_len=forced, **kw)
+    R = int(np.sum(Kp))
+    glog = {(r, 0): d.debug_logits(r) for r in range(R)}
+    d.select_and_compact()
+    s = 0
+    while d.n_active() > 0:
+        s += 1
+        d.decode_step()
+        res = d.results()
+        for r in range(R):
+            if res["len"][r] == s + 1:
+                glog[(r, s)] = d.debug_logits(r)
+        d.select_and_compact()
+    return d.results(), glog
+
+
+# std 0.02 is the configs' init recipe (tolerance: north_star's 2e-2).  std 0.08 is a stress case outside the recipe:
+# sharper softmaxes amplify the bf16 rounding of q, k, P and the activations, so it gets twice the tolerance.
+@pytest.mark.parametrize("qk_norm,std,tol", [(False, 0.02, LOGIT_TOL_BF16), (True, 0.02, LOGIT_TOL_BF16), (False, 0.08, 2 * LOGIT_TOL_BF16)])
+def test_small_bf16_model_matches_oracle(qk_norm, std, tol):
+    from paper_2605_30859_b200 import api
+    cfg = dict(SMALL, qk_norm=qk_norm)
+    seed, G, P, max_new, K, T = 5, 3, 70, 40, 2, 1.0
+    rng = np.random.default_rng(seed)
+    prompts = [rng.integers(0, cfg["vocab"] - 1, size=n).astype(np.int32) for n in (70, 33, 64)]
+    Kp = np.asarray([4, 5, 3], dtype=np.int32)
+    forced = wl.make_forced_len(Kp, dict(kind="lognormal", mu=2.8, sigma=0.7, lo=2, hi=60), seed)
+    d, host = make_ctx(cfg, seed, G, 5, P, max_new, page=64, flags=api.FLAG_DUMP_LOGITS, std=std)
+    gpu, glog = run_stepwise(d, prompts, Kp, K, T, seed, forced)
+    orc = ro.rollout_stepwise(host, prompts, Kp, K, max_new, T, seed, forced_len=forced, teacher=gpu["tokens"], keep_logits=True)
+    for k in ("len", "status", "sel", "sel_mask", "close_step"):
+        assert np.array_equal(gpu[k], orc[k]), k
+    assert set(glog.keys()) == set(orc["logits"].keys())
+    worst = max(rel_inf(glog[k], orc["logits"][k]) for k in glog)
+    assert worst < tol, worst
+    near = 0
+    for (r, s), zg in glog.items():
+        err = float(np.max(np.abs(zg - orc["logits"][(r, s)]))) / T
+        if orc["margins"][r, s] > 2 * err + 1e-3:
+            forced_here = s + 1 == orc["len"][r] and gpu["tokens"][r, s] == cfg["vocab"] - 1
+            assert forced_here or orc["oracle_tokens"][r, s] == gpu["tokens"][r, s], (r, s)
+        else:
+            near += 1
+    assert near <= len(glog) // 10, (near, len(glog))
+    cnt = d.counters()
+    assert cnt["n_generated_tokens"] == orc["n_generated_tokens"] and cnt["n_steps"] == orc["n_steps"]
+    d.close()
+
+
+def test_bf16_rollout_loop_equals_stepwise_and_is_deterministic():
+    """darts_rollout_host (async loop, stale row-count upper bounds) gives the same result as the step-by-step calls."""
+    from paper_2605_30859_b200 import api
+    cfg = dict(SMALL)
+    seed, G, P, max_new, K = 8, 4, 64, 48, 2
+    prompts = wl.make_prompts(G, P, cfg["vocab"], seed)
+    Kp = np.full(G, 4, dtype=np.int32)
+    forced = wl.make_forced_len(Kp, dict(kind="lognormal", mu=3.0, sigma=0.6, lo=2, hi=48), seed)
+    d, _ = make_ctx(cfg, seed, G, 4, P, max_new, page=64, flags=api.FLAG_DUMP_LOGITS, std=0.08)
+    a, _ = run_stepwise(d, list(prompts), Kp, K, 1.0, 3, forced)
+    b = d.rollout_host(prompts, Kp, K, max_new, 1.0, 3, forced_len=forced)
+    c = d.rollout_host(prompts, Kp, K, max_new, 1.0, 3, forced_len=forced)
+    for k in ("tokens", "len", "status", "sel", "sel_mask"):
+        assert np.array_equal(a[k], b[k]), k
+        assert np.array_equal(b[k], c[k]), k
+    assert np.any(b["status"] == PRUNED)
+    d.close()

@@ -1,0 +1,54 @@
+"""-m gpu parity of the tcgen05/TMEM GEMM (through the C-ABI hook darts_debug_gemm_bf16) against oracle.linear."""
+import numpy as np
+import pytest
+import torch
+
+from oracle.linear import linear
+from paper_2605_30859_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    from paper_2605_30859_b200 import api
+    d = api.Darts(dict(cfg=dict(wl.CONFIGS["c2"]["model"])), page_size=64, n_pages=64, max_rows=8, max_prompts=2, max_prompt_len=64, max_new=64)
+    yield d
+    d.close()
+
+
+def _mk(shape, seed, scale=1.0):
+    g = torch.Generator(device="cuda").manual_seed(seed)
+    return (torch.randn(*shape, generator=g, device="cuda") * scale).to(torch.bfloat16)
+
+
+@pytest.mark.parametrize("rows,N,K,S", [
+    (1, 128, 64, 1),          # one row, one k-block
+    (16, 256, 256, 1),
+    (37, 132, 192, 3),        # ragged rows (3 boxes of 16), ragged N (tail tile, N % 128 != 0), ragged split
+    (128, 384, 512, 2),       # full tile
+    (200, 512, 1024, 4),      # two row tiles, second one ragged
+    (300, 1000, 2560, 5),     # three row tiles, K of config 3
+    (64, 6144, 2560, 4),      # config-3 QKV shape at 64 rows
+])
+def test_gemm_matches_oracle(ctx, rows, N, K, S):
+    X, W = _mk((rows, K), rows + N), _mk((N, K), K + S, 0.05)
+    got = ctx.debug_gemm_bf16(X, W, split_k=S).cpu().numpy().astype(np.float64)
+    ref = linear(X.float().cpu().numpy(), W.float().cpu().numpy())
+    # bf16 products are exact in fp32; only the fp32 accumulation order differs: ~K * 2^-24 relative to sum |x w|
+    tol = 4 * K * 2.0 ** -24 * float(np.max(np.abs(X.float().cpu().numpy()) @ np.abs(W.float().cpu().numpy()).T))
+    assert np.max(np.abs(got - ref)) <= tol, (np.max(np.abs(got - ref)), tol)
+
+
+def test_gemm_is_deterministic_and_split_order_fixed(ctx):
+    X, W = _mk((50, 1024), 1), _mk((256, 1024), 2, 0.05)
+    a = ctx.debug_gemm_bf16(X, W, split_k=4)
+    b = ctx.debug_gemm_bf16(X, W, split_k=4)
+    assert torch.equal(a, b)
+
+
+def test_gemm_rejects_bad_shapes(ctx):
+    from paper_2605_30859_b200 import api
+    with pytest.raises(api.DartsError) as e:
+        ctx.debug_gemm_bf16(_mk((4, 100), 0), _mk((8, 100), 1))
+    assert e.value.code == api.ERR_UNSUPPORTED

@@ -160,3 +160,14 @@ def test_moe_route_tie_prefers_lower_expert_id():
     layer = dict(wr=np.zeros((5, 3)))                       # all logits equal -> experts 0,1
     ids, w = tr.moe_route(layer, cfg, np.ones(3))
     assert ids.tolist() == [0, 1] and np.allclose(w, 0.5)
+
+
+def test_linear_matches_written_out_sum():
+    """oracle.linear: y[r,n] = sum_k x[r,k] W[n,k] (non-square W so a transposed operand cannot pass)."""
+    from oracle.linear import linear, linear_loops
+    rng = np.random.default_rng(0)
+    x, W = rng.standard_normal((3, 5)), rng.standard_normal((4, 5))
+    y = linear(x, W)
+    assert y.shape == (3, 4)
+    assert np.allclose(y, linear_loops(x, W), rtol=0, atol=1e-13)
+    assert abs(y[1, 2] - sum(x[1, k] * W[2, k] for k in range(5))) < 1e-13
