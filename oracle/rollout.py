@@ -30,6 +30,7 @@ import numpy as np
 from . import ACTIVE, VALID, TRUNC, PRUNED, MODE_AUTO
 from .sampling import sample_token
 from .selection import apply_stop, compact, group_mode, group_rule, sel_mask, select_dual
+from . import transformer as _tf
 from .transformer import decode_one, prefill
 
 
@@ -61,9 +62,12 @@ def rollout_stepwise(model, prompts, Kp, K, max_new, T, seed, forced_len=None, L
     M_up = 2 * K if M_up is None else M_up
     G, Kp, offs, R, row_i, row_j = _setup(prompts, Kp)
 
-    z0, kv0 = [], []
+    z0, kv0, gap0 = [], [], []
+    router_gap = {}                                          # (r, s) -> smallest router gap seen (R13; MoE models only)
     for i in range(G):                                       # one prefill per prompt (:134)
+        _tf.ROUTER_GAPS = [] if keep_logits else None
         z, kv = prefill(model, prompts[i])
+        gap0.append(min(_tf.ROUTER_GAPS) if _tf.ROUTER_GAPS else np.inf)
         z0.append(z)
         kv0.append(kv)
     kv = [[(a.copy(), b.copy()) for a, b in kv0[row_i[r]]] for r in range(R)]  # private copies
@@ -87,10 +91,14 @@ def rollout_stepwise(model, prompts, Kp, K, max_new, T, seed, forced_len=None, L
             i, j = int(row_i[r]), int(row_j[r])
             if s == 0:
                 z = z0[i]
+                gap = gap0[i]
             else:
+                _tf.ROUTER_GAPS = [] if keep_logits else None
                 z = decode_one(model, kv[r], tokens[r, s - 1], len(prompts[i]) + s - 1)
+                gap = min(_tf.ROUTER_GAPS) if _tf.ROUTER_GAPS else np.inf
             if keep_logits and (logit_filter is None or logit_filter(r, s)):
                 logits[(r, s)] = z.copy()
+                router_gap[(r, s)] = gap
             tok, margin = sample_token(z, T, seed, i, j, s)
             otok[r, s], margins[r, s] = tok, margin
             if teacher is not None:
@@ -111,7 +119,8 @@ def rollout_stepwise(model, prompts, Kp, K, max_new, T, seed, forced_len=None, L
 
     out = dict(tokens=tokens, len=length, status=status, sel=sel, sel_mask=mask,
                close_step=close_step, n_steps=s, margins=margins, oracle_tokens=otok,
-               logits=logits, n_active_hist=n_active_hist)
+               logits=logits, router_gap=router_gap, n_active_hist=n_active_hist)
+    _tf.ROUTER_GAPS = None
     return _finish(out, G, K, offs)
 
 

@@ -104,11 +104,20 @@ def qkv_project(layer, cfg, a, pos):
     return q, k, v
 
 
+# DESIGN.md R13: when this is a list, every routing decision appends the probability gap between the
+# k-th and (k+1)-th expert (tests use it to set aside rows whose discrete expert choice is a near-tie).
+# Pure instrumentation: it does not change any value computed here.
+ROUTER_GAPS = None
+
+
 def moe_route(layer, cfg, b):
     """b [d] -> (expert ids [top_k] in selection order, weights [top_k] summing to 1)."""
     p = softmax(f64(layer["wr"]) @ b)
     # top-k by p, ties -> lower expert id: stable sort of -p keeps lower ids first
     order = np.argsort(-p, kind="stable")[: cfg["top_k"]]
+    if ROUTER_GAPS is not None and cfg["top_k"] < len(p):
+        ps = np.sort(p)[::-1]
+        ROUTER_GAPS.append(float(ps[cfg["top_k"] - 1] - ps[cfg["top_k"]]))
     w = p[order] / np.sum(p[order])
     return order, w
 

@@ -101,25 +101,30 @@ size_t carve(darts_ctx *c, void *base) {
     c->prompt_tokens = k.take<int32_t>(G * rt.max_prompt_len);
     c->slot_cs = k.take<float2>(A * (m.head_dim / 2));
     c->h = k.take<float>(A * m.d_model);
+    if (m.n_experts) {
+      size_t RK = A * m.top_k;
+      c->moe_logits = k.take<float>(A * m.n_experts);
+      c->moe_eid = k.take<int32_t>(RK);
+      c->moe_pos = k.take<int32_t>(RK);
+      c->moe_w = k.take<float>(RK);
+    }
     if (c->tc_path) {
-      size_t maxN = std::max<size_t>(std::max<size_t>(c->n_qkv, 2 * F), m.d_model);
+      size_t maxN = std::max<size_t>(std::max<size_t>(c->n_qkv, 2 * F), m.n_experts ? (size_t)m.top_k * m.d_model : (size_t)m.d_model);
       c->part_bytes = std::max<size_t>(A * maxN * 4, (size_t)64 << 20);
       c->part = k.take<float>(c->part_bytes / 4);
       c->top2 = k.take<float>((size_t)ceil_div(m.vocab, 128) * R * 4);
       if (rt.flags & DARTS_FLAG_DUMP_LOGITS) c->logits = k.take<float>(R * m.vocab);
       if (m.n_experts) {
         size_t RK = A * m.top_k;
-        c->moe_eid = k.take<int32_t>(RK);
-        c->moe_pos = k.take<int32_t>(RK);
         c->moe_tok = k.take<int32_t>(RK);
-        c->moe_w = k.take<float>(RK);
         c->moe_off = k.take<int32_t>(m.n_experts + 1);
-        c->moe_cnt = k.take<int32_t>(m.n_experts);
+        c->moe_cnt = k.take<int32_t>((size_t)m.n_layers * m.n_experts);
         c->xs = k.take<char>(RK * m.d_model * 2);
       }
     } else {
       c->qkv32 = k.take<float>(A * c->n_qkv);
-      c->gu32 = k.take<float>(A * 2 * F);
+      if (m.n_experts) c->moe_y = k.take<float>(A * m.top_k * m.d_model);
+      else c->gu32 = k.take<float>(A * 2 * F);
       c->logits = k.take<float>(R * m.vocab);
     }
     c->z0 = k.take<float>(G * m.vocab);
@@ -146,6 +151,11 @@ darts_status validate(const darts_model_desc *m, const darts_runtime_desc *rt, c
     snprintf(err, n, "runtime sizes must be positive"); return DARTS_ERR_INVALID_ARG;
   }
   if (m->vocab > 0 && m->n_experts == 0 && m->ffn <= 0) { snprintf(err, n, "dense model needs ffn > 0"); return DARTS_ERR_INVALID_ARG; }
+  if (m->n_experts < 0 || (m->n_experts > 0 && (m->top_k <= 0 || m->top_k > m->n_experts || m->top_k > 32 || m->expert_ffn <= 0))) {
+    snprintf(err, n, "MoE needs 0 < top_k <= min(n_experts, 32) and expert_ffn > 0"); return DARTS_ERR_INVALID_ARG;
+  }
+  if (m->n_experts > 256) { snprintf(err, n, "n_experts > 256"); return DARTS_ERR_UNSUPPORTED; }
+  if (m->vocab > 0 && m->d_model % 4) { snprintf(err, n, "d_model must be a multiple of 4"); return DARTS_ERR_UNSUPPORTED; }
   return DARTS_OK;
 }
 
@@ -207,6 +217,7 @@ darts_status forward_layers_tc(darts_ctx *c, int rows_ub, const int32_t *n_rows_
   const int d = m.d_model, qd = m.n_q_heads * m.head_dim, F = m.ffn, L = m.n_layers;
   TRY(launch_embed(c, c->slot_tok, 0, rows_ub, n_rows_dev));
   TRY(launch_rope_table(c, rows_ub, n_rows_dev));
+  TRY(launch_moe_begin_pass(c));
   TRY(launch_rmsnorm(c, c->h, c->attn_norm[0], c->xn, rows_ub, n_rows_dev));
   for (int l = 0; l < L; ++l) {
     TcGemm g = tc_gemm(c, &c->tm_xn, &c->tm_wqkv[l], c->n_qkv, d, rows_ub, n_rows_dev);

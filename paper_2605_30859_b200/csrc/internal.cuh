@@ -89,8 +89,8 @@ struct darts_ctx {
   CUtensorMap *tm_wqkv, *tm_wo, *tm_wgu, *tm_wd, *tm_wgu_e, *tm_wd_e;   // host arrays [n_layers]
   CUtensorMap tm_lm, tm_xn, tm_ao, tm_act, tm_xs, tm_hl;                      // activations: 16-row boxes
   // MoE (kernels_moe.cu)
-  int32_t *moe_eid, *moe_pos, *moe_off, *moe_cnt, *moe_tok;
-  float *moe_w;
+  int32_t *moe_eid, *moe_pos, *moe_off, *moe_cnt, *moe_tok;   // moe_cnt: [n_layers][E], zeroed once per forward pass
+  float *moe_w, *moe_logits, *moe_y;   // gates [rows*top_k]; router logits [rows][E]; generic path expert outputs [rows*top_k][d]
   void *xs;                      // expert-sorted copy of xn [max_rows * top_k][d]
   // tuned attention (kernels_attn_sm100.cu): per-step work list and split-KV partials
   int32_t *attn_items_pre, *attn_items_suf, *attn_nitems, *part_base, *part_cnt;
@@ -170,6 +170,7 @@ darts_status launch_attention(darts_ctx *c, int layer, const void *q, void *out,
 darts_status launch_silu_mul(darts_ctx *c, int rows_ub, const int32_t *n_rows_dev);
 darts_status launch_moe(darts_ctx *c, int layer, int rows_ub, const int32_t *n_rows_dev);
 darts_status launch_moe_tc(darts_ctx *c, int layer, const void *next_norm, int rows_ub, const int32_t *n_rows_dev);
+darts_status launch_moe_begin_pass(darts_ctx *c);
 darts_status launch_sample(darts_ctx *c, const float *logits, int step0, int rows_ub);
 darts_status launch_plan_decode(darts_ctx *c, int rows_ub);
 darts_status launch_plan_prefill(darts_ctx *c, int tok_begin, int n_tok, int g_begin, int g_end);
