@@ -201,8 +201,12 @@ darts_status darts_debug_set_last_tokens(darts_ctx *ctx, const int32_t *tokens_h
 
 /* Parity hook for the tcgen05 GEMM that carries every projection of the bf16 path:
  * C[rows][N] (fp32) = X[rows][K] . W[N][K]^T with bf16 X, W.  All pointers DEVICE.  split_k >= 1 K-splits are
- * computed as separate partials in `scratch` (>= split_k * rows * N floats) and added in split order.
+ * computed as separate partials in `scratch` (>= split_k * rows * N floats) and added in split order into C
+ * (C == NULL: leave the partials in `scratch`, no reduction).
  * Needs K % 64 == 0 and N % 4 == 0 (DARTS_ERR_UNSUPPORTED otherwise).  Asynchronous on the ctx stream. */
+/* split_k == 0 selects the stream-K weight-streaming kernel (the one the decode projections use); its pieces need
+ * darts_debug_gemm_scratch_floats(...) floats of scratch. */
+darts_status darts_debug_gemm_scratch_floats(darts_ctx *ctx, int32_t rows, int32_t N, int32_t K, int32_t split_k, size_t *out);
 darts_status darts_debug_gemm_bf16(darts_ctx *ctx, const void *X, const void *W, float *C, float *scratch, int32_t rows,
                                    int32_t N, int32_t K, int32_t split_k);
 

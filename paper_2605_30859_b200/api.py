@@ -83,6 +83,7 @@ darts_get_attention_times = _sig("darts_get_attention_times", _ctx, _vp, _i32, C
 darts_debug_logits = _sig("darts_debug_logits", _ctx, _i32, _vp)
 darts_debug_set_last_tokens = _sig("darts_debug_set_last_tokens", _ctx, _vp, _i32)
 darts_debug_gemm_bf16 = _sig("darts_debug_gemm_bf16", _ctx, _vp, _vp, _vp, _vp, _i32, _i32, _i32, _i32)
+darts_debug_gemm_scratch_floats = _sig("darts_debug_gemm_scratch_floats", _ctx, _i32, _i32, _i32, _i32, C.POINTER(C.c_size_t))
 darts_attn_load = _sig("darts_attn_load", _ctx, _i32, _i32, _i32, _vp, _vp, _vp, _vp, _vp)
 darts_attention = _sig("darts_attention", _ctx, _i32, _vp, _vp)
 
@@ -254,15 +255,20 @@ class Darts:
         t = np.ascontiguousarray(tokens, dtype=np.int32)
         self._check(darts_debug_set_last_tokens(self.ctx, _np_ptr(t), len(t)))
 
-    def debug_gemm_bf16(self, X, W, split_k=1):
-        """C = X @ W.T on the tcgen05 GEMM (bf16 device tensors X [rows,K], W [N,K]); returns fp32 [rows,N] on device."""
+    def debug_gemm_bf16(self, X, W, split_k=1, scratch=None, reduce=True):
+        """C = X @ W.T on the tcgen05 GEMM (bf16 device tensors X [rows,K], W [N,K]); returns fp32 [rows,N] on device
+        (reduce=False: only the split-K partials are computed, into `scratch`)."""
         rows, K = X.shape
         N = W.shape[0]
-        out = torch.empty(rows, N, dtype=torch.float32, device="cuda")
-        scratch = torch.empty(split_k * rows * N, dtype=torch.float32, device="cuda")
-        self._check(darts_debug_gemm_bf16(self.ctx, X.data_ptr(), W.data_ptr(), out.data_ptr(), scratch.data_ptr(), rows, N, K, split_k))
+        out = torch.empty(rows, N, dtype=torch.float32, device="cuda") if reduce else None
+        if scratch is None:
+            need = C.c_size_t()
+            self._check(darts_debug_gemm_scratch_floats(self.ctx, rows, N, K, split_k, C.byref(need)))
+            scratch = torch.empty(need.value, dtype=torch.float32, device="cuda")
+        self._check(darts_debug_gemm_bf16(self.ctx, X.data_ptr(), W.data_ptr(), out.data_ptr() if reduce else None, scratch.data_ptr(),
+                                          rows, N, K, split_k))
         self._scratch = scratch
-        return out
+        return out if reduce else scratch
 
     # ---- attention-only (config 2) -----------------------------------------------------------------
     def attn_load(self, G, P, Kp, k_prefix, v_prefix, suffix_len, k_suffix, v_suffix):

@@ -1,5 +1,7 @@
 // C-ABI entry points (include/darts.h): workspace carving, prefill, decode step, selection/compaction,
 // the rollout loop and result read-back.  Host logic only; every step of the path runs in the kernels.
+#include <stdlib.h>
+
 #include <algorithm>
 #include <new>
 #include <vector>
@@ -109,8 +111,17 @@ size_t carve(darts_ctx *c, void *base) {
       c->moe_w = k.take<float>(RK);
     }
     if (c->tc_path) {
+      // stream-K pieces [slots][rows][N]: whole-tile mode (1 slot) for the prefill-sized passes, up to 16 slots for decode rows
       size_t maxN = std::max<size_t>(std::max<size_t>(c->n_qkv, 2 * F), m.n_experts ? (size_t)m.top_k * m.d_model : (size_t)m.d_model);
-      c->part_bytes = std::max<size_t>(A * maxN * 4, (size_t)64 << 20);
+      size_t dec = 0;
+      const int sms = c->n_sms > 0 ? c->n_sms : 148;       // host-only sizing assumes a full B200; darts_create re-checks
+      int shapes[4][2] = {{c->n_qkv, m.d_model}, {m.d_model, qd_}, {m.n_experts ? 0 : 2 * m.ffn, m.d_model}, {m.n_experts ? 0 : m.d_model, m.ffn}};
+      for (auto &sh : shapes)
+        if (sh[0] > 0) {
+          dec = std::max(dec, (size_t)sk_plan(sms, sh[0], sh[1], rt.max_rows, 0, false).slots * R * sh[0] * 4);
+          dec = std::max(dec, (size_t)sk_plan(sms, sh[0], sh[1], (int)A, 0, true).slots * A * sh[0] * 4);
+        }
+      c->part_bytes = std::max<size_t>(std::max<size_t>(A * maxN * 4, dec), (size_t)64 << 20);
       c->part = k.take<float>(c->part_bytes / 4);
       c->top2 = k.take<float>((size_t)ceil_div(m.vocab, 128) * R * 4);
       if (rt.flags & DARTS_FLAG_DUMP_LOGITS) c->logits = k.take<float>(R * m.vocab);
@@ -118,6 +129,8 @@ size_t carve(darts_ctx *c, void *base) {
         size_t RK = A * m.top_k;
         c->moe_tok = k.take<int32_t>(RK);
         c->moe_off = k.take<int32_t>(m.n_experts + 1);
+        c->moe_rb = k.take<int32_t>(4 * ((size_t)m.n_experts + RK / SK_ROWBLOCK + 1));
+        c->moe_nrb = k.take<int32_t>(1);
         c->moe_cnt = k.take<int32_t>((size_t)m.n_layers * m.n_experts);
         c->xs = k.take<char>(RK * m.d_model * 2);
       }
@@ -202,13 +215,13 @@ darts_status forward_layers(darts_ctx *c, int rows_ub, const int32_t *n_rows_dev
   return DARTS_OK;
 }
 
-// Tensor-core path (bf16): every projection on tcgen05, split-K partials reduced inside the consumer kernels, the
-// residual add fused with the next RMSNorm.  Leaves xn = rmsnorm(h_L) * final_norm for the LM head.
-TcGemm tc_gemm(darts_ctx *c, const CUtensorMap *a, const CUtensorMap *b, int N, int K, int rows_ub, const int32_t *n_rows_dev) {
-  TcGemm g{};
-  g.a_map = a; g.b_map = b; g.C = c->part; g.N = N; g.K = K; g.rows_ub = rows_ub; g.n_rows_dev = n_rows_dev;
-  g.S = tc_pick_split(c, N, K, rows_ub, 0);
-  g.split_stride = (size_t)rows_ub * N;
+// Tensor-core path (bf16): every projection on the stream-K tcgen05 kernel, its pieces reduced inside the consumer
+// kernels, the residual add fused with the next RMSNorm.  Leaves xn = rmsnorm(h_L) * final_norm for the LM head.
+SkGemm sk_gemm(darts_ctx *c, const XMaps *x, const CUtensorMap *w, int N, int K, int rows_ub, const int32_t *n_rows_dev) {
+  SkGemm g{};
+  g.w_map = w; g.x_maps = x; g.C = c->part; g.N = N; g.rows_ub = rows_ub; g.n_rows_dev = n_rows_dev;
+  g.plan = sk_plan(c->n_sms, N, K, rows_ub, 0, n_rows_dev == nullptr);
+  g.slot_stride = (size_t)rows_ub * N;
   return g;
 }
 
@@ -220,21 +233,21 @@ darts_status forward_layers_tc(darts_ctx *c, int rows_ub, const int32_t *n_rows_
   TRY(launch_moe_begin_pass(c));
   TRY(launch_rmsnorm(c, c->h, c->attn_norm[0], c->xn, rows_ub, n_rows_dev));
   for (int l = 0; l < L; ++l) {
-    TcGemm g = tc_gemm(c, &c->tm_xn, &c->tm_wqkv[l], c->n_qkv, d, rows_ub, n_rows_dev);
-    TRY(launch_gemm_tc(c, g));
-    TRY(launch_rope_append_part(c, l, g.S, rows_ub, n_rows_dev));
+    SkGemm g = sk_gemm(c, &c->xm_xn, &c->tm_wqkv[l], c->n_qkv, d, rows_ub, n_rows_dev);
+    TRY(launch_gemm_sk(c, g));
+    TRY(launch_rope_append_sk(c, l, sk_view(g), rows_ub, n_rows_dev));
     TRY(launch_attention(c, l, c->q, c->ao, rows_ub, n_rows_dev));
-    g = tc_gemm(c, &c->tm_ao, &c->tm_wo[l], d, qd, rows_ub, n_rows_dev);
-    TRY(launch_gemm_tc(c, g));
-    TRY(launch_add_rmsnorm(c, c->part, g.S, g.split_stride, c->mlp_norm[l], rows_ub, n_rows_dev));
+    g = sk_gemm(c, &c->xm_ao, &c->tm_wo[l], d, qd, rows_ub, n_rows_dev);
+    TRY(launch_gemm_sk(c, g));
+    TRY(launch_add_rmsnorm_sk(c, sk_view(g), c->mlp_norm[l], rows_ub, n_rows_dev));
     const void *next_norm = l + 1 < L ? c->attn_norm[l + 1] : c->final_norm;
     if (m.n_experts == 0) {
-      g = tc_gemm(c, &c->tm_xn, &c->tm_wgu[l], 2 * F, d, rows_ub, n_rows_dev);
-      TRY(launch_gemm_tc(c, g));
-      TRY(launch_silu_mul_part(c, g.S, rows_ub, n_rows_dev));
-      g = tc_gemm(c, &c->tm_act, &c->tm_wd[l], d, F, rows_ub, n_rows_dev);
-      TRY(launch_gemm_tc(c, g));
-      TRY(launch_add_rmsnorm(c, c->part, g.S, g.split_stride, next_norm, rows_ub, n_rows_dev));
+      g = sk_gemm(c, &c->xm_xn, &c->tm_wgu[l], 2 * F, d, rows_ub, n_rows_dev);
+      TRY(launch_gemm_sk(c, g));
+      TRY(launch_silu_mul_sk(c, sk_view(g), rows_ub, n_rows_dev));
+      g = sk_gemm(c, &c->xm_act, &c->tm_wd[l], d, F, rows_ub, n_rows_dev);
+      TRY(launch_gemm_sk(c, g));
+      TRY(launch_add_rmsnorm_sk(c, sk_view(g), next_norm, rows_ub, n_rows_dev));
     } else {
       TRY(launch_moe_tc(c, l, next_norm, rows_ub, n_rows_dev));
     }
@@ -270,9 +283,15 @@ darts_status make_maps(darts_ctx *c) {
   TRY(tc_make_map(c, &c->tm_lm, c->lm_head, m.vocab, d, 128));
   TRY(tc_make_map(c, &c->tm_xn, c->xn, c->act_rows, d, 16));
   TRY(tc_make_map(c, &c->tm_ao, c->ao, c->act_rows, qd, 16));
+  TRY(tc_make_xmaps(c, &c->xm_xn, c->xn, c->act_rows, d));
+  TRY(tc_make_xmaps(c, &c->xm_ao, c->ao, c->act_rows, qd));
   TRY(tc_make_map(c, &c->tm_hl, c->hlast, c->rt.max_prompts, d, 16));
-  if (m.n_experts == 0) TRY(tc_make_map(c, &c->tm_act, c->act, c->act_rows, m.ffn, 16));
-  else {
+  if (m.n_experts == 0) {
+    TRY(tc_make_map(c, &c->tm_act, c->act, c->act_rows, m.ffn, 16));
+    TRY(tc_make_xmaps(c, &c->xm_act, c->act, c->act_rows, m.ffn));
+  } else {
+    TRY(tc_make_xmaps(c, &c->xm_act, c->act, (long long)c->act_rows * m.top_k, m.expert_ffn));
+    TRY(tc_make_xmaps(c, &c->xm_xs, c->xs, (long long)c->act_rows * m.top_k, d));
     TRY(tc_make_map(c, &c->tm_act, c->act, (long long)c->act_rows * m.top_k, m.expert_ffn, 16));
     TRY(tc_make_map(c, &c->tm_xs, c->xs, (long long)c->act_rows * m.top_k, d, 16));
   }
@@ -411,6 +430,7 @@ darts_status darts_create(const darts_model_desc *m, const darts_weights *w, con
   if (need > rt->workspace_bytes) FAIL(c, DARTS_ERR_WORKSPACE_TOO_SMALL, "workspace %zu < %zu bytes", rt->workspace_bytes, need);
   if (((uintptr_t)rt->workspace & 255) != 0) FAIL(c, DARTS_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
   c->has_weights = m->vocab > 0;
+  c->use_pdl = getenv("DARTS_NO_PDL") == nullptr;
   if (c->has_weights) {
     int L = m->n_layers;
     c->embed = w->embed; c->final_norm = w->final_norm; c->lm_head = w->lm_head;
@@ -638,18 +658,38 @@ darts_status darts_debug_set_last_tokens(darts_ctx *c, const int32_t *tokens_hos
   return DARTS_OK;
 }
 
+darts_status darts_debug_gemm_scratch_floats(darts_ctx *c, int32_t rows, int32_t N, int32_t K, int32_t split_k, size_t *out) {
+  if (!c || !out || rows <= 0 || N <= 0 || K <= 0 || split_k < 0) return DARTS_ERR_INVALID_ARG;
+  if (!tc_shape_ok(N, K)) FAIL(c, DARTS_ERR_UNSUPPORTED, "tcgen05 GEMM needs K %% 64 == 0, N %% 4 == 0");
+  int slots = split_k > 0 ? split_k : sk_plan(c->n_sms, N, K, rows, 0, true).slots;
+  *out = (size_t)slots * rows * N;
+  return DARTS_OK;
+}
+
 darts_status darts_debug_gemm_bf16(darts_ctx *c, const void *X, const void *W, float *C, float *scratch, int32_t rows, int32_t N, int32_t K,
                                    int32_t split_k) {
   if (!c) return DARTS_ERR_INVALID_ARG;
   if (c->sticky) return c->sticky;
-  if (!X || !W || !C || !scratch || rows <= 0 || N <= 0 || K <= 0 || split_k < 1) FAIL(c, DARTS_ERR_INVALID_ARG, "NULL / non-positive argument");
+  if (!X || !W || !scratch || rows <= 0 || N <= 0 || K <= 0 || split_k < 0) FAIL(c, DARTS_ERR_INVALID_ARG, "NULL / non-positive argument");
   if (!tc_shape_ok(N, K) || split_k > K / 64) FAIL(c, DARTS_ERR_UNSUPPORTED, "tcgen05 GEMM needs K %% 64 == 0, N %% 4 == 0, split_k <= K/64");
   CUtensorMap ta, tb;
+  if (split_k == 0) {                                        // the stream-K weight-streaming kernel; scratch >= slots * rows * N floats
+    XMaps xm;
+    TRY(tc_make_xmaps(c, &xm, X, rows, K));
+    TRY(tc_make_map(c, &tb, W, N, K, 128));
+    SkGemm g{};
+    g.w_map = &tb; g.x_maps = &xm; g.C = scratch; g.N = N; g.rows_ub = rows; g.slot_stride = (size_t)rows * N;
+    g.plan = sk_plan(c->n_sms, N, K, rows, 0, true);
+    TRY(launch_gemm_sk(c, g));
+    if (!C) return DARTS_OK;
+    return launch_sk_reduce(c, sk_view(g), C, rows);
+  }
   TRY(tc_make_map(c, &ta, X, rows, K, 16));
   TRY(tc_make_map(c, &tb, W, N, K, 128));
   TcGemm g{};
   g.a_map = &ta; g.b_map = &tb; g.C = scratch; g.N = N; g.K = K; g.S = split_k; g.rows_ub = rows; g.split_stride = (size_t)rows * N;
   TRY(launch_gemm_tc(c, g));
+  if (!C) return DARTS_OK;                                   // partials only (timing the GEMM kernel alone)
   return launch_sum_partials(c, scratch, C, split_k, (size_t)rows * N);
 }
 

@@ -40,6 +40,8 @@ __device__ __forceinline__ size_t kv_elem(const KvGeom &g, int page, int head, i
   return (size_t)page * g.page_elems + ((size_t)head * 2 + kv) * g.tile_elems + (size_t)tok * g.hd + dd;
 }
 
+struct XMaps { CUtensorMap m[5]; };   // one activation matrix [rows][K] with boxes of 16, 32, 64, 128, 256 rows
+
 struct darts_ctx {
   darts_model_desc m;
   darts_runtime_desc rt;
@@ -83,13 +85,15 @@ struct darts_ctx {
   int32_t attn_rows;
   // tensor-core path (bf16, kernels_gemm_tc.cu): split-K partial buffer, LM-head top-2 partials, tensor maps
   bool tc_path;                  // every GEMM of this model runs on tcgen05
+  bool use_pdl;                  // launch the stream-K GEMMs as programmatic dependents (DARTS_NO_PDL=1 in the environment disables)
   float *part;                   // [S][rows][N] fp32 partials of the GEMM in flight
   size_t part_bytes;
   float *top2;                   // float4 [vocab tiles][max_rows]
   CUtensorMap *tm_wqkv, *tm_wo, *tm_wgu, *tm_wd, *tm_wgu_e, *tm_wd_e;   // host arrays [n_layers]
   CUtensorMap tm_lm, tm_xn, tm_ao, tm_act, tm_xs, tm_hl;                      // activations: 16-row boxes
+  XMaps xm_xn, xm_ao, xm_act, xm_xs;                                            // the same matrices for the stream-K kernel
   // MoE (kernels_moe.cu)
-  int32_t *moe_eid, *moe_pos, *moe_off, *moe_cnt, *moe_tok;   // moe_cnt: [n_layers][E], zeroed once per forward pass
+  int32_t *moe_eid, *moe_pos, *moe_off, *moe_cnt, *moe_tok, *moe_rb, *moe_nrb;   // moe_rb: row blocks {row0, nrows, expert, -}   // moe_cnt: [n_layers][E], zeroed once per forward pass
   float *moe_w, *moe_logits, *moe_y;   // gates [rows*top_k]; router logits [rows][E]; generic path expert outputs [rows*top_k][d]
   void *xs;                      // expert-sorted copy of xn [max_rows * top_k][d]
   // tuned attention (kernels_attn_sm100.cu): per-step work list and split-KV partials
@@ -147,6 +151,12 @@ template <typename T> __device__ __forceinline__ T from_f(float x);
 template <> __device__ __forceinline__ float from_f<float>(float x) { return x; }
 template <> __device__ __forceinline__ __nv_bfloat16 from_f<__nv_bfloat16>(float x) { return __float2bfloat16_rn(x); }
 
+// Programmatic dependent launch (PDL): a kernel that calls pdl_trigger() lets the NEXT kernel of the stream start its
+// prologue (and, for the GEMMs, its weight prefetch) while this one is still running; a kernel launched with the PDL
+// attribute must call pdl_wait() before it touches anything an earlier kernel wrote.  Both are no-ops otherwise.
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 __device__ __forceinline__ float warp_sum(float v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
@@ -196,8 +206,44 @@ struct TcGemm {
 };
 darts_status launch_gemm_tc(darts_ctx *c, const TcGemm &g);
 darts_status tc_make_map(darts_ctx *c, CUtensorMap *out, const void *base, long long rows, int K, int box_rows);
+darts_status tc_make_xmaps(darts_ctx *c, XMaps *out, const void *base, long long rows, int K);
 bool tc_shape_ok(int N, int K);
 int tc_pick_split(const darts_ctx *c, int N, int K, int rows_ub, int n_groups);
+// stream-K weight-streaming GEMM (kernels_gemm_sk.cu)
+#define SK_ROWBLOCK 256            // activation rows per MMA N block
+struct SkPlan { int nkb, n_wtiles, P, unit_tile, slots, stage_bytes, n_stages, tm_cols; };
+struct SkGemm {
+  const CUtensorMap *w_map;           // weights [N (x groups)][K], 128-row boxes
+  const XMaps *x_maps;
+  float *C;                           // pieces [slot][rows][N]
+  size_t slot_stride;
+  int N, rows_ub;
+  const int32_t *n_rows_dev;
+  const int32_t *rb_list, *n_rb_dev;  // grouped: {row0, nrows, group id, -} per row block, count on the device
+  int w_rows_per_group;               // grouped: weight row base of a block = group id * w_rows_per_group
+  SkPlan plan;
+};
+// What a consumer needs to add the pieces of element (row, col) in slot order.
+struct SkView {
+  const float *part;
+  size_t slot_stride;
+  int N, nkb, n_wtiles, P, unit_tile;
+};
+// CTA that owns unit u when T units are cut into P ranges [c*T/P, (c+1)*T/P)
+__host__ __device__ __forceinline__ int sk_owner(int u, int P, int T) { return ((u + 1) * P - 1) / T; }
+__host__ __device__ __forceinline__ int sk_npieces(const SkView &v, int n_rb, int col, int row) {
+  if (v.unit_tile) return 1;
+  int T = v.n_wtiles * n_rb * v.nkb;
+  int t = (col >> 7) * n_rb + row / SK_ROWBLOCK;
+  return sk_owner(t * v.nkb + v.nkb - 1, v.P, T) - sk_owner(t * v.nkb, v.P, T) + 1;
+}
+SkPlan sk_plan(int n_sms, int N, int K, int rows_ub, int n_rb_ub_grouped, bool rows_exact);
+darts_status launch_gemm_sk(darts_ctx *c, const SkGemm &g);
+darts_status launch_sk_reduce(darts_ctx *c, const SkView &v, float *out, int rows);
+inline SkView sk_view(const SkGemm &g) { return SkView{g.C, g.slot_stride, g.N, g.plan.nkb, g.plan.n_wtiles, g.plan.P, g.plan.unit_tile}; }
+darts_status launch_add_rmsnorm_sk(darts_ctx *c, const SkView &v, const void *w, int rows_ub, const int32_t *n_rows_dev);
+darts_status launch_silu_mul_sk(darts_ctx *c, const SkView &v, int rows_ub, const int32_t *n_rows_dev);
+darts_status launch_rope_append_sk(darts_ctx *c, int layer, const SkView &v, int rows_ub, const int32_t *n_rows_dev);
 // consumers of the split-K partials (kernels_fused.cu)
 darts_status launch_rope_append_part(darts_ctx *c, int layer, int S, int rows_ub, const int32_t *n_rows_dev);
 darts_status launch_add_rmsnorm(darts_ctx *c, const float *part, int S, size_t split_stride, const void *w, int rows_ub, const int32_t *n_rows_dev);

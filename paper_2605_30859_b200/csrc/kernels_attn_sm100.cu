@@ -312,6 +312,7 @@ __global__ void __launch_bounds__(THREADS, 2) attn_main_k(Params p) {
 __global__ void attn_merge_k(const float *__restrict__ part_ml, const float *__restrict__ part_acc, const int32_t *__restrict__ part_base,
                              const int32_t *__restrict__ part_cnt, __nv_bfloat16 *__restrict__ out, int Hq, float c,
                              const int32_t *n_rows_dev, int rows_ub) {
+  pdl_trigger();
   int slot = blockIdx.x;
   int R = n_rows_dev ? min(*n_rows_dev, rows_ub) : rows_ub;
   if (slot >= R) return;

@@ -41,6 +41,7 @@ darts_status launch_embed(darts_ctx *c, const int32_t *slot_tok, int, int rows_u
 template <typename T>
 __global__ void rmsnorm_k(const float *__restrict__ h, const T *__restrict__ w, T *__restrict__ out, int d, float eps,
                           const int32_t *n_rows_dev, int rows_ub) {
+  pdl_trigger();
   int slot = blockIdx.x;
   if (slot >= live_rows(n_rows_dev, rows_ub)) return;
   const float *x = h + (size_t)slot * d;

@@ -3,6 +3,8 @@
 //   add_rmsnorm    h += sum_s P_s (O-proj / down-proj residual), then xn = rmsnorm(h) * w for the next GEMM
 //   silu_mul_part  act = silu(sum_s gate_s) * (sum_s up_s)
 //   (rope_append_k in kernels_basic.cu does the same for the QKV partials)
+#include <algorithm>
+
 #include "internal.cuh"
 
 namespace {
@@ -88,6 +90,147 @@ __global__ void sum_partials_k(const float *__restrict__ part, float *__restrict
   out[i] = v;
 }
 
+// ---- consumers of the stream-K pieces (kernels_gemm_sk.cu): element (row, col) = sum of its tile's pieces in slot order.
+
+// Piece loads are issued four at a time before their adds (memory-level parallelism at a low register cost, so that
+// occupancy hides the rest of the latency); the adds run in slot order.
+__device__ __forceinline__ float4 sk_sum4(const SkView &v, int np, size_t idx) {
+  const float4 *p = reinterpret_cast<const float4 *>(v.part + idx);
+  const size_t st = v.slot_stride / 4;
+  float4 a = __ldg(p);
+  for (int s0 = 1; s0 < np; s0 += 4) {
+    float4 x[4];
+#pragma unroll
+    for (int s = 0; s < 4; ++s)
+      if (s0 + s < np) x[s] = __ldg(p + (size_t)(s0 + s) * st);
+#pragma unroll
+    for (int s = 0; s < 4; ++s)
+      if (s0 + s < np) { a.x += x[s].x; a.y += x[s].y; a.z += x[s].z; a.w += x[s].w; }
+  }
+  return a;
+}
+
+__device__ __forceinline__ uint2 pack4_bf16(float a, float b, float c, float d) {
+  __nv_bfloat162 o0 = __floats2bfloat162_rn(a, b), o1 = __floats2bfloat162_rn(c, d);
+  uint2 o;
+  o.x = *reinterpret_cast<uint32_t *>(&o0);
+  o.y = *reinterpret_cast<uint32_t *>(&o1);
+  return o;
+}
+
+// h[slot] += pieces;  out = rmsnorm(h[slot]) * w.   One CTA per slot, one float4 per thread per pass (d % 4 == 0).
+__global__ void __launch_bounds__(256) add_rmsnorm_sk_k(float *__restrict__ h, SkView v, const __nv_bfloat16 *__restrict__ w,
+                                                        __nv_bfloat16 *__restrict__ out, int d, float eps, const int32_t *n_rows_dev, int rows_ub) {
+  pdl_trigger();
+  const int slot = blockIdx.x, live = live_rows(n_rows_dev, rows_ub);
+  if (slot >= live) return;
+  const int n_rb = (live + SK_ROWBLOCK - 1) / SK_ROWBLOCK;
+  float4 *hr = reinterpret_cast<float4 *>(h + (size_t)slot * d);
+  float ss = 0.f;
+  for (int k = threadIdx.x; k < d / 4; k += blockDim.x) {
+    float4 a = sk_sum4(v, sk_npieces(v, n_rb, 4 * k, slot), (size_t)slot * d + 4 * k);
+    float4 x = hr[k];
+    x.x += a.x; x.y += a.y; x.z += a.z; x.w += a.w;
+    hr[k] = x;
+    ss += x.x * x.x + x.y * x.y + x.z * x.z + x.w * x.w;
+  }
+  __shared__ float red[32];
+  ss = warp_sum(ss);
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = ss;
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    float t = threadIdx.x < (blockDim.x >> 5) ? red[threadIdx.x] : 0.f;
+    t = warp_sum(t);
+    if (threadIdx.x == 0) red[0] = t;
+  }
+  __syncthreads();
+  const float r = 1.0f / sqrtf(red[0] / d + eps);
+  for (int k = threadIdx.x; k < d / 4; k += blockDim.x) {
+    float4 x = hr[k];                                       // written by this thread above
+    const __nv_bfloat162 *wp = reinterpret_cast<const __nv_bfloat162 *>(w + 4 * k);
+    float2 w0 = __bfloat1622float2(wp[0]), w1 = __bfloat1622float2(wp[1]);
+    *reinterpret_cast<uint2 *>(out + (size_t)slot * d + 4 * k) = pack4_bf16(x.x * r * w0.x, x.y * r * w0.y, x.z * r * w1.x, x.w * r * w1.y);
+  }
+}
+
+// act[slot][k] = silu(g) * u with g = pieces(slot, k), u = pieces(slot, F + k)
+__global__ void __launch_bounds__(256) silu_mul_sk_k(SkView v, __nv_bfloat16 *__restrict__ act, int F, const int32_t *n_rows_dev, int rows_ub) {
+  pdl_trigger();
+  const int slot = blockIdx.y, live = live_rows(n_rows_dev, rows_ub);
+  if (slot >= live) return;
+  const int k = (blockIdx.x * blockDim.x + threadIdx.x) * 4;
+  if (k >= F) return;
+  const int n_rb = (live + SK_ROWBLOCK - 1) / SK_ROWBLOCK;
+  const size_t row = (size_t)slot * 2 * F;
+  float4 g = sk_sum4(v, sk_npieces(v, n_rb, k, slot), row + k), u = sk_sum4(v, sk_npieces(v, n_rb, F + k, slot), row + F + k);
+  auto f = [](float gg, float uu) { return gg / (1.0f + expf(-gg)) * uu; };
+  *reinterpret_cast<uint2 *>(act + (size_t)slot * F + k) = pack4_bf16(f(g.x, u.x), f(g.y, u.y), f(g.z, u.z), f(g.w, u.w));
+}
+
+// (QK-norm) + RoPE + KV append from the QKV pieces.  One warp per (slot, head); lane l owns elements 4l..4l+3 of the
+// head's rotate-half pairs: x1 = head[4j..], x2 = head[hd/2 + 4j..] for j < hd/8 (hd in {64, 128, 256}; hd % 8 == 0).
+__global__ void __launch_bounds__(128) rope_append_sk_k(SkView v, __nv_bfloat16 *__restrict__ q_out, __nv_bfloat16 *__restrict__ kv_layer,
+                                                       const int32_t *__restrict__ slot_dst_page, const int32_t *__restrict__ slot_dst_off,
+                                                       const float2 *__restrict__ cs, const __nv_bfloat16 *__restrict__ q_norm,
+                                                       const __nv_bfloat16 *__restrict__ k_norm, int Hq, int Hkv, int hd, float eps, KvGeom geo,
+                                                       const int32_t *n_rows_dev, int rows_ub) {
+  pdl_trigger();
+  const int slot = blockIdx.y, live = live_rows(n_rows_dev, rows_ub);
+  if (slot >= live) return;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int head = blockIdx.x * 4 + warp;
+  if (head >= Hq + 2 * Hkv) return;
+  const int n_rb = (live + SK_ROWBLOCK - 1) / SK_ROWBLOCK;
+  const int half = hd >> 1, col0 = head * hd;
+  const size_t row = (size_t)slot * (Hq + 2 * Hkv) * hd + col0;
+  const int page = slot_dst_page[slot], off = slot_dst_off[slot];
+  const bool is_q = head < Hq, is_v = head >= Hq + Hkv;
+  if (!is_q && page < 0) return;
+  const bool act = lane < half / 4;                        // hd <= 256: one pass, the head lives in <= 32 lanes
+  const int p = 4 * lane;
+  float a1[4] = {0.f, 0.f, 0.f, 0.f}, a2[4] = {0.f, 0.f, 0.f, 0.f};
+  if (act) {
+    float4 x1 = sk_sum4(v, sk_npieces(v, n_rb, col0 + p, slot), row + p);
+    float4 x2 = sk_sum4(v, sk_npieces(v, n_rb, col0 + half + p, slot), row + half + p);
+    a1[0] = x1.x; a1[1] = x1.y; a1[2] = x1.z; a1[3] = x1.w;
+    a2[0] = x2.x; a2[1] = x2.y; a2[2] = x2.z; a2[3] = x2.w;
+  }
+  if (is_v) {
+    if (act) {
+#pragma unroll
+      for (int e = 0; e < 4; ++e) {
+        kv_layer[kv_elem(geo, page, head - Hq - Hkv, 1, off, p + e)] = __float2bfloat16_rn(a1[e]);
+        kv_layer[kv_elem(geo, page, head - Hq - Hkv, 1, off, half + p + e)] = __float2bfloat16_rn(a2[e]);
+      }
+    }
+    return;
+  }
+  const __nv_bfloat16 *nw = is_q ? q_norm : k_norm;
+  if (nw) {                                                // per-head RMSNorm (warp-uniform branch)
+    float ss = 0.f;
+#pragma unroll
+    for (int e = 0; e < 4; ++e) ss += a1[e] * a1[e] + a2[e] * a2[e];
+    ss = warp_sum(ss);
+    const float r = 1.0f / sqrtf(ss / hd + eps);
+    if (act) {
+#pragma unroll
+      for (int e = 0; e < 4; ++e) { a1[e] *= r * __bfloat162float(nw[p + e]); a2[e] *= r * __bfloat162float(nw[half + p + e]); }
+    }
+  }
+  if (!act) return;
+  __nv_bfloat16 *qdst = q_out + (size_t)slot * Hq * hd + (size_t)head * hd;
+#pragma unroll
+  for (int e = 0; e < 4; ++e) {
+    const float2 t = cs[(size_t)slot * half + p + e];
+    const __nv_bfloat16 y1 = __float2bfloat16_rn(a1[e] * t.x - a2[e] * t.y), y2 = __float2bfloat16_rn(a2[e] * t.x + a1[e] * t.y);
+    if (is_q) { qdst[p + e] = y1; qdst[half + p + e] = y2; }
+    else {
+      kv_layer[kv_elem(geo, page, head - Hq, 0, off, p + e)] = y1;
+      kv_layer[kv_elem(geo, page, head - Hq, 0, off, half + p + e)] = y2;
+    }
+  }
+}
+
 darts_status post(darts_ctx *c, const char *what) {
   c->launches++;
   cudaError_t e = cudaGetLastError();
@@ -125,4 +268,31 @@ darts_status launch_gather_rows_bf16(darts_ctx *c, const void *src, void *dst, i
 darts_status launch_sum_partials(darts_ctx *c, const float *part, float *out, int S, size_t n) {
   sum_partials_k<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(part, out, S, n);
   return post(c, "sum_partials");
+}
+
+darts_status launch_add_rmsnorm_sk(darts_ctx *c, const SkView &v, const void *w, int rows_ub, const int32_t *n_rows_dev) {
+  if (rows_ub <= 0) return DARTS_OK;
+  int d = c->m.d_model;
+  add_rmsnorm_sk_k<<<rows_ub, 256, 0, c->stream>>>(c->h, v, (const __nv_bfloat16 *)w, (__nv_bfloat16 *)c->xn, d, c->m.rms_eps, n_rows_dev, rows_ub);
+  return post(c, "add_rmsnorm_sk");
+}
+
+darts_status launch_silu_mul_sk(darts_ctx *c, const SkView &v, int rows_ub, const int32_t *n_rows_dev) {
+  if (rows_ub <= 0) return DARTS_OK;
+  int F = c->m.ffn;
+  dim3 grid((F / 4 + 255) / 256, rows_ub);
+  silu_mul_sk_k<<<grid, 256, 0, c->stream>>>(v, (__nv_bfloat16 *)c->act, F, n_rows_dev, rows_ub);
+  return post(c, "silu_mul_sk");
+}
+
+darts_status launch_rope_append_sk(darts_ctx *c, int layer, const SkView &v, int rows_ub, const int32_t *n_rows_dev) {
+  if (rows_ub <= 0) return DARTS_OK;
+  using T = __nv_bfloat16;
+  int nh = c->m.n_q_heads + 2 * c->m.n_kv_heads;
+  dim3 grid((nh + 3) / 4, rows_ub);
+  rope_append_sk_k<<<grid, 128, 0, c->stream>>>(v, (T *)c->q, (T *)c->kv_pool + (size_t)layer * c->kv_layer_elems, c->slot_dst_page, c->slot_dst_off,
+                                                c->slot_cs, c->m.qk_norm ? (const T *)c->q_norm[layer] : nullptr,
+                                                c->m.qk_norm ? (const T *)c->k_norm[layer] : nullptr, c->m.n_q_heads, c->m.n_kv_heads, c->m.head_dim,
+                                                c->m.rms_eps, c->geom(), n_rows_dev, rows_ub);
+  return post(c, "rope_append_sk");
 }

@@ -1,0 +1,298 @@
+// Weight-streaming tcgen05 / TMEM GEMM for the projections of the bf16 path:
+//     P[slot][r][n] = sum_{k in piece} X[r][k] W[n][k]
+//
+// Decode projections are bound by streaming the weights from HBM once per step, so the kernel is built
+// around the weight stream, not around the (small) activation matrix:
+//   * "swap-AB": the 128-row MMA dimension M is a tile of WEIGHT rows, the MMA N dimension is the block of activation
+//     rows (runtime N = live rows rounded up to 16, at most 256), so tensor work and activation loads scale with the
+//     live row count and every weight byte is fetched once per 256-row block;
+//   * persistent, one CTA per SM, stream-K: the (weight tile, row block, k-block) units of a GEMM are cut into gridDim.x
+//     equal contiguous ranges, so every SM streams the same number of weight bytes whatever the tile count (152 tiles
+//     on 148 SMs would otherwise cost two waves).  A tile that straddles CTAs is emitted as several partial "pieces";
+//     piece s of a tile is written to slot s (slot = CTA index - first CTA of the tile), and the consumer kernels add
+//     the pieces in slot order (internal.cuh: sk_npieces) — deterministic, no atomics;
+//   * a deep TMA ring (stage = 16 KB of weights + 2 KB per 16 live rows; as many stages as fit in ~200 KB) keeps
+//     >= 100 KB of weight loads in flight per SM, which is what it takes to cover HBM latency at 44 GB/s per SM;
+//   * two TMEM accumulators: the epilogue warps drain piece i while the MMA warp accumulates piece i+1.
+// Warp roles: warp 0 TMA producer, warp 1 MMA issuer (+ TMEM alloc), warps 2-5 epilogue (TMEM lane = weight row,
+// column = activation row; a warp's 32 lanes store 32 consecutive output columns of one row: coalesced 128 B).
+// Grouped mode (MoE): row blocks come from a device list {row0, nrows, weight row base}, units are whole tiles.
+#include <algorithm>
+
+#include "internal.cuh"
+#include "sm100_ptx.cuh"
+
+namespace {
+
+using namespace ptx;
+
+constexpr int BMW = 128, BK = 64;
+constexpr int W_STAGE_BYTES = BMW * BK * 2;      // 16 KB
+constexpr int BOX_ROWS = 16, BOX_BYTES = BOX_ROWS * BK * 2;
+constexpr int MAX_STAGES = 10;
+constexpr int SK_THREADS = 192;
+constexpr int SMEM_BUDGET = 200 * 1024;
+
+struct SkParams {
+  float *C;
+  size_t slot_stride;
+  int N, nkb, n_wtiles, w_rows_per_group;
+  int rows_ub;
+  const int32_t *n_rows_dev;
+  const int32_t *rb_list, *n_rb_dev;             // grouped mode
+  int unit_tile;
+  int stage_bytes, n_stages, tm_cols;            // tm_cols: columns of ONE accumulator (power of two >= 32)
+};
+
+struct SkBars {
+  unsigned long long full[MAX_STAGES], empty[MAX_STAGES], acc_full[2], acc_empty[2];
+  uint32_t tmem_base;
+};
+
+struct Piece {
+  int wtile, row0, nrows, wbase, kb0, kb1, slot;
+};
+
+// Walks the pieces of CTA `cta`; the three roles call it with identical arguments and so see the same sequence.
+struct PieceIter {
+  int u, u1, T, P, nkb, n_rb, unit_tile, cta, w_rows_per_group;
+  const int32_t *rb_list;
+  int live;
+  __device__ bool next(Piece &p) {
+    if (u >= u1) return false;
+    int tile = unit_tile ? u : u / nkb;
+    p.kb0 = unit_tile ? 0 : u - tile * nkb;
+    p.kb1 = unit_tile ? nkb : min(nkb, p.kb0 + (u1 - u));
+    p.wtile = tile / n_rb;
+    int rb = tile - p.wtile * n_rb;
+    if (rb_list) { p.row0 = rb_list[4 * rb]; p.nrows = rb_list[4 * rb + 1]; p.wbase = rb_list[4 * rb + 2] * w_rows_per_group; }
+    else { p.row0 = rb * SK_ROWBLOCK; p.nrows = min(SK_ROWBLOCK, live - p.row0); p.wbase = 0; }
+    p.slot = unit_tile ? 0 : cta - sk_owner(tile * nkb, P, T);
+    u += unit_tile ? 1 : p.kb1 - p.kb0;
+    return true;
+  }
+};
+
+__global__ void __launch_bounds__(SK_THREADS, 1) gemm_sk_k(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ XMaps tmX,
+                                                           SkParams p) {
+  extern __shared__ unsigned char smem_raw[];
+  unsigned char *stage_base = reinterpret_cast<unsigned char *>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  SkBars &bar = *reinterpret_cast<SkBars *>(stage_base + (size_t)p.n_stages * p.stage_bytes);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+  // ---- this CTA's unit range (uniform over the CTA; leave before any barrier / TMEM allocation if it is empty)
+  PieceIter it0;
+  it0.rb_list = p.rb_list; it0.w_rows_per_group = p.w_rows_per_group; it0.nkb = p.nkb; it0.unit_tile = p.unit_tile; it0.P = gridDim.x; it0.cta = blockIdx.x;
+  if (p.rb_list) { pdl_wait(); it0.n_rb = *p.n_rb_dev; it0.live = 0; }
+  else { it0.live = p.n_rows_dev ? min(*p.n_rows_dev, p.rows_ub) : p.rows_ub; it0.n_rb = (it0.live + SK_ROWBLOCK - 1) / SK_ROWBLOCK; }
+  if (it0.n_rb <= 0) return;
+  it0.T = p.n_wtiles * it0.n_rb * (p.unit_tile ? 1 : p.nkb);
+  it0.u = (int)((long long)blockIdx.x * it0.T / gridDim.x);
+  it0.u1 = (int)((long long)(blockIdx.x + 1) * it0.T / gridDim.x);
+  if (it0.u >= it0.u1) return;
+
+  if (threadIdx.x == 0) {
+    prefetch_tmap(&tmW);
+    for (int b = 0; b < 5; ++b) prefetch_tmap(&tmX.m[b]);
+    for (int s = 0; s < p.n_stages; ++s) { mbar_init(&bar.full[s], 1); mbar_init(&bar.empty[s], 1); }
+    for (int b = 0; b < 2; ++b) { mbar_init(&bar.acc_full[b], 1); mbar_init(&bar.acc_empty[b], 4); }
+    fence_mbar_init();
+  }
+  if (warp == 1) tmem_alloc(&bar.tmem_base, 2 * p.tm_cols);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = bar.tmem_base;
+
+  if (warp == 0) {
+    // ------------------------------------------------------------------------------------------ TMA producer
+    // The whole warp walks the ring; lane 0 arms the barrier and fetches the weight tile; the activation rows
+    // (rounded up to 16) are fetched as the binary decomposition of their count into boxes of 256/128/64/32/16 rows,
+    // lane b taking the box of 16 << b rows: at most five bulk-tensor copies per stage, issued by one warp instruction
+    // (the copy COUNT, not the bytes, is what bounds a single-producer TMA ring).
+    // Programmatic dependent launch: this kernel may start while the kernel that produces X is still running.  The weights
+    // do not depend on it, so the first ring-full of weight tiles is requested BEFORE griddepcontrol.wait; only the
+    // activation boxes wait.  (Grouped mode reads its row-block list first and therefore waits at the top.)
+    int n_pre = 0;
+    if (!p.rb_list) {
+      PieceIter it = it0;
+      Piece pc;
+      while (n_pre < p.n_stages && it.next(pc)) {
+        const int n16 = (pc.nrows + BOX_ROWS - 1) / BOX_ROWS;
+        for (int kb = pc.kb0; kb < pc.kb1 && n_pre < p.n_stages; ++kb, ++n_pre)
+          if (lane == 0) {
+            unsigned char *st = stage_base + (size_t)n_pre * p.stage_bytes;
+            mbar_expect_tx(&bar.full[n_pre], W_STAGE_BYTES + n16 * BOX_BYTES);
+            tma_load_2d_hint(st, &tmW, kb * BK, pc.wbase + pc.wtile * BMW, &bar.full[n_pre], HINT_EVICT_FIRST);
+          }
+      }
+    }
+    pdl_wait();
+    PieceIter it = it0;
+    Piece pc;
+    int stage = 0, phase = 0, i = 0;
+    while (it.next(pc)) {
+      const int n16 = (pc.nrows + BOX_ROWS - 1) / BOX_ROWS;
+      const int tx = W_STAGE_BYTES + n16 * BOX_BYTES;
+      const int wrow = pc.wbase + pc.wtile * BMW;
+      const bool mine = lane < 5 && ((n16 >> lane) & 1);
+      const int my_row = (n16 & ~((2 << lane) - 1)) * BOX_ROWS;          // rows covered by the larger boxes
+      for (int kb = pc.kb0; kb < pc.kb1; ++kb, ++i) {
+        unsigned char *st = stage_base + (size_t)stage * p.stage_bytes;
+        if (i >= n_pre) {
+          mbar_wait(&bar.empty[stage], phase ^ 1);
+          if (lane == 0) {
+            mbar_expect_tx(&bar.full[stage], tx);
+            tma_load_2d_hint(st, &tmW, kb * BK, wrow, &bar.full[stage], HINT_EVICT_FIRST);        // weights: streamed once
+          }
+          __syncwarp();
+        }
+        if (mine)
+          tma_load_2d_hint(st + W_STAGE_BYTES + my_row * (BK * 2), &tmX.m[lane], kb * BK, pc.row0 + my_row, &bar.full[stage], HINT_EVICT_LAST);
+        if (++stage == p.n_stages) { stage = 0; phase ^= 1; }
+      }
+    }
+  } else if (warp == 1) {
+    // ------------------------------------------------------------------------------------------ MMA issuer
+    if (lane == 0) {
+      PieceIter it = it0;
+      Piece pc;
+      int stage = 0, phase = 0, piece = 0;
+      while (it.next(pc)) {
+        const int buf = piece & 1, use = piece >> 1;
+        const uint32_t idesc = umma_idesc_bf16(BMW, (pc.nrows + 15) & ~15);
+        mbar_wait(&bar.acc_empty[buf], (use & 1) ^ 1);
+        tc_fence_after();
+        const uint32_t d = tmem + (uint32_t)(buf * p.tm_cols);
+        for (int kb = pc.kb0; kb < pc.kb1; ++kb) {
+          mbar_wait(&bar.full[stage], phase);
+          tc_fence_after();
+          const uint32_t sa = smem_u32(stage_base + (size_t)stage * p.stage_bytes);
+          const uint64_t dw = umma_desc_sw128(sa), dx = umma_desc_sw128(sa + W_STAGE_BYTES);
+#pragma unroll
+          for (int k = 0; k < BK / 16; ++k) mma_bf16_ss(d, dw + 2 * k, dx + 2 * k, idesc, (kb > pc.kb0 || k > 0) ? 1u : 0u);
+          mma_commit(&bar.empty[stage]);
+          if (++stage == p.n_stages) { stage = 0; phase ^= 1; }
+        }
+        mma_commit(&bar.acc_full[buf]);
+        ++piece;
+      }
+    }
+  } else {
+    // ------------------------------------------------------------------------------------------ epilogue
+    const int q = warp & 3;                                // TMEM lane quadrant this warp may read
+    PieceIter it = it0;
+    Piece pc;
+    int piece = 0;
+    while (it.next(pc)) {
+      const int buf = piece & 1, use = piece >> 1;
+      mbar_wait(&bar.acc_full[buf], use & 1);
+      tc_fence_after();
+      const int n = pc.wtile * BMW + q * 32 + lane;        // output column = weight row
+      const bool n_ok = n < p.N;
+      float *dst = p.C + (size_t)pc.slot * p.slot_stride + (size_t)pc.row0 * p.N + n;
+      const uint32_t src = tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)(buf * p.tm_cols);
+#pragma unroll 1
+      for (int c = 0; c < pc.nrows; c += 32) {
+        uint32_t v[32];
+        tmem_ld32(src + c, v);
+        tmem_ld_wait();
+        if (n_ok) {
+#pragma unroll
+          for (int j = 0; j < 32; ++j)
+            if (c + j < pc.nrows) dst[(size_t)(c + j) * p.N] = __uint_as_float(v[j]);
+        }
+      }
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&bar.acc_empty[buf]);
+      ++piece;
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) tmem_dealloc(tmem, 2 * p.tm_cols);
+}
+
+// out[r][n] = sum of the pieces of (r, n) in slot order (debug / test hook)
+__global__ void sk_reduce_k(SkView v, float *__restrict__ out, int rows) {
+  size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= (size_t)rows * v.N) return;
+  int r = (int)(i / v.N), n = (int)(i % v.N);
+  int n_rb = (rows + SK_ROWBLOCK - 1) / SK_ROWBLOCK;
+  int np = sk_npieces(v, n_rb, n, r);
+  float a = v.part[i];
+  for (int s = 1; s < np; ++s) a += v.part[(size_t)s * v.slot_stride + i];
+  out[i] = a;
+}
+
+}  // namespace
+
+// Host-side plan: mode, grid, slots.  rows_ub bounds the live rows (dense; rows_exact: it IS the row count) or the rows
+// of one group (grouped, at most n_rb_ub_grouped row blocks in all).
+SkPlan sk_plan(int n_sms, int N, int K, int rows_ub, int n_rb_ub_grouped, bool rows_exact) {
+  SkPlan pl{};
+  pl.nkb = K / BK;
+  pl.n_wtiles = (N + BMW - 1) / BMW;
+  const bool grouped = n_rb_ub_grouped > 0;
+  const int n_rb_ub = grouped ? n_rb_ub_grouped : (rows_ub + SK_ROWBLOCK - 1) / SK_ROWBLOCK;
+  const long long tiles_ub = (long long)pl.n_wtiles * n_rb_ub;
+  pl.unit_tile = grouped || tiles_ub >= 8LL * n_sms;
+  if (pl.unit_tile) {
+    pl.P = (int)std::min<long long>(n_sms, tiles_ub);
+    pl.slots = 1;
+  } else {
+    const int T_min = pl.n_wtiles * pl.nkb * (rows_exact ? n_rb_ub : 1);   // fewest units a launch can see
+    pl.P = std::max(1, std::min(n_sms, T_min / 4));                        // >= 4 k-blocks (64 KB of weights) per CTA
+    for (;;) {
+      const int per = T_min / pl.P;                                        // every CTA range holds >= per units
+      pl.slots = std::min(pl.nkb, (pl.nkb + per - 1) / per + 1);
+      if (pl.slots <= 16 || pl.P == 1) break;                              // consumers hold <= 16 pieces in registers
+      pl.P = std::max(1, pl.P * 3 / 4);
+    }
+  }
+  int cap = std::min(SK_ROWBLOCK, (rows_ub + 15) & ~15);
+  pl.stage_bytes = W_STAGE_BYTES + cap / BOX_ROWS * BOX_BYTES;
+  pl.n_stages = std::min(MAX_STAGES, SMEM_BUDGET / pl.stage_bytes);
+  pl.tm_cols = 32;
+  while (pl.tm_cols < cap) pl.tm_cols *= 2;
+  return pl;
+}
+
+darts_status launch_gemm_sk(darts_ctx *c, const SkGemm &g) {
+  if (g.rows_ub <= 0) return DARTS_OK;
+  const SkPlan &pl = g.plan;
+  SkParams p{};
+  p.C = g.C; p.slot_stride = g.slot_stride; p.N = g.N; p.nkb = pl.nkb; p.n_wtiles = pl.n_wtiles; p.rows_ub = g.rows_ub; p.n_rows_dev = g.n_rows_dev;
+  p.rb_list = g.rb_list; p.n_rb_dev = g.n_rb_dev; p.w_rows_per_group = g.w_rows_per_group; p.unit_tile = pl.unit_tile; p.stage_bytes = pl.stage_bytes; p.n_stages = pl.n_stages;
+  p.tm_cols = pl.tm_cols;
+  size_t smem = (size_t)pl.n_stages * pl.stage_bytes + sizeof(SkBars) + 1024;
+  static bool attr = false;
+  if (!attr) {
+    CUDA_TRY(c, cudaFuncSetAttribute(gemm_sk_k, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET + (int)sizeof(SkBars) + 2048));
+    attr = true;
+  }
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = dim3(pl.P); cfg.blockDim = dim3(SK_THREADS); cfg.dynamicSmemBytes = smem; cfg.stream = c->stream;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = c->use_pdl ? 1 : 0;
+  cudaLaunchKernelEx(&cfg, gemm_sk_k, *g.w_map, *g.x_maps, p);
+  c->launches++;
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) {
+    snprintf(c->err, sizeof(c->err), "launch gemm_sk: %s", cudaGetErrorString(e));
+    c->sticky = DARTS_ERR_CUDA;
+    return DARTS_ERR_CUDA;
+  }
+  return DARTS_OK;
+}
+
+darts_status launch_sk_reduce(darts_ctx *c, const SkView &v, float *out, int rows) {
+  size_t n = (size_t)rows * v.N;
+  sk_reduce_k<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(v, out, rows);
+  c->launches++;
+  if (cudaGetLastError() != cudaSuccess) FAIL(c, DARTS_ERR_CUDA, "launch sk_reduce failed");
+  return DARTS_OK;
+}

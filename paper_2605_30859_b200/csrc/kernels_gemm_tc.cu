@@ -240,6 +240,14 @@ darts_status tc_make_map(darts_ctx *c, CUtensorMap *out, const void *base, long 
   return DARTS_OK;
 }
 
+darts_status tc_make_xmaps(darts_ctx *c, XMaps *out, const void *base, long long rows, int K) {
+  for (int b = 0; b < 5; ++b) {
+    darts_status s = tc_make_map(c, &out->m[b], base, rows, K, 16 << b);
+    if (s != DARTS_OK) return s;
+  }
+  return DARTS_OK;
+}
+
 bool tc_shape_ok(int N, int K) { return K % BK == 0 && K >= BK && N % 4 == 0; }
 
 // Split-K factor: fill ~2 CTAs per SM, keep >= 4 k-blocks per split, stay inside the partial buffer.  Depends on the

@@ -11,6 +11,8 @@
 //   moe_expert_simt_k (fp32 / generic path) one CTA per (slot, k): the expert's SwiGLU MLP as warp dot products
 //   moe_combine_k    h += sum_k w_k y_k in selection order (+ the next RMSNorm on the tensor-core path)
 // Weight bytes streamed per step scale with the DISTINCT experts hit: groups with no rows exit before any load.
+#include <algorithm>
+
 #include "internal.cuh"
 
 namespace {
@@ -136,29 +138,34 @@ __global__ void __launch_bounds__(128) moe_topk_k(const float *__restrict__ logi
 // One CTA per expert (tensor-core path).  off[e] = sum_{e'<e} cnt[e'];  the expert's assignments keep their slot
 // order (stable), so the layout of xs is a pure function of the routing.  xs[off[e] + rank] = xn[slot of assignment].
 __global__ void __launch_bounds__(256) moe_place_k(const int32_t *__restrict__ cnt, const int32_t *__restrict__ eid, int32_t *__restrict__ pos,
-                                                   int32_t *__restrict__ tok, int32_t *__restrict__ off_out, const __nv_bfloat16 *__restrict__ xn,
+                                                   int32_t *__restrict__ tok, int32_t *__restrict__ off_out, int32_t *__restrict__ rb_list,
+                                                   int32_t *__restrict__ n_rb_out, const __nv_bfloat16 *__restrict__ xn,
                                                    __nv_bfloat16 *__restrict__ xs, int E, int top_k, int d, const int32_t *n_rows_dev,
                                                    int rows_ub) {
-  __shared__ int s_red[8];
-  __shared__ int s_off;
+  __shared__ int s_red[8], s_redb[8];
+  __shared__ int s_off, s_blk;
   const int e = blockIdx.x, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int n_assign = live_rows(n_rows_dev, rows_ub) * top_k;
-  int part = 0;
-  for (int q = threadIdx.x; q < e; q += blockDim.x) part += cnt[q];
+  int part = 0, partb = 0;                               // rows / 256-row blocks of the experts before this one
+  for (int q = threadIdx.x; q < e; q += blockDim.x) { int cq = cnt[q]; part += cq; partb += (cq + SK_ROWBLOCK - 1) / SK_ROWBLOCK; }
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
-  if (lane == 0) s_red[warp] = part;
+  for (int o = 16; o > 0; o >>= 1) { part += __shfl_xor_sync(0xffffffffu, part, o); partb += __shfl_xor_sync(0xffffffffu, partb, o); }
+  if (lane == 0) { s_red[warp] = part; s_redb[warp] = partb; }
   __syncthreads();
   if (threadIdx.x == 0) {
-    int t = 0;
-    for (int w = 0; w < 8; ++w) t += s_red[w];
-    s_off = t;
+    int t = 0, tb = 0;
+    for (int w = 0; w < 8; ++w) { t += s_red[w]; tb += s_redb[w]; }
+    s_off = t; s_blk = tb;
     off_out[e] = t;
-    if (e == E - 1) off_out[E] = t + cnt[e];
+    if (e == E - 1) { off_out[E] = t + cnt[e]; *n_rb_out = tb + (cnt[e] + SK_ROWBLOCK - 1) / SK_ROWBLOCK; }
   }
   __syncthreads();
   const int off = s_off, mine = cnt[e];
   if (mine == 0) return;
+  for (int i = threadIdx.x; i < (mine + SK_ROWBLOCK - 1) / SK_ROWBLOCK; i += blockDim.x) {   // this expert's row blocks for the grouped GEMM
+    int32_t *rb = rb_list + 4 * (s_blk + i);
+    rb[0] = off + i * SK_ROWBLOCK; rb[1] = min(SK_ROWBLOCK, mine - i * SK_ROWBLOCK); rb[2] = e; rb[3] = 0;
+  }
   if (warp == 0) {
     int base = off;
     for (int a0 = 0; a0 < n_assign; a0 += 32) {
@@ -340,25 +347,24 @@ darts_status launch_moe_tc(darts_ctx *c, int layer, const void *next_norm, int r
   int32_t *cnt = c->moe_cnt + (size_t)layer * E;
   darts_status s;
   if ((s = route<T>(c, layer, rows_ub, n_rows_dev, cnt)) != DARTS_OK) return s;
-  moe_place_k<<<E, 256, 0, c->stream>>>(cnt, c->moe_eid, c->moe_pos, c->moe_tok, c->moe_off, (const T *)c->xn, (T *)c->xs, E, m.top_k, d, n_rows_dev,
-                                        rows_ub);
+  moe_place_k<<<E, 256, 0, c->stream>>>(cnt, c->moe_eid, c->moe_pos, c->moe_tok, c->moe_off, c->moe_rb, c->moe_nrb, (const T *)c->xn, (T *)c->xs, E,
+                                        m.top_k, d, n_rows_dev, rows_ub);
   if ((s = post(c, "moe_place")) != DARTS_OK) return s;
-  TcGemm g{};
-  g.a_map = &c->tm_xs; g.b_map = &c->tm_wgu_e[layer]; g.C = c->part; g.N = 2 * F; g.K = d; g.rows_ub = rows_ub;   // <= rows_ub rows per expert
-  g.n_rows_dev = nullptr; g.n_groups = E; g.grp_off = c->moe_off; g.b_rows_per_group = 2 * F;
-  g.S = tc_pick_split(c, g.N, g.K, rows_ub, E);
-  if ((size_t)g.S * RK * g.N * 4 > c->part_bytes) g.S = 1;
-  g.split_stride = (size_t)RK * g.N;
-  if ((s = launch_gemm_tc(c, g)) != DARTS_OK) return s;
+  // grouped stream-K GEMMs: one row block per (expert, <= 256 of its rows); experts nobody chose cost nothing
+  const int n_rb_ub = std::min(E, RK) + RK / SK_ROWBLOCK;
+  SkGemm g{};
+  g.w_map = &c->tm_wgu_e[layer]; g.x_maps = &c->xm_xs; g.C = c->part; g.N = 2 * F; g.rows_ub = rows_ub;      // <= rows_ub rows per expert
+  g.rb_list = c->moe_rb; g.n_rb_dev = c->moe_nrb; g.w_rows_per_group = 2 * F;
+  g.plan = sk_plan(c->n_sms, g.N, d, rows_ub, n_rb_ub, false);
+  g.slot_stride = 0;
+  if ((s = launch_gemm_sk(c, g)) != DARTS_OK) return s;
   dim3 grid((F / 4 + 255) / 256, RK);
-  moe_silu_mul_k<<<grid, 256, 0, c->stream>>>(c->part, g.S, g.split_stride, (T *)c->act, F, m.top_k, n_rows_dev, rows_ub);
+  moe_silu_mul_k<<<grid, 256, 0, c->stream>>>(c->part, 1, 0, (T *)c->act, F, m.top_k, n_rows_dev, rows_ub);
   if ((s = post(c, "moe_silu_mul")) != DARTS_OK) return s;
-  g.a_map = &c->tm_act; g.b_map = &c->tm_wd_e[layer]; g.N = d; g.K = F; g.b_rows_per_group = d;
-  g.S = tc_pick_split(c, g.N, g.K, rows_ub, E);
-  if ((size_t)g.S * RK * g.N * 4 > c->part_bytes) g.S = 1;
-  g.split_stride = (size_t)RK * g.N;
-  if ((s = launch_gemm_tc(c, g)) != DARTS_OK) return s;
-  moe_combine_k<T><<<rows_ub, 256, 0, c->stream>>>(c->h, c->part, g.S, g.split_stride, c->moe_pos, c->moe_w, m.top_k, (const T *)next_norm, (T *)c->xn, d,
+  g.w_map = &c->tm_wd_e[layer]; g.x_maps = &c->xm_act; g.N = d; g.w_rows_per_group = d;
+  g.plan = sk_plan(c->n_sms, g.N, F, rows_ub, n_rb_ub, false);
+  if ((s = launch_gemm_sk(c, g)) != DARTS_OK) return s;
+  moe_combine_k<T><<<rows_ub, 256, 0, c->stream>>>(c->h, c->part, 1, 0, c->moe_pos, c->moe_w, m.top_k, (const T *)next_norm, (T *)c->xn, d,
                                                    m.rms_eps, n_rows_dev, rows_ub);
   return post(c, "moe_combine");
 }

@@ -30,6 +30,17 @@ def _mk(shape, seed, scale=1.0):
     (200, 512, 1024, 4),      # two row tiles, second one ragged
     (300, 1000, 2560, 5),     # three row tiles, K of config 3
     (64, 6144, 2560, 4),      # config-3 QKV shape at 64 rows
+    # S = 0: the stream-K weight-streaming kernel (swap-AB, persistent) the decode projections run on
+    (1, 128, 64, 0),
+    (16, 256, 256, 0),
+    (37, 132, 192, 0),        # ragged rows, ragged N
+    (200, 512, 1024, 0),      # 13 row boxes, pieces straddling CTAs
+    (256, 384, 512, 0),       # one full 256-row block
+    (300, 1000, 2560, 0),     # two row blocks, the second ragged
+    (700, 640, 1024, 0),      # three row blocks
+    (64, 6144, 2560, 0),      # config-3 QKV shape
+    (130, 2560, 9728, 0),     # config-3 down projection: few tiles, long K (many pieces per tile)
+    (2048, 19456, 256, 0),    # whole-tile mode (tiles >= 8 x SMs), prefill-like
 ])
 def test_gemm_matches_oracle(ctx, rows, N, K, S):
     X, W = _mk((rows, K), rows + N), _mk((N, K), K + S, 0.05)
@@ -40,10 +51,11 @@ def test_gemm_matches_oracle(ctx, rows, N, K, S):
     assert np.max(np.abs(got - ref)) <= tol, (np.max(np.abs(got - ref)), tol)
 
 
-def test_gemm_is_deterministic_and_split_order_fixed(ctx):
+@pytest.mark.parametrize("S", [4, 0])
+def test_gemm_is_deterministic_and_split_order_fixed(ctx, S):
     X, W = _mk((50, 1024), 1), _mk((256, 1024), 2, 0.05)
-    a = ctx.debug_gemm_bf16(X, W, split_k=4)
-    b = ctx.debug_gemm_bf16(X, W, split_k=4)
+    a = ctx.debug_gemm_bf16(X, W, split_k=S)
+    b = ctx.debug_gemm_bf16(X, W, split_k=S)
     assert torch.equal(a, b)
 
 
