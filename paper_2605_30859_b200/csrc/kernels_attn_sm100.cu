@@ -150,6 +150,8 @@ __global__ void __launch_bounds__(THREADS, 2) attn_main_k(Params p) {
     for (int s = 0; s < STAGES; ++s) { mbar_init(&sm.full[s], 1); mbar_init(&sm.empty[s], N_CONS); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
+  pdl_trigger();
+  pdl_wait();                                    // q, the KV rows appended this step and the plan come from earlier kernels
   __syncthreads();
   int n_pre = p.n_items[0], n_suf = p.n_items[1];
   long long total = (long long)(n_pre + n_suf) * p.Hkv;
@@ -313,12 +315,13 @@ __global__ void attn_merge_k(const float *__restrict__ part_ml, const float *__r
                              const int32_t *__restrict__ part_cnt, __nv_bfloat16 *__restrict__ out, int Hq, float c,
                              const int32_t *n_rows_dev, int rows_ub) {
   pdl_trigger();
+  pdl_wait();
   int slot = blockIdx.x;
   int R = n_rows_dev ? min(*n_rows_dev, rows_ub) : rows_ub;
   if (slot >= R) return;
   int lane = threadIdx.x & 31;
   int base = part_base[slot], cnt = part_cnt[slot];
-  for (int h = threadIdx.x >> 5; h < Hq; h += blockDim.x >> 5) {
+  for (int h = blockIdx.y * (blockDim.x >> 5) + (threadIdx.x >> 5); h < Hq; h += gridDim.y * (blockDim.x >> 5)) {   // one head per warp
     float M = -INFINITY;
     for (int k = 0; k < cnt; ++k) M = fmaxf(M, part_ml[((size_t)(base + k) * Hq + h) * 2]);
     float L = 0.f;
@@ -467,10 +470,10 @@ darts_status launch_attention_sm100(darts_ctx *c, int layer, const void *q, void
   p.page_elems = c->kv_page_elems; p.tile_elems = c->kv_tile_elems;
   p.c = 1.4426950408889634f / sqrtf((float)HD);
   int grid = c->n_sms * 2;
-  attn_main_k<<<grid, THREADS, smem, c->stream>>>(p);
+  launch_pdl(c, attn_main_k, dim3(grid), dim3(THREADS), smem, p);
   c->launches++;
   if (cudaGetLastError() != cudaSuccess) FAIL(c, DARTS_ERR_CUDA, "launch attn_main failed: %s", cudaGetErrorString(cudaGetLastError()));
-  attn_merge_k<<<rows_ub, 256, 0, c->stream>>>(c->part_ml, c->part_acc, c->part_base, c->part_cnt, (__nv_bfloat16 *)out, p.Hq, p.c, n_rows_dev, rows_ub);
+  launch_pdl(c, attn_merge_k, dim3(rows_ub, (p.Hq + 7) / 8), dim3(256), 0, c->part_ml, c->part_acc, c->part_base, c->part_cnt, (__nv_bfloat16 *)out, p.Hq, p.c, n_rows_dev, rows_ub);
   c->launches++;
   if (cudaGetLastError() != cudaSuccess) FAIL(c, DARTS_ERR_CUDA, "launch attn_merge failed");
   return DARTS_OK;

@@ -122,6 +122,7 @@ __device__ __forceinline__ uint2 pack4_bf16(float a, float b, float c, float d) 
 __global__ void __launch_bounds__(256) add_rmsnorm_sk_k(float *__restrict__ h, SkView v, const __nv_bfloat16 *__restrict__ w,
                                                         __nv_bfloat16 *__restrict__ out, int d, float eps, const int32_t *n_rows_dev, int rows_ub) {
   pdl_trigger();
+  pdl_wait();
   const int slot = blockIdx.x, live = live_rows(n_rows_dev, rows_ub);
   if (slot >= live) return;
   const int n_rb = (live + SK_ROWBLOCK - 1) / SK_ROWBLOCK;
@@ -156,6 +157,7 @@ __global__ void __launch_bounds__(256) add_rmsnorm_sk_k(float *__restrict__ h, S
 // act[slot][k] = silu(g) * u with g = pieces(slot, k), u = pieces(slot, F + k)
 __global__ void __launch_bounds__(256) silu_mul_sk_k(SkView v, __nv_bfloat16 *__restrict__ act, int F, const int32_t *n_rows_dev, int rows_ub) {
   pdl_trigger();
+  pdl_wait();
   const int slot = blockIdx.y, live = live_rows(n_rows_dev, rows_ub);
   if (slot >= live) return;
   const int k = (blockIdx.x * blockDim.x + threadIdx.x) * 4;
@@ -175,6 +177,7 @@ __global__ void __launch_bounds__(128) rope_append_sk_k(SkView v, __nv_bfloat16 
                                                        const __nv_bfloat16 *__restrict__ k_norm, int Hq, int Hkv, int hd, float eps, KvGeom geo,
                                                        const int32_t *n_rows_dev, int rows_ub) {
   pdl_trigger();
+  pdl_wait();
   const int slot = blockIdx.y, live = live_rows(n_rows_dev, rows_ub);
   if (slot >= live) return;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -273,7 +276,7 @@ darts_status launch_sum_partials(darts_ctx *c, const float *part, float *out, in
 darts_status launch_add_rmsnorm_sk(darts_ctx *c, const SkView &v, const void *w, int rows_ub, const int32_t *n_rows_dev) {
   if (rows_ub <= 0) return DARTS_OK;
   int d = c->m.d_model;
-  add_rmsnorm_sk_k<<<rows_ub, 256, 0, c->stream>>>(c->h, v, (const __nv_bfloat16 *)w, (__nv_bfloat16 *)c->xn, d, c->m.rms_eps, n_rows_dev, rows_ub);
+  launch_pdl(c, add_rmsnorm_sk_k, dim3(rows_ub), dim3(256), 0, c->h, v, (const __nv_bfloat16 *)w, (__nv_bfloat16 *)c->xn, d, c->m.rms_eps, n_rows_dev, rows_ub);
   return post(c, "add_rmsnorm_sk");
 }
 
@@ -281,7 +284,7 @@ darts_status launch_silu_mul_sk(darts_ctx *c, const SkView &v, int rows_ub, cons
   if (rows_ub <= 0) return DARTS_OK;
   int F = c->m.ffn;
   dim3 grid((F / 4 + 255) / 256, rows_ub);
-  silu_mul_sk_k<<<grid, 256, 0, c->stream>>>(v, (__nv_bfloat16 *)c->act, F, n_rows_dev, rows_ub);
+  launch_pdl(c, silu_mul_sk_k, grid, dim3(256), 0, v, (__nv_bfloat16 *)c->act, F, n_rows_dev, rows_ub);
   return post(c, "silu_mul_sk");
 }
 
@@ -290,7 +293,7 @@ darts_status launch_rope_append_sk(darts_ctx *c, int layer, const SkView &v, int
   using T = __nv_bfloat16;
   int nh = c->m.n_q_heads + 2 * c->m.n_kv_heads;
   dim3 grid((nh + 3) / 4, rows_ub);
-  rope_append_sk_k<<<grid, 128, 0, c->stream>>>(v, (T *)c->q, (T *)c->kv_pool + (size_t)layer * c->kv_layer_elems, c->slot_dst_page, c->slot_dst_off,
+  launch_pdl(c, rope_append_sk_k, grid, dim3(128), 0, v, (T *)c->q, (T *)c->kv_pool + (size_t)layer * c->kv_layer_elems, c->slot_dst_page, c->slot_dst_off,
                                                 c->slot_cs, c->m.qk_norm ? (const T *)c->q_norm[layer] : nullptr,
                                                 c->m.qk_norm ? (const T *)c->k_norm[layer] : nullptr, c->m.n_q_heads, c->m.n_kv_heads, c->m.head_dim,
                                                 c->m.rms_eps, c->geom(), n_rows_dev, rows_ub);

@@ -80,6 +80,7 @@ __global__ void __launch_bounds__(SK_THREADS, 1) gemm_sk_k(const __grid_constant
   SkBars &bar = *reinterpret_cast<SkBars *>(stage_base + (size_t)p.n_stages * p.stage_bytes);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
+  pdl_trigger();
   // ---- this CTA's unit range (uniform over the CTA; leave before any barrier / TMEM allocation if it is empty)
   PieceIter it0;
   it0.rb_list = p.rb_list; it0.w_rows_per_group = p.w_rows_per_group; it0.nkb = p.nkb; it0.unit_tile = p.unit_tile; it0.P = gridDim.x; it0.cta = blockIdx.x;
@@ -272,13 +273,7 @@ darts_status launch_gemm_sk(darts_ctx *c, const SkGemm &g) {
     CUDA_TRY(c, cudaFuncSetAttribute(gemm_sk_k, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET + (int)sizeof(SkBars) + 2048));
     attr = true;
   }
-  cudaLaunchConfig_t cfg{};
-  cfg.gridDim = dim3(pl.P); cfg.blockDim = dim3(SK_THREADS); cfg.dynamicSmemBytes = smem; cfg.stream = c->stream;
-  cudaLaunchAttribute at[1];
-  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  at[0].val.programmaticStreamSerializationAllowed = 1;
-  cfg.attrs = at; cfg.numAttrs = c->use_pdl ? 1 : 0;
-  cudaLaunchKernelEx(&cfg, gemm_sk_k, *g.w_map, *g.x_maps, p);
+  launch_pdl(c, gemm_sk_k, dim3(pl.P), dim3(SK_THREADS), smem, *g.w_map, *g.x_maps, p);
   c->launches++;
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) {
