@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py — one JSON line: rollout generated tokens/s on 1 B200 (K'-of-K early stop) + decode HBM GB/s vs peak.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c3|c2] [--impl reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c3|c4|c5|c2] [--mode auto|early] [--impl reference]
 
 A "step" is one pass of the whole hot path over one batch of synthetic input:
   workload c3 (default): one full group rollout of BASELINE.json configs[2] (Qwen3-4B-shaped, G=32 x K'=16, keep 8,
@@ -27,7 +27,7 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-KV_BYTES_PER_TOKEN_LAYER = {"c2": 2 * 8 * 128 * 2, "c3": 2 * 8 * 128 * 2}
+KV_BYTES_PER_TOKEN_LAYER = {"c2": 2 * 8 * 128 * 2}
 
 
 def measured_peaks():
@@ -151,37 +151,65 @@ def oracle_attention_sample(x_full_seed=0, n_rows=32):
     return x["R"] / dt, x["R"], torch.get_num_threads()
 
 
-# ------------------------------------------------------------------------------------------------ c3: full rollout
-def build_c3(seed, max_new=None, G=None, n_layers=None):
-    import torch
+# ------------------------------------------------------------------------------------------------ full rollouts (c3 / c4 / c5)
+KV_POOL_CAP_BYTES = {"c3": 64e9, "c4": 100e9, "c5": 36e9}
+
+
+def build_rollout(name, seed, max_new=None, G=None, n_layers=None, flags=None):
     from paper_2605_30859_b200 import api, workloads as wl
-    c = wl.CONFIGS["c3"]
+    c = wl.CONFIGS[name]
     cfg = dict(c["model"])
     if n_layers:
         cfg["n_layers"] = n_layers
     G = c["G"] if G is None else G
     max_new = c["max_new"] if max_new is None else max_new
     model = wl.make_model(cfg, seed=seed, device="cuda")
-    R = G * c["Kp"]
+    Kp_max = c["Kp"] if isinstance(c["Kp"], int) else max(c["Kp"])
+    R = G * Kp_max
     page = 64
-    # pool: prefix + every row's worst case is far too much; size for the expected peak (~42 GB at full size) with margin
+    # pool: every row's worst case is far too much; size for the expected peak with margin
     kv_page_bytes = cfg["n_layers"] * 2 * cfg["n_kv_heads"] * page * cfg["head_dim"] * 2
-    n_pages = min(G * (c["P"] // page) + R * (max_new // page + 1), int(64e9 // kv_page_bytes))
+    n_pages = min(G * ((c["P"] + page - 1) // page) + R * (max_new // page + 1), int(KV_POOL_CAP_BYTES[name] // kv_page_bytes))
     d = api.Darts(model, page_size=page, n_pages=n_pages, max_rows=R, max_prompts=G, max_prompt_len=c["P"], max_new=max_new,
-                  flags=api.FLAG_PROFILE_ATTENTION)
+                  flags=api.FLAG_PROFILE_ATTENTION if flags is None else flags)
     return d, model, c, cfg, G, max_new
 
 
 def rollout_algo_attention_bytes(lens, Kp, P, kvb):
-    """Algorithmic KV bytes the attention of ONE layer must read over a whole rollout (prefix once per active group)."""
-    lens = np.asarray(lens).reshape(-1, Kp)
+    """Algorithmic KV bytes the attention of ONE layer must read over a whole rollout (prefix once per active group).
+    lens: final lengths per row (group-major), Kp: [G] rows per group."""
+    lens = np.asarray(lens)
+    offs = np.concatenate([[0], np.cumsum(Kp)])
+    grp = np.repeat(np.arange(len(Kp)), Kp)
     total, per_step = 0, []
     for s in range(1, int(lens.max())):
         act = lens > s                              # rows that are fed token s-1 at decode step s
-        b = (int(act.sum()) * s + int(act.any(axis=1).sum()) * P) * kvb
+        n_groups = len(np.unique(grp[act]))
+        b = (int(act.sum()) * s + n_groups * P) * kvb
         per_step.append(b)
         total += b
     return total, per_step
+
+
+def oracle_rollout_sample(name, model_gpu, cfg, P, n_tokens=1, seed=0):
+    """cpu_baseline / reference arm: the oracle (oracle/, numpy fp64) decoding `n_tokens` tokens of ONE trajectory of
+    the workload's model at context P.  The prompt's KV is drawn N(0,1) instead of being prefilled (an oracle prefill
+    of P tokens at this size takes minutes); per-token cost is what the sample measures."""
+    import torch
+    from oracle import transformer as otf
+    from oracle.sampling import sample_token
+    from paper_2605_30859_b200 import workloads as wl
+    host = wl.host_model(model_gpu)                 # bf16 bits copied to the host; up-cast to fp64 inside the oracle
+    rng = np.random.default_rng(seed)
+    Hkv, hd = cfg["n_kv_heads"], cfg["head_dim"]
+    kv = [(rng.standard_normal((P, Hkv, hd)), rng.standard_normal((P, Hkv, hd))) for _ in range(cfg["n_layers"])]
+    tok = 1
+    t0 = time.perf_counter()
+    for s in range(n_tokens):
+        z = otf.decode_one(host, kv, tok, P + s)
+        tok, _ = sample_token(z, 1.0, seed, 0, 0, s + 1)
+    dt = time.perf_counter() - t0
+    return n_tokens / dt, dt, os.cpu_count()
 
 
 def main():
@@ -190,7 +218,8 @@ def main():
     ap.add_argument("--steps", type=int, default=2)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours")
-    ap.add_argument("--workload", default="c2")
+    ap.add_argument("--workload", default="c3", choices=["c2", "c3", "c4", "c5"])
+    ap.add_argument("--mode", default="auto", choices=["auto", "early"], help="early: force shortest-only + early stop (DESIGN.md R17 variant)")
     ap.add_argument("--max-new", type=int, default=None, help="debug only: shorten the rollout (INVALID as a bench number)")
     ap.add_argument("--G", type=int, default=None, help="debug only")
     ap.add_argument("--layers", type=int, default=None, help="debug only")
@@ -207,6 +236,7 @@ def main():
     sampler = ClockSampler(local) if rank == 0 else None
     line = dict(n_gpus=world, steps=args.steps, warmup=args.warmup, higher_is_better=True, scaling="weak", vs_baseline=None,
                 dtype="bf16", data="synthetic")
+    cpu_model = None
 
     if args.workload == "c2":
         barrier(world)
@@ -222,94 +252,105 @@ def main():
                                   kernel="attn_main_k+attn_merge_k", peak_source=peaks["source"]),
                     gpu_launches=res["launches"])
     else:
-        d, model, c, cfg, G, max_new = build_c3(seed=0, max_new=args.max_new, G=args.G, n_layers=args.layers)
-        Kp, K, P = c["Kp"], c["K"], c["P"]
-        R = G * Kp
-        kvb = KV_BYTES_PER_TOKEN_LAYER["c3"]
-        host_in = []
-        for it in range(args.warmup + 2 * args.steps):
-            xin = wl.rollout_inputs("c3", seed=1000 * rank + it, G=G, max_new=max_new)
-            host_in.append(xin)
+        name = args.workload
+        d, model, c, cfg, G, max_new = build_rollout(name, seed=0, max_new=args.max_new, G=args.G, n_layers=args.layers)
+        K, P = c["K"], c["P"]
+        mode = api.MODE_SHORTEST_EARLY_STOP if args.mode == "early" else api.MODE_AUTO
+        kvb = 2 * cfg["n_kv_heads"] * cfg["head_dim"] * 2
+        n_runs = args.warmup + 2 * args.steps
+        host_in = [wl.rollout_inputs(name, seed=1000 * rank + it, G=G, max_new=max_new) for it in range(n_runs)]
         pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
-        gen_tokens, dev_ms, e2e_ms, attn_ms, attn_bytes, steps_count = [], [], [], [], [], []
-        launches0 = None
+        gen_tokens, kept_tokens, dev_ms, e2e_ms, e2e_tokens, attn_ms, attn_bytes, steps_count, near = [], [], [], [], [], [], [], [], []
+        launches = 0
         it = 0
         for phase, n in (("warmup", args.warmup), ("device", args.steps), ("e2e", args.steps)):
-            if phase == "device":
+            if phase != "warmup":
                 barrier(world)
-                launches0 = d.counters()["kernel_launches"]
-                t_dev0 = time.perf_counter()
             for _ in range(n):
                 xin = host_in[it]; it += 1
                 if phase == "e2e":
                     p_pin, f_pin = pin(xin["prompts"]), pin(xin["forced_len"])
                     t0 = time.perf_counter()
-                    out = d.rollout_host(p_pin.numpy(), xin["Kp"], K, max_new, 1.0, 7 + it, forced_len=f_pin.numpy())
+                    out = d.rollout_host(p_pin.numpy(), xin["Kp"], K, max_new, 1.0, 7 + it, forced_len=f_pin.numpy(), mode=mode)
                     e2e_ms.append((time.perf_counter() - t0) * 1e3)
-                    gen = int(out["len"].sum())
-                    e2e_tokens = gen
+                    e2e_tokens.append(int(out["len"].sum()))
                 else:
-                    p_dev = torch.from_numpy(xin["prompts"]).cuda()
-                    f_dev = torch.from_numpy(xin["forced_len"]).cuda()
+                    toks = torch.from_numpy(np.ascontiguousarray(xin["prompts"])).cuda()
+                    f_dev = torch.from_numpy(np.ascontiguousarray(xin["forced_len"])).cuda()
+                    l0 = d.counters()["kernel_launches"]
                     torch.cuda.synchronize()
                     a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                     a.record(d.stream)
-                    d.rollout(p_dev, G, Kp, K, max_new, 1.0, 7 + it, forced_len_dev=f_dev)
+                    d.prefill_device(toks, P, xin["Kp"], K, temperature=1.0, seed=7 + it, forced_len_dev=f_dev, mode=mode, max_len=max_new)
+                    d.run_to_completion()
                     b.record(d.stream)
                     torch.cuda.synchronize()
                     if phase == "device":
                         dev_ms.append(a.elapsed_time(b))
                         cnt = d.counters()
-                        gen_tokens.append(cnt["n_generated_tokens"])
-                        steps_count.append(cnt["n_steps"])
+                        launches += cnt["kernel_launches"] - l0
+                        gen_tokens.append(cnt["n_generated_tokens"]); kept_tokens.append(cnt["n_kept_tokens"])
+                        steps_count.append(cnt["n_steps"]); near.append(cnt["n_near_ties"])
                         res = d.results()
-                        tot, per_step = rollout_algo_attention_bytes(res["len"], Kp, P, kvb)
+                        tot, per_step = rollout_algo_attention_bytes(res["len"], xin["Kp"], P, kvb)
                         t_ms = d.attention_times()
-                        n = min(len(t_ms), len(per_step))
-                        attn_ms.append(float(np.sum(t_ms[:n])))
-                        attn_bytes.append(float(np.sum(per_step[:n])))
-            if phase == "device":
+                        m = min(len(t_ms), len(per_step))
+                        attn_ms.append(float(np.sum(t_ms[:m])))
+                        attn_bytes.append(float(np.sum(per_step[:m])))
+            if phase != "warmup":
                 barrier(world)
-                launches = d.counters()["kernel_launches"] - launches0
         tot_ms = allreduce(world, float(np.sum(dev_ms)), "MAX")
         tot_tok = allreduce(world, float(np.sum(gen_tokens)), "SUM")
         tot_e2e_ms = allreduce(world, float(np.sum(e2e_ms)), "MAX")
-        e2e_tok = allreduce(world, float(e2e_tokens * 0 + sum(int(0) for _ in ()) + 0), "SUM") if False else None
+        tot_e2e_tok = allreduce(world, float(np.sum(e2e_tokens)), "SUM")
         ach = float(np.sum(attn_bytes)) / (float(np.sum(attn_ms)) * 1e-3) / 1e9 if np.sum(attn_ms) > 0 else 0.0
-        h2d = int(host_in[0]["prompts"].nbytes + host_in[0]["forced_len"].nbytes)
+        R = int(host_in[0]["Kp"].sum())
+        h2d = int(host_in[0]["prompts"].nbytes + host_in[0]["forced_len"].nbytes + host_in[0]["Kp"].nbytes)
         d2h = int(R * max_new * 8 + R * 5 + G * (K * 4 + 4 * 4))
-        # e2e tokens: re-count from the e2e phase inputs (same distribution as the device phase)
+        attn_share = float(np.sum(attn_ms)) * cfg["n_layers"] / max(float(np.sum(dev_ms)), 1e-9)
+        rule = {"c3": "K'=16 >= 2K: shortest-only + early stop", "c4": "K' in {8,12,16}: early stop only for K'=16 prompts, dual-end otherwise",
+                "c5": "K'=12 < 2K: dual-end, no early stop"}[name] if args.mode == "auto" else "forced shortest-only + early stop (variant, DESIGN.md R17)"
         line.update(metric="rollout generated tokens/s on 1 B200 (K'-of-K early stop)", value=tot_tok / (tot_ms * 1e-3), unit="tokens/s",
-                    ms_per_step=tot_ms / args.steps,
-                    config=dict(workload=f"c3: Qwen3-4B-shaped bf16 ({cfg['n_layers']} layers), G={G} x K'={Kp}, keep {K}, P={P}, max_new={max_new}, "
-                                         "forced-EOS lognormal(7.2,0.9), mode AUTO (K'>=2K: shortest-only + early stop)",
-                                l2="per-step working set (8 GB weights + KV) >> 126 MB L2, no flush",
-                                steps_per_rollout=int(np.mean(steps_count)), generated_tokens_per_rollout=int(np.mean(gen_tokens))),
+                    ms_per_step=tot_ms / max(1, args.steps),
+                    config=dict(workload=f"{name}: {cfg['n_layers']} layers d={cfg['d_model']} bf16, G={G} prompts of {P}, K'={c['Kp']}, keep {K}, "
+                                         f"max_new={max_new}, forced-EOS {c['forced']['kind']}, rule: {rule}",
+                                l2="per-step working set (weights + KV, > 8 GB) >> 126 MB L2, no flush",
+                                decode_steps_per_rollout=int(np.mean(steps_count)), generated_tokens_per_rollout=int(np.mean(gen_tokens)),
+                                kept_tokens_per_rollout=int(np.mean(kept_tokens)), near_ties_per_rollout=int(np.mean(near)),
+                                ms_per_decode_step=float(np.sum(dev_ms) / max(1, np.sum(steps_count)))),
                     roofline=dict(bound="hbm", achieved=ach, peak=peaks["hbm"], unit="GB/s", frac=ach / peaks["hbm"], traffic=None,
-                                  kernel="attn_main_k+attn_merge_k (layer 0 of every decode step, CUDA events inside the rollout)",
-                                  peak_source=peaks["source"]),
+                                  kernel="attn_main_k+attn_merge_k (layer 0 of every decode step, CUDA events on the library's stream inside the rollout)",
+                                  share_of_step=attn_share, peak_source=peaks["source"]),
                     gpu_launches=int(launches))
-        line["e2e"] = dict(value=None, unit="tokens/s", h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h, ms_per_step=tot_e2e_ms / max(1, args.steps))
-        line["_e2e_ms"] = tot_e2e_ms
+        line["e2e"] = dict(value=tot_e2e_tok / (tot_e2e_ms * 1e-3) if tot_e2e_ms > 0 else None, unit="tokens/s", h2d_bytes_per_step=h2d,
+                           d2h_bytes_per_step=d2h, ms_per_step=tot_e2e_ms / max(1, args.steps), api="darts_rollout_host (pinned host buffers in, host results out)")
         if args.max_new or args.G or args.layers:
             line["config"]["INVALID"] = "debug flags shrink the workload"
         d.close()
+        if rank == 0 and not args.no_cpu_baseline:
+            cpu_model = dict(cfg=model["cfg"], layers=[{k: v.cpu() for k, v in L.items()} for L in model["layers"]],
+                             **{k: model[k].cpu() for k in ("embed", "lm_head", "final_norm")})
         del model
         torch.cuda.empty_cache()
-        # attention microbench (config 2) alongside: the kernel timed alone
+        # attention microbench (config 2) alongside: the dominant kernel timed alone on BASELINE.json configs[1]
         if rank == 0:
             res2, _ = attention_microbench(10, 3)
             a2 = res2["algo_bytes"] / (res2["ms"] * 1e-3) / 1e9
-            line["attention_c2"] = dict(ms=res2["ms"], achieved_GBps=a2, frac_of_measured_peak=a2 / peaks["hbm"], rows=res2["rows"])
+            line["attention_c2"] = dict(ms=res2["ms"], achieved_GBps=a2, frac_of_measured_peak=a2 / peaks["hbm"], rows=res2["rows"],
+                                        ncu_traffic_over_algorithmic=1.075, ncu_source="profiles/r1_attention_c2.md")
 
     if rank == 0:
         line["clocks"] = sampler.stop()
         if not args.no_cpu_baseline:
-            v, n, cores = oracle_attention_sample()
-            line["cpu_baseline"] = dict(value=v, unit="attention rows/s" if args.workload == "c2" else "attention rows/s (oracle, c2 rows)", cores=cores,
-                                        kind="oracle", sample=f"{n} rows of config 2 (1 prompt group), oracle.attention.attention_row, numpy fp64")
-        if "_e2e_ms" in line:
-            line.pop("_e2e_ms")
+            if args.workload == "c2":
+                v, n, cores = oracle_attention_sample()
+                line["cpu_baseline"] = dict(value=v, unit="attention rows/s", cores=cores, kind="oracle",
+                                            sample=f"{n} rows of config 2 (1 prompt group), oracle.attention.attention_row, numpy fp64")
+            else:
+                v, dt, cores = oracle_rollout_sample(args.workload, cpu_model, cfg, P)
+                line["cpu_baseline"] = dict(value=v, unit="tokens/s", cores=cores, kind="oracle",
+                                            sample=f"1 decode token of one {args.workload} trajectory at context {P} (oracle.transformer.decode_one, numpy fp64, "
+                                                   f"prompt KV drawn at random instead of prefilled), {dt:.1f} s")
         print(json.dumps(line))
     if world > 1:
         import torch.distributed as dist
@@ -317,13 +358,43 @@ def main():
 
 
 def reference_arm(args):
+    """The tier's reference arm: the oracle as it stands on the host cores, same metric / config, bounded sample per step."""
     rank = int(os.environ.get("RANK", 0))
     if rank != 0:
         return
-    v, n, cores = oracle_attention_sample()
-    print(json.dumps(dict(impl="reference", metric="decode attention rows/s", value=v, unit="rows/s", n_gpus=args.gpus, steps=args.steps,
-                          warmup=args.warmup, higher_is_better=True, cpu_baseline=dict(value=v, kind="oracle", cores=cores, sample=f"{n} rows"),
-                          e2e=dict(value=v, unit="rows/s", h2d_bytes_per_step=0, d2h_bytes_per_step=0))))
+    import torch
+    from paper_2605_30859_b200 import workloads as wl
+    name = args.workload
+    if name == "c2":
+        v, n, cores = oracle_attention_sample()
+        print(json.dumps(dict(impl="reference", metric="decode attention rows (generated tokens)/s, one step over all rows", value=v, unit="tokens/s",
+                              n_gpus=args.gpus, steps=args.steps, warmup=args.warmup, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64",
+                              data="synthetic", config=dict(workload="c2 (sample of rows)"),
+                              cpu_baseline=dict(value=v, unit="tokens/s", kind="oracle", cores=cores, sample=f"{n} rows"),
+                              e2e=dict(value=v, unit="tokens/s", h2d_bytes_per_step=0, d2h_bytes_per_step=0))))
+        return
+    c = wl.CONFIGS[name]
+    cfg = dict(c["model"])
+    if args.layers:
+        cfg["n_layers"] = args.layers
+    dev = "cuda" if torch.cuda.is_available() else "cpu"      # the device only draws the seeded weights; the oracle runs on the host
+    model = wl.make_model(cfg, seed=0, device=dev)
+    cpu_model = dict(cfg=model["cfg"], layers=[{k: v.cpu() for k, v in L.items()} for L in model["layers"]],
+                     **{k: model[k].cpu() for k in ("embed", "lm_head", "final_norm")})
+    del model
+    for _ in range(min(args.warmup, 1)):                       # one untimed token pages the weights in
+        oracle_rollout_sample(name, cpu_model, cfg, c["P"])
+    tok, secs, cores = 0, 0.0, 0
+    for _ in range(args.steps):
+        v, dt, cores = oracle_rollout_sample(name, cpu_model, cfg, c["P"])
+        tok += 1; secs += dt
+    v = tok / secs
+    sample = f"each step = 1 decode token of one {name} trajectory at context {c['P']} (oracle.transformer.decode_one, numpy fp64)"
+    print(json.dumps(dict(impl="reference", metric="rollout generated tokens/s on 1 B200 (K'-of-K early stop)", value=v, unit="tokens/s", n_gpus=args.gpus,
+                          steps=args.steps, warmup=args.warmup, ms_per_step=secs / max(1, args.steps) * 1e3, higher_is_better=True, scaling="weak",
+                          vs_baseline=None, dtype="f64", data="synthetic", config=dict(workload=f"{name} (bounded sample: {sample})"),
+                          cpu_baseline=dict(value=v, unit="tokens/s", kind="oracle", cores=cores, sample=sample),
+                          e2e=dict(value=v, unit="tokens/s", h2d_bytes_per_step=0, d2h_bytes_per_step=0))))
 
 
 if __name__ == "__main__":

@@ -183,6 +183,22 @@ class Darts:
         self.G, self.R, self.K = G, int(Kp.sum()), K
         self._keep_inputs = (toks, fl)
 
+    def prefill_device(self, prompts_dev, P, Kp, K, temperature=1.0, seed=0, forced_len_dev=None, L_long=1, M_up=0, mode=MODE_AUTO,
+                       max_len=None):
+        """darts_prefill with inputs already resident in HBM: prompts_dev [G,P] int32 (cuda), forced_len_dev [G, max Kp] int32 (cuda)."""
+        assert prompts_dev.is_cuda and prompts_dev.dtype == torch.int32 and prompts_dev.is_contiguous()
+        assert max_len is None or max_len == self.max_new
+        G = prompts_dev.shape[0]
+        Kp = np.ascontiguousarray(Kp, dtype=np.int32)
+        offs = (np.arange(G + 1) * P).astype(np.int32)
+        if forced_len_dev is not None:
+            assert forced_len_dev.is_cuda and forced_len_dev.dtype == torch.int32 and tuple(forced_len_dev.shape) == (G, int(Kp.max()))
+        pol = Policy(K=K, L_long=L_long, M_up=M_up, mode=mode)
+        self._check(darts_prefill(self.ctx, prompts_dev.data_ptr(), _np_ptr(offs), G, _np_ptr(Kp),
+                                  forced_len_dev.data_ptr() if forced_len_dev is not None else None, C.byref(pol), temperature, seed))
+        self.G, self.R, self.K = G, int(Kp.sum()), K
+        self._keep_inputs = (prompts_dev, forced_len_dev)
+
     def decode_step(self):
         self._check(darts_decode_step(self.ctx))
 

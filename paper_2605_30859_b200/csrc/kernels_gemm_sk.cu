@@ -193,15 +193,22 @@ __global__ void __launch_bounds__(SK_THREADS, 1) gemm_sk_k(const __grid_constant
       const bool n_ok = n < p.N;
       float *dst = p.C + (size_t)pc.slot * p.slot_stride + (size_t)pc.row0 * p.N + n;
       const uint32_t src = tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)(buf * p.tm_cols);
+      const size_t ldc = (size_t)p.N;
 #pragma unroll 1
       for (int c = 0; c < pc.nrows; c += 32) {
         uint32_t v[32];
         tmem_ld32(src + c, v);
         tmem_ld_wait();
         if (n_ok) {
+          float *q = dst + (size_t)c * ldc;                // one pointer bump per store, no per-element predicate on full chunks
+          if (c + 32 <= pc.nrows) {
 #pragma unroll
-          for (int j = 0; j < 32; ++j)
-            if (c + j < pc.nrows) dst[(size_t)(c + j) * p.N] = __uint_as_float(v[j]);
+            for (int j = 0; j < 32; ++j, q += ldc) *q = __uint_as_float(v[j]);
+          } else {
+#pragma unroll
+            for (int j = 0; j < 32; ++j, q += ldc)
+              if (c + j < pc.nrows) *q = __uint_as_float(v[j]);
+          }
         }
       }
       tc_fence_before();

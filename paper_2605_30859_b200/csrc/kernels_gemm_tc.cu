@@ -64,10 +64,10 @@ __global__ void __launch_bounds__(GEMM_THREADS) gemm_tc_k(const __grid_constant_
   int row_begin, row_end;
   if (p.grp_off) { row_begin = p.grp_off[grp]; row_end = p.grp_off[grp + 1]; }
   else { row_begin = 0; row_end = p.n_rows_dev ? min(*p.n_rows_dev, p.rows_ub) : p.rows_ub; }
-  const int m0 = row_begin + blockIdx.y * BM;
+  const int m0 = row_begin + blockIdx.x * BM;             // row tiles vary fastest: the CTAs that share a weight tile run together (L2 reuse)
   if (m0 >= row_end) return;
   const int live = min(BM, row_end - m0);                // live rows of this tile
-  const int n0 = blockIdx.x * BN;
+  const int n0 = blockIdx.y * BN;
   const int nkb = p.K / BK;
   const int kb0 = (int)((long long)split * nkb / p.S), kb1 = (int)((long long)(split + 1) * nkb / p.S);
 
@@ -179,7 +179,7 @@ __global__ void __launch_bounds__(GEMM_THREADS) gemm_tc_k(const __grid_constant_
             }
           }
         }
-        if (row_ok) p.top2[(size_t)blockIdx.x * p.rows_ub + r] = make_float4(b1, b2, __int_as_float(i1), 0.f);
+        if (row_ok) p.top2[(size_t)blockIdx.y * p.rows_ub + r] = make_float4(b1, b2, __int_as_float(i1), 0.f);
       }
     }
   }
@@ -267,7 +267,7 @@ darts_status launch_gemm_tc(darts_ctx *c, const TcGemm &g) {
   p.C = g.C; p.split_stride = g.split_stride; p.N = g.N; p.K = g.K; p.S = g.S; p.rows_ub = g.rows_ub; p.n_rows_dev = g.n_rows_dev;
   p.grp_off = g.grp_off; p.b_rows_per_group = g.b_rows_per_group;
   int groups = g.grp_off ? g.n_groups : 1;
-  dim3 grid((g.N + 127) / 128, (g.rows_ub + BM - 1) / BM, groups * g.S);
+  dim3 grid((g.rows_ub + BM - 1) / BM, (g.N + 127) / 128, groups * g.S);
   if (!g.sample) return launch_cfg<128, 3, EPI_STORE>(c, *g.a_map, *g.b_map, p, grid);
   p.top2 = (float4 *)c->top2; p.logits_dump = (c->rt.flags & DARTS_FLAG_DUMP_LOGITS) ? c->logits : nullptr;
   p.row_list = c->row_list; p.row_prompt = c->row_prompt; p.row_sample = c->row_sample; p.row_len = c->row_len;
