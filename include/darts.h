@@ -210,6 +210,19 @@ darts_status darts_debug_gemm_scratch_floats(darts_ctx *ctx, int32_t rows, int32
 darts_status darts_debug_gemm_bf16(darts_ctx *ctx, const void *X, const void *W, float *C, float *scratch, int32_t rows,
                                    int32_t N, int32_t K, int32_t split_k);
 
+/* ---- Adaptive redundancy allocation (§4.2.2; App. B Eq. 6-9 :384-411; App. C Alg. 1 :413-462) --------
+ * Host-only helpers for the step upstream of the rollout: per-prompt length variances (darts_results.len_var) -> EMA ->
+ * total budget -> greedy plan Kp[G] for the next darts_prefill.  All pointers HOST.  No context, no GPU work.
+ * darts_update_variance_ema: var_ema[i] <- (1-beta) var_ema[i] + beta len_var[i]; var_ema[i] < 0 means "no history".
+ * darts_redundancy_budget:   M* = rho/(lambda k) (Eq. 8), *M_total_out = clip(floor(M*), K G, 2 K G) (Eq. 9).
+ * darts_allocate_redundancy: Alg. 1 with w_i = min-max normalised sqrt(var_ema[i]) (all equal: 1), marginal gain
+ *   w_i (1/M'_i - 1/(M'_i+1)) (R18), ties -> smallest i; needs G M_low <= M_total; the plan sums to
+ *   min(M_total, G M_up).  DARTS_ERR_INVALID_ARG on NULLs, non-positive sizes or negative / NaN variances. */
+darts_status darts_update_variance_ema(float *var_ema_host, const float *len_var_host, int32_t G, float beta);
+darts_status darts_redundancy_budget(double rho, double lambda, double k, int32_t G, int32_t K, int64_t *M_total_out);
+darts_status darts_allocate_redundancy(const float *var_ema_host, int32_t G, int64_t M_total, int32_t M_low, int32_t M_up,
+                                       int32_t *Kp_out_host);
+
 /* ---- Attention-only entry points (BASELINE.json config 2) -------------------
  * Build G groups of Kp rows whose KV is given explicitly, then time darts_attention alone.
  * k_prefix/v_prefix: DEVICE [G][P][n_kv_heads][head_dim]; suffix_len: HOST [R]; k_suffix/v_suffix:

@@ -84,6 +84,9 @@ darts_debug_logits = _sig("darts_debug_logits", _ctx, _i32, _vp)
 darts_debug_set_last_tokens = _sig("darts_debug_set_last_tokens", _ctx, _vp, _i32)
 darts_debug_gemm_bf16 = _sig("darts_debug_gemm_bf16", _ctx, _vp, _vp, _vp, _vp, _i32, _i32, _i32, _i32)
 darts_debug_gemm_scratch_floats = _sig("darts_debug_gemm_scratch_floats", _ctx, _i32, _i32, _i32, _i32, C.POINTER(C.c_size_t))
+darts_update_variance_ema = _sig("darts_update_variance_ema", _vp, _vp, _i32, _f32)
+darts_redundancy_budget = _sig("darts_redundancy_budget", C.c_double, C.c_double, C.c_double, _i32, _i32, C.POINTER(C.c_int64))
+darts_allocate_redundancy = _sig("darts_allocate_redundancy", _vp, _i32, C.c_int64, _i32, _i32, _vp)
 darts_attn_load = _sig("darts_attn_load", _ctx, _i32, _i32, _i32, _vp, _vp, _vp, _vp, _vp)
 darts_attention = _sig("darts_attention", _ctx, _i32, _vp, _vp)
 
@@ -112,6 +115,33 @@ def model_desc(cfg, eos_id=None):
     m.rope_theta, m.rms_eps = float(cfg["rope_theta"]), float(cfg["rms_eps"])
     m.eos_id = int(cfg["vocab"] - 1 if eos_id is None else eos_id)
     return m
+
+
+def update_variance_ema(var_ema, len_var, beta):
+    """In-place EMA of the per-prompt length variances (float32 arrays)."""
+    assert var_ema.dtype == np.float32 and var_ema.flags.c_contiguous
+    lv = np.ascontiguousarray(len_var, dtype=np.float32)
+    st = darts_update_variance_ema(_np_ptr(var_ema), _np_ptr(lv), len(var_ema), beta)
+    if st != OK:
+        raise DartsError(st, "darts_update_variance_ema")
+    return var_ema
+
+
+def redundancy_budget(rho, lam, k, G, K):
+    out = C.c_int64()
+    st = darts_redundancy_budget(rho, lam, k, G, K, C.byref(out))
+    if st != OK:
+        raise DartsError(st, "darts_redundancy_budget")
+    return out.value
+
+
+def allocate_redundancy(var_ema, M_total, M_low, M_up):
+    v = np.ascontiguousarray(var_ema, dtype=np.float32)
+    out = np.empty(len(v), np.int32)
+    st = darts_allocate_redundancy(_np_ptr(v), len(v), M_total, M_low, M_up, _np_ptr(out))
+    if st != OK:
+        raise DartsError(st, "darts_allocate_redundancy")
+    return out
 
 
 class Darts:
