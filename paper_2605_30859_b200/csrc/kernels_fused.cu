@@ -110,6 +110,29 @@ __device__ __forceinline__ float4 sk_sum4(const SkView &v, int np, size_t idx) {
   return a;
 }
 
+// Two elements at once (gate / up, the two halves of a rotary pair): both first pieces, then both tails, so the loads of the two
+// sums overlap instead of forming two dependent round trips to L2.
+__device__ __forceinline__ void sk_sum4x2(const SkView &v, int npa, size_t ia, int npb, size_t ib, float4 &a, float4 &b) {
+  const float4 *pa = reinterpret_cast<const float4 *>(v.part + ia), *pb = reinterpret_cast<const float4 *>(v.part + ib);
+  const size_t st = v.slot_stride / 4;
+  a = __ldg(pa);
+  b = __ldg(pb);
+  const int np = max(npa, npb);
+  for (int s0 = 1; s0 < np; s0 += 2) {
+    float4 xa[2], xb[2];
+#pragma unroll
+    for (int s = 0; s < 2; ++s) {
+      if (s0 + s < npa) xa[s] = __ldg(pa + (size_t)(s0 + s) * st);
+      if (s0 + s < npb) xb[s] = __ldg(pb + (size_t)(s0 + s) * st);
+    }
+#pragma unroll
+    for (int s = 0; s < 2; ++s) {
+      if (s0 + s < npa) { a.x += xa[s].x; a.y += xa[s].y; a.z += xa[s].z; a.w += xa[s].w; }
+      if (s0 + s < npb) { b.x += xb[s].x; b.y += xb[s].y; b.z += xb[s].z; b.w += xb[s].w; }
+    }
+  }
+}
+
 __device__ __forceinline__ uint2 pack4_bf16(float a, float b, float c, float d) {
   __nv_bfloat162 o0 = __floats2bfloat162_rn(a, b), o1 = __floats2bfloat162_rn(c, d);
   uint2 o;
@@ -129,8 +152,8 @@ __global__ void __launch_bounds__(256) add_rmsnorm_sk_k(float *__restrict__ h, S
   float4 *hr = reinterpret_cast<float4 *>(h + (size_t)slot * d);
   float ss = 0.f;
   for (int k = threadIdx.x; k < d / 4; k += blockDim.x) {
+    float4 x = hr[k];                                       // in flight together with the piece loads
     float4 a = sk_sum4(v, sk_npieces(v, n_rb, 4 * k, slot), (size_t)slot * d + 4 * k);
-    float4 x = hr[k];
     x.x += a.x; x.y += a.y; x.z += a.z; x.w += a.w;
     hr[k] = x;
     ss += x.x * x.x + x.y * x.y + x.z * x.z + x.w * x.w;
@@ -164,7 +187,8 @@ __global__ void __launch_bounds__(256) silu_mul_sk_k(SkView v, __nv_bfloat16 *__
   if (k >= F) return;
   const int n_rb = (live + SK_ROWBLOCK - 1) / SK_ROWBLOCK;
   const size_t row = (size_t)slot * 2 * F;
-  float4 g = sk_sum4(v, sk_npieces(v, n_rb, k, slot), row + k), u = sk_sum4(v, sk_npieces(v, n_rb, F + k, slot), row + F + k);
+  float4 g, u;
+  sk_sum4x2(v, sk_npieces(v, n_rb, k, slot), row + k, sk_npieces(v, n_rb, F + k, slot), row + F + k, g, u);
   auto f = [](float gg, float uu) { return gg / (1.0f + expf(-gg)) * uu; };
   *reinterpret_cast<uint2 *>(act + (size_t)slot * F + k) = pack4_bf16(f(g.x, u.x), f(g.y, u.y), f(g.z, u.z), f(g.w, u.w));
 }
@@ -193,8 +217,8 @@ __global__ void __launch_bounds__(128) rope_append_sk_k(SkView v, __nv_bfloat16 
   const int p = 4 * lane;
   float a1[4] = {0.f, 0.f, 0.f, 0.f}, a2[4] = {0.f, 0.f, 0.f, 0.f};
   if (act) {
-    float4 x1 = sk_sum4(v, sk_npieces(v, n_rb, col0 + p, slot), row + p);
-    float4 x2 = sk_sum4(v, sk_npieces(v, n_rb, col0 + half + p, slot), row + half + p);
+    float4 x1, x2;
+    sk_sum4x2(v, sk_npieces(v, n_rb, col0 + p, slot), row + p, sk_npieces(v, n_rb, col0 + half + p, slot), row + half + p, x1, x2);
     a1[0] = x1.x; a1[1] = x1.y; a1[2] = x1.z; a1[3] = x1.w;
     a2[0] = x2.x; a2[1] = x2.y; a2[2] = x2.z; a2[3] = x2.w;
   }

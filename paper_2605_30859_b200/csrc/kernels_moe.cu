@@ -18,7 +18,7 @@
 namespace {
 
 constexpr int RROWS = 4;       // slots per router CTA (Wr tile reuse)
-constexpr int REXP = 32;       // experts per router CTA
+constexpr int REXP = 8;        // experts per router CTA (one per warp: the grid, not a loop, covers the experts)
 constexpr int MAX_E_PER_LANE = 8;   // E <= 256
 
 __device__ __forceinline__ int live_rows(const int32_t *n_rows_dev, int rows_ub) { return n_rows_dev ? min(*n_rows_dev, rows_ub) : rows_ub; }
@@ -39,6 +39,8 @@ template <typename T>
 __global__ void __launch_bounds__(256) moe_router_k(const float *__restrict__ h, const T *__restrict__ wnorm, const float *__restrict__ wr,
                                                     float *__restrict__ logits, int d, int E, float eps, const int32_t *n_rows_dev,
                                                     int rows_ub) {
+  pdl_trigger();
+  pdl_wait();
   extern __shared__ float xs[];                       // [RROWS][d] normalised rows
   __shared__ float red[RROWS][8];
   const int n = live_rows(n_rows_dev, rows_ub);
@@ -68,8 +70,9 @@ __global__ void __launch_bounds__(256) moe_router_k(const float *__restrict__ h,
   for (int e = blockIdx.y * REXP + warp; e < min(E, (int)(blockIdx.y + 1) * REXP); e += 8) {
     float acc[RROWS] = {};
     const float4 *wrow = reinterpret_cast<const float4 *>(wr + (size_t)e * d);
+#pragma unroll 4
     for (int k4 = lane; k4 < d / 4; k4 += 32) {
-      float4 w = wrow[k4];
+      float4 w = __ldg(wrow + k4);
 #pragma unroll
       for (int r = 0; r < RROWS; ++r) {
         float4 x = *reinterpret_cast<const float4 *>(&xs[r * d + 4 * k4]);
@@ -88,6 +91,8 @@ __global__ void __launch_bounds__(256) moe_router_k(const float *__restrict__ h,
 __global__ void __launch_bounds__(128) moe_topk_k(const float *__restrict__ logits, int E, int top_k, int32_t *__restrict__ eid,
                                                   float *__restrict__ gate, int32_t *__restrict__ pos, int32_t *__restrict__ cnt,
                                                   const int32_t *n_rows_dev, int rows_ub) {
+  pdl_trigger();
+  pdl_wait();
   const int n = live_rows(n_rows_dev, rows_ub);
   const int slot = blockIdx.x * 4 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
   if (slot >= n) return;
@@ -142,6 +147,8 @@ __global__ void __launch_bounds__(256) moe_place_k(const int32_t *__restrict__ c
                                                    int32_t *__restrict__ n_rb_out, const __nv_bfloat16 *__restrict__ xn,
                                                    __nv_bfloat16 *__restrict__ xs, int E, int top_k, int d, const int32_t *n_rows_dev,
                                                    int rows_ub) {
+  pdl_trigger();
+  pdl_wait();
   __shared__ int s_red[8], s_redb[8];
   __shared__ int s_off, s_blk;
   const int e = blockIdx.x, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -193,6 +200,8 @@ __global__ void __launch_bounds__(256) moe_place_k(const int32_t *__restrict__ c
 // act[p][f] = silu(g) * u over the expert-sorted rows p < live * top_k;  g = sum_s P_s[p][f], u = sum_s P_s[p][F + f].
 __global__ void __launch_bounds__(256) moe_silu_mul_k(const float *__restrict__ part, int S, size_t split_stride, __nv_bfloat16 *__restrict__ act,
                                                       int F, int top_k, const int32_t *n_rows_dev, int rows_ub) {
+  pdl_trigger();
+  pdl_wait();
   int p = blockIdx.y;
   if (p >= live_rows(n_rows_dev, rows_ub) * top_k) return;
   int k = (blockIdx.x * blockDim.x + threadIdx.x) * 4;
@@ -217,6 +226,8 @@ template <typename T>
 __global__ void __launch_bounds__(256) moe_expert_simt_k(const T *__restrict__ xn, const T *__restrict__ wgu_e, const T *__restrict__ wd_e,
                                                          const int32_t *__restrict__ eid, float *__restrict__ y, int d, int F, int top_k,
                                                          const int32_t *n_rows_dev, int rows_ub) {
+  pdl_trigger();
+  pdl_wait();
   extern __shared__ float sm_f[];                      // x [d], act [F]
   float *x = sm_f, *act = sm_f + d;
   const int a = blockIdx.x, slot = a / top_k;
@@ -247,6 +258,8 @@ __global__ void __launch_bounds__(256) moe_combine_k(float *__restrict__ h, cons
                                                      const int32_t *__restrict__ pos, const float *__restrict__ gate, int top_k,
                                                      const T *__restrict__ wnorm, T *__restrict__ out, int d, float eps,
                                                      const int32_t *n_rows_dev, int rows_ub) {
+  pdl_trigger();
+  pdl_wait();
   int slot = blockIdx.x;
   if (slot >= live_rows(n_rows_dev, rows_ub)) return;
   float4 *hr = reinterpret_cast<float4 *>(h + (size_t)slot * d);
@@ -294,11 +307,11 @@ darts_status route(darts_ctx *c, int layer, int rows_ub, const int32_t *n_rows_d
     CUDA_TRY(c, cudaFuncSetAttribute(moe_router_k<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     attr = true;
   }
-  moe_router_k<T><<<grid, 256, smem, c->stream>>>(c->h, (const T *)c->mlp_norm[layer], (const float *)c->wr[layer], c->moe_logits, m.d_model,
+  launch_pdl(c, moe_router_k<T>, grid, dim3(256), smem, c->h, (const T *)c->mlp_norm[layer], (const float *)c->wr[layer], c->moe_logits, m.d_model,
                                                   m.n_experts, m.rms_eps, n_rows_dev, rows_ub);
   darts_status s = post(c, "moe_router");
   if (s != DARTS_OK) return s;
-  moe_topk_k<<<(rows_ub + 3) / 4, 128, 0, c->stream>>>(c->moe_logits, m.n_experts, m.top_k, c->moe_eid, c->moe_w, c->moe_pos, cnt, n_rows_dev, rows_ub);
+  launch_pdl(c, moe_topk_k, dim3((rows_ub + 3) / 4), dim3(128), 0, c->moe_logits, m.n_experts, m.top_k, c->moe_eid, c->moe_w, c->moe_pos, cnt, n_rows_dev, rows_ub);
   return post(c, "moe_topk");
 }
 
@@ -347,7 +360,7 @@ darts_status launch_moe_tc(darts_ctx *c, int layer, const void *next_norm, int r
   int32_t *cnt = c->moe_cnt + (size_t)layer * E;
   darts_status s;
   if ((s = route<T>(c, layer, rows_ub, n_rows_dev, cnt)) != DARTS_OK) return s;
-  moe_place_k<<<E, 256, 0, c->stream>>>(cnt, c->moe_eid, c->moe_pos, c->moe_tok, c->moe_off, c->moe_rb, c->moe_nrb, (const T *)c->xn, (T *)c->xs, E,
+  launch_pdl(c, moe_place_k, dim3(E), dim3(256), 0, cnt, c->moe_eid, c->moe_pos, c->moe_tok, c->moe_off, c->moe_rb, c->moe_nrb, (const T *)c->xn, (T *)c->xs, E,
                                         m.top_k, d, n_rows_dev, rows_ub);
   if ((s = post(c, "moe_place")) != DARTS_OK) return s;
   // grouped stream-K GEMMs: one row block per (expert, <= 256 of its rows); experts nobody chose cost nothing
@@ -359,12 +372,12 @@ darts_status launch_moe_tc(darts_ctx *c, int layer, const void *next_norm, int r
   g.slot_stride = 0;
   if ((s = launch_gemm_sk(c, g)) != DARTS_OK) return s;
   dim3 grid((F / 4 + 255) / 256, RK);
-  moe_silu_mul_k<<<grid, 256, 0, c->stream>>>(c->part, 1, 0, (T *)c->act, F, m.top_k, n_rows_dev, rows_ub);
+  launch_pdl(c, moe_silu_mul_k, grid, dim3(256), 0, c->part, 1, (size_t)0, (T *)c->act, F, m.top_k, n_rows_dev, rows_ub);
   if ((s = post(c, "moe_silu_mul")) != DARTS_OK) return s;
   g.w_map = &c->tm_wd_e[layer]; g.x_maps = &c->xm_act; g.N = d; g.w_rows_per_group = d;
   g.plan = sk_plan(c->n_sms, g.N, F, rows_ub, n_rb_ub, false);
   if ((s = launch_gemm_sk(c, g)) != DARTS_OK) return s;
-  moe_combine_k<T><<<rows_ub, 256, 0, c->stream>>>(c->h, c->part, 1, 0, c->moe_pos, c->moe_w, m.top_k, (const T *)next_norm, (T *)c->xn, d,
+  launch_pdl(c, moe_combine_k<T>, dim3(rows_ub), dim3(256), 0, c->h, c->part, 1, (size_t)0, c->moe_pos, c->moe_w, m.top_k, (const T *)next_norm, (T *)c->xn, d,
                                                    m.rms_eps, n_rows_dev, rows_ub);
   return post(c, "moe_combine");
 }
