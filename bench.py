@@ -224,10 +224,15 @@ def main():
     ap.add_argument("--G", type=int, default=None, help="debug only")
     ap.add_argument("--layers", type=int, default=None, help="debug only")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--profile-step", type=int, default=None,
+                    help="profiling aid (prints no bench line): run the workload's rollout step by step up to this decode step, then bracket "
+                         "two more steps with cudaProfilerStart/Stop (use with `ncu --profile-from-start off`)")
     args = ap.parse_args()
 
     if args.impl == "reference":
         return reference_arm(args)
+    if args.profile_step is not None:
+        return profile_steps(args)
 
     import torch
     from paper_2605_30859_b200 import api, workloads as wl
@@ -355,6 +360,37 @@ def main():
     if world > 1:
         import torch.distributed as dist
         dist.destroy_process_group()
+
+
+def profile_steps(args):
+    """Rollout of the chosen workload through the step calls of the C-ABI; the two steps after --profile-step are the profiled range."""
+    import torch
+    from paper_2605_30859_b200 import api, workloads as wl
+    torch.cuda.set_device(0)
+    name = args.workload
+    d, model, c, cfg, G, max_new = build_rollout(name, seed=0, max_new=args.max_new, G=args.G, n_layers=args.layers)
+    xin = wl.rollout_inputs(name, seed=0, G=G, max_new=max_new)
+    toks = torch.from_numpy(np.ascontiguousarray(xin["prompts"])).cuda()
+    f_dev = torch.from_numpy(np.ascontiguousarray(xin["forced_len"])).cuda()
+    mode = api.MODE_SHORTEST_EARLY_STOP if args.mode == "early" else api.MODE_AUTO
+    d.prefill_device(toks, c["P"], xin["Kp"], c["K"], temperature=1.0, seed=7, forced_len_dev=f_dev, mode=mode)
+    d.select_and_compact()
+    for _ in range(args.profile_step):
+        d.decode_step()
+        d.select_and_compact()
+    n0 = d.n_active()
+    torch.cuda.synchronize()
+    torch.cuda.profiler.start()
+    for _ in range(2):
+        d.decode_step()
+        d.select_and_compact()
+    torch.cuda.synchronize()
+    torch.cuda.profiler.stop()
+    res = d.results()
+    act = res["status"] == 0
+    print(json.dumps(dict(profiled_steps=[args.profile_step + 1, args.profile_step + 2], active_rows=int(n0),
+                          mean_suffix_tokens=float(res["len"][act].mean()) if act.any() else 0.0, workload=name)))
+    d.close()
 
 
 def reference_arm(args):

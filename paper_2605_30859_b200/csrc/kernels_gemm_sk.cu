@@ -114,6 +114,9 @@ __global__ void __launch_bounds__(SK_THREADS, 1) gemm_sk_k(const __grid_constant
     // Programmatic dependent launch: this kernel may start while the kernel that produces X is still running.  The weights
     // do not depend on it, so the first ring-full of weight tiles is requested BEFORE griddepcontrol.wait; only the
     // activation boxes wait.  (Grouped mode reads its row-block list first and therefore waits at the top.)
+    // One row block: every weight byte is used once (evict-first).  Several row blocks re-read a weight tile a few k-blocks
+    // later: keep it in L2 (evict-last), or the second pass goes back to HBM (measured: 2x DRAM reads on the gate/up GEMM).
+    const uint64_t w_hint = (!p.rb_list && it0.n_rb > 1) ? HINT_EVICT_LAST : HINT_EVICT_FIRST;
     int n_pre = 0;
     if (!p.rb_list) {
       PieceIter it = it0;
@@ -124,7 +127,7 @@ __global__ void __launch_bounds__(SK_THREADS, 1) gemm_sk_k(const __grid_constant
           if (lane == 0) {
             unsigned char *st = stage_base + (size_t)n_pre * p.stage_bytes;
             mbar_expect_tx(&bar.full[n_pre], W_STAGE_BYTES + n16 * BOX_BYTES);
-            tma_load_2d_hint(st, &tmW, kb * BK, pc.wbase + pc.wtile * BMW, &bar.full[n_pre], HINT_EVICT_FIRST);
+            tma_load_2d_hint(st, &tmW, kb * BK, pc.wbase + pc.wtile * BMW, &bar.full[n_pre], w_hint);
           }
       }
     }
@@ -144,7 +147,7 @@ __global__ void __launch_bounds__(SK_THREADS, 1) gemm_sk_k(const __grid_constant
           mbar_wait(&bar.empty[stage], phase ^ 1);
           if (lane == 0) {
             mbar_expect_tx(&bar.full[stage], tx);
-            tma_load_2d_hint(st, &tmW, kb * BK, wrow, &bar.full[stage], HINT_EVICT_FIRST);        // weights: streamed once
+            tma_load_2d_hint(st, &tmW, kb * BK, wrow, &bar.full[stage], w_hint);
           }
           __syncwarp();
         }
