@@ -74,15 +74,20 @@ class ClockSampler:
 
 
 def dist_setup(n):
+    """One process per GPU (torchrun env).  The ranks are independent replicas: the process group only
+    carries the barriers and the max / sum of the timing reduction — NCCL on GPUs, gloo when there is no GPU (CPU tests)."""
     import torch
     rank, world = int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
     local = int(os.environ.get("LOCAL_RANK", 0))
+    cuda = torch.cuda.is_available()
+    if cuda:
+        torch.cuda.set_device(local if world > 1 else 0)
     if world > 1:
         import torch.distributed as dist
-        torch.cuda.set_device(local)
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    else:
-        torch.cuda.set_device(0)
+        if cuda:
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        else:
+            dist.init_process_group("gloo")
     return rank, world, local
 
 
@@ -91,7 +96,8 @@ def barrier(world):
     if world > 1:
         import torch.distributed as dist
         dist.barrier()
-    torch.cuda.synchronize()
+    if torch.cuda.is_available():
+        torch.cuda.synchronize()
 
 
 def allreduce(world, x, op):
@@ -99,9 +105,16 @@ def allreduce(world, x, op):
     if world == 1:
         return x
     import torch.distributed as dist
-    t = torch.tensor([x], dtype=torch.float64, device="cuda")
+    t = torch.tensor([x], dtype=torch.float64, device="cuda" if torch.cuda.is_available() else "cpu")
     dist.all_reduce(t, op=getattr(dist.ReduceOp, op))
     return float(t.item())
+
+
+def aggregate(world, local_ms, local_units):
+    """Whole-job throughput of N independent replicas: units of all ranks / the slowest rank's time (max over ranks)."""
+    ms = allreduce(world, float(local_ms), "MAX")
+    units = allreduce(world, float(local_units), "SUM")
+    return units / (ms * 1e-3), ms, units
 
 
 # ------------------------------------------------------------------------------------------------ c2: attention step
@@ -304,10 +317,8 @@ def main():
                         attn_bytes.append(float(np.sum(per_step[:m])))
             if phase != "warmup":
                 barrier(world)
-        tot_ms = allreduce(world, float(np.sum(dev_ms)), "MAX")
-        tot_tok = allreduce(world, float(np.sum(gen_tokens)), "SUM")
-        tot_e2e_ms = allreduce(world, float(np.sum(e2e_ms)), "MAX")
-        tot_e2e_tok = allreduce(world, float(np.sum(e2e_tokens)), "SUM")
+        value, tot_ms, tot_tok = aggregate(world, np.sum(dev_ms), np.sum(gen_tokens))
+        e2e_value, tot_e2e_ms, tot_e2e_tok = aggregate(world, max(np.sum(e2e_ms), 1e-9), np.sum(e2e_tokens))
         ach = float(np.sum(attn_bytes)) / (float(np.sum(attn_ms)) * 1e-3) / 1e9 if np.sum(attn_ms) > 0 else 0.0
         R = int(host_in[0]["Kp"].sum())
         h2d = int(host_in[0]["prompts"].nbytes + host_in[0]["forced_len"].nbytes + host_in[0]["Kp"].nbytes)
@@ -315,7 +326,7 @@ def main():
         attn_share = float(np.sum(attn_ms)) * cfg["n_layers"] / max(float(np.sum(dev_ms)), 1e-9)
         rule = {"c3": "K'=16 >= 2K: shortest-only + early stop", "c4": "K' in {8,12,16}: early stop only for K'=16 prompts, dual-end otherwise",
                 "c5": "K'=12 < 2K: dual-end, no early stop"}[name] if args.mode == "auto" else "forced shortest-only + early stop (variant, DESIGN.md R17)"
-        line.update(metric="rollout generated tokens/s on 1 B200 (K'-of-K early stop)", value=tot_tok / (tot_ms * 1e-3), unit="tokens/s",
+        line.update(metric="rollout generated tokens/s on 1 B200 (K'-of-K early stop)", value=value, unit="tokens/s",
                     ms_per_step=tot_ms / max(1, args.steps),
                     config=dict(workload=f"{name}: {cfg['n_layers']} layers d={cfg['d_model']} bf16, G={G} prompts of {P}, K'={c['Kp']}, keep {K}, "
                                          f"max_new={max_new}, forced-EOS {c['forced']['kind']}, rule: {rule}",
@@ -327,7 +338,7 @@ def main():
                                   kernel="attn_main_k+attn_merge_k (layer 0 of every decode step, CUDA events on the library's stream inside the rollout)",
                                   share_of_step=attn_share, peak_source=peaks["source"]),
                     gpu_launches=int(launches))
-        line["e2e"] = dict(value=tot_e2e_tok / (tot_e2e_ms * 1e-3) if tot_e2e_ms > 0 else None, unit="tokens/s", h2d_bytes_per_step=h2d,
+        line["e2e"] = dict(value=e2e_value if tot_e2e_tok > 0 else None, unit="tokens/s", h2d_bytes_per_step=h2d,
                            d2h_bytes_per_step=d2h, ms_per_step=tot_e2e_ms / max(1, args.steps), api="darts_rollout_host (pinned host buffers in, host results out)")
         if args.max_new or args.G or args.layers:
             line["config"]["INVALID"] = "debug flags shrink the workload"
