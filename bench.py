@@ -165,6 +165,11 @@ def oracle_attention_sample(x_full_seed=0, n_rows=32):
 
 
 # ------------------------------------------------------------------------------------------------ full rollouts (c3 / c4 / c5)
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE attn_main_k launch from an `ncu --set full` capture (profiles/), with the
+# algorithmic bytes of that same launch beside it (launches differ in size over a rollout; `achieved` is the rollout average)
+NCU_ATTENTION_TRAFFIC = {"c3": dict(dram_bytes=1.2947e9, algorithmic_bytes=1.2322e9, ratio=1.051,
+                                    launch="decode step 1001: 289 rows, mean suffix 1003 tokens, 19 open groups",
+                                    source="profiles/r1_gemm_sk.md (ncu --set full, bench.py --profile-step 1000)")}
 KV_POOL_CAP_BYTES = {"c3": 64e9, "c4": 100e9, "c5": 36e9}
 
 
@@ -334,7 +339,8 @@ def main():
                                 decode_steps_per_rollout=int(np.mean(steps_count)), generated_tokens_per_rollout=int(np.mean(gen_tokens)),
                                 kept_tokens_per_rollout=int(np.mean(kept_tokens)), near_ties_per_rollout=int(np.mean(near)),
                                 ms_per_decode_step=float(np.sum(dev_ms) / max(1, np.sum(steps_count)))),
-                    roofline=dict(bound="hbm", achieved=ach, peak=peaks["hbm"], unit="GB/s", frac=ach / peaks["hbm"], traffic=None,
+                    roofline=dict(bound="hbm", achieved=ach, peak=peaks["hbm"], unit="GB/s", frac=ach / peaks["hbm"],
+                                  traffic=NCU_ATTENTION_TRAFFIC.get(name, {}).get("dram_bytes"), traffic_detail=NCU_ATTENTION_TRAFFIC.get(name),
                                   kernel="attn_main_k+attn_merge_k (layer 0 of every decode step, CUDA events on the library's stream inside the rollout)",
                                   share_of_step=attn_share, peak_source=peaks["source"]),
                     gpu_launches=int(launches))

@@ -42,6 +42,7 @@ struct SkParams {
   const int32_t *rb_list, *n_rb_dev;             // grouped mode
   int unit_tile;
   int stage_bytes, n_stages, tm_cols;            // tm_cols: columns of ONE accumulator (power of two >= 32)
+  int rb_rows, n_acc;                            // rows per row block (256 | 512 = two fused N blocks sharing the weight tile); TMEM accumulators (2 | 1)
 };
 
 struct SkBars {
@@ -55,7 +56,7 @@ struct Piece {
 
 // Walks the pieces of CTA `cta`; the three roles call it with identical arguments and so see the same sequence.
 struct PieceIter {
-  int u, u1, T, P, nkb, n_rb, unit_tile, cta, w_rows_per_group;
+  int u, u1, T, P, nkb, n_rb, unit_tile, cta, w_rows_per_group, rb_rows;
   const int32_t *rb_list;
   int live;
   __device__ bool next(Piece &p) {
@@ -66,7 +67,7 @@ struct PieceIter {
     p.wtile = tile / n_rb;
     int rb = tile - p.wtile * n_rb;
     if (rb_list) { p.row0 = rb_list[4 * rb]; p.nrows = rb_list[4 * rb + 1]; p.wbase = rb_list[4 * rb + 2] * w_rows_per_group; }
-    else { p.row0 = rb * SK_ROWBLOCK; p.nrows = min(SK_ROWBLOCK, live - p.row0); p.wbase = 0; }
+    else { p.row0 = rb * rb_rows; p.nrows = min(rb_rows, live - p.row0); p.wbase = 0; }
     p.slot = unit_tile ? 0 : cta - sk_owner(tile * nkb, P, T);
     u += unit_tile ? 1 : p.kb1 - p.kb0;
     return true;
@@ -83,9 +84,9 @@ __global__ void __launch_bounds__(SK_THREADS, 1) gemm_sk_k(const __grid_constant
   pdl_trigger();
   // ---- this CTA's unit range (uniform over the CTA; leave before any barrier / TMEM allocation if it is empty)
   PieceIter it0;
-  it0.rb_list = p.rb_list; it0.w_rows_per_group = p.w_rows_per_group; it0.nkb = p.nkb; it0.unit_tile = p.unit_tile; it0.P = gridDim.x; it0.cta = blockIdx.x;
+  it0.rb_list = p.rb_list; it0.w_rows_per_group = p.w_rows_per_group; it0.nkb = p.nkb; it0.unit_tile = p.unit_tile; it0.P = gridDim.x; it0.cta = blockIdx.x; it0.rb_rows = p.rb_rows;
   if (p.rb_list) { pdl_wait(); it0.n_rb = *p.n_rb_dev; it0.live = 0; }
-  else { it0.live = p.n_rows_dev ? min(*p.n_rows_dev, p.rows_ub) : p.rows_ub; it0.n_rb = (it0.live + SK_ROWBLOCK - 1) / SK_ROWBLOCK; }
+  else { it0.live = p.n_rows_dev ? min(*p.n_rows_dev, p.rows_ub) : p.rows_ub; it0.n_rb = (it0.live + p.rb_rows - 1) / p.rb_rows; }
   if (it0.n_rb <= 0) return;
   it0.T = p.n_wtiles * it0.n_rb * (p.unit_tile ? 1 : p.nkb);
   it0.u = (int)((long long)blockIdx.x * it0.T / gridDim.x);
@@ -99,7 +100,7 @@ __global__ void __launch_bounds__(SK_THREADS, 1) gemm_sk_k(const __grid_constant
     for (int b = 0; b < 2; ++b) { mbar_init(&bar.acc_full[b], 1); mbar_init(&bar.acc_empty[b], 4); }
     fence_mbar_init();
   }
-  if (warp == 1) tmem_alloc(&bar.tmem_base, 2 * p.tm_cols);
+  if (warp == 1) tmem_alloc(&bar.tmem_base, p.n_acc * p.tm_cols);
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
@@ -139,8 +140,11 @@ __global__ void __launch_bounds__(SK_THREADS, 1) gemm_sk_k(const __grid_constant
       const int n16 = (pc.nrows + BOX_ROWS - 1) / BOX_ROWS;
       const int tx = W_STAGE_BYTES + n16 * BOX_BYTES;
       const int wrow = pc.wbase + pc.wtile * BMW;
-      const bool mine = lane < 5 && ((n16 >> lane) & 1);
-      const int my_row = (n16 & ~((2 << lane) - 1)) * BOX_ROWS;          // rows covered by the larger boxes
+      // sub-block A = rows [0, 256) on lanes 0-4, sub-block B = rows [256, 512) on lanes 8-12 (only with rb_rows = 512)
+      const int sub = lane >> 3, bit = lane & 7;
+      const int n16s = sub == 0 ? min(n16, 16) : n16 - min(n16, 16);
+      const bool mine = sub < 2 && bit < 5 && ((n16s >> bit) & 1);
+      const int my_row = sub * 256 + (n16s & ~((2 << bit) - 1)) * BOX_ROWS;   // rows covered by the larger boxes of this sub-block
       for (int kb = pc.kb0; kb < pc.kb1; ++kb, ++i) {
         unsigned char *st = stage_base + (size_t)stage * p.stage_bytes;
         if (i >= n_pre) {
@@ -152,7 +156,7 @@ __global__ void __launch_bounds__(SK_THREADS, 1) gemm_sk_k(const __grid_constant
           __syncwarp();
         }
         if (mine)
-          tma_load_2d_hint(st + W_STAGE_BYTES + my_row * (BK * 2), &tmX.m[lane], kb * BK, pc.row0 + my_row, &bar.full[stage], HINT_EVICT_LAST);
+          tma_load_2d_hint(st + W_STAGE_BYTES + my_row * (BK * 2), &tmX.m[bit], kb * BK, pc.row0 + my_row, &bar.full[stage], HINT_EVICT_LAST);
         if (++stage == p.n_stages) { stage = 0; phase ^= 1; }
       }
     }
@@ -163,8 +167,9 @@ __global__ void __launch_bounds__(SK_THREADS, 1) gemm_sk_k(const __grid_constant
       Piece pc;
       int stage = 0, phase = 0, piece = 0;
       while (it.next(pc)) {
-        const int buf = piece & 1, use = piece >> 1;
-        const uint32_t idesc = umma_idesc_bf16(BMW, (pc.nrows + 15) & ~15);
+        const int buf = piece % p.n_acc, use = piece / p.n_acc;
+        const int nA = min(pc.nrows, 256), nB = pc.nrows - nA;                  // two MMA N blocks share the weight tile of a stage
+        const uint32_t idesc = umma_idesc_bf16(BMW, (nA + 15) & ~15), idescB = umma_idesc_bf16(BMW, (nB + 15) & ~15);
         mbar_wait(&bar.acc_empty[buf], (use & 1) ^ 1);
         tc_fence_after();
         const uint32_t d = tmem + (uint32_t)(buf * p.tm_cols);
@@ -175,6 +180,11 @@ __global__ void __launch_bounds__(SK_THREADS, 1) gemm_sk_k(const __grid_constant
           const uint64_t dw = umma_desc_sw128(sa), dx = umma_desc_sw128(sa + W_STAGE_BYTES);
 #pragma unroll
           for (int k = 0; k < BK / 16; ++k) mma_bf16_ss(d, dw + 2 * k, dx + 2 * k, idesc, (kb > pc.kb0 || k > 0) ? 1u : 0u);
+          if (nB > 0) {
+            const uint64_t dxb = umma_desc_sw128(sa + W_STAGE_BYTES + 256 * BK * 2);
+#pragma unroll
+            for (int k = 0; k < BK / 16; ++k) mma_bf16_ss(d + 256, dw + 2 * k, dxb + 2 * k, idescB, (kb > pc.kb0 || k > 0) ? 1u : 0u);
+          }
           mma_commit(&bar.empty[stage]);
           if (++stage == p.n_stages) { stage = 0; phase ^= 1; }
         }
@@ -189,7 +199,7 @@ __global__ void __launch_bounds__(SK_THREADS, 1) gemm_sk_k(const __grid_constant
     Piece pc;
     int piece = 0;
     while (it.next(pc)) {
-      const int buf = piece & 1, use = piece >> 1;
+      const int buf = piece % p.n_acc, use = piece / p.n_acc;
       mbar_wait(&bar.acc_full[buf], use & 1);
       tc_fence_after();
       const int n = pc.wtile * BMW + q * 32 + lane;        // output column = weight row
@@ -222,7 +232,7 @@ __global__ void __launch_bounds__(SK_THREADS, 1) gemm_sk_k(const __grid_constant
   }
   tc_fence_before();
   __syncthreads();
-  if (warp == 1) tmem_dealloc(tmem, 2 * p.tm_cols);
+  if (warp == 1) tmem_dealloc(tmem, p.n_acc * p.tm_cols);
 }
 
 // out[r][n] = sum of the pieces of (r, n) in slot order (debug / test hook)
@@ -230,7 +240,7 @@ __global__ void sk_reduce_k(SkView v, float *__restrict__ out, int rows) {
   size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= (size_t)rows * v.N) return;
   int r = (int)(i / v.N), n = (int)(i % v.N);
-  int n_rb = (rows + SK_ROWBLOCK - 1) / SK_ROWBLOCK;
+  int n_rb = (rows + v.rb_rows - 1) / v.rb_rows;
   int np = sk_npieces(v, n_rb, n, r);
   float a = v.part[i];
   for (int s = 1; s < np; ++s) a += v.part[(size_t)s * v.slot_stride + i];
@@ -246,7 +256,11 @@ SkPlan sk_plan(int n_sms, int N, int K, int rows_ub, int n_rb_ub_grouped, bool r
   pl.nkb = K / BK;
   pl.n_wtiles = (N + BMW - 1) / BMW;
   const bool grouped = n_rb_ub_grouped > 0;
-  const int n_rb_ub = grouped ? n_rb_ub_grouped : (rows_ub + SK_ROWBLOCK - 1) / SK_ROWBLOCK;
+  // 257..384 decode rows: one 512-row block = two MMA N blocks per stage that share the weight tile (one pass over the weights,
+  // one TMEM accumulator of 512 columns, 3 stages).  Measured on c3: step time -4 % at 288 rows, -2 % at 384, but +7 % at 512
+  // (2 stages, no epilogue overlap), so above 384 rows the 256-row blocks with two accumulators stay.
+  pl.rb_rows = (!grouped && rows_ub > SK_ROWBLOCK && rows_ub <= 384) ? 2 * SK_ROWBLOCK : SK_ROWBLOCK;
+  const int n_rb_ub = grouped ? n_rb_ub_grouped : (rows_ub + pl.rb_rows - 1) / pl.rb_rows;
   const long long tiles_ub = (long long)pl.n_wtiles * n_rb_ub;
   pl.unit_tile = grouped || tiles_ub >= 8LL * n_sms;
   if (pl.unit_tile) {
@@ -262,11 +276,12 @@ SkPlan sk_plan(int n_sms, int N, int K, int rows_ub, int n_rb_ub_grouped, bool r
       pl.P = std::max(1, pl.P * 3 / 4);
     }
   }
-  int cap = std::min(SK_ROWBLOCK, (rows_ub + 15) & ~15);
+  int cap = std::min(pl.rb_rows, (rows_ub + 15) & ~15);
   pl.stage_bytes = W_STAGE_BYTES + cap / BOX_ROWS * BOX_BYTES;
   pl.n_stages = std::min(MAX_STAGES, SMEM_BUDGET / pl.stage_bytes);
   pl.tm_cols = 32;
   while (pl.tm_cols < cap) pl.tm_cols *= 2;
+  pl.n_acc = pl.tm_cols > 256 ? 1 : 2;
   return pl;
 }
 
@@ -276,7 +291,7 @@ darts_status launch_gemm_sk(darts_ctx *c, const SkGemm &g) {
   SkParams p{};
   p.C = g.C; p.slot_stride = g.slot_stride; p.N = g.N; p.nkb = pl.nkb; p.n_wtiles = pl.n_wtiles; p.rows_ub = g.rows_ub; p.n_rows_dev = g.n_rows_dev;
   p.rb_list = g.rb_list; p.n_rb_dev = g.n_rb_dev; p.w_rows_per_group = g.w_rows_per_group; p.unit_tile = pl.unit_tile; p.stage_bytes = pl.stage_bytes; p.n_stages = pl.n_stages;
-  p.tm_cols = pl.tm_cols;
+  p.tm_cols = pl.tm_cols; p.rb_rows = pl.rb_rows; p.n_acc = pl.n_acc;
   size_t smem = (size_t)pl.n_stages * pl.stage_bytes + sizeof(SkBars) + 1024;
   static bool attr = false;
   if (!attr) {

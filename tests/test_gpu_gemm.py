@@ -36,7 +36,9 @@ def _mk(shape, seed, scale=1.0):
     (37, 132, 192, 0),        # ragged rows, ragged N
     (200, 512, 1024, 0),      # 13 row boxes, pieces straddling CTAs
     (256, 384, 512, 0),       # one full 256-row block
-    (300, 1000, 2560, 0),     # two row blocks, the second ragged
+    (300, 1000, 2560, 0),     # 257..512 rows: ONE 512-row block = two fused MMA N blocks (256 + 44) sharing the weight tile
+    (512, 640, 512, 0),       # both fused N blocks full
+    (289, 2560, 4096, 0),     # config-3 O projection at the row count of the profiled step
     (700, 640, 1024, 0),      # three row blocks
     (64, 6144, 2560, 0),      # config-3 QKV shape
     (130, 2560, 9728, 0),     # config-3 down projection: few tiles, long K (many pieces per tile)
