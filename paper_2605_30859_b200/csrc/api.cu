@@ -80,13 +80,15 @@ size_t carve(darts_ctx *c, void *base) {
   c->slot_nsuf = k.take<int32_t>(A);
   c->forced_stage = k.take<int32_t>(G * DARTS_MAX_KP);
   if (attention_sm100_supported(c)) {
-    size_t max_parts = R * ((size_t)ceil_div(rt.max_prompt_len, 512) + 2) + (size_t)rt.n_pages / 8 + 16;
+    size_t npc_max = (size_t)ceil_div(rt.max_prompt_len, 512);
+    size_t max_parts = R * (npc_max + 2) + (size_t)rt.n_pages / 8 + 16;
+    if (model) max_parts = std::max(max_parts, A * npc_max + 16);            // a prefill pass: one partial per (prompt token, chunk)
     c->attn_max_items = (int)max_parts;
     c->attn_items_pre = k.take<int32_t>(max_parts * 6);
     c->attn_items_suf = k.take<int32_t>(max_parts * 6);
     c->attn_nitems = k.take<int32_t>(4);
-    c->part_base = k.take<int32_t>(R);
-    c->part_cnt = k.take<int32_t>(R);
+    c->part_base = k.take<int32_t>(A);
+    c->part_cnt = k.take<int32_t>(A);
     c->part_ml = k.take<float>(max_parts * m.n_q_heads * 2);
     c->part_acc = k.take<float>(max_parts * m.n_q_heads * m.head_dim);
   }
@@ -349,8 +351,9 @@ darts_status prefill_impl(darts_ctx *c, const int32_t *prompt_tokens_dev, bool t
     int g1 = g0, ntok = 0;
     while (g1 < G && ntok + plen[g1] <= chunk) ntok += plen[g1++];
     int tb = tok_off[g0];
-    c->attn_plan_valid = false;                      // prefill is causal per token: generic kernel
     TRY(launch_plan_prefill(c, tb, ntok, g0, g1));
+    c->attn_plan_valid = attention_sm100_supported(c);                            // causal plan: blocks of query positions x 512-token chunks
+    if (c->attn_plan_valid) TRY(launch_attention_plan_sm100(c, ntok, nullptr, true));
     if (c->tc_path) {
       TRY(forward_layers_tc(c, ntok, nullptr));
       TRY(launch_gather_rows_bf16(c, c->xn, c->hlast, tb, g0, g1));             // final-normed hidden of each prompt's last token

@@ -100,7 +100,7 @@ struct darts_ctx {
   int32_t *attn_items_pre, *attn_items_suf, *attn_nitems, *part_base, *part_cnt;
   float *part_ml, *part_acc;
   int attn_max_items;
-  bool attn_plan_valid;
+  bool attn_plan_valid, attn_causal;   // attn_causal: the current plan is a prefill pass (row-wise causal masks)
   int n_sms;
 
   // policy / sampling
@@ -263,6 +263,6 @@ darts_status launch_silu_mul_part(darts_ctx *c, int S, int rows_ub, const int32_
 darts_status launch_sample_finalize(darts_ctx *c, int n_tiles, int rows_ub);
 darts_status launch_sum_partials(darts_ctx *c, const float *part, float *out, int S, size_t n);
 darts_status launch_gather_rows_bf16(darts_ctx *c, const void *src, void *dst, int tok_begin, int g_begin, int g_end);
-darts_status launch_attention_plan_sm100(darts_ctx *c, int rows_ub, const int32_t *n_rows_dev);
+darts_status launch_attention_plan_sm100(darts_ctx *c, int rows_ub, const int32_t *n_rows_dev, bool prefill = false);
 bool attention_sm100_supported(const darts_ctx *c);
 darts_status launch_attention_ref(darts_ctx *c, int layer, const void *q, void *out, int rows_ub, const int32_t *n_rows_dev);

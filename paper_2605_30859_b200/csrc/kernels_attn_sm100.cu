@@ -77,7 +77,8 @@ struct Params {
   const __nv_bfloat16 *q;                   // [slot][Hq][128]
   const __nv_bfloat16 *kv_layer;
   const int32_t *items_pre, *items_suf, *n_items;   // n_items[0] = prefix items, [1] = suffix items
-  const int32_t *slot_prompt, *slot_row, *g_prefix_pages, *row_pages, *part_base;
+  const int32_t *slot_prompt, *slot_row, *slot_npre, *g_prefix_pages, *row_pages, *part_base;
+  int causal;                               // prefill pass: query row of slot s sees tokens < slot_npre[s] only
   float *part_ml, *part_acc;
   int mpp, msp, Hq, Hkv, rep;
   size_t page_elems, tile_elems;
@@ -186,6 +187,7 @@ __global__ void __launch_bounds__(THREADS, 2) attn_main_k(Params p) {
     const int32_t *it = item < n_pre ? p.items_pre + (size_t)item * ITEM_INTS : p.items_suf + (size_t)(item - n_pre) * ITEM_INTS;
     int first = it[0], n_slots = it[1], n_tok = it[3], chunk_k = it[4];
     int n_rows = n_slots * p.rep;
+    const int tok_begin = it[2] * PAGE;                            // first token of this item within its page table
     bool rowsplit = n_rows > 16;
     int mt = rowsplit ? warp : 0;                                  // m-tile this warp works on
     bool warp_has_rows = mt * 16 < n_rows;
@@ -204,6 +206,13 @@ __global__ void __launch_bounds__(THREADS, 2) attn_main_k(Params p) {
         Qa[ks][3] = q1 ? *reinterpret_cast<const uint32_t *>(q1 + d + 8) : 0u;
       }
     }
+    // per-row token limit inside this item (rows g and g+8 of the warp's m-tile): n_tok, or the causal bound of a prefill pass
+    int lim0 = n_tok, lim1 = n_tok;
+    if (p.causal) {
+      int r0 = mt * 16 + g, r1 = r0 + 8;
+      lim0 = r0 < n_rows ? min(n_tok, p.slot_npre[first + r0 / p.rep] - tok_begin) : 0;
+      lim1 = r1 < n_rows ? min(n_tok, p.slot_npre[first + r1 / p.rep] - tok_begin) : 0;
+    }
     float O[16][4];
 #pragma unroll
     for (int nt = 0; nt < 16; ++nt) O[nt][0] = O[nt][1] = O[nt][2] = O[nt][3] = 0.f;
@@ -213,6 +222,7 @@ __global__ void __launch_bounds__(THREADS, 2) attn_main_k(Params p) {
       mbar_wait(&sm.full[stage], phase);
       uint32_t sK = smem_u32(sm.stage[stage]), sV = sK + PAGE * HD * 2;
       int valid = min(PAGE, n_tok - pg * PAGE);
+      const int v0 = lim0 - pg * PAGE, v1 = lim1 - pg * PAGE;       // row-wise valid tokens of this page (may be <= 0 or >= PAGE)
       if (!rowsplit) {
         int tok0 = warp * 16;                                      // this warp's 16 tokens of the page
         if (tok0 < valid) {
@@ -221,8 +231,10 @@ __global__ void __launch_bounds__(THREADS, 2) attn_main_k(Params p) {
 #pragma unroll
           for (int nt = 0; nt < 2; ++nt) {
             int tk = tok0 + nt * 8 + 2 * t;
-            if (tk >= valid) { S[nt][0] = -INFINITY; S[nt][2] = -INFINITY; }
-            if (tk + 1 >= valid) { S[nt][1] = -INFINITY; S[nt][3] = -INFINITY; }
+            if (tk >= v0) S[nt][0] = -INFINITY;
+            if (tk + 1 >= v0) S[nt][1] = -INFINITY;
+            if (tk >= v1) S[nt][2] = -INFINITY;
+            if (tk + 1 >= v1) S[nt][3] = -INFINITY;
           }
           uint32_t P[2][2];
           softmax_update<2>(S, m, l, O, P, p.c);
@@ -232,12 +244,14 @@ __global__ void __launch_bounds__(THREADS, 2) attn_main_k(Params p) {
         float S[8][4] = {};
 #pragma unroll
         for (int np = 0; np < 4; ++np) qk_16tok(sK, np * 16, Qa, S[2 * np], S[2 * np + 1], lane);
-        if (valid < PAGE) {
+        if (min(v0, v1) < PAGE) {
 #pragma unroll
           for (int nt = 0; nt < 8; ++nt) {
             int tk = nt * 8 + 2 * t;
-            if (tk >= valid) { S[nt][0] = -INFINITY; S[nt][2] = -INFINITY; }
-            if (tk + 1 >= valid) { S[nt][1] = -INFINITY; S[nt][3] = -INFINITY; }
+            if (tk >= v0) S[nt][0] = -INFINITY;
+            if (tk + 1 >= v0) S[nt][1] = -INFINITY;
+            if (tk >= v1) S[nt][2] = -INFINITY;
+            if (tk + 1 >= v1) S[nt][3] = -INFINITY;
           }
         }
         uint32_t P[8][2];
@@ -371,8 +385,8 @@ __device__ __forceinline__ int scan1024(int v, int *total, int *smem) {
 
 __global__ void attn_plan_k(const int32_t *__restrict__ slot_prompt, const int32_t *__restrict__ slot_npre,
                             const int32_t *__restrict__ slot_nsuf, int32_t *items_pre, int32_t *items_suf, int32_t *n_items,
-                            int32_t *part_base, int32_t *part_cnt, int rep, int no_share, int max_items, const int32_t *n_rows_dev,
-                            int rows_ub) {
+                            int32_t *part_base, int32_t *part_cnt, int rep, int no_share, int prefill, int max_items,
+                            const int32_t *n_rows_dev, int rows_ub) {
   __shared__ int sm[33];
   __shared__ int b_part, b_pre, b_suf;
   int n = n_rows_dev ? min(*n_rows_dev, rows_ub) : rows_ub;
@@ -381,16 +395,30 @@ __global__ void attn_plan_k(const int32_t *__restrict__ slot_prompt, const int32
   int RB = 64 / rep;                                   // slots per ROWSPLIT item (64 query rows)
   for (int base = 0; base < n; base += blockDim.x) {
     int slot = base + threadIdx.x;
-    int npc = 0, nsc = 0, gsize = 0, nblk = 0;
+    int npc = 0, nsc = 0, gsize = 0, nblk = 0, npre_items = 0;
     if (slot < n) {
       npc = (slot_npre[slot] + CH_TOK - 1) / CH_TOK;
       nsc = (slot_nsuf[slot] + CH_TOK - 1) / CH_TOK;
       int pr = slot_prompt[slot];
-      bool leader = no_share || slot == 0 || slot_prompt[slot - 1] != pr;
-      if (leader) {
-        gsize = 1;
-        if (!no_share) while (slot + gsize < n && slot_prompt[slot + gsize] == pr) ++gsize;
-        nblk = gsize * rep <= 16 ? 1 : (gsize + RB - 1) / RB;
+      if (prefill) {
+        // causal pass over prompt tokens: slot = token at position npre-1.  A block = RB consecutive positions of one prompt
+        // (RB divides the 512-token chunk, so its slots need the same chunks); its items run up to the block's LAST position
+        // and the kernel masks row-wise (Params::causal).
+        bool leader = (slot_npre[slot] - 1) % RB == 0;
+        if (leader) {
+          gsize = 1;
+          while (gsize < RB && slot + gsize < n && slot_prompt[slot + gsize] == pr) ++gsize;
+          nblk = 1;
+          npre_items = slot_npre[slot + gsize - 1];
+        }
+      } else {
+        bool leader = no_share || slot == 0 || slot_prompt[slot - 1] != pr;
+        if (leader) {
+          gsize = 1;
+          if (!no_share) while (slot + gsize < n && slot_prompt[slot + gsize] == pr) ++gsize;
+          nblk = gsize * rep <= 16 ? 1 : (gsize + RB - 1) / RB;
+          npre_items = slot_npre[slot];
+        }
       }
     }
     int tp, tq, ts;
@@ -410,7 +438,7 @@ __global__ void attn_plan_k(const int32_t *__restrict__ slot_prompt, const int32
           it[0] = slot + b * per;
           it[1] = min(per, gsize - b * per);
           it[2] = ck * CH_PAGES;
-          it[3] = min(CH_TOK, slot_npre[slot] - ck * CH_TOK);
+          it[3] = min(CH_TOK, npre_items - ck * CH_TOK);
           it[4] = ck;
           it[5] = 1;
         }
@@ -435,11 +463,12 @@ __global__ void attn_plan_k(const int32_t *__restrict__ slot_prompt, const int32
 size_t attn_sm100_smem_bytes() { return sizeof(Smem) + 128; }
 
 // Plan once per decode step (the lengths are the same for every layer), then per layer: main + merge.
-darts_status launch_attention_plan_sm100(darts_ctx *c, int rows_ub, const int32_t *n_rows_dev) {
+darts_status launch_attention_plan_sm100(darts_ctx *c, int rows_ub, const int32_t *n_rows_dev, bool prefill) {
   int rep = c->m.n_q_heads / c->m.n_kv_heads;
   attn_plan_k<<<1, 1024, 0, c->stream>>>(c->slot_prompt, c->slot_npre, c->slot_nsuf, c->attn_items_pre, c->attn_items_suf, c->attn_nitems,
-                                         c->part_base, c->part_cnt, rep, (c->rt.flags & DARTS_FLAG_NO_PREFIX_SHARING) ? 1 : 0,
+                                         c->part_base, c->part_cnt, rep, (c->rt.flags & DARTS_FLAG_NO_PREFIX_SHARING) ? 1 : 0, prefill ? 1 : 0,
                                          c->attn_max_items, n_rows_dev, rows_ub);
+  c->attn_causal = prefill;
   c->launches++;
   if (cudaGetLastError() != cudaSuccess) FAIL(c, DARTS_ERR_CUDA, "launch attn_plan failed");
   return DARTS_OK;
@@ -464,7 +493,7 @@ darts_status launch_attention_sm100(darts_ctx *c, int layer, const void *q, void
   p.q = (const __nv_bfloat16 *)q;
   p.kv_layer = (const __nv_bfloat16 *)c->kv_pool + (size_t)layer * c->kv_layer_elems;
   p.items_pre = c->attn_items_pre; p.items_suf = c->attn_items_suf; p.n_items = c->attn_nitems;
-  p.slot_prompt = c->slot_prompt; p.slot_row = c->slot_row; p.g_prefix_pages = c->g_prefix_pages; p.row_pages = c->row_pages;
+  p.slot_prompt = c->slot_prompt; p.slot_row = c->slot_row; p.slot_npre = c->slot_npre; p.causal = c->attn_causal ? 1 : 0; p.g_prefix_pages = c->g_prefix_pages; p.row_pages = c->row_pages;
   p.part_base = c->part_base; p.part_ml = c->part_ml; p.part_acc = c->part_acc;
   p.mpp = c->max_prefix_pages; p.msp = c->max_suffix_pages; p.Hq = c->m.n_q_heads; p.Hkv = c->m.n_kv_heads; p.rep = p.Hq / p.Hkv;
   p.page_elems = c->kv_page_elems; p.tile_elems = c->kv_tile_elems;
