@@ -97,8 +97,8 @@ __global__ void sum_partials_k(const float *__restrict__ part, float *__restrict
 __device__ __forceinline__ float4 sk_sum4(const SkView &v, int np, size_t idx) {
   const float4 *p = reinterpret_cast<const float4 *>(v.part + idx);
   const size_t st = v.slot_stride / 4;
-  float4 a = __ldg(p);
-  for (int s0 = 1; s0 < np; s0 += 4) {
+  float4 a = make_float4(0.f, 0.f, 0.f, 0.f);              // 0 + x == x: the sum is still piece 0 + piece 1 + ... in slot order
+  for (int s0 = 0; s0 < np; s0 += 4) {
     float4 x[4];
 #pragma unroll
     for (int s = 0; s < 4; ++s)
