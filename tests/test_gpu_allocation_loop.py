@@ -1,0 +1,56 @@
+"""-m gpu: the DARTS loop around the rollout (SURVEY.md 8(f) f1 feeding 8(a)): rollout -> per-prompt length variance (by-product of
+the selection kernel) -> EMA -> Eq. 9 budget -> Alg. 1 plan -> next rollout with per-prompt K' (a mix of dual-end prompts, K' < 2K,
+and shortest-only + early-stop prompts, K' = 2K).  Every stage is compared with the oracle; integer results bit-exact."""
+import numpy as np
+import pytest
+
+from oracle import PRUNED, allocation as al, rollout as ro
+from paper_2605_30859_b200 import workloads as wl
+from tests.gpu_util import make_ctx
+
+pytestmark = pytest.mark.gpu
+
+
+def test_rollout_variance_allocation_next_rollout():
+    from paper_2605_30859_b200 import api
+    c = wl.CONFIGS["c1"]
+    cfg, G, K, max_new, seed = c["model"], 6, 4, 48, 11
+    prompts = wl.make_prompts(G, c["P"], cfg["vocab"], seed)
+    # long-tail severity differs per prompt: sigma of the forced-EOS lognormal grows with the prompt index
+    rng = np.random.default_rng(seed)
+    def forced_for(Kp):
+        f = np.zeros((G, int(Kp.max())), np.int32)
+        for i in range(G):
+            f[i, :Kp[i]] = np.clip(np.round(rng.lognormal(2.8, 0.15 + 0.2 * i, size=Kp[i])), 3, max_new)
+        return f
+    d, host = make_ctx(cfg, seed, G, 2 * K, c["P"], max_new, page=16)
+    # ---- rollout 1: uniform K' = 6 (dual-end everywhere)
+    Kp1 = np.full(G, 6, np.int32)
+    f1 = forced_for(Kp1)
+    g1 = d.rollout_host(prompts, Kp1, K, max_new, 1.0, seed, forced_len=f1)
+    o1 = ro.rollout_stepwise(host, prompts, Kp1, K, max_new, 1.0, seed, forced_len=f1, teacher=g1["tokens"])
+    assert np.array_equal(g1["len"], o1["len"]) and np.array_equal(g1["sel"], o1["sel"])
+    # the variance by-product of select_k against the plain definition on the oracle's lengths
+    offs = np.concatenate([[0], np.cumsum(Kp1)])
+    var_ref = np.array([np.var(o1["len"][offs[i]:offs[i + 1]].astype(np.float64)) for i in range(G)])
+    assert np.allclose(g1["len_var"], var_ref, rtol=1e-5, atol=1e-4)
+    # ---- EMA -> budget -> plan, library vs oracle
+    ema = np.full(G, -1.0, np.float32)
+    api.update_variance_ema(ema, g1["len_var"], 0.5)
+    assert np.allclose(ema, al.ema_update(np.full(G, -1.0), g1["len_var"].astype(np.float64), 0.5))
+    M_total = api.redundancy_budget(rho=0.9, lam=0.02, k=1.0, G=G, K=K)
+    assert M_total == al.budget(0.9, 0.02, 1.0, G, K) and G * K <= M_total <= 2 * G * K
+    Kp2 = api.allocate_redundancy(ema, M_total, K, 2 * K)
+    assert np.array_equal(Kp2, al.greedy_allocate(ema.astype(np.float64), M_total, K, 2 * K))
+    assert Kp2.sum() == M_total and Kp2.max() == 2 * K and Kp2.min() < 2 * K      # both branches of Alg. 2 occur
+    # ---- rollout 2 with the plan: AUTO mode picks dual-end / early stop per prompt
+    f2 = forced_for(Kp2)
+    g2 = d.rollout_host(prompts, Kp2, K, max_new, 1.0, seed + 1, forced_len=f2)
+    o2 = ro.rollout_stepwise(host, prompts, Kp2, K, max_new, 1.0, seed + 1, forced_len=f2, teacher=g2["tokens"])
+    for key in ("len", "status", "sel", "sel_mask", "close_step"):
+        assert np.array_equal(g2[key], o2[key]), key
+    offs2 = np.concatenate([[0], np.cumsum(Kp2)])
+    for i in range(G):
+        pruned = np.any(g2["status"][offs2[i]:offs2[i + 1]] == PRUNED)
+        assert not pruned or Kp2[i] >= 2 * K                                         # only saturated prompts stop early
+    d.close()
