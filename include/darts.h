@@ -36,7 +36,8 @@
  *     router wr [E][d] always F32.
  *   - Rows (trajectories) are numbered group-major: row = sum_{i'<i} Kp[i'] + j.
  *   - KV cache (library-owned, inside the workspace): pages of page_size tokens,
- *     [layer][page][K|V][kv_head][token][head_dim]; a row's page table is
+ *     [layer][page][kv_head][K|V][token][head_dim] (the K and V tiles of one (page, head) are adjacent; for bf16 /
+ *     head_dim 128 the 16-byte chunks of a token row are XOR-permuted by token & 7); a row's page table is
  *     [its prompt's shared prefix pages || its own suffix pages]; the suffix starts on a fresh page,
  *     so the K' samples of a prompt share the prefix pages without any copy.
  */

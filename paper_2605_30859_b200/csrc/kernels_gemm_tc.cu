@@ -1,4 +1,5 @@
-// tcgen05 / TMEM GEMM for the bf16 path:   P[s][r][n] = sum_{k in split s} X[r][k] W[n][k]
+// tcgen05 / TMEM tile GEMM (the LM head with its fused sampling epilogue; also the prefill logits and the
+// split-K parity hook):   P[s][r][n] = sum_{k in split s} X[r][k] W[n][k].   The layer projections run on kernels_gemm_sk.cu.
 //
 // One CTA computes a 128 (activation rows) x BN (weight rows) tile of one K-split:
 //   warp 0   TMA producer: per 64-wide k-block one box of W (BN x 64, 128-byte swizzle) and ceil(live rows / 16) boxes

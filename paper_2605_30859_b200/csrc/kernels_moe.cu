@@ -7,7 +7,7 @@
 //   moe_topk_k       one warp per slot: softmax, k rounds of warp arg-max, renormalised gates, per-expert counts
 //   moe_place_k      (tensor-core path) one CTA per expert: exclusive scan of the counts, stable ballot ranking of the
 //                    expert's assignments, gather of their bf16 activation rows into the expert-sorted matrix xs
-//   [grouped tcgen05 GEMMs of kernels_gemm_tc.cu: gate/up then down, one group per expert]
+//   [grouped stream-K tcgen05 GEMMs of kernels_gemm_sk.cu: gate/up then down, one row block per (expert, <= 256 rows)]
 //   moe_expert_simt_k (fp32 / generic path) one CTA per (slot, k): the expert's SwiGLU MLP as warp dot products
 //   moe_combine_k    h += sum_k w_k y_k in selection order (+ the next RMSNorm on the tensor-core path)
 // Weight bytes streamed per step scale with the DISTINCT experts hit: groups with no rows exit before any load.
