@@ -3,6 +3,8 @@
 //   add_rmsnorm    h += sum_s P_s (O-proj / down-proj residual), then xn = rmsnorm(h) * w for the next GEMM
 //   silu_mul_part  act = silu(sum_s gate_s) * (sum_s up_s)
 //   (rope_append_k in kernels_basic.cu does the same for the QKV partials)
+#include <stdlib.h>
+
 #include <algorithm>
 
 #include "internal.cuh"
@@ -177,6 +179,80 @@ __global__ void __launch_bounds__(256) add_rmsnorm_sk_k(float *__restrict__ h, S
   }
 }
 
+// Same operation with the slot's row held in registers (d / 4 <= ITERS * 256): every load of the row — the residual and up to four
+// pieces per element — is issued before the first add, and the row is read once (the two-pass version above re-reads h and walks
+// its elements one dependent round trip at a time, which is what a launch of 16 CTAs spends its 10 us on).
+template <int ITERS>
+__global__ void __launch_bounds__(256) add_rmsnorm_sk_reg_k(float *__restrict__ h, SkView v, const __nv_bfloat16 *__restrict__ w,
+                                                           __nv_bfloat16 *__restrict__ out, int d, float eps, const int32_t *n_rows_dev,
+                                                           int rows_ub) {
+  pdl_trigger();
+  pdl_wait();
+  const int slot = blockIdx.x, live = live_rows(n_rows_dev, rows_ub);
+  if (slot >= live) return;
+  const int n_rb = (live + v.rb_rows - 1) / v.rb_rows;
+  float4 *hr = reinterpret_cast<float4 *>(h + (size_t)slot * d);
+  const size_t st = v.slot_stride / 4;
+  float4 x[ITERS], acc[ITERS];
+  int np[ITERS];
+  const float4 *pp[ITERS];
+  int npmax = 0;
+#pragma unroll
+  for (int it = 0; it < ITERS; ++it) {
+    const int k = threadIdx.x + it * 256;
+    const bool ok = k < d / 4;
+    np[it] = ok ? sk_npieces(v, n_rb, 4 * k, slot) : 0;
+    pp[it] = reinterpret_cast<const float4 *>(v.part + (size_t)slot * d) + (ok ? k : 0);
+    x[it] = ok ? hr[k] : make_float4(0.f, 0.f, 0.f, 0.f);
+    acc[it] = make_float4(0.f, 0.f, 0.f, 0.f);
+    npmax = max(npmax, np[it]);
+  }
+  for (int s0 = 0; s0 < npmax; s0 += 4) {
+    float4 y[ITERS][4];
+#pragma unroll
+    for (int it = 0; it < ITERS; ++it)
+#pragma unroll
+      for (int s = 0; s < 4; ++s)
+        if (s0 + s < np[it]) y[it][s] = __ldg(pp[it] + (size_t)(s0 + s) * st);
+#pragma unroll
+    for (int it = 0; it < ITERS; ++it)
+#pragma unroll
+      for (int s = 0; s < 4; ++s)
+        if (s0 + s < np[it]) { acc[it].x += y[it][s].x; acc[it].y += y[it][s].y; acc[it].z += y[it][s].z; acc[it].w += y[it][s].w; }
+  }
+  float ss = 0.f;
+#pragma unroll
+  for (int it = 0; it < ITERS; ++it) {
+    x[it].x += acc[it].x; x[it].y += acc[it].y; x[it].z += acc[it].z; x[it].w += acc[it].w;
+    const int k = threadIdx.x + it * 256;
+    if (k < d / 4) {
+      hr[k] = x[it];
+      ss += x[it].x * x[it].x + x[it].y * x[it].y + x[it].z * x[it].z + x[it].w * x[it].w;
+    }
+  }
+  __shared__ float red[32];
+  ss = warp_sum(ss);
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = ss;
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    float t = threadIdx.x < (blockDim.x >> 5) ? red[threadIdx.x] : 0.f;
+    t = warp_sum(t);
+    if (threadIdx.x == 0) red[0] = t;
+  }
+  __syncthreads();
+  const float r = 1.0f / sqrtf(red[0] / d + eps);
+#pragma unroll
+  for (int it = 0; it < ITERS; ++it) {
+    const int k = threadIdx.x + it * 256;
+    if (k < d / 4) {
+      const __nv_bfloat162 *wp = reinterpret_cast<const __nv_bfloat162 *>(w + 4 * k);
+      float2 w0 = __bfloat1622float2(wp[0]), w1 = __bfloat1622float2(wp[1]);
+      *reinterpret_cast<uint2 *>(out + (size_t)slot * d + 4 * k) =
+          pack4_bf16(x[it].x * r * w0.x, x[it].y * r * w0.y, x[it].z * r * w1.x, x[it].w * r * w1.y);
+    }
+  }
+}
+
 // act[slot][k] = silu(g) * u with g = pieces(slot, k), u = pieces(slot, F + k)
 __global__ void __launch_bounds__(256) silu_mul_sk_k(SkView v, __nv_bfloat16 *__restrict__ act, int F, const int32_t *n_rows_dev, int rows_ub) {
   pdl_trigger();
@@ -299,8 +375,16 @@ darts_status launch_sum_partials(darts_ctx *c, const float *part, float *out, in
 
 darts_status launch_add_rmsnorm_sk(darts_ctx *c, const SkView &v, const void *w, int rows_ub, const int32_t *n_rows_dev) {
   if (rows_ub <= 0) return DARTS_OK;
-  int d = c->m.d_model;
-  launch_pdl(c, add_rmsnorm_sk_k, dim3(rows_ub), dim3(256), 0, c->h, v, (const __nv_bfloat16 *)w, (__nv_bfloat16 *)c->xn, d, c->m.rms_eps, n_rows_dev, rows_ub);
+  // the register-resident variant pays with occupancy (101-175 registers): it is for launches that cannot fill the SMs anyway
+  static const int reg_max = getenv("DARTS_ADDNORM_REG_MAX") ? atoi(getenv("DARTS_ADDNORM_REG_MAX")) : 128;
+  int d = c->m.d_model, iters = rows_ub <= reg_max ? (d / 4 + 255) / 256 : 99;
+  const __nv_bfloat16 *wn = (const __nv_bfloat16 *)w;
+  __nv_bfloat16 *xn = (__nv_bfloat16 *)c->xn;
+  if (iters == 1) launch_pdl(c, add_rmsnorm_sk_reg_k<1>, dim3(rows_ub), dim3(256), 0, c->h, v, wn, xn, d, c->m.rms_eps, n_rows_dev, rows_ub);
+  else if (iters == 2) launch_pdl(c, add_rmsnorm_sk_reg_k<2>, dim3(rows_ub), dim3(256), 0, c->h, v, wn, xn, d, c->m.rms_eps, n_rows_dev, rows_ub);
+  else if (iters == 3) launch_pdl(c, add_rmsnorm_sk_reg_k<3>, dim3(rows_ub), dim3(256), 0, c->h, v, wn, xn, d, c->m.rms_eps, n_rows_dev, rows_ub);
+  else if (iters == 4) launch_pdl(c, add_rmsnorm_sk_reg_k<4>, dim3(rows_ub), dim3(256), 0, c->h, v, wn, xn, d, c->m.rms_eps, n_rows_dev, rows_ub);
+  else launch_pdl(c, add_rmsnorm_sk_k, dim3(rows_ub), dim3(256), 0, c->h, v, wn, xn, d, c->m.rms_eps, n_rows_dev, rows_ub);
   return post(c, "add_rmsnorm_sk");
 }
 
