@@ -177,6 +177,15 @@ darts_status darts_rollout(darts_ctx *ctx, const int32_t *prompts, int32_t promp
 /* Same loop after a caller-issued darts_prefill (ragged prompts, per-prompt Kp, explicit policy). */
 darts_status darts_run_to_completion(darts_ctx *ctx, darts_results *out);
 
+/* Token-level streaming hook (§4.3.2 "ship token chunks to the trainer once a threshold accumulates"; rollout side
+ * only — the consumer is the caller's).  Same loop as darts_run_to_completion; every chunk_steps lock-step iterations the tokens
+ * of steps [step_begin, step_end) are copied to pinned host memory on a second stream (overlapping the following decode steps) and
+ * fn(user, step_begin, step_end, n_rows, tokens) is called on the calling thread, in step order, with tokens = HOST
+ * [n_rows][step_end - step_begin] row-major (-1 where a row had already stopped; a trailing chunk may hold only -1).  The buffer is
+ * valid during the call only.  The chunks together cover steps [0, n_steps).  The library owns the two pinned staging buffers. */
+typedef void (*darts_chunk_fn)(void *user, int32_t step_begin, int32_t step_end, int32_t n_rows, const int32_t *tokens_host);
+darts_status darts_run_to_completion_streaming(darts_ctx *ctx, int32_t chunk_steps, darts_chunk_fn fn, void *user, darts_results *out);
+
 /* End-to-end convenience with HOST inputs (bench `e2e`): copies prompts / forced_len host->device,
  * runs the rollout, copies results device->host. */
 darts_status darts_rollout_host(darts_ctx *ctx, const int32_t *prompts_host, int32_t prompt_len, int32_t G,

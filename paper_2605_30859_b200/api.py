@@ -74,6 +74,8 @@ darts_decode_step = _sig("darts_decode_step", _ctx)
 darts_select_and_compact = _sig("darts_select_and_compact", _ctx, _vp)
 darts_rollout = _sig("darts_rollout", _ctx, _vp, _i32, _i32, _i32, _i32, _i32, _f32, _u64, _vp, C.POINTER(Results))
 darts_run_to_completion = _sig("darts_run_to_completion", _ctx, C.POINTER(Results))
+ChunkFn = C.CFUNCTYPE(None, C.c_void_p, _i32, _i32, _i32, C.POINTER(C.c_int32))
+darts_run_to_completion_streaming = _sig("darts_run_to_completion_streaming", _ctx, _i32, ChunkFn, C.c_void_p, C.POINTER(Results))
 darts_rollout_host = _sig("darts_rollout_host", _ctx, _vp, _i32, _i32, _vp, _vp, C.POINTER(Policy), _i32, _f32, _u64,
                           C.POINTER(Results))
 darts_get_results = _sig("darts_get_results", _ctx, C.POINTER(Results))
@@ -242,6 +244,13 @@ class Darts:
 
     def run_to_completion(self):
         self._check(darts_run_to_completion(self.ctx, None))
+
+    def run_to_completion_streaming(self, chunk_steps, on_chunk):
+        """on_chunk(step_begin, step_end, tokens) with tokens an int32 numpy array [n_rows, step_end - step_begin] (copied)."""
+        def tramp(_user, s0, s1, n_rows, ptr):
+            on_chunk(s0, s1, np.ctypeslib.as_array(ptr, shape=(n_rows, s1 - s0)).copy())
+        cb = ChunkFn(tramp)
+        self._check(darts_run_to_completion_streaming(self.ctx, chunk_steps, cb, None, None))
 
     def rollout(self, prompts_dev, G, Kp, K, max_len, temperature, seed, forced_len_dev=None):
         """north_star signature: device prompts [G,P] int32, scalar K'."""

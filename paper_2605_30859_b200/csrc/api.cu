@@ -468,6 +468,11 @@ darts_status darts_destroy(darts_ctx *c) {
   if (c->ev[0]) cudaEventDestroy(c->ev[0]);
   if (c->ev[1]) cudaEventDestroy(c->ev[1]);
   for (cudaEvent_t e : c->prof_ev) cudaEventDestroy(e);
+  if (c->copy_stream) {
+    cudaStreamSynchronize(c->copy_stream);
+    cudaStreamDestroy(c->copy_stream);
+    for (int b = 0; b < 2; ++b) { cudaEventDestroy(c->ev_copy_ready[b]); cudaEventDestroy(c->ev_copy_done[b]); if (c->chunk_stage[b]) cudaFreeHost(c->chunk_stage[b]); }
+  }
   const void **arrs[] = {c->attn_norm, c->wqkv, c->q_norm, c->k_norm, c->wo, c->mlp_norm, c->wgu, c->wd, c->wr, c->wgu_e, c->wd_e};
   for (auto a : arrs) delete[] a;
   CUtensorMap *maps[] = {c->tm_wqkv, c->tm_wo, c->tm_wgu, c->tm_wd, c->tm_wgu_e, c->tm_wd_e};
@@ -566,8 +571,43 @@ darts_status darts_get_counters(darts_ctx *c, darts_counters *o) {
   return DARTS_OK;
 }
 
-darts_status darts_run_to_completion(darts_ctx *c, darts_results *out) {
-  if (!c) return DARTS_ERR_INVALID_ARG;
+// Token-level streaming (§4.3.2, App. E :481-489, rollout side only): every
+// `chunk_steps` lock-step iterations the token columns produced since the last chunk are copied device->host on a second
+// stream (ordered after the step that produced them by an event, overlapping the following steps) and handed to `fn`.
+struct ChunkStream {
+  darts_ctx *c;
+  int chunk;
+  darts_chunk_fn fn;
+  void *user;
+  int flushed = 0;
+  int pend_s0[2] = {0, 0}, pend_s1[2] = {0, 0};
+  bool pending[2] = {false, false};
+  int next_slot = 0;
+
+  darts_status drain(int b) {
+    if (!pending[b]) return DARTS_OK;
+    CUDA_TRY(c, cudaEventSynchronize(c->ev_copy_done[b]));
+    fn(user, pend_s0[b], pend_s1[b], c->R, c->chunk_stage[b]);
+    pending[b] = false;
+    return DARTS_OK;
+  }
+  darts_status issue(int s0, int s1) {
+    int b = next_slot;
+    next_slot ^= 1;
+    darts_status st = drain(b);                               // slots alternate, so chunks are delivered in step order
+    if (st != DARTS_OK) return st;
+    CUDA_TRY(c, cudaEventRecord(c->ev_copy_ready[b], c->stream));
+    CUDA_TRY(c, cudaStreamWaitEvent(c->copy_stream, c->ev_copy_ready[b], 0));
+    CUDA_TRY(c, cudaMemcpy2DAsync(c->chunk_stage[b], (size_t)(s1 - s0) * 4, c->tokens_out + s0, (size_t)c->rt.max_new * 4, (size_t)(s1 - s0) * 4,
+                                  (size_t)c->R, cudaMemcpyDeviceToHost, c->copy_stream));
+    CUDA_TRY(c, cudaEventRecord(c->ev_copy_done[b], c->copy_stream));
+    pend_s0[b] = s0; pend_s1[b] = s1; pending[b] = true;
+    flushed = s1;
+    return DARTS_OK;
+  }
+};
+
+static darts_status run_loop(darts_ctx *c, darts_results *out, ChunkStream *cs) {
   if (c->sticky) return c->sticky;
   if (!c->prefilled) FAIL(c, DARTS_ERR_BAD_STATE, "darts_run_to_completion before darts_prefill");
   TRY(darts_select_and_compact(c, nullptr));
@@ -580,12 +620,50 @@ darts_status darts_run_to_completion(darts_ctx *c, darts_results *out) {
     TRY(darts_select_and_compact(c, nullptr));
     CUDA_TRY(c, cudaEventRecord(c->ev[it & 1], c->stream));
     if (it >= 1) CUDA_TRY(c, cudaEventSynchronize(c->ev[(it + 1) & 1]));
+    if (cs && it + 2 - cs->flushed >= cs->chunk && cs->flushed + cs->chunk <= c->max_len)   // token columns [0, it + 2) are enqueued
+      TRY(cs->issue(cs->flushed, cs->flushed + cs->chunk));
   }
   CUDA_TRY(c, cudaStreamSynchronize(c->stream));
   int32_t na = 0;
   TRY(darts_n_active(c, &na));
   if (na != 0) FAIL(c, DARTS_ERR_BAD_STATE, "rollout loop ended with %d active rows", na);
+  if (cs) {
+    DevState st;
+    CUDA_TRY(c, cudaMemcpy(&st, c->st, sizeof(st), cudaMemcpyDeviceToHost));
+    while (cs->flushed < st.step) TRY(cs->issue(cs->flushed, std::min(st.step, cs->flushed + cs->chunk)));
+    TRY(cs->drain(cs->next_slot));
+    TRY(cs->drain(cs->next_slot ^ 1));
+  }
   return out ? darts_get_results(c, out) : DARTS_OK;
+}
+
+darts_status darts_run_to_completion(darts_ctx *c, darts_results *out) {
+  if (!c) return DARTS_ERR_INVALID_ARG;
+  return run_loop(c, out, nullptr);
+}
+
+darts_status darts_run_to_completion_streaming(darts_ctx *c, int32_t chunk_steps, darts_chunk_fn fn, void *user, darts_results *out) {
+  if (!c) return DARTS_ERR_INVALID_ARG;
+  if (!fn || chunk_steps <= 0) FAIL(c, DARTS_ERR_INVALID_ARG, "chunk_steps must be positive and fn non-NULL");
+  if (!c->prefilled) FAIL(c, DARTS_ERR_BAD_STATE, "darts_run_to_completion_streaming before darts_prefill");
+  size_t need = (size_t)c->R * chunk_steps * 4;
+  if (!c->copy_stream) {
+    CUDA_TRY(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+    for (int b = 0; b < 2; ++b) {
+      CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev_copy_ready[b], cudaEventDisableTiming));
+      CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev_copy_done[b], cudaEventDisableTiming));
+    }
+  }
+  if (need > c->chunk_stage_bytes) {
+    for (int b = 0; b < 2; ++b) {
+      if (c->chunk_stage[b]) cudaFreeHost(c->chunk_stage[b]);
+      c->chunk_stage[b] = nullptr;
+      CUDA_TRY(c, cudaHostAlloc((void **)&c->chunk_stage[b], need, cudaHostAllocDefault));
+    }
+    c->chunk_stage_bytes = need;
+  }
+  ChunkStream cs{c, chunk_steps, fn, user};
+  return run_loop(c, out, &cs);
 }
 
 static darts_status rollout_common(darts_ctx *c, const int32_t *prompts_dev, bool in_place, int32_t prompt_len, int32_t G,

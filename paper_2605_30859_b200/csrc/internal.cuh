@@ -123,6 +123,11 @@ struct darts_ctx {
   std::vector<cudaEvent_t> prof_ev;
   int prof_n;
   bool in_decode;
+  // token-level streaming (darts_run_to_completion_streaming): copy stream, pinned double buffer, events
+  cudaStream_t copy_stream;
+  int32_t *chunk_stage[2];
+  size_t chunk_stage_bytes;
+  cudaEvent_t ev_copy_ready[2], ev_copy_done[2];
   char err[512];
   darts_status sticky;
 };
