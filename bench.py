@@ -209,6 +209,29 @@ def rollout_algo_attention_bytes(lens, Kp, P, kvb):
     return total, per_step
 
 
+def rollout_algo_step_bytes(cfg, lens, Kp, P):
+    """Algorithmic HBM bytes of the whole decode path over a rollout: per lock-step iteration the active weights
+    once (MoE: the experts actually hit, in expectation E (1 - (1 - k/E)^R) per layer), every active row's own suffix KV, each open
+    group's prefix KV once, and the appended K/V — summed over the steps the final lengths imply.  Activations are ignored."""
+    L, d, hd, Hq, Hkv, V = cfg["n_layers"], cfg["d_model"], cfg["head_dim"], cfg["n_q_heads"], cfg["n_kv_heads"], cfg["vocab"]
+    attn_w = (Hq + 2 * Hkv) * hd * d + Hq * hd * d
+    dense_w = L * (attn_w + 3 * d * cfg["ffn"]) + V * d if not cfg["n_experts"] else L * (attn_w + cfg["n_experts"] * d * 2) + V * d
+    expert_w = 3 * d * cfg["expert_ffn"] if cfg["n_experts"] else 0
+    kvb = 2 * Hkv * hd * 2 * L
+    lens = np.asarray(lens)
+    grp = np.repeat(np.arange(len(Kp)), Kp)
+    total = 0.0
+    for s in range(1, int(lens.max())):
+        act = lens > s
+        R = int(act.sum())
+        w = dense_w * 2
+        if cfg["n_experts"]:
+            E, k = cfg["n_experts"], cfg["top_k"]
+            w += L * E * (1.0 - (1.0 - k / E) ** R) * expert_w * 2
+        total += w + (R * s + len(np.unique(grp[act])) * P + R) * kvb
+    return total
+
+
 def oracle_rollout_sample(name, model_gpu, cfg, P, n_tokens=1, seed=0):
     """cpu_baseline / reference arm: the oracle (oracle/, numpy fp64) decoding `n_tokens` tokens of ONE trajectory of
     the workload's model at context P.  The prompt's KV is drawn N(0,1) instead of being prefilled (an oracle prefill
@@ -283,7 +306,7 @@ def main():
         n_runs = args.warmup + 2 * args.steps
         host_in = [wl.rollout_inputs(name, seed=1000 * rank + it, G=G, max_new=max_new) for it in range(n_runs)]
         pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
-        gen_tokens, kept_tokens, dev_ms, e2e_ms, e2e_tokens, attn_ms, attn_bytes, steps_count, near = [], [], [], [], [], [], [], [], []
+        gen_tokens, kept_tokens, dev_ms, e2e_ms, e2e_tokens, attn_ms, attn_bytes, steps_count, near, step_bytes = [], [], [], [], [], [], [], [], [], []
         launches = 0
         it = 0
         for phase, n in (("warmup", args.warmup), ("device", args.steps), ("e2e", args.steps)):
@@ -315,6 +338,7 @@ def main():
                         gen_tokens.append(cnt["n_generated_tokens"]); kept_tokens.append(cnt["n_kept_tokens"])
                         steps_count.append(cnt["n_steps"]); near.append(cnt["n_near_ties"])
                         res = d.results()
+                        step_bytes.append(rollout_algo_step_bytes(cfg, res["len"], xin["Kp"], P))
                         tot, per_step = rollout_algo_attention_bytes(res["len"], xin["Kp"], P, kvb)
                         t_ms = d.attention_times()
                         m = min(len(t_ms), len(per_step))
@@ -344,6 +368,10 @@ def main():
                                   kernel="attn_main_k+attn_merge_k (layer 0 of every decode step, CUDA events on the library's stream inside the rollout)",
                                   share_of_step=attn_share, peak_source=peaks["source"]),
                     gpu_launches=int(launches))
+        step_gbps = float(np.sum(step_bytes)) / (float(np.sum(dev_ms)) * 1e-3) / 1e9
+        line["decode_path_roofline"] = dict(bound="hbm", achieved=step_gbps, peak=peaks["hbm"], unit="GB/s", frac=step_gbps / peaks["hbm"],
+                                            what="algorithmic bytes of ALL kernels of the rollout (active weights once per step, suffix KV per row, "
+                                                 "prefix KV once per open group, KV appends) / device time of the rollout incl. prefill")
         line["e2e"] = dict(value=e2e_value if tot_e2e_tok > 0 else None, unit="tokens/s", h2d_bytes_per_step=h2d,
                            d2h_bytes_per_step=d2h, ms_per_step=tot_e2e_ms / max(1, args.steps), api="darts_rollout_host (pinned host buffers in, host results out)")
         if args.max_new or args.G or args.layers:
