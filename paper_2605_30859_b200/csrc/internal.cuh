@@ -228,7 +228,7 @@ bool tc_shape_ok(int N, int K);
 int tc_pick_split(const darts_ctx *c, int N, int K, int rows_ub, int n_groups);
 // stream-K weight-streaming GEMM (kernels_gemm_sk.cu)
 #define SK_ROWBLOCK 256            // activation rows per MMA N block
-struct SkPlan { int nkb, n_wtiles, P, unit_tile, slots, stage_bytes, n_stages, tm_cols, rb_rows, n_acc; };
+struct SkPlan { int nkb, n_wtiles, P, unit_tile, slots, stage_bytes, n_stages, tm_cols, n_acc; };   // stage / TMEM fields: grouped mode only
 struct SkGemm {
   const CUtensorMap *w_map;           // weights [N (x groups)][K], 128-row boxes
   const XMaps *x_maps;
@@ -244,20 +244,24 @@ struct SkGemm {
 struct SkView {
   const float *part;
   size_t slot_stride;
-  int N, nkb, n_wtiles, P, unit_tile, rb_rows;   // rb_rows: activation rows per row block (256, or 512 = two fused MMA N blocks)
+  int N, nkb, n_wtiles, P, unit_tile;
 };
+// Activation rows per row block of a DENSE launch, decided from the LIVE row count on the device (never from the host's stale upper
+// bound: the block size fixes where a tile's pieces are cut, i.e. the fp32 summation order, and that must not depend on timing).
+// 257..384 live rows: one 512-row block = two MMA N blocks per stage sharing the weight tile; otherwise 256-row blocks.
+__host__ __device__ __forceinline__ int sk_rb_rows(int live) { return (live > SK_ROWBLOCK && live <= 384) ? 2 * SK_ROWBLOCK : SK_ROWBLOCK; }
 // CTA that owns unit u when T units are cut into P ranges [c*T/P, (c+1)*T/P)
 __host__ __device__ __forceinline__ int sk_owner(int u, int P, int T) { return ((u + 1) * P - 1) / T; }
-__host__ __device__ __forceinline__ int sk_npieces(const SkView &v, int n_rb, int col, int row) {
+__host__ __device__ __forceinline__ int sk_npieces(const SkView &v, int n_rb, int rb_rows, int col, int row) {
   if (v.unit_tile) return 1;
   int T = v.n_wtiles * n_rb * v.nkb;
-  int t = (col >> 7) * n_rb + row / v.rb_rows;
+  int t = (col >> 7) * n_rb + row / rb_rows;
   return sk_owner(t * v.nkb + v.nkb - 1, v.P, T) - sk_owner(t * v.nkb, v.P, T) + 1;
 }
 SkPlan sk_plan(int n_sms, int N, int K, int rows_ub, int n_rb_ub_grouped, bool rows_exact);
 darts_status launch_gemm_sk(darts_ctx *c, const SkGemm &g);
 darts_status launch_sk_reduce(darts_ctx *c, const SkView &v, float *out, int rows);
-inline SkView sk_view(const SkGemm &g) { return SkView{g.C, g.slot_stride, g.N, g.plan.nkb, g.plan.n_wtiles, g.plan.P, g.plan.unit_tile, g.plan.rb_rows}; }
+inline SkView sk_view(const SkGemm &g) { return SkView{g.C, g.slot_stride, g.N, g.plan.nkb, g.plan.n_wtiles, g.plan.P, g.plan.unit_tile}; }
 darts_status launch_add_rmsnorm_sk(darts_ctx *c, const SkView &v, const void *w, int rows_ub, const int32_t *n_rows_dev);
 darts_status launch_silu_mul_sk(darts_ctx *c, const SkView &v, int rows_ub, const int32_t *n_rows_dev);
 darts_status launch_rope_append_sk(darts_ctx *c, int layer, const SkView &v, int rows_ub, const int32_t *n_rows_dev);

@@ -150,12 +150,12 @@ __global__ void __launch_bounds__(256) add_rmsnorm_sk_k(float *__restrict__ h, S
   pdl_wait();
   const int slot = blockIdx.x, live = live_rows(n_rows_dev, rows_ub);
   if (slot >= live) return;
-  const int n_rb = (live + v.rb_rows - 1) / v.rb_rows;
+  const int rbr = sk_rb_rows(live), n_rb = (live + rbr - 1) / rbr;
   float4 *hr = reinterpret_cast<float4 *>(h + (size_t)slot * d);
   float ss = 0.f;
   for (int k = threadIdx.x; k < d / 4; k += blockDim.x) {
     float4 x = hr[k];                                       // in flight together with the piece loads
-    float4 a = sk_sum4(v, sk_npieces(v, n_rb, 4 * k, slot), (size_t)slot * d + 4 * k);
+    float4 a = sk_sum4(v, sk_npieces(v, n_rb, rbr, 4 * k, slot), (size_t)slot * d + 4 * k);
     x.x += a.x; x.y += a.y; x.z += a.z; x.w += a.w;
     hr[k] = x;
     ss += x.x * x.x + x.y * x.y + x.z * x.z + x.w * x.w;
@@ -190,7 +190,7 @@ __global__ void __launch_bounds__(256) add_rmsnorm_sk_reg_k(float *__restrict__ 
   pdl_wait();
   const int slot = blockIdx.x, live = live_rows(n_rows_dev, rows_ub);
   if (slot >= live) return;
-  const int n_rb = (live + v.rb_rows - 1) / v.rb_rows;
+  const int rbr = sk_rb_rows(live), n_rb = (live + rbr - 1) / rbr;
   float4 *hr = reinterpret_cast<float4 *>(h + (size_t)slot * d);
   const size_t st = v.slot_stride / 4;
   float4 x[ITERS], acc[ITERS];
@@ -201,7 +201,7 @@ __global__ void __launch_bounds__(256) add_rmsnorm_sk_reg_k(float *__restrict__ 
   for (int it = 0; it < ITERS; ++it) {
     const int k = threadIdx.x + it * 256;
     const bool ok = k < d / 4;
-    np[it] = ok ? sk_npieces(v, n_rb, 4 * k, slot) : 0;
+    np[it] = ok ? sk_npieces(v, n_rb, rbr, 4 * k, slot) : 0;
     pp[it] = reinterpret_cast<const float4 *>(v.part + (size_t)slot * d) + (ok ? k : 0);
     x[it] = ok ? hr[k] : make_float4(0.f, 0.f, 0.f, 0.f);
     acc[it] = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -261,10 +261,10 @@ __global__ void __launch_bounds__(256) silu_mul_sk_k(SkView v, __nv_bfloat16 *__
   if (slot >= live) return;
   const int k = (blockIdx.x * blockDim.x + threadIdx.x) * 4;
   if (k >= F) return;
-  const int n_rb = (live + v.rb_rows - 1) / v.rb_rows;
+  const int rbr = sk_rb_rows(live), n_rb = (live + rbr - 1) / rbr;
   const size_t row = (size_t)slot * 2 * F;
   float4 g, u;
-  sk_sum4x2(v, sk_npieces(v, n_rb, k, slot), row + k, sk_npieces(v, n_rb, F + k, slot), row + F + k, g, u);
+  sk_sum4x2(v, sk_npieces(v, n_rb, rbr, k, slot), row + k, sk_npieces(v, n_rb, rbr, F + k, slot), row + F + k, g, u);
   auto f = [](float gg, float uu) { return gg / (1.0f + expf(-gg)) * uu; };
   *reinterpret_cast<uint2 *>(act + (size_t)slot * F + k) = pack4_bf16(f(g.x, u.x), f(g.y, u.y), f(g.z, u.z), f(g.w, u.w));
 }
@@ -283,7 +283,7 @@ __global__ void __launch_bounds__(128) rope_append_sk_k(SkView v, __nv_bfloat16 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int head = blockIdx.x * 4 + warp;
   if (head >= Hq + 2 * Hkv) return;
-  const int n_rb = (live + v.rb_rows - 1) / v.rb_rows;
+  const int rbr = sk_rb_rows(live), n_rb = (live + rbr - 1) / rbr;
   const int half = hd >> 1, col0 = head * hd;
   const size_t row = (size_t)slot * (Hq + 2 * Hkv) * hd + col0;
   const int page = slot_dst_page[slot], off = slot_dst_off[slot];
@@ -294,7 +294,7 @@ __global__ void __launch_bounds__(128) rope_append_sk_k(SkView v, __nv_bfloat16 
   float a1[4] = {0.f, 0.f, 0.f, 0.f}, a2[4] = {0.f, 0.f, 0.f, 0.f};
   if (act) {
     float4 x1, x2;
-    sk_sum4x2(v, sk_npieces(v, n_rb, col0 + p, slot), row + p, sk_npieces(v, n_rb, col0 + half + p, slot), row + half + p, x1, x2);
+    sk_sum4x2(v, sk_npieces(v, n_rb, rbr, col0 + p, slot), row + p, sk_npieces(v, n_rb, rbr, col0 + half + p, slot), row + half + p, x1, x2);
     a1[0] = x1.x; a1[1] = x1.y; a1[2] = x1.z; a1[3] = x1.w;
     a2[0] = x2.x; a2[1] = x2.y; a2[2] = x2.z; a2[3] = x2.w;
   }

@@ -42,7 +42,7 @@ struct SkParams {
   const int32_t *rb_list, *n_rb_dev;             // grouped mode
   int unit_tile;
   int stage_bytes, n_stages, tm_cols;            // tm_cols: columns of ONE accumulator (power of two >= 32)
-  int rb_rows, n_acc;                            // rows per row block (256 | 512 = two fused N blocks sharing the weight tile); TMEM accumulators (2 | 1)
+  int n_acc;                                     // TMEM accumulators: 2 (epilogue overlaps the next piece) | 1 (one 512-column accumulator)
 };
 
 struct SkBars {
@@ -78,15 +78,26 @@ __global__ void __launch_bounds__(SK_THREADS, 1) gemm_sk_k(const __grid_constant
                                                            SkParams p) {
   extern __shared__ unsigned char smem_raw[];
   unsigned char *stage_base = reinterpret_cast<unsigned char *>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
-  SkBars &bar = *reinterpret_cast<SkBars *>(stage_base + (size_t)p.n_stages * p.stage_bytes);
+  SkBars &bar = *reinterpret_cast<SkBars *>(stage_base + SMEM_BUDGET);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
   pdl_trigger();
   // ---- this CTA's unit range (uniform over the CTA; leave before any barrier / TMEM allocation if it is empty)
   PieceIter it0;
-  it0.rb_list = p.rb_list; it0.w_rows_per_group = p.w_rows_per_group; it0.nkb = p.nkb; it0.unit_tile = p.unit_tile; it0.P = gridDim.x; it0.cta = blockIdx.x; it0.rb_rows = p.rb_rows;
+  it0.rb_list = p.rb_list; it0.w_rows_per_group = p.w_rows_per_group; it0.nkb = p.nkb; it0.unit_tile = p.unit_tile; it0.P = gridDim.x; it0.cta = blockIdx.x; it0.rb_rows = SK_ROWBLOCK;
   if (p.rb_list) { pdl_wait(); it0.n_rb = *p.n_rb_dev; it0.live = 0; }
-  else { it0.live = p.n_rows_dev ? min(*p.n_rows_dev, p.rows_ub) : p.rows_ub; it0.n_rb = (it0.live + p.rb_rows - 1) / p.rb_rows; }
+  else {
+    // dense: block size, ring depth and TMEM split follow the LIVE row count (device value), not the host's bound
+    it0.live = p.n_rows_dev ? min(*p.n_rows_dev, p.rows_ub) : p.rows_ub;
+    it0.rb_rows = sk_rb_rows(it0.live);
+    it0.n_rb = (it0.live + it0.rb_rows - 1) / it0.rb_rows;
+    const int cap = (min(it0.rb_rows, it0.live) + 15) & ~15;
+    p.stage_bytes = W_STAGE_BYTES + cap / BOX_ROWS * BOX_BYTES;
+    p.n_stages = min(MAX_STAGES, SMEM_BUDGET / p.stage_bytes);
+    p.tm_cols = 32;
+    while (p.tm_cols < cap) p.tm_cols *= 2;
+    p.n_acc = p.tm_cols > 256 ? 1 : 2;
+  }
   if (it0.n_rb <= 0) return;
   it0.T = p.n_wtiles * it0.n_rb * (p.unit_tile ? 1 : p.nkb);
   it0.u = (int)((long long)blockIdx.x * it0.T / gridDim.x);
@@ -240,8 +251,8 @@ __global__ void sk_reduce_k(SkView v, float *__restrict__ out, int rows) {
   size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= (size_t)rows * v.N) return;
   int r = (int)(i / v.N), n = (int)(i % v.N);
-  int n_rb = (rows + v.rb_rows - 1) / v.rb_rows;
-  int np = sk_npieces(v, n_rb, n, r);
+  int rbr = sk_rb_rows(rows), n_rb = (rows + rbr - 1) / rbr;
+  int np = sk_npieces(v, n_rb, rbr, n, r);
   float a = v.part[i];
   for (int s = 1; s < np; ++s) a += v.part[(size_t)s * v.slot_stride + i];
   out[i] = a;
@@ -256,11 +267,7 @@ SkPlan sk_plan(int n_sms, int N, int K, int rows_ub, int n_rb_ub_grouped, bool r
   pl.nkb = K / BK;
   pl.n_wtiles = (N + BMW - 1) / BMW;
   const bool grouped = n_rb_ub_grouped > 0;
-  // 257..384 decode rows: one 512-row block = two MMA N blocks per stage that share the weight tile (one pass over the weights,
-  // one TMEM accumulator of 512 columns, 3 stages).  Measured on c3: step time -4 % at 288 rows, -2 % at 384, but +7 % at 512
-  // (2 stages, no epilogue overlap), so above 384 rows the 256-row blocks with two accumulators stay.
-  pl.rb_rows = (!grouped && rows_ub > SK_ROWBLOCK && rows_ub <= 384) ? 2 * SK_ROWBLOCK : SK_ROWBLOCK;
-  const int n_rb_ub = grouped ? n_rb_ub_grouped : (rows_ub + pl.rb_rows - 1) / pl.rb_rows;
+  const int n_rb_ub = grouped ? n_rb_ub_grouped : (rows_ub + SK_ROWBLOCK - 1) / SK_ROWBLOCK;   // dense 512-row blocks only lower it
   const long long tiles_ub = (long long)pl.n_wtiles * n_rb_ub;
   pl.unit_tile = grouped || tiles_ub >= 8LL * n_sms;
   if (pl.unit_tile) {
@@ -276,7 +283,7 @@ SkPlan sk_plan(int n_sms, int N, int K, int rows_ub, int n_rb_ub_grouped, bool r
       pl.P = std::max(1, pl.P * 3 / 4);
     }
   }
-  int cap = std::min(pl.rb_rows, (rows_ub + 15) & ~15);
+  int cap = std::min(SK_ROWBLOCK, (rows_ub + 15) & ~15);              // grouped mode; dense launches derive these on the device
   pl.stage_bytes = W_STAGE_BYTES + cap / BOX_ROWS * BOX_BYTES;
   pl.n_stages = std::min(MAX_STAGES, SMEM_BUDGET / pl.stage_bytes);
   pl.tm_cols = 32;
@@ -291,8 +298,8 @@ darts_status launch_gemm_sk(darts_ctx *c, const SkGemm &g) {
   SkParams p{};
   p.C = g.C; p.slot_stride = g.slot_stride; p.N = g.N; p.nkb = pl.nkb; p.n_wtiles = pl.n_wtiles; p.rows_ub = g.rows_ub; p.n_rows_dev = g.n_rows_dev;
   p.rb_list = g.rb_list; p.n_rb_dev = g.n_rb_dev; p.w_rows_per_group = g.w_rows_per_group; p.unit_tile = pl.unit_tile; p.stage_bytes = pl.stage_bytes; p.n_stages = pl.n_stages;
-  p.tm_cols = pl.tm_cols; p.rb_rows = pl.rb_rows; p.n_acc = pl.n_acc;
-  size_t smem = (size_t)pl.n_stages * pl.stage_bytes + sizeof(SkBars) + 1024;
+  p.tm_cols = pl.tm_cols; p.n_acc = pl.n_acc;
+  size_t smem = SMEM_BUDGET + sizeof(SkBars) + 1024;
   static bool attr = false;
   if (!attr) {
     CUDA_TRY(c, cudaFuncSetAttribute(gemm_sk_k, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET + (int)sizeof(SkBars) + 2048));

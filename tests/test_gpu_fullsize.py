@@ -89,3 +89,27 @@ def test_c4_width_sampled_rows_match_oracle():
 def test_c5_width_sampled_rows_match_oracle():
     # 128 experts, top-8, expert ffn 768, 32 q / 4 kv heads; prompt cut to 128 tokens (the oracle walks the experts in Python)
     _case("c5", [2, 11], P=128, steps=2, gap_tol=3e-4)
+
+
+def test_c3_width_rollout_is_bitwise_repeatable_across_row_count_buckets():
+    """The asynchronous loop sizes grids from a stale host-side bound of the live row count; nothing a row computes may depend on that
+    bound.  512 rows thinning out through the 384 / 256 / 128 row buckets (short forced-EOS lengths), three runs, identical bits."""
+    import torch
+    from paper_2605_30859_b200 import api
+    c = wl.CONFIGS["c3"]
+    cfg = dict(c["model"], n_layers=2)
+    G, P, K, max_new = c["G"], c["P"], c["K"], 48
+    model = wl.make_model(cfg, seed=5, device="cuda")
+    x = wl.rollout_inputs("c3", seed=5, max_new=max_new)
+    forced = wl.make_forced_len(x["Kp"], dict(kind="lognormal", mu=2.6, sigma=0.7, lo=2, hi=max_new), 5)
+    R = int(x["Kp"].sum())
+    d = api.Darts(model, page_size=64, n_pages=G * (P // 64) + R * 2 + 8, max_rows=R, max_prompts=G, max_prompt_len=P, max_new=max_new)
+    runs = [d.rollout_host(x["prompts"], x["Kp"], K, max_new, 1.0, 9, forced_len=forced, mode=api.MODE_DUAL_END) for _ in range(3)]
+    lens = runs[0]["len"]
+    assert lens.max() > 30 and np.sum(lens > 8) < 400 and np.sum(lens > 16) < 200          # the batch really crosses the buckets
+    for r in runs[1:]:
+        for k in ("tokens", "len", "status", "sel", "margin"):
+            assert np.array_equal(runs[0][k], r[k]), k
+    d.close()
+    del model
+    torch.cuda.empty_cache()
