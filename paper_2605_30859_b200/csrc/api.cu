@@ -80,8 +80,8 @@ size_t carve(darts_ctx *c, void *base) {
   c->slot_nsuf = k.take<int32_t>(A);
   c->forced_stage = k.take<int32_t>(G * DARTS_MAX_KP);
   if (attention_sm100_supported(c)) {
-    size_t npc_max = (size_t)ceil_div(rt.max_prompt_len, 512);
-    size_t max_parts = R * (npc_max + 2) + (size_t)rt.n_pages / 8 + 16;
+    size_t npc_max = (size_t)ceil_div(rt.max_prompt_len, ATTN_CHUNK_TOKENS);
+    size_t max_parts = R * (npc_max + 2) + (size_t)rt.n_pages / ATTN_CHUNK_PAGES + 16;
     if (model) max_parts = std::max(max_parts, A * npc_max + 16);            // a prefill pass: one partial per (prompt token, chunk)
     c->attn_max_items = (int)max_parts;
     c->attn_items_pre = k.take<int32_t>(max_parts * 6);

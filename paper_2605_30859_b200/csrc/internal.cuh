@@ -11,6 +11,10 @@
 
 #include "darts.h"
 
+#ifndef ATTN_CHUNK_PAGES
+#define ATTN_CHUNK_PAGES 8        // pages (of 64 tokens) per split-KV work item of the tuned attention kernel
+#endif
+#define ATTN_CHUNK_TOKENS (ATTN_CHUNK_PAGES * 64)
 #define DARTS_MAX_KP 32          // a group's pool is ranked by one warp (include/darts.h: Kp[i] <= 32)
 #define NEAR_TIE_MARGIN 1e-3f    // north_star: "bit-exact wherever the Gumbel-max margin exceeds 1e-3"
 

@@ -18,7 +18,7 @@
 
 namespace {
 
-constexpr int CH_PAGES = 8;                 // pages per item
+constexpr int CH_PAGES = ATTN_CHUNK_PAGES;   // pages per item
 constexpr int PAGE = 64, HD = 128;
 constexpr int CH_TOK = CH_PAGES * PAGE;
 constexpr int STAGES = 3;
