@@ -77,6 +77,45 @@ def measure(workload="c3", rows=(16, 32, 64, 128, 192, 256, 384, 512), steps=24,
     return out
 
 
+def predict_rollout(workload, b, t, seed=0, layers=None):
+    """Eq. 4 on this GPU: T = sum over lock-step iterations of PTL(active rows), with PTL interpolated from the measured
+    points (prefill not included), against the measured device time of the same rollout.  PTL(b) is measured at context = prompt
+    length; Eq. 4 has no context-length term, so the prediction misses the growth of the KV reads — the difference is reported."""
+    import torch
+    from . import api, workloads as wl
+    c = wl.CONFIGS[workload]
+    cfg = dict(c["model"])
+    if layers:
+        cfg["n_layers"] = layers
+    G, P, K, max_new = c["G"], c["P"], c["K"], c["max_new"]
+    model = wl.make_model(cfg, seed=seed, device="cuda")
+    x = wl.rollout_inputs(workload, seed=seed)
+    R = int(x["Kp"].sum())
+    page = 64
+    kv_page_bytes = cfg["n_layers"] * 2 * cfg["n_kv_heads"] * page * cfg["head_dim"] * 2
+    n_pages = min(G * ((P + page - 1) // page) + R * (max_new // page + 1), int(100e9 // kv_page_bytes))
+    d = api.Darts(model, page_size=page, n_pages=n_pages, max_rows=R, max_prompts=G, max_prompt_len=P, max_new=max_new)
+    toks = torch.from_numpy(x["prompts"]).cuda()
+    f_dev = torch.from_numpy(x["forced_len"]).cuda()
+    ms = []
+    for _ in range(2):                                       # the second run is the measurement
+        d.prefill_device(toks, P, x["Kp"], K, temperature=1.0, seed=seed, forced_len_dev=f_dev)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(d.stream)
+        d.run_to_completion()
+        e1.record(d.stream)
+        torch.cuda.synchronize()
+        ms.append(e0.elapsed_time(e1))
+    lens = d.results()["len"]
+    d.close()
+    steps = int(lens.max())
+    rows = [int((lens > s).sum()) for s in range(1, steps)]
+    pred = float(sum(np.interp(r, b, t) for r in rows))      # Eq. 4 written per step: same sum as over sorted length differences
+    return dict(decode_steps=len(rows), measured_ms=ms[-1], eq4_ms=pred, ratio=ms[-1] / pred,
+                note="PTL(b) measured at context = prompt length; the excess is KV traffic growing with the generated length")
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--workload", default="c3")
@@ -84,6 +123,8 @@ def main():
     ap.add_argument("--steps", type=int, default=24)
     ap.add_argument("--P", type=int, default=None)
     ap.add_argument("--layers", type=int, default=None)
+    ap.add_argument("--predict", action="store_true",
+                    help="also run one rollout of the workload and compare its device time with Eq. 4 evaluated on the fitted PTL(b)")
     a = ap.parse_args()
     pts = measure(a.workload, tuple(int(x) for x in a.rows.split(",")), a.steps, a.P, layers=a.layers)
     b, t = [p["rows"] for p in pts], [p["ms_median"] for p in pts]
@@ -91,6 +132,8 @@ def main():
     if len(b) >= 4:
         knots, vals, rmse = fit_piecewise3(b, t)
         res["fit"] = dict(knots=knots, ms_at_knots=vals, rmse_ms=rmse)
+    if a.predict:
+        res["eq4"] = predict_rollout(a.workload, b, t, layers=a.layers)
     json.dump(res, sys.stdout)
     print()
 
