@@ -220,16 +220,12 @@ struct TcGemm {
   size_t split_stride;
   int N, K, S, rows_ub;
   const int32_t *n_rows_dev;
-  int n_groups;                       // grouped (MoE): blockIdx.z / S = group
-  const int32_t *grp_off;
-  int b_rows_per_group;
   bool sample;                        // LM head: fused temperature + Gumbel-max epilogue -> ctx->top2
 };
 darts_status launch_gemm_tc(darts_ctx *c, const TcGemm &g);
 darts_status tc_make_map(darts_ctx *c, CUtensorMap *out, const void *base, long long rows, int K, int box_rows);
 darts_status tc_make_xmaps(darts_ctx *c, XMaps *out, const void *base, long long rows, int K);
 bool tc_shape_ok(int N, int K);
-int tc_pick_split(const darts_ctx *c, int N, int K, int rows_ub, int n_groups);
 // stream-K weight-streaming GEMM (kernels_gemm_sk.cu)
 #define SK_ROWBLOCK 256            // activation rows per MMA N block
 struct SkPlan { int nkb, n_wtiles, P, unit_tile, slots, stage_bytes, n_stages, tm_cols, n_acc; };   // stage / TMEM fields: grouped mode only
@@ -270,9 +266,6 @@ darts_status launch_add_rmsnorm_sk(darts_ctx *c, const SkView &v, const void *w,
 darts_status launch_silu_mul_sk(darts_ctx *c, const SkView &v, int rows_ub, const int32_t *n_rows_dev);
 darts_status launch_rope_append_sk(darts_ctx *c, int layer, const SkView &v, int rows_ub, const int32_t *n_rows_dev);
 // consumers of the split-K partials (kernels_fused.cu)
-darts_status launch_rope_append_part(darts_ctx *c, int layer, int S, int rows_ub, const int32_t *n_rows_dev);
-darts_status launch_add_rmsnorm(darts_ctx *c, const float *part, int S, size_t split_stride, const void *w, int rows_ub, const int32_t *n_rows_dev);
-darts_status launch_silu_mul_part(darts_ctx *c, int S, int rows_ub, const int32_t *n_rows_dev);
 darts_status launch_sample_finalize(darts_ctx *c, int n_tiles, int rows_ub);
 darts_status launch_sum_partials(darts_ctx *c, const float *part, float *out, int S, size_t n);
 darts_status launch_gather_rows_bf16(darts_ctx *c, const void *src, void *dst, int tok_begin, int g_begin, int g_end);

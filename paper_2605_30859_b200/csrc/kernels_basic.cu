@@ -153,18 +153,6 @@ __global__ void rope_append_k(const float *__restrict__ qkv, T *__restrict__ q_o
   }
 }
 
-darts_status launch_rope_append_part(darts_ctx *c, int layer, int S, int rows_ub, const int32_t *n_rows_dev) {
-  if (rows_ub <= 0) return DARTS_OK;
-  int nh = c->m.n_q_heads + 2 * c->m.n_kv_heads;
-  dim3 grid((nh + 3) / 4, rows_ub);
-  using T = __nv_bfloat16;
-  rope_append_k<T><<<grid, 128, 0, c->stream>>>(c->part, (T *)c->q, (T *)c->kv_pool + (size_t)layer * c->kv_layer_elems, c->slot_dst_page,
-                                                c->slot_dst_off, c->slot_cs, c->m.qk_norm ? (const T *)c->q_norm[layer] : nullptr,
-                                                c->m.qk_norm ? (const T *)c->k_norm[layer] : nullptr, c->m.n_q_heads, c->m.n_kv_heads,
-                                                c->m.head_dim, c->m.rms_eps, c->geom(), S, (size_t)rows_ub * c->n_qkv, n_rows_dev, rows_ub);
-  return post_launch(c, "rope_append_part");
-}
-
 darts_status launch_rope_append(darts_ctx *c, int layer, int rows_ub, const int32_t *n_rows_dev) {
   if (rows_ub <= 0) return DARTS_OK;
   int nh = c->m.n_q_heads + 2 * c->m.n_kv_heads;

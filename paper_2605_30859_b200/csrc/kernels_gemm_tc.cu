@@ -12,7 +12,6 @@
 // Decode GEMMs are weight-streaming (HBM-bound) below ~250 active rows: the grid is filled by splitting K
 // (deterministic: every split writes its own partial, the consumer kernel adds them in split order).  Rows of the
 // 128-row MMA tile beyond the live row count hold stale shared memory; they only produce their own (never stored) rows.
-// Grouped mode (MoE): blockIdx.z / S selects a group with its own row range (grp_off) and weight slab.
 #include "internal.cuh"
 #include "philox.cuh"
 #include "sm100_ptx.cuh"
@@ -34,8 +33,6 @@ struct GemmParams {
   int N, K, S;
   int rows_ub;
   const int32_t *n_rows_dev;      // live row count on the device (nullable)
-  const int32_t *grp_off;         // grouped: [n_groups + 1] row offsets; null = one group starting at row 0
-  int b_rows_per_group;           // grouped: weight rows per group (0 = dense)
   // EPI_SAMPLE
   float4 *top2;                   // [n_tiles][rows] (best y, second y, bits(best index), -)
   float *logits_dump;             // optional [rows][N]
@@ -59,12 +56,12 @@ __global__ void __launch_bounds__(GEMM_THREADS) gemm_tc_k(const __grid_constant_
   using Smem = GemmSmem<BN, STAGES>;
   Smem &sm = *reinterpret_cast<Smem *>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int grp = blockIdx.z / p.S, split = blockIdx.z % p.S;
+  const int split = blockIdx.z;
 
   // ---- which rows does this tile cover? (uniform over the CTA; exit before any barrier / TMEM allocation)
   int row_begin, row_end;
-  if (p.grp_off) { row_begin = p.grp_off[grp]; row_end = p.grp_off[grp + 1]; }
-  else { row_begin = 0; row_end = p.n_rows_dev ? min(*p.n_rows_dev, p.rows_ub) : p.rows_ub; }
+  row_begin = 0;
+  row_end = p.n_rows_dev ? min(*p.n_rows_dev, p.rows_ub) : p.rows_ub;
   const int m0 = row_begin + blockIdx.x * BM;             // row tiles vary fastest: the CTAs that share a weight tile run together (L2 reuse)
   if (m0 >= row_end) return;
   const int live = min(BM, row_end - m0);                // live rows of this tile
@@ -90,7 +87,7 @@ __global__ void __launch_bounds__(GEMM_THREADS) gemm_tc_k(const __grid_constant_
     if (lane == 0) {
       const int nbox = (live + A_BOX_ROWS - 1) / A_BOX_ROWS;
       const int tx = nbox * (A_BOX_ROWS * BK * 2) + BN * BK * 2;
-      const int brow = grp * p.b_rows_per_group + n0;
+      const int brow = n0;
       int stage = 0, phase = 0;
       for (int kb = kb0; kb < kb1; ++kb) {
         mbar_wait(&sm.empty[stage], phase ^ 1);
@@ -251,24 +248,11 @@ darts_status tc_make_xmaps(darts_ctx *c, XMaps *out, const void *base, long long
 
 bool tc_shape_ok(int N, int K) { return K % BK == 0 && K >= BK && N % 4 == 0; }
 
-// Split-K factor: fill ~2 CTAs per SM, keep >= 4 k-blocks per split, stay inside the partial buffer.  Depends on the
-// shape and on the number of 128-row tiles only (batch invariance holds within a row-count bucket).
-int tc_pick_split(const darts_ctx *c, int N, int K, int rows_ub, int n_groups) {
-  int tiles = ((N + 127) / 128) * ((rows_ub + BM - 1) / BM) * (n_groups > 0 ? n_groups : 1);
-  int nkb = K / BK, S = 1;
-  while (tiles * S * 2 <= 2 * c->n_sms && nkb / (S * 2) >= 4 && S * 2 <= 16 &&
-         (size_t)(S * 2) * (size_t)rows_ub * (size_t)N * 4 <= c->part_bytes)
-    S *= 2;
-  return S;
-}
-
 darts_status launch_gemm_tc(darts_ctx *c, const TcGemm &g) {
   if (g.rows_ub <= 0) return DARTS_OK;
   GemmParams p{};
   p.C = g.C; p.split_stride = g.split_stride; p.N = g.N; p.K = g.K; p.S = g.S; p.rows_ub = g.rows_ub; p.n_rows_dev = g.n_rows_dev;
-  p.grp_off = g.grp_off; p.b_rows_per_group = g.b_rows_per_group;
-  int groups = g.grp_off ? g.n_groups : 1;
-  dim3 grid((g.rows_ub + BM - 1) / BM, (g.N + 127) / 128, groups * g.S);
+  dim3 grid((g.rows_ub + BM - 1) / BM, (g.N + 127) / 128, g.S);
   if (!g.sample) return launch_cfg<128, 3, EPI_STORE>(c, *g.a_map, *g.b_map, p, grid);
   p.top2 = (float4 *)c->top2; p.logits_dump = (c->rt.flags & DARTS_FLAG_DUMP_LOGITS) ? c->logits : nullptr;
   p.row_list = c->row_list; p.row_prompt = c->row_prompt; p.row_sample = c->row_sample; p.row_len = c->row_len;
