@@ -234,22 +234,25 @@ darts_status forward_layers_tc(darts_ctx *c, int rows_ub, const int32_t *n_rows_
   TRY(launch_rope_table(c, rows_ub, n_rows_dev));
   TRY(launch_moe_begin_pass(c));
   TRY(launch_rmsnorm(c, c->h, c->attn_norm[0], c->xn, rows_ub, n_rows_dev));
+  // DARTS_SKIP (profiling aid): bit k drops the k-th kernel class of every layer so that the change of the step time gives that class's
+  // LIVE cost (launch-list times are serialised and cold); results are garbage in that mode.
+  const unsigned sk = c->skip_mask;
   for (int l = 0; l < L; ++l) {
     SkGemm g = sk_gemm(c, &c->xm_xn, &c->tm_wqkv[l], c->n_qkv, d, rows_ub, n_rows_dev);
-    TRY(launch_gemm_sk(c, g));
-    TRY(launch_rope_append_sk(c, l, sk_view(g), rows_ub, n_rows_dev));
-    TRY(launch_attention(c, l, c->q, c->ao, rows_ub, n_rows_dev));
+    if (!(sk & 1)) TRY(launch_gemm_sk(c, g));
+    if (!(sk & 2)) TRY(launch_rope_append_sk(c, l, sk_view(g), rows_ub, n_rows_dev));
+    if ((sk & 12) != 12) TRY(launch_attention(c, l, c->q, c->ao, rows_ub, n_rows_dev));
     g = sk_gemm(c, &c->xm_ao, &c->tm_wo[l], d, qd, rows_ub, n_rows_dev);
-    TRY(launch_gemm_sk(c, g));
-    TRY(launch_add_rmsnorm_sk(c, sk_view(g), c->mlp_norm[l], rows_ub, n_rows_dev));
+    if (!(sk & 16)) TRY(launch_gemm_sk(c, g));
+    if (!(sk & 32)) TRY(launch_add_rmsnorm_sk(c, sk_view(g), c->mlp_norm[l], rows_ub, n_rows_dev));
     const void *next_norm = l + 1 < L ? c->attn_norm[l + 1] : c->final_norm;
     if (m.n_experts == 0) {
       g = sk_gemm(c, &c->xm_xn, &c->tm_wgu[l], 2 * F, d, rows_ub, n_rows_dev);
-      TRY(launch_gemm_sk(c, g));
-      TRY(launch_silu_mul_sk(c, sk_view(g), rows_ub, n_rows_dev));
+      if (!(sk & 64)) TRY(launch_gemm_sk(c, g));
+      if (!(sk & 128)) TRY(launch_silu_mul_sk(c, sk_view(g), rows_ub, n_rows_dev));
       g = sk_gemm(c, &c->xm_act, &c->tm_wd[l], d, F, rows_ub, n_rows_dev);
-      TRY(launch_gemm_sk(c, g));
-      TRY(launch_add_rmsnorm_sk(c, sk_view(g), next_norm, rows_ub, n_rows_dev));
+      if (!(sk & 256)) TRY(launch_gemm_sk(c, g));
+      if (!(sk & 512)) TRY(launch_add_rmsnorm_sk(c, sk_view(g), next_norm, rows_ub, n_rows_dev));
     } else {
       TRY(launch_moe_tc(c, l, next_norm, rows_ub, n_rows_dev));
     }
@@ -434,6 +437,7 @@ darts_status darts_create(const darts_model_desc *m, const darts_weights *w, con
   if (((uintptr_t)rt->workspace & 255) != 0) FAIL(c, DARTS_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
   c->has_weights = m->vocab > 0;
   c->use_pdl = getenv("DARTS_NO_PDL") == nullptr;
+  c->skip_mask = getenv("DARTS_SKIP") ? (unsigned)strtoul(getenv("DARTS_SKIP"), nullptr, 0) : 0u;
   if (c->has_weights) {
     int L = m->n_layers;
     c->embed = w->embed; c->final_norm = w->final_norm; c->lm_head = w->lm_head;

@@ -89,6 +89,7 @@ struct darts_ctx {
   int32_t attn_rows;
   // tensor-core path (bf16, kernels_gemm_tc.cu): split-K partial buffer, LM-head top-2 partials, tensor maps
   bool tc_path;                  // every GEMM of this model runs on tcgen05
+  unsigned skip_mask;            // profiling aid (env DARTS_SKIP, bit per kernel class of a layer): skipped launches leave stale data — timing only
   bool use_pdl;                  // launch the stream-K GEMMs as programmatic dependents (DARTS_NO_PDL=1 in the environment disables)
   float *part;                   // [S][rows][N] fp32 partials of the GEMM in flight
   size_t part_bytes;

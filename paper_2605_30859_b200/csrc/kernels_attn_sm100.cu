@@ -499,10 +499,10 @@ darts_status launch_attention_sm100(darts_ctx *c, int layer, const void *q, void
   p.page_elems = c->kv_page_elems; p.tile_elems = c->kv_tile_elems;
   p.c = 1.4426950408889634f / sqrtf((float)HD);
   int grid = c->n_sms * 2;
-  launch_pdl(c, attn_main_k, dim3(grid), dim3(THREADS), smem, p);
+  if (!(c->skip_mask & 4)) launch_pdl(c, attn_main_k, dim3(grid), dim3(THREADS), smem, p);
   c->launches++;
   if (cudaGetLastError() != cudaSuccess) FAIL(c, DARTS_ERR_CUDA, "launch attn_main failed: %s", cudaGetErrorString(cudaGetLastError()));
-  launch_pdl(c, attn_merge_k, dim3(rows_ub, (p.Hq + 7) / 8), dim3(256), 0, c->part_ml, c->part_acc, c->part_base, c->part_cnt, (__nv_bfloat16 *)out, p.Hq, p.c, n_rows_dev, rows_ub);
+  if (!(c->skip_mask & 8)) launch_pdl(c, attn_merge_k, dim3(rows_ub, (p.Hq + 7) / 8), dim3(256), 0, c->part_ml, c->part_acc, c->part_base, c->part_cnt, (__nv_bfloat16 *)out, p.Hq, p.c, n_rows_dev, rows_ub);
   c->launches++;
   if (cudaGetLastError() != cudaSuccess) FAIL(c, DARTS_ERR_CUDA, "launch attn_merge failed");
   return DARTS_OK;

@@ -29,7 +29,7 @@ __device__ __forceinline__ Top2 top2_merge(const Top2 &a, const Top2 &b) {
 __device__ __forceinline__ void finish_row(DevState *st, int row, int slot, int s, const Top2 &t, int32_t *row_len, uint8_t *row_status,
                                            const int32_t *row_forced, int32_t *row_last_tok, int32_t *row_slot, int32_t *row_slot_step,
                                            int32_t *tokens_out, float *margin_out, int max_new_stride, int max_len, int eos_id) {
-  int tok = t.i1;
+  int tok = t.i1 == 0x7fffffff ? 0 : t.i1;              // every y was NaN (cannot happen with finite weights): stay inside the vocabulary
   float margin = t.b1 - t.b2;
   int len = s + 1;
   uint8_t status = DARTS_ROW_ACTIVE;
