@@ -490,6 +490,7 @@ const char *darts_last_error(const darts_ctx *c) { return c ? c->err : "NULL con
 darts_status darts_prefill(darts_ctx *c, const int32_t *prompt_tokens, const int32_t *prompt_offsets_host, int32_t G,
                            const int32_t *Kp_host, const int32_t *forced_len, const darts_policy *policy, float temperature, uint64_t seed) {
   if (!c) return DARTS_ERR_INVALID_ARG;
+  c->max_len = c->rt.max_new;                      // the step-wise API always runs to the context's limit (darts_rollout* pass their own)
   return prefill_impl(c, prompt_tokens, false, prompt_offsets_host, G, Kp_host, forced_len, policy, temperature, seed);
 }
 

@@ -85,3 +85,21 @@ def test_all_rows_stop_at_their_first_token_and_all_rows_truncate(cfg, page, tol
     for key in ("len", "status", "sel", "sel_mask", "close_step"):
         assert np.array_equal(g[key], orc[key]), key
     d.close()
+
+
+def test_stepwise_api_is_not_limited_by_an_earlier_shorter_rollout():
+    """darts_rollout* take max_len per call; a later darts_prefill + darts_run_to_completion must run to the context's own limit."""
+    c = wl.CONFIGS["c1"]
+    x = wl.rollout_inputs("c1", seed=2)
+    d, host = make_ctx(c["model"], 2, c["G"], c["Kp"], c["P"], c["max_new"], page=16)
+    short = d.rollout_host(x["prompts"], x["Kp"], x["K"], 6, 1.0, 4, forced_len=None, mode=MODE_DUAL_END)
+    assert short["len"].max() <= 6 and np.any(short["status"] == TRUNC)
+    d.prefill(list(x["prompts"]), x["Kp"], x["K"], temperature=1.0, seed=4, forced_len=x["forced_len"], mode=MODE_DUAL_END)
+    d.run_to_completion()
+    full = d.results()
+    orc = ro.rollout_stepwise(host, x["prompts"], x["Kp"], x["K"], c["max_new"], 1.0, 4, forced_len=x["forced_len"], mode=MODE_DUAL_END,
+                              teacher=full["tokens"])
+    assert full["len"].max() > 6
+    for key in ("len", "status", "sel"):
+        assert np.array_equal(full[key], orc[key]), key
+    d.close()
