@@ -12,10 +12,18 @@ from tests.gpu_util import make_ctx
 pytestmark = pytest.mark.gpu
 
 
-@pytest.mark.parametrize("seed", range(24))
-def test_random_policies_match_oracle_bit_exact(seed):
+BF16 = dict(n_layers=2, d_model=256, n_q_heads=4, n_kv_heads=2, head_dim=128, ffn=512, vocab=1024, n_experts=0, top_k=0, expert_ffn=0,
+            qk_norm=False, rope_theta=1.0e6, rms_eps=1.0e-6, dtype="bf16")
+BF16_MOE = dict(BF16, ffn=0, n_experts=8, top_k=2, expert_ffn=128)
+
+
+@pytest.mark.parametrize("seed,kind", [(s, "f32") for s in range(24)] + [(s, "bf16") for s in range(24, 30)] + [(s, "moe") for s in range(30, 34)])
+def test_random_policies_match_oracle_bit_exact(seed, kind):
     rng = np.random.default_rng(100 + seed)
-    cfg = dict(wl.CONFIGS["c1"]["model"], vocab=int(rng.choice([64, 512])))       # vocab 64: natural EOS fires now and then
+    if kind == "f32":
+        cfg = dict(wl.CONFIGS["c1"]["model"], vocab=int(rng.choice([64, 512])))   # vocab 64: natural EOS fires now and then
+    else:
+        cfg = dict(BF16 if kind == "bf16" else BF16_MOE)                          # tensor-core path: stream-K GEMMs, tuned attention
     G = int(rng.integers(1, 6))
     K = int(rng.integers(1, 7))
     Kp = rng.integers(K, min(32, 3 * K) + 1, size=G).astype(np.int32)
@@ -36,7 +44,7 @@ def test_random_policies_match_oracle_bit_exact(seed):
             forced[i, :Kp[i]] = 0
         else:              # fewer than K valid rows
             forced[i, :Kp[i]] = np.where(rng.random(Kp[i]) < 0.3, rng.integers(1, max_new + 1, size=Kp[i]), 10 * max_new)
-    d, host = make_ctx(cfg, seed, G, int(Kp.max()), P, max_new, page=8, std=0.3)
+    d, host = make_ctx(cfg, seed, G, int(Kp.max()), P, max_new, page=8 if kind == "f32" else 64, std=0.3 if kind == "f32" else 0.05)
     d.prefill(prompts, Kp, K, temperature=1.0, seed=seed, forced_len=forced, L_long=L_long, M_up=M_up, mode=mode)
     d.run_to_completion()
     gpu = d.results()
