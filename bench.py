@@ -276,6 +276,9 @@ def main():
         return profile_steps(args)
 
     import torch
+    from paper_2605_30859_b200 import build as _build
+    if not os.path.exists(_build.LIB):                       # build step (nvcc, sm_100a), not a fallback: without the library nothing runs
+        _build.build()
     from paper_2605_30859_b200 import api, workloads as wl
     rank, world, local = dist_setup(args.gpus)
     peaks = measured_peaks()
