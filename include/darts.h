@@ -29,6 +29,12 @@
  *   - There is no CPU fallback and no other backend: on a device that is not sm_100 every entry
  *     point that needs the GPU returns DARTS_ERR_UNSUPPORTED.
  *
+ * Environment (read at darts_create; diagnostics only, never needed for correct use)
+ *   DARTS_NO_PDL=1           launch every kernel as an ordinary stream launch (no programmatic dependent launch)
+ *   DARTS_SKIP=<bitmask>     profiling aid: drop one kernel class of every layer (results are garbage; see
+ *                            profiles/r1_live_cost_by_kernel.md).  Never set it outside a timing experiment.
+ *   DARTS_ADDNORM_REG_MAX=n  row bound under which the register-resident add + RMSNorm kernel is used (default 128)
+ *
  * Layouts
  *   - Projections are [out_features, in_features] row-major in the model dtype (F32 or BF16).
  *     wqkv rows: n_q_heads q-heads, then n_kv_heads k-heads, then n_kv_heads v-heads (head_dim rows each).
