@@ -111,6 +111,8 @@ size_t carve(darts_ctx *c, void *base) {
       c->moe_eid = k.take<int32_t>(RK);
       c->moe_pos = k.take<int32_t>(RK);
       c->moe_w = k.take<float>(RK);
+      c->moe_arrive_n = A / 4 + 1;
+      c->moe_arrive = k.take<int32_t>(c->moe_arrive_n);         // router arrival counters, one per block of 4 slots; zero between launches
     }
     if (c->tc_path) {
       // stream-K pieces [slots][rows][N]: whole-tile mode (1 slot) for the prefill-sized passes, up to 16 slots for decode rows
@@ -460,6 +462,7 @@ darts_status darts_create(const darts_model_desc *m, const darts_weights *w, con
   CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev[0], cudaEventDisableTiming));
   CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev[1], cudaEventDisableTiming));
   CUDA_TRY(c, cudaMemsetAsync(c->st, 0, sizeof(DevState), c->stream));
+  if (c->moe_arrive) CUDA_TRY(c, cudaMemsetAsync(c->moe_arrive, 0, c->moe_arrive_n * sizeof(int32_t), c->stream));
   // The pool must hold finite values everywhere: a partially filled page is multiplied by zero probabilities.
   CUDA_TRY(c, cudaMemsetAsync(c->kv_pool, 0, (size_t)m->n_layers * c->kv_layer_elems * c->elt, c->stream));
   return DARTS_OK;

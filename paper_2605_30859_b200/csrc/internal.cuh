@@ -98,7 +98,8 @@ struct darts_ctx {
   CUtensorMap tm_lm, tm_xn, tm_ao, tm_act, tm_xs, tm_hl;                      // activations: 16-row boxes
   XMaps xm_xn, xm_ao, xm_act, xm_xs;                                            // the same matrices for the stream-K kernel
   // MoE (kernels_moe.cu)
-  int32_t *moe_eid, *moe_pos, *moe_off, *moe_cnt, *moe_tok, *moe_rb, *moe_nrb;   // moe_rb: row blocks {row0, nrows, expert, -}   // moe_cnt: [n_layers][E], zeroed once per forward pass
+  int32_t *moe_eid, *moe_pos, *moe_off, *moe_cnt, *moe_tok, *moe_rb, *moe_nrb, *moe_arrive;
+  size_t moe_arrive_n;   // moe_rb: row blocks {row0, nrows, expert, -}   // moe_cnt: [n_layers][E], zeroed once per forward pass
   float *moe_w, *moe_logits, *moe_y;   // gates [rows*top_k]; router logits [rows][E]; generic path expert outputs [rows*top_k][d]
   void *xs;                      // expert-sorted copy of xn [max_rows * top_k][d]
   // tuned attention (kernels_attn_sm100.cu): per-step work list and split-KV partials

@@ -3,8 +3,9 @@
 //   w = p_top / sum(p_top);  m = sum_e w_e expert_e(b);  h += m.
 // Kernels (all sized from a host upper bound of the row count, live count read on the device):
 //   moe_router_k     router logits [slot][E] straight from the fp32 residual stream (the bf16 xn is NOT used: the
-//                    discrete top-k decision is taken in fp32 on both sides, R13)
-//   moe_topk_k       one warp per slot: softmax, k rounds of warp arg-max, renormalised gates, per-expert counts
+//                    discrete top-k decision is taken in fp32 on both sides, R13); the last CTA to finish a block of
+//                    slots then takes their top-k, one warp per slot: softmax, k rounds of warp arg-max, renormalised
+//                    gates, per-expert counts
 //   moe_place_k      (tensor-core path) one CTA per expert: exclusive scan of the counts, stable ballot ranking of the
 //                    expert's assignments, gather of their bf16 activation rows into the expert-sorted matrix xs
 //   [grouped stream-K tcgen05 GEMMs of kernels_gemm_sk.cu: gate/up then down, one row block per (expert, <= 256 rows)]
@@ -35,14 +36,64 @@ darts_status post(darts_ctx *c, const char *what) {
 }
 
 // grid (ceil(rows_ub / RROWS), ceil(E / REXP)), 256 threads, dynamic smem RROWS * d floats.  d % 4 == 0.
+// One warp per slot.  Ordering is taken on the logits (monotone in p, so identical to ordering by p in exact arithmetic).
+__device__ __forceinline__ void topk_row(const float *logits, int E, int top_k, int32_t *__restrict__ eid, float *__restrict__ gate,
+                                         int32_t *__restrict__ pos, int32_t *__restrict__ cnt, int slot, int lane) {
+  float z[MAX_E_PER_LANE];
+  float mx = -INFINITY;
+#pragma unroll
+  for (int q = 0; q < MAX_E_PER_LANE; ++q) {
+    int e = q * 32 + lane;
+    z[q] = e < E ? __ldcg(&logits[(size_t)slot * E + e]) : -INFINITY;
+    mx = fmaxf(mx, z[q]);
+  }
+  mx = warp_max(mx);
+  float sum = 0.f;
+#pragma unroll
+  for (int q = 0; q < MAX_E_PER_LANE; ++q) sum += (q * 32 + lane) < E ? expf(z[q] - mx) : 0.f;
+  sum = warp_sum(sum);
+  unsigned taken = 0;
+  float my_p = 0.f, psum = 0.f;
+  int my_e = -1;
+  for (int k = 0; k < top_k; ++k) {
+    float bz = -INFINITY;
+    int be = 0x7fffffff;
+#pragma unroll
+    for (int q = 0; q < MAX_E_PER_LANE; ++q) {
+      int e = q * 32 + lane;
+      if (e < E && !((taken >> q) & 1u) && (z[q] > bz)) { bz = z[q]; be = e; }     // ascending e: strict > keeps the lower id
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      float oz = __shfl_xor_sync(0xffffffffu, bz, o);
+      int oe = __shfl_xor_sync(0xffffffffu, be, o);
+      if (oz > bz || (oz == bz && oe < be)) { bz = oz; be = oe; }
+    }
+    if ((be & 31) == lane) taken |= 1u << (be >> 5);
+    float p = expf(bz - mx) / sum;
+    psum += p;
+    if (lane == k) { my_p = p; my_e = be; }
+  }
+  if (lane < top_k) {
+    int a = slot * top_k + lane;
+    eid[a] = my_e;
+    gate[a] = my_p / psum;
+    pos[a] = a;                                        // identity; moe_place_k overwrites it on the tensor-core path
+    if (cnt) atomicAdd(&cnt[my_e], 1);
+  }
+}
+
+
 template <typename T>
 __global__ void __launch_bounds__(256) moe_router_k(const float *__restrict__ h, const T *__restrict__ wnorm, const float *__restrict__ wr,
-                                                    float *__restrict__ logits, int d, int E, float eps, const int32_t *n_rows_dev,
-                                                    int rows_ub) {
+                                                    float *logits, int d, int E, float eps, int top_k, int32_t *__restrict__ eid,
+                                                    float *__restrict__ gate, int32_t *__restrict__ pos, int32_t *__restrict__ cnt,
+                                                    int32_t *arrive, const int32_t *n_rows_dev, int rows_ub) {
   pdl_trigger();
   pdl_wait();
   extern __shared__ float xs[];                       // [RROWS][d] normalised rows
   __shared__ float red[RROWS][8];
+  __shared__ int s_last;
   const int n = live_rows(n_rows_dev, rows_ub);
   const int s0 = blockIdx.x * RROWS;
   if (s0 >= n) return;
@@ -85,59 +136,15 @@ __global__ void __launch_bounds__(256) moe_router_k(const float *__restrict__ h,
       if (lane == 0 && s0 + r < n) logits[(size_t)(s0 + r) * E + e] = v;
     }
   }
-}
-
-// One warp per slot.  Ordering is taken on the logits (monotone in p, so identical to ordering by p in exact arithmetic).
-__global__ void __launch_bounds__(128) moe_topk_k(const float *__restrict__ logits, int E, int top_k, int32_t *__restrict__ eid,
-                                                  float *__restrict__ gate, int32_t *__restrict__ pos, int32_t *__restrict__ cnt,
-                                                  const int32_t *n_rows_dev, int rows_ub) {
-  pdl_trigger();
-  pdl_wait();
-  const int n = live_rows(n_rows_dev, rows_ub);
-  const int slot = blockIdx.x * 4 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
-  if (slot >= n) return;
-  float z[MAX_E_PER_LANE];
-  float mx = -INFINITY;
-#pragma unroll
-  for (int q = 0; q < MAX_E_PER_LANE; ++q) {
-    int e = q * 32 + lane;
-    z[q] = e < E ? logits[(size_t)slot * E + e] : -INFINITY;
-    mx = fmaxf(mx, z[q]);
-  }
-  mx = warp_max(mx);
-  float sum = 0.f;
-#pragma unroll
-  for (int q = 0; q < MAX_E_PER_LANE; ++q) sum += (q * 32 + lane) < E ? expf(z[q] - mx) : 0.f;
-  sum = warp_sum(sum);
-  unsigned taken = 0;
-  float my_p = 0.f, psum = 0.f;
-  int my_e = -1;
-  for (int k = 0; k < top_k; ++k) {
-    float bz = -INFINITY;
-    int be = 0x7fffffff;
-#pragma unroll
-    for (int q = 0; q < MAX_E_PER_LANE; ++q) {
-      int e = q * 32 + lane;
-      if (e < E && !((taken >> q) & 1u) && (z[q] > bz)) { bz = z[q]; be = e; }     // ascending e: strict > keeps the lower id
-    }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-      float oz = __shfl_xor_sync(0xffffffffu, bz, o);
-      int oe = __shfl_xor_sync(0xffffffffu, be, o);
-      if (oz > bz || (oz == bz && oe < be)) { bz = oz; be = oe; }
-    }
-    if ((be & 31) == lane) taken |= 1u << (be >> 5);
-    float p = expf(bz - mx) / sum;
-    psum += p;
-    if (lane == k) { my_p = p; my_e = be; }
-  }
-  if (lane < top_k) {
-    int a = slot * top_k + lane;
-    eid[a] = my_e;
-    gate[a] = my_p / psum;
-    pos[a] = a;                                        // identity; moe_place_k overwrites it on the tensor-core path
-    if (cnt) atomicAdd(&cnt[my_e], 1);
-  }
+  // the CTA that completes a slot block's logits (last of gridDim.y to arrive) takes its top-k: one warp per slot
+  __threadfence();
+  __syncthreads();
+  if (threadIdx.x == 0) s_last = atomicAdd(&arrive[blockIdx.x], 1) == (int)gridDim.y - 1;
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  if (threadIdx.x == 0) arrive[blockIdx.x] = 0;       // ready for the next layer's launch
+  if (warp < RROWS && s0 + warp < n) topk_row(logits, E, top_k, eid, gate, pos, cnt, s0 + warp, lane);
 }
 
 // One CTA per expert (tensor-core path).  off[e] = sum_{e'<e} cnt[e'];  the expert's assignments keep their slot
@@ -308,11 +315,8 @@ darts_status route(darts_ctx *c, int layer, int rows_ub, const int32_t *n_rows_d
     attr = true;
   }
   launch_pdl(c, moe_router_k<T>, grid, dim3(256), smem, c->h, (const T *)c->mlp_norm[layer], (const float *)c->wr[layer], c->moe_logits, m.d_model,
-                                                  m.n_experts, m.rms_eps, n_rows_dev, rows_ub);
-  darts_status s = post(c, "moe_router");
-  if (s != DARTS_OK) return s;
-  launch_pdl(c, moe_topk_k, dim3((rows_ub + 3) / 4), dim3(128), 0, c->moe_logits, m.n_experts, m.top_k, c->moe_eid, c->moe_w, c->moe_pos, cnt, n_rows_dev, rows_ub);
-  return post(c, "moe_topk");
+             m.n_experts, m.rms_eps, m.top_k, c->moe_eid, c->moe_w, c->moe_pos, cnt, c->moe_arrive, n_rows_dev, rows_ub);
+  return post(c, "moe_router");
 }
 
 }  // namespace
