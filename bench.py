@@ -306,7 +306,7 @@ def main():
         K, P = c["K"], c["P"]
         mode = api.MODE_SHORTEST_EARLY_STOP if args.mode == "early" else api.MODE_AUTO
         kvb = 2 * cfg["n_kv_heads"] * cfg["head_dim"] * 2
-        n_runs = args.warmup + 2 * args.steps
+        n_runs = args.warmup + args.steps                     # the e2e phase re-runs the device phase's inputs and seeds: same work, comparable numbers
         host_in = [wl.rollout_inputs(name, seed=1000 * rank + it, G=G, max_new=max_new) for it in range(n_runs)]
         pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
         gen_tokens, kept_tokens, dev_ms, e2e_ms, e2e_tokens, attn_ms, attn_bytes, steps_count, near, step_bytes = [], [], [], [], [], [], [], [], [], []
@@ -315,6 +315,8 @@ def main():
         for phase, n in (("warmup", args.warmup), ("device", args.steps), ("e2e", args.steps)):
             if phase != "warmup":
                 barrier(world)
+            if phase == "e2e":
+                it = args.warmup
             for _ in range(n):
                 xin = host_in[it]; it += 1
                 if phase == "e2e":
