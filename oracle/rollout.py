@@ -22,13 +22,14 @@ Each row owns a private copy of its prompt's KV (no prefix sharing here, on purp
 Returned dict: tokens [R, max_new] int32 (-1 beyond len), len [R], status [R],
 sel [G, K] (sample indices j), sel_mask [G], close_step [G], n_steps,
 n_generated_tokens (all rows, incl. pruned), n_kept_tokens, margins [R, max_new],
+logprobs [R, max_new] (log softmax(z/T) of the token the sampler drew at each step),
 oracle_tokens [R, max_new] (the oracle's own argmax, differs from `tokens` only under
 teacher forcing), logits (dict (r,s)->z, only if keep_logits).
 """
 import numpy as np
 
 from . import ACTIVE, VALID, TRUNC, PRUNED, MODE_AUTO
-from .sampling import sample_token
+from .sampling import sample_token, token_logprob
 from .selection import apply_stop, compact, group_mode, group_rule, sel_mask, select_dual
 from . import transformer as _tf
 from .transformer import decode_one, prefill
@@ -75,6 +76,7 @@ def rollout_stepwise(model, prompts, Kp, K, max_new, T, seed, forced_len=None, L
     tokens = -np.ones((R, max_new), dtype=np.int32)
     otok = -np.ones((R, max_new), dtype=np.int32)
     margins = np.full((R, max_new), np.nan)
+    logprobs = np.full((R, max_new), np.nan)                # of the DRAWN token (before a forced EOS or a teacher replaces it)
     length = np.zeros(R, dtype=np.int32)
     status = np.full(R, ACTIVE, dtype=np.uint8)
     sel = -np.ones((G, K), dtype=np.int32)
@@ -101,6 +103,7 @@ def rollout_stepwise(model, prompts, Kp, K, max_new, T, seed, forced_len=None, L
                 router_gap[(r, s)] = gap
             tok, margin = sample_token(z, T, seed, i, j, s)
             otok[r, s], margins[r, s] = tok, margin
+            logprobs[r, s] = token_logprob(z, T, tok)
             if teacher is not None:
                 tok = int(teacher[r][s])
             length[r] = s + 1
@@ -118,7 +121,7 @@ def rollout_stepwise(model, prompts, Kp, K, max_new, T, seed, forced_len=None, L
         s += 1
 
     out = dict(tokens=tokens, len=length, status=status, sel=sel, sel_mask=mask,
-               close_step=close_step, n_steps=s, margins=margins, oracle_tokens=otok,
+               close_step=close_step, n_steps=s, margins=margins, logprobs=logprobs, oracle_tokens=otok,
                logits=logits, router_gap=router_gap, n_active_hist=n_active_hist)
     _tf.ROUTER_GAPS = None
     return _finish(out, G, K, offs)

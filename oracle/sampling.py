@@ -9,10 +9,14 @@ only requires that the M'_i trajectories of a prompt be independent samples
     token = argmax_v y_v           ties -> lowest v
     margin = y_(1) - y_(2)         (top-1 minus top-2; the near-tie measure)
     T == 0  ->  y = z (greedy)
+    logprob = log softmax(z / T)[token]   (T == 0: log softmax(z)[token]) — SURVEY.md 8(a) row 7 "optionally log-prob":
+              the sampling policy's log-probability of the token it drew, written out as its definition
 
 argmax_v (z_v/T + g_v) with i.i.d. standard Gumbel g is an exact sample from
 softmax(z/T) (the Gumbel-max trick) — that closed form is the pin
-(tests/test_oracle_sampling.py, chi-square against softmax).
+(tests/test_oracle_sampling.py, chi-square against softmax).  token_logprob is pinned there against
+scipy.special.log_softmax, the closed forms (uniform logits: -ln V; two logits: log-sigmoid of their difference / T),
+normalisation (sum_v exp = 1) and shift invariance.
 """
 import numpy as np
 
@@ -41,3 +45,12 @@ def sample_token(z, T, seed, i, j, s):
     y = perturbed_logits(z, T, seed, i, j, s)
     v1, y1, y2 = top2(y)
     return v1, float(y1 - y2)
+
+
+def token_logprob(z, T, v):
+    """log softmax(z / T)[v] in fp64 (T == 0: temperature 1), by the definition with the maximum subtracted."""
+    zt = np.asarray(z, dtype=np.float64)
+    if T != 0:
+        zt = zt / T
+    m = np.max(zt)
+    return float(zt[v] - (m + np.log(np.sum(np.exp(zt - m)))))
