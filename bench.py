@@ -356,7 +356,7 @@ def main():
         ach = float(np.sum(attn_bytes)) / (float(np.sum(attn_ms)) * 1e-3) / 1e9 if np.sum(attn_ms) > 0 else 0.0
         R = int(host_in[0]["Kp"].sum())
         h2d = int(host_in[0]["prompts"].nbytes + host_in[0]["forced_len"].nbytes + host_in[0]["Kp"].nbytes)
-        d2h = int(R * max_new * 8 + R * 5 + G * (K * 4 + 4 * 4))
+        d2h = int(R * max_new * 12 + R * 5 + G * (K * 4 + 4 * 4))     # tokens, margins, log-probs; len, status; sel, mask, close step, mean, var
         attn_share = float(np.sum(attn_ms)) * cfg["n_layers"] / max(float(np.sum(dev_ms)), 1e-9)
         rule = {"c3": "K'=16 >= 2K: shortest-only + early stop", "c4": "K' in {8,12,16}: early stop only for K'=16 prompts, dual-end otherwise",
                 "c5": "K'=12 < 2K: dual-end, no early stop"}[name] if args.mode == "auto" else "forced shortest-only + early stop (variant, DESIGN.md R17)"

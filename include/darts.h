@@ -132,6 +132,9 @@ typedef struct {
   uint32_t *sel_mask;                  /* [G] bitset of sel */
   int32_t *close_step;                 /* [G] step index at which the group closed */
   float *len_mean, *len_var;           /* [G] mean / population variance of the pool's lengths (sigma_L^2) */
+  float *logprob;                      /* [n_rows][max_new] log softmax(z / T) of the token the sampler DREW at each step (T == 0: of
+                                        * softmax(z)); where a forced stop replaced the draw by EOS the value is still the draw's.
+                                        * 0 beyond len.  fp32, accumulated per 128-id vocab tile then merged. */
 } darts_results;
 
 typedef struct {
@@ -186,10 +189,13 @@ darts_status darts_run_to_completion(darts_ctx *ctx, darts_results *out);
 /* Token-level streaming hook (§4.3.2 "ship token chunks to the trainer once a threshold accumulates"; rollout side
  * only — the consumer is the caller's).  Same loop as darts_run_to_completion; every chunk_steps lock-step iterations the tokens
  * of steps [step_begin, step_end) are copied to pinned host memory on a second stream (overlapping the following decode steps) and
- * fn(user, step_begin, step_end, n_rows, tokens) is called on the calling thread, in step order, with tokens = HOST
- * [n_rows][step_end - step_begin] row-major (-1 where a row had already stopped; a trailing chunk may hold only -1).  The buffer is
+ * fn(user, step_begin, step_end, n_rows, tokens, logprob) is called on the calling thread, in step order, with tokens = HOST
+ * [n_rows][step_end - step_begin] row-major (-1 where a row had already stopped; a trailing chunk may hold only -1) and logprob the
+ * same shape in fp32 (darts_results.logprob's values: the sampling policy's log-probability of each drawn token, 0 where tokens is
+ * -1) — what the trainer's old-policy pass would otherwise recompute with a teacher-forced forward over the chunk.  The buffers are
  * valid during the call only.  The chunks together cover steps [0, n_steps).  The library owns the two pinned staging buffers. */
-typedef void (*darts_chunk_fn)(void *user, int32_t step_begin, int32_t step_end, int32_t n_rows, const int32_t *tokens_host);
+typedef void (*darts_chunk_fn)(void *user, int32_t step_begin, int32_t step_end, int32_t n_rows, const int32_t *tokens_host,
+                               const float *logprob_host);
 darts_status darts_run_to_completion_streaming(darts_ctx *ctx, int32_t chunk_steps, darts_chunk_fn fn, void *user, darts_results *out);
 
 /* End-to-end convenience with HOST inputs (bench `e2e`): copies prompts / forced_len host->device,

@@ -50,7 +50,7 @@ class Policy(C.Structure):
 
 
 class Results(C.Structure):
-    _fields_ = [(n, _vp) for n in ("tokens", "len", "status", "margin", "sel", "sel_mask", "close_step", "len_mean", "len_var")]
+    _fields_ = [(n, _vp) for n in ("tokens", "len", "status", "margin", "sel", "sel_mask", "close_step", "len_mean", "len_var", "logprob")]
 
 
 class Counters(C.Structure):
@@ -74,7 +74,7 @@ darts_decode_step = _sig("darts_decode_step", _ctx)
 darts_select_and_compact = _sig("darts_select_and_compact", _ctx, _vp)
 darts_rollout = _sig("darts_rollout", _ctx, _vp, _i32, _i32, _i32, _i32, _i32, _f32, _u64, _vp, C.POINTER(Results))
 darts_run_to_completion = _sig("darts_run_to_completion", _ctx, C.POINTER(Results))
-ChunkFn = C.CFUNCTYPE(None, C.c_void_p, _i32, _i32, _i32, C.POINTER(C.c_int32))
+ChunkFn = C.CFUNCTYPE(None, C.c_void_p, _i32, _i32, _i32, C.POINTER(C.c_int32), C.POINTER(C.c_float))
 darts_run_to_completion_streaming = _sig("darts_run_to_completion_streaming", _ctx, _i32, ChunkFn, C.c_void_p, C.POINTER(Results))
 darts_rollout_host = _sig("darts_rollout_host", _ctx, _vp, _i32, _i32, _vp, _vp, C.POINTER(Policy), _i32, _f32, _u64,
                           C.POINTER(Results))
@@ -246,9 +246,9 @@ class Darts:
         self._check(darts_run_to_completion(self.ctx, None))
 
     def run_to_completion_streaming(self, chunk_steps, on_chunk):
-        """on_chunk(step_begin, step_end, tokens) with tokens an int32 numpy array [n_rows, step_end - step_begin] (copied)."""
-        def tramp(_user, s0, s1, n_rows, ptr):
-            on_chunk(s0, s1, np.ctypeslib.as_array(ptr, shape=(n_rows, s1 - s0)).copy())
+        """on_chunk(step_begin, step_end, tokens, logprob): int32 / float32 numpy arrays [n_rows, step_end - step_begin] (copied)."""
+        def tramp(_user, s0, s1, n_rows, ptr, lp):
+            on_chunk(s0, s1, np.ctypeslib.as_array(ptr, shape=(n_rows, s1 - s0)).copy(), np.ctypeslib.as_array(lp, shape=(n_rows, s1 - s0)).copy())
         cb = ChunkFn(tramp)
         self._check(darts_run_to_completion_streaming(self.ctx, chunk_steps, cb, None, None))
 
@@ -278,7 +278,8 @@ class Darts:
         R, G, K, mn = self.R, self.G, self.K, self.max_new
         bufs = dict(tokens=np.empty((R, mn), np.int32), len=np.empty(R, np.int32), status=np.empty(R, np.uint8),
                     margin=np.empty((R, mn), np.float32), sel=np.empty((G, K), np.int32), sel_mask=np.empty(G, np.uint32),
-                    close_step=np.empty(G, np.int32), len_mean=np.empty(G, np.float32), len_var=np.empty(G, np.float32))
+                    close_step=np.empty(G, np.int32), len_mean=np.empty(G, np.float32), len_var=np.empty(G, np.float32),
+                    logprob=np.empty((R, mn), np.float32))
         res = Results(**{k: _np_ptr(v) for k, v in bufs.items()})
         return bufs, res
 

@@ -102,6 +102,7 @@ size_t carve(darts_ctx *c, void *base) {
     size_t F = Fm;
     c->tokens_out = k.take<int32_t>(R * rt.max_new);
     c->margin_out = k.take<float>(R * rt.max_new);
+    c->logprob_out = k.take<float>(R * rt.max_new);
     c->prompt_tokens = k.take<int32_t>(G * rt.max_prompt_len);
     c->slot_cs = k.take<float2>(A * (m.head_dim / 2));
     c->h = k.take<float>(A * m.d_model);
@@ -128,6 +129,7 @@ size_t carve(darts_ctx *c, void *base) {
       c->part_bytes = std::max<size_t>(std::max<size_t>(A * maxN * 4, dec), (size_t)64 << 20);
       c->part = k.take<float>(c->part_bytes / 4);
       c->top2 = k.take<float>((size_t)ceil_div(m.vocab, 128) * R * 4);
+      c->lse = k.take<float>((size_t)ceil_div(m.vocab, 128) * R * 2);
       if (rt.flags & DARTS_FLAG_DUMP_LOGITS) c->logits = k.take<float>(R * m.vocab);
       if (m.n_experts) {
         size_t RK = A * m.top_k;
@@ -348,6 +350,7 @@ darts_status prefill_impl(darts_ctx *c, const int32_t *prompt_tokens_dev, bool t
   CUDA_TRY(c, cudaMemcpyAsync(c->g_prefix_pages, pre_pages.data(), pre_pages.size() * 4, cudaMemcpyHostToDevice, s));
   CUDA_TRY(c, cudaMemsetAsync(c->tokens_out, 0xFF, (size_t)R * c->rt.max_new * 4, s));
   CUDA_TRY(c, cudaMemsetAsync(c->margin_out, 0, (size_t)R * c->rt.max_new * 4, s));
+  CUDA_TRY(c, cudaMemsetAsync(c->logprob_out, 0, (size_t)R * c->rt.max_new * 4, s));
   CUDA_TRY(c, cudaMemsetAsync(c->g_sel, 0xFF, (size_t)G * DARTS_MAX_KP * 4, s));
   TRY(launch_init_rows(c, forced_len_dev, n_prefix_pages));
   // one causal pass per PROMPT, in chunks of whole prompts
@@ -558,6 +561,7 @@ darts_status darts_get_results(darts_ctx *c, darts_results *o) {
   size_t R = c->R, G = c->G, mn = c->rt.max_new;
   if (o->tokens) CUDA_TRY(c, cudaMemcpy(o->tokens, c->tokens_out, R * mn * 4, cudaMemcpyDeviceToHost));
   if (o->margin) CUDA_TRY(c, cudaMemcpy(o->margin, c->margin_out, R * mn * 4, cudaMemcpyDeviceToHost));
+  if (o->logprob) CUDA_TRY(c, cudaMemcpy(o->logprob, c->logprob_out, R * mn * 4, cudaMemcpyDeviceToHost));
   if (o->len) CUDA_TRY(c, cudaMemcpy(o->len, c->row_len, R * 4, cudaMemcpyDeviceToHost));
   if (o->status) CUDA_TRY(c, cudaMemcpy(o->status, c->row_status, R, cudaMemcpyDeviceToHost));
   if (o->sel) CUDA_TRY(c, cudaMemcpy(o->sel, c->g_sel, G * c->pol.K * 4, cudaMemcpyDeviceToHost));
@@ -595,7 +599,7 @@ struct ChunkStream {
   darts_status drain(int b) {
     if (!pending[b]) return DARTS_OK;
     CUDA_TRY(c, cudaEventSynchronize(c->ev_copy_done[b]));
-    fn(user, pend_s0[b], pend_s1[b], c->R, c->chunk_stage[b]);
+    fn(user, pend_s0[b], pend_s1[b], c->R, c->chunk_stage[b], (const float *)(c->chunk_stage[b] + (size_t)c->R * (pend_s1[b] - pend_s0[b])));
     pending[b] = false;
     return DARTS_OK;
   }
@@ -608,6 +612,8 @@ struct ChunkStream {
     CUDA_TRY(c, cudaStreamWaitEvent(c->copy_stream, c->ev_copy_ready[b], 0));
     CUDA_TRY(c, cudaMemcpy2DAsync(c->chunk_stage[b], (size_t)(s1 - s0) * 4, c->tokens_out + s0, (size_t)c->rt.max_new * 4, (size_t)(s1 - s0) * 4,
                                   (size_t)c->R, cudaMemcpyDeviceToHost, c->copy_stream));
+    CUDA_TRY(c, cudaMemcpy2DAsync(c->chunk_stage[b] + (size_t)c->R * (s1 - s0), (size_t)(s1 - s0) * 4, c->logprob_out + s0, (size_t)c->rt.max_new * 4,
+                                  (size_t)(s1 - s0) * 4, (size_t)c->R, cudaMemcpyDeviceToHost, c->copy_stream));   // log-probs behind the tokens
     CUDA_TRY(c, cudaEventRecord(c->ev_copy_done[b], c->copy_stream));
     pend_s0[b] = s0; pend_s1[b] = s1; pending[b] = true;
     flushed = s1;
@@ -654,7 +660,7 @@ darts_status darts_run_to_completion_streaming(darts_ctx *c, int32_t chunk_steps
   if (!c) return DARTS_ERR_INVALID_ARG;
   if (!fn || chunk_steps <= 0) FAIL(c, DARTS_ERR_INVALID_ARG, "chunk_steps must be positive and fn non-NULL");
   if (!c->prefilled) FAIL(c, DARTS_ERR_BAD_STATE, "darts_run_to_completion_streaming before darts_prefill");
-  size_t need = (size_t)c->R * chunk_steps * 4;
+  size_t need = (size_t)c->R * chunk_steps * 8;              // tokens + their log-probabilities
   if (!c->copy_stream) {
     CUDA_TRY(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
     for (int b = 0; b < 2; ++b) {

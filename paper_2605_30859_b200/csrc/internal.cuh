@@ -75,6 +75,7 @@ struct darts_ctx {
   uint8_t *row_status;
   int32_t *tokens_out;
   float *margin_out;
+  float *logprob_out;            // [max_rows][max_new] log softmax(z/T) of the drawn token
   int32_t *g_off, *g_Kp, *g_plen, *g_closed, *g_sel, *g_close_step, *g_prefix_pages, *g_tok_off;
   uint32_t *g_mask;
   float *g_len_mean, *g_len_var;
@@ -94,6 +95,7 @@ struct darts_ctx {
   float *part;                   // [S][rows][N] fp32 partials of the GEMM in flight
   size_t part_bytes;
   float *top2;                   // float4 [vocab tiles][max_rows]
+  float *lse;                    // float2 [vocab tiles][max_rows]
   CUtensorMap *tm_wqkv, *tm_wo, *tm_wgu, *tm_wd, *tm_wgu_e, *tm_wd_e;   // host arrays [n_layers]
   CUtensorMap tm_lm, tm_xn, tm_ao, tm_act, tm_xs, tm_hl;                      // activations: 16-row boxes
   XMaps xm_xn, xm_ao, xm_act, xm_xs;                                            // the same matrices for the stream-K kernel

@@ -34,7 +34,8 @@ struct GemmParams {
   int rows_ub;
   const int32_t *n_rows_dev;      // live row count on the device (nullable)
   // EPI_SAMPLE
-  float4 *top2;                   // [n_tiles][rows] (best y, second y, bits(best index), -)
+  float4 *top2;                   // [n_tiles][rows] (best y, second y, bits(best index), z/T of the best)
+  float2 *lse;                    // [n_tiles][rows] (max, sum e^(z/T - max)) over the tile: log-probability of the drawn token
   float *logits_dump;             // optional [rows][N]
   const int32_t *row_list, *row_prompt, *row_sample, *row_len;
   float temperature;
@@ -145,8 +146,9 @@ __global__ void __launch_bounds__(GEMM_THREADS) gemm_tc_k(const __grid_constant_
           int row = p.row_list[r];
           pi = p.row_prompt[row]; pj = p.row_sample[row]; ps = p.row_len[row];
         }
-        float b1 = -INFINITY, b2 = -INFINITY;
+        float b1 = -INFINITY, b2 = -INFINITY, z1 = 0.f;
         int i1 = 0x7fffffff;
+        float lm = -INFINITY, ls = 0.f;
 #pragma unroll 1
         for (int c = 0; c < BN; c += 32) {
           uint32_t v[32];
@@ -166,18 +168,26 @@ __global__ void __launch_bounds__(GEMM_THREADS) gemm_tc_k(const __grid_constant_
               if (vid < p.N) {
                 uint32_t x[4];
                 if (p.temperature != 0.f) philox4x32_10((uint32_t)(vid >> 2), (uint32_t)ps, (uint32_t)pj, (uint32_t)pi, p.k0, p.k1, x);
+                float zt[4];
 #pragma unroll
                 for (int e = 0; e < 4; ++e) {
                   float z = __uint_as_float(v[j + e]);
-                  float y = p.temperature != 0.f ? z / p.temperature + gumbel_from_bits(x[e]) : z;
-                  if (y > b1) { b2 = b1; b1 = y; i1 = vid + e; }       // ids ascend: strict > keeps the lowest id on ties
+                  zt[e] = p.temperature != 0.f ? z / p.temperature : z;
+                  float y = p.temperature != 0.f ? zt[e] + gumbel_from_bits(x[e]) : z;
+                  if (y > b1) { b2 = b1; b1 = y; i1 = vid + e; z1 = zt[e]; }       // ids ascend: strict > keeps the lowest id on ties
                   else if (y > b2) b2 = y;
                 }
+                float mn = fmaxf(fmaxf(lm, fmaxf(zt[0], zt[1])), fmaxf(zt[2], zt[3]));     // running log-sum-exp of z / T, four at a time
+                ls = ls * __expf(lm - mn) + ((__expf(zt[0] - mn) + __expf(zt[1] - mn)) + (__expf(zt[2] - mn) + __expf(zt[3] - mn)));
+                lm = mn;
               }
             }
           }
         }
-        if (row_ok) p.top2[(size_t)blockIdx.y * p.rows_ub + r] = make_float4(b1, b2, __int_as_float(i1), 0.f);
+        if (row_ok) {
+          p.top2[(size_t)blockIdx.y * p.rows_ub + r] = make_float4(b1, b2, __int_as_float(i1), z1);
+          p.lse[(size_t)blockIdx.y * p.rows_ub + r] = make_float2(lm, ls);
+        }
       }
     }
   }
@@ -254,7 +264,7 @@ darts_status launch_gemm_tc(darts_ctx *c, const TcGemm &g) {
   p.C = g.C; p.split_stride = g.split_stride; p.N = g.N; p.K = g.K; p.S = g.S; p.rows_ub = g.rows_ub; p.n_rows_dev = g.n_rows_dev;
   dim3 grid((g.rows_ub + BM - 1) / BM, (g.N + 127) / 128, g.S);
   if (!g.sample) return launch_cfg<128, 3, EPI_STORE>(c, *g.a_map, *g.b_map, p, grid);
-  p.top2 = (float4 *)c->top2; p.logits_dump = (c->rt.flags & DARTS_FLAG_DUMP_LOGITS) ? c->logits : nullptr;
+  p.top2 = (float4 *)c->top2; p.lse = (float2 *)c->lse; p.logits_dump = (c->rt.flags & DARTS_FLAG_DUMP_LOGITS) ? c->logits : nullptr;
   p.row_list = c->row_list; p.row_prompt = c->row_prompt; p.row_sample = c->row_sample; p.row_len = c->row_len;
   p.temperature = c->temperature; p.k0 = (uint32_t)(c->seed & 0xffffffffu); p.k1 = (uint32_t)(c->seed >> 32);
   return launch_cfg<128, 3, EPI_SAMPLE>(c, *g.a_map, *g.b_map, p, grid);

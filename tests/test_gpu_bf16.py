@@ -3,6 +3,7 @@ teacher-forced (R12): the oracle consumes the GPU's tokens, logits mus
 (north_star), tokens must agree wherever the oracle's margin exceeds twice the measured logit error."""
 import numpy as np
 import pytest
+from oracle.sampling import token_logprob
 
 from oracle import PRUNED, MODE_DUAL_END
 from oracle import rollout as ro
@@ -60,6 +61,11 @@ def test_small_bf16_model_matches_oracle(qk_norm, std, tol):
         if orc["margins"][r, s] > 2 * err + 1e-3:
             forced_here = s + 1 == orc["len"][r] and gpu["tokens"][r, s] == cfg["vocab"] - 1
             assert forced_here or orc["oracle_tokens"][r, s] == gpu["tokens"][r, s], (r, s)
+            # log-probability of the drawn token: |d logprob| <= 2 max|d z| / T
+            assert abs(gpu["logprob"][r, s] - orc["logprobs"][r, s]) <= 2 * err + 1e-3, (r, s)
+            if not forced_here:                             # and tightly against the definition on the GPU's own fp32 logits
+                lp = token_logprob(zg, T, int(gpu["tokens"][r, s]))
+                assert abs(gpu["logprob"][r, s] - lp) < 1e-4 * (1 + abs(lp)), (r, s, gpu["logprob"][r, s], lp)
         else:
             near += 1
     assert near <= len(glog) // 10, (near, len(glog))

@@ -36,6 +36,9 @@ def compare_rollout(gpu, orc, G, K):
                 near += 1
             if orc["margins"][r, s] > MARGIN and forced_or_same:
                 assert abs(gpu["margin"][r, s] - orc["margins"][r, s]) < 1e-3
+            if orc["margins"][r, s] > MARGIN:               # both sides drew the same token (a forced EOS replaces it afterwards)
+                assert abs(gpu["logprob"][r, s] - orc["logprobs"][r, s]) < 2e-4, (r, s, gpu["logprob"][r, s], orc["logprobs"][r, s])
+        assert np.all(gpu["logprob"][r, orc["len"][r]:] == 0.0)
     return near
 
 

@@ -7,7 +7,7 @@ import numpy as np
 import pytest
 
 from oracle import transformer as otf
-from oracle.sampling import sample_token
+from oracle.sampling import sample_token, token_logprob
 from paper_2605_30859_b200 import workloads as wl
 from tests.gpu_util import rel_inf
 
@@ -66,6 +66,9 @@ def _case(name, prompts_sampled, P=None, steps=3, gap_tol=0.0):
             err = float(np.max(np.abs(zg - z))) / T
             if margin > 2 * err + 1e-3:
                 assert tok == gpu["tokens"][r, s], (r, s, margin, err)
+                assert abs(gpu["logprob"][r, s] - token_logprob(z, T, tok)) <= 2 * err + 1e-3, (r, s)
+                lp = token_logprob(zg, T, tok)               # the fused log-sum-exp against the definition on the GPU's own logits
+                assert abs(gpu["logprob"][r, s] - lp) < 1e-4 * (1 + abs(lp)), (r, s, gpu["logprob"][r, s], lp)
             else:
                 near += 1
     otf.ROUTER_GAPS = None

@@ -1,5 +1,6 @@
 """-m gpu: token-level streaming hook (rollout side): the chunks delivered while the rollout runs
-reassemble to exactly the tokens of the finished rollout, cover steps [0, n_steps) in order, and the result equals the plain loop's."""
+reassemble to exactly the tokens (and their log-probabilities) of the finished rollout, cover steps [0, n_steps) in order, and the
+result equals the plain loop's."""
 import numpy as np
 import pytest
 
@@ -18,14 +19,17 @@ def test_chunks_reassemble_to_the_rollout(chunk):
     n_steps = d.counters()["n_steps"]
     got = []
     d.prefill(list(x["prompts"]), x["Kp"], x["K"], temperature=1.0, seed=3, forced_len=x["forced_len"])
-    d.run_to_completion_streaming(chunk, lambda s0, s1, t: got.append((s0, s1, t)))
+    d.run_to_completion_streaming(chunk, lambda s0, s1, t, lp: got.append((s0, s1, t, lp)))
     res = d.results()
-    for k in ("tokens", "len", "status", "sel"):
+    for k in ("tokens", "len", "status", "sel", "logprob"):
         assert np.array_equal(res[k], ref[k]), k
     assert got[0][0] == 0 and all(a[1] == b[0] for a, b in zip(got, got[1:]))          # contiguous, in step order
-    assert all(0 < s1 - s0 <= chunk and t.shape == (32, s1 - s0) for s0, s1, t in got)
+    assert all(0 < s1 - s0 <= chunk and t.shape == (32, s1 - s0) and lp.shape == t.shape for s0, s1, t, lp in got)
     assert got[-1][1] >= n_steps
-    stream = np.concatenate([t for _, _, t in got], axis=1)
+    stream = np.concatenate([g[2] for g in got], axis=1)
+    stream_lp = np.concatenate([g[3] for g in got], axis=1)
     assert np.array_equal(stream[:, :n_steps], ref["tokens"][:, :n_steps])
     assert np.all(stream[:, n_steps:] == -1)
+    assert np.array_equal(stream_lp[:, :n_steps], ref["logprob"][:, :n_steps])        # bitwise: same kernels, same order
+    assert np.all(stream_lp[stream < 0] == 0.0) and np.all(stream_lp <= 0.0)
     d.close()
