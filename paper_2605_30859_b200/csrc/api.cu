@@ -128,8 +128,8 @@ size_t carve(darts_ctx *c, void *base) {
         }
       c->part_bytes = std::max<size_t>(std::max<size_t>(A * maxN * 4, dec), (size_t)64 << 20);
       c->part = k.take<float>(c->part_bytes / 4);
-      c->top2 = k.take<float>((size_t)ceil_div(m.vocab, 128) * R * 4);
-      c->lse = k.take<float>((size_t)ceil_div(m.vocab, 128) * R * 2);
+      c->top2 = k.take<float>((size_t)4 * ceil_div(m.vocab, 128) * R * 4);    // one entry per (vocab tile, warp quadrant, row)
+      c->lse = k.take<float>((size_t)4 * ceil_div(m.vocab, 128) * R * 2);
       if (rt.flags & DARTS_FLAG_DUMP_LOGITS) c->logits = k.take<float>(R * m.vocab);
       if (m.n_experts) {
         size_t RK = A * m.top_k;
@@ -442,6 +442,7 @@ darts_status darts_create(const darts_model_desc *m, const darts_weights *w, con
   if (((uintptr_t)rt->workspace & 255) != 0) FAIL(c, DARTS_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
   c->has_weights = m->vocab > 0;
   c->use_pdl = getenv("DARTS_NO_PDL") == nullptr;
+  c->lm_sk_max_rows = getenv("DARTS_LM_SK_MAX_ROWS") ? atoi(getenv("DARTS_LM_SK_MAX_ROWS")) : (1 << 30);
   c->skip_mask = getenv("DARTS_SKIP") ? (unsigned)strtoul(getenv("DARTS_SKIP"), nullptr, 0) : 0u;
   if (c->has_weights) {
     int L = m->n_layers;
@@ -515,8 +516,14 @@ darts_status darts_decode_step(darts_ctx *c) {
   struct Leave { darts_ctx *c; ~Leave() { c->in_decode = false; } } leave{c};
   if (c->tc_path) {
     TRY(forward_layers_tc(c, ub, n));
-    TRY(lm_head_tc(c, &c->tm_xn, nullptr, ub, n, true));                          // logits never reach HBM (unless DUMP_LOGITS)
-    TRY(launch_sample_finalize(c, ceil_div(c->m.vocab, 128), ub));
+    // logits never reach HBM (unless DUMP_LOGITS): swap-AB persistent kernel with the sampling epilogue, 4 entries per vocab tile
+    if (ub <= c->lm_sk_max_rows && sk_sample_supported(c, ub)) {
+      TRY(launch_gemm_sk_sample(c, &c->tm_lm, &c->xm_xn, c->m.vocab, c->m.d_model, ub, n));
+      TRY(launch_sample_finalize(c, 4 * ceil_div(c->m.vocab, 128), ub));
+    } else {
+      TRY(lm_head_tc(c, &c->tm_xn, nullptr, ub, n, true));
+      TRY(launch_sample_finalize(c, ceil_div(c->m.vocab, 128), ub));
+    }
   } else {
     TRY(forward_layers(c, ub, n));
     TRY(launch_rmsnorm(c, c->h, c->final_norm, c->xn, ub, n));

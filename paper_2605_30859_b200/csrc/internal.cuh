@@ -91,6 +91,8 @@ struct darts_ctx {
   // tensor-core path (bf16, kernels_gemm_tc.cu): split-K partial buffer, LM-head top-2 partials, tensor maps
   bool tc_path;                  // every GEMM of this model runs on tcgen05
   unsigned skip_mask;            // profiling aid (env DARTS_SKIP, bit per kernel class of a layer): skipped launches leave stale data — timing only
+  int lm_sk_max_rows;            // decode LM head: swap-AB persistent kernel up to this many rows (host bound), 128x128 tile kernel above
+                                 // (default: always; DARTS_LM_SK_MAX_ROWS=0 in the environment selects the tile kernel, an A/B aid)
   bool use_pdl;                  // launch the stream-K GEMMs as programmatic dependents (DARTS_NO_PDL=1 in the environment disables)
   float *part;                   // [S][rows][N] fp32 partials of the GEMM in flight
   size_t part_bytes;
@@ -265,6 +267,8 @@ __host__ __device__ __forceinline__ int sk_npieces(const SkView &v, int n_rb, in
 SkPlan sk_plan(int n_sms, int N, int K, int rows_ub, int n_rb_ub_grouped, bool rows_exact);
 darts_status launch_gemm_sk(darts_ctx *c, const SkGemm &g);
 darts_status launch_sk_reduce(darts_ctx *c, const SkView &v, float *out, int rows);
+bool sk_sample_supported(const darts_ctx *c, int rows_ub);
+darts_status launch_gemm_sk_sample(darts_ctx *c, const CUtensorMap *w_map, const XMaps *x_maps, int N, int K, int rows_ub, const int32_t *n_rows_dev);
 inline SkView sk_view(const SkGemm &g) { return SkView{g.C, g.slot_stride, g.N, g.plan.nkb, g.plan.n_wtiles, g.plan.P, g.plan.unit_tile}; }
 darts_status launch_add_rmsnorm_sk(darts_ctx *c, const SkView &v, const void *w, int rows_ub, const int32_t *n_rows_dev);
 darts_status launch_silu_mul_sk(darts_ctx *c, const SkView &v, int rows_ub, const int32_t *n_rows_dev);

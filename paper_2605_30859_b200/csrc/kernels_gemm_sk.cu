@@ -17,9 +17,14 @@
 // Warp roles: warp 0 TMA producer, warp 1 MMA issuer (+ TMEM alloc), warps 2-5 epilogue (TMEM lane = weight row,
 // column = activation row; a warp's 32 lanes store 32 consecutive output columns of one row: coalesced 128 B).
 // Grouped mode (MoE): row blocks come from a device list {row0, nrows, weight row base}, units are whole tiles.
+// Sampling mode (EPI_SAMPLE, the LM head of a decode step): whole (vocab tile, 256-row block) units; the
+// epilogue never stores the logits: each warp transposes its 32 ids x 32 rows blocks through shared memory so that a thread owns a
+// row, perturbs that row's 32 logits (z / T + Gumbel from Philox keyed by the row), keeps best / second / argbest and the
+// log-sum-exp of z / T in registers, and leaves one entry per (tile, warp quadrant, row) for sample_finalize_k to merge.
 #include <algorithm>
 
 #include "internal.cuh"
+#include "philox.cuh"
 #include "sm100_ptx.cuh"
 
 namespace {
@@ -44,6 +49,21 @@ struct SkParams {
   int stage_bytes, n_stages, tm_cols;            // tm_cols: columns of ONE accumulator (power of two >= 32)
   int n_acc;                                     // TMEM accumulators: 2 (epilogue overlaps the next piece) | 1 (one 512-column accumulator)
 };
+
+struct SkSampleArgs {
+  float4 *top2;                                  // [4 * n_wtiles][rows_ub] (best y, second y, bits(argbest), z/T of the best)
+  float2 *lse;                                   // [4 * n_wtiles][rows_ub] (max, sum e^(z/T - max))
+  float *logits_dump;                            // [rows][N] or NULL
+  const int32_t *row_list, *row_prompt, *row_sample, *row_len;
+  float temperature;
+  uint32_t k0, k1;
+};
+enum { SK_EPI_PIECES = 0, SK_EPI_SAMPLE = 1 };
+constexpr int SK_TILE_OFF = 512;                 // behind the barriers: 32 x 33 fp32 transpose tiles, one per epilogue warp
+constexpr int SK_SAMPLE_EPI_WARPS = 8;           // two per TMEM lane quadrant (alternate 32-column chunks): one warp per scheduler cannot hide its own latencies
+constexpr int SK_TILE_BYTES = SK_SAMPLE_EPI_WARPS * 32 * 33 * 4;
+constexpr int SK_SAMPLE_RING = 184 * 1024;       // the ring gives 16 KB to the tiles
+constexpr int SK_SAMPLE_THREADS = 64 + SK_SAMPLE_EPI_WARPS * 32;
 
 struct SkBars {
   unsigned long long full[MAX_STAGES], empty[MAX_STAGES], acc_full[2], acc_empty[2];
@@ -74,11 +94,13 @@ struct PieceIter {
   }
 };
 
-__global__ void __launch_bounds__(SK_THREADS, 1) gemm_sk_k(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ XMaps tmX,
-                                                           SkParams p) {
+template <int EPI>
+__global__ void __launch_bounds__(EPI == SK_EPI_SAMPLE ? SK_SAMPLE_THREADS : SK_THREADS, 1) gemm_sk_k(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ XMaps tmX,
+                                                           SkParams p, SkSampleArgs sa) {
   extern __shared__ unsigned char smem_raw[];
   unsigned char *stage_base = reinterpret_cast<unsigned char *>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
-  SkBars &bar = *reinterpret_cast<SkBars *>(stage_base + SMEM_BUDGET);
+  constexpr int RING = EPI == SK_EPI_SAMPLE ? SK_SAMPLE_RING : SMEM_BUDGET;
+  SkBars &bar = *reinterpret_cast<SkBars *>(stage_base + RING);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
   pdl_trigger();
@@ -89,11 +111,11 @@ __global__ void __launch_bounds__(SK_THREADS, 1) gemm_sk_k(const __grid_constant
   else {
     // dense: block size, ring depth and TMEM split follow the LIVE row count (device value), not the host's bound
     it0.live = p.n_rows_dev ? min(*p.n_rows_dev, p.rows_ub) : p.rows_ub;
-    it0.rb_rows = sk_rb_rows(it0.live);
+    it0.rb_rows = EPI == SK_EPI_SAMPLE ? SK_ROWBLOCK : sk_rb_rows(it0.live);   // sampling needs both accumulators (epilogue overlap)
     it0.n_rb = (it0.live + it0.rb_rows - 1) / it0.rb_rows;
     const int cap = (min(it0.rb_rows, it0.live) + 15) & ~15;
     p.stage_bytes = W_STAGE_BYTES + cap / BOX_ROWS * BOX_BYTES;
-    p.n_stages = min(MAX_STAGES, SMEM_BUDGET / p.stage_bytes);
+    p.n_stages = min(MAX_STAGES, RING / p.stage_bytes);
     p.tm_cols = 32;
     while (p.tm_cols < cap) p.tm_cols *= 2;
     p.n_acc = p.tm_cols > 256 ? 1 : 2;
@@ -108,7 +130,7 @@ __global__ void __launch_bounds__(SK_THREADS, 1) gemm_sk_k(const __grid_constant
     prefetch_tmap(&tmW);
     for (int b = 0; b < 5; ++b) prefetch_tmap(&tmX.m[b]);
     for (int s = 0; s < p.n_stages; ++s) { mbar_init(&bar.full[s], 1); mbar_init(&bar.empty[s], 1); }
-    for (int b = 0; b < 2; ++b) { mbar_init(&bar.acc_full[b], 1); mbar_init(&bar.acc_empty[b], 4); }
+    for (int b = 0; b < 2; ++b) { mbar_init(&bar.acc_full[b], 1); mbar_init(&bar.acc_empty[b], EPI == SK_EPI_SAMPLE ? SK_SAMPLE_EPI_WARPS : 4); }
     fence_mbar_init();
   }
   if (warp == 1) tmem_alloc(&bar.tmem_base, p.n_acc * p.tm_cols);
@@ -206,39 +228,111 @@ __global__ void __launch_bounds__(SK_THREADS, 1) gemm_sk_k(const __grid_constant
   } else {
     // ------------------------------------------------------------------------------------------ epilogue
     const int q = warp & 3;                                // TMEM lane quadrant this warp may read
-    PieceIter it = it0;
-    Piece pc;
-    int piece = 0;
-    while (it.next(pc)) {
-      const int buf = piece % p.n_acc, use = piece / p.n_acc;
-      mbar_wait(&bar.acc_full[buf], use & 1);
-      tc_fence_after();
-      const int n = pc.wtile * BMW + q * 32 + lane;        // output column = weight row
-      const bool n_ok = n < p.N;
-      float *dst = p.C + (size_t)pc.slot * p.slot_stride + (size_t)pc.row0 * p.N + n;
-      const uint32_t src = tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)(buf * p.tm_cols);
-      const size_t ldc = (size_t)p.N;
+    if constexpr (EPI == SK_EPI_SAMPLE) {
+      // A TMEM lane is a vocabulary id and a column an activation row; sampling wants the opposite (one thread walking the ids of ONE
+      // row: Philox block shared by 4 consecutive ids, running top-2 and log-sum-exp in registers, no warp-wide step).  Each 32 x 32
+      // (id x row) block is therefore transposed through a padded shared-memory tile private to the warp.
+      const int half = (warp - 2) >> 2;                    // the two warps of a quadrant take alternate 32-column chunks
+      float *tile = reinterpret_cast<float *>(stage_base + RING + SK_TILE_OFF) + (half * 4 + q) * (32 * 33);
+      pdl_wait();
+      const float T = sa.temperature;
+      PieceIter it = it0;
+      Piece pc;
+      int piece = 0;
+      while (it.next(pc)) {
+        const int buf = piece % p.n_acc, use = piece / p.n_acc;
+        mbar_wait(&bar.acc_full[buf], use & 1);
+        tc_fence_after();
+        const int nb = pc.wtile * BMW + q * 32;              // first vocabulary id of this warp (multiple of 32)
+        const uint32_t src = tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)(buf * p.tm_cols);
+        const size_t ent = (size_t)(pc.wtile * 4 + q) * p.rows_ub + pc.row0;
 #pragma unroll 1
-      for (int c = 0; c < pc.nrows; c += 32) {
-        uint32_t v[32];
-        tmem_ld32(src + c, v);
-        tmem_ld_wait();
-        if (n_ok) {
-          float *q = dst + (size_t)c * ldc;                // one pointer bump per store, no per-element predicate on full chunks
-          if (c + 32 <= pc.nrows) {
+        for (int c = half * 32; c < pc.nrows; c += 32 * (SK_SAMPLE_EPI_WARPS / 4)) {
+          uint32_t v[32];
+          tmem_ld32(src + c, v);
+          tmem_ld_wait();
+          if (sa.logits_dump && nb + lane < p.N) {
 #pragma unroll
-            for (int j = 0; j < 32; ++j, q += ldc) *q = __uint_as_float(v[j]);
-          } else {
+            for (int j = 0; j < 32; ++j)
+              if (c + j < pc.nrows) sa.logits_dump[(size_t)(pc.row0 + c + j) * p.N + nb + lane] = __uint_as_float(v[j]);
+          }
 #pragma unroll
-            for (int j = 0; j < 32; ++j, q += ldc)
-              if (c + j < pc.nrows) *q = __uint_as_float(v[j]);
+          for (int j = 0; j < 32; ++j) tile[lane * 33 + j] = __uint_as_float(v[j]);       // bank (lane + j) % 32: conflict-free
+          __syncwarp();
+          const bool row_ok = c + lane < pc.nrows;
+          int pi = 0, pj = 0, ps = 0;
+          if (row_ok) {
+            const int row = sa.row_list[pc.row0 + c + lane];
+            pi = sa.row_prompt[row]; pj = sa.row_sample[row]; ps = sa.row_len[row];
+          }
+          float b1 = -INFINITY, b2 = -INFINITY, z1 = 0.f, lm = -INFINITY, ls = 0.f;
+          int i1 = 0x7fffffff;
+#pragma unroll
+          for (int k = 0; k < 32; k += 4) {
+            const int vid = nb + k;                          // multiple of 4: one Philox block serves 4 vocabulary ids
+            if (vid < p.N) {                                 // warp-uniform (N % 4 == 0)
+              uint32_t x[4];
+              if (T != 0.f) philox4x32_10((uint32_t)(vid >> 2), (uint32_t)ps, (uint32_t)pj, (uint32_t)pi, sa.k0, sa.k1, x);
+              float zt[4];
+#pragma unroll
+              for (int e = 0; e < 4; ++e) {
+                const float z = tile[(k + e) * 33 + lane];   // consecutive lanes, consecutive words
+                zt[e] = T != 0.f ? z / T : z;
+                const float y = T != 0.f ? zt[e] + gumbel_from_bits(x[e]) : z;
+                if (y > b1) { b2 = b1; b1 = y; i1 = vid + e; z1 = zt[e]; }          // ids ascend: strict > keeps the lowest id on ties
+                else if (y > b2) b2 = y;
+              }
+              const float mn = fmaxf(fmaxf(lm, fmaxf(zt[0], zt[1])), fmaxf(zt[2], zt[3]));
+              ls = ls * __expf(lm - mn) + ((__expf(zt[0] - mn) + __expf(zt[1] - mn)) + (__expf(zt[2] - mn) + __expf(zt[3] - mn)));
+              lm = mn;
+            }
+          }
+          __syncwarp();                                      // the tile is rewritten by the next chunk
+          if (row_ok) {
+            sa.top2[ent + c + lane] = make_float4(b1, b2, __int_as_float(i1), z1);
+            sa.lse[ent + c + lane] = make_float2(lm, ls);
           }
         }
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&bar.acc_empty[buf]);
+        ++piece;
       }
-      tc_fence_before();
-      __syncwarp();
-      if (lane == 0) mbar_arrive(&bar.acc_empty[buf]);
-      ++piece;
+    } else {
+      PieceIter it = it0;
+      Piece pc;
+      int piece = 0;
+      while (it.next(pc)) {
+        const int buf = piece % p.n_acc, use = piece / p.n_acc;
+        mbar_wait(&bar.acc_full[buf], use & 1);
+        tc_fence_after();
+        const int n = pc.wtile * BMW + q * 32 + lane;        // output column = weight row
+        const bool n_ok = n < p.N;
+        float *dst = p.C + (size_t)pc.slot * p.slot_stride + (size_t)pc.row0 * p.N + n;
+        const uint32_t src = tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)(buf * p.tm_cols);
+        const size_t ldc = (size_t)p.N;
+#pragma unroll 1
+        for (int c = 0; c < pc.nrows; c += 32) {
+          uint32_t v[32];
+          tmem_ld32(src + c, v);
+          tmem_ld_wait();
+          if (n_ok) {
+            float *q = dst + (size_t)c * ldc;                // one pointer bump per store, no per-element predicate on full chunks
+            if (c + 32 <= pc.nrows) {
+#pragma unroll
+              for (int j = 0; j < 32; ++j, q += ldc) *q = __uint_as_float(v[j]);
+            } else {
+#pragma unroll
+              for (int j = 0; j < 32; ++j, q += ldc)
+                if (c + j < pc.nrows) *q = __uint_as_float(v[j]);
+            }
+          }
+        }
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&bar.acc_empty[buf]);
+        ++piece;
+      }
     }
   }
   tc_fence_before();
@@ -302,14 +396,44 @@ darts_status launch_gemm_sk(darts_ctx *c, const SkGemm &g) {
   size_t smem = SMEM_BUDGET + sizeof(SkBars) + 1024;
   static bool attr = false;
   if (!attr) {
-    CUDA_TRY(c, cudaFuncSetAttribute(gemm_sk_k, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET + (int)sizeof(SkBars) + 2048));
+    CUDA_TRY(c, cudaFuncSetAttribute(gemm_sk_k<SK_EPI_PIECES>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET + (int)sizeof(SkBars) + 2048));
     attr = true;
   }
-  launch_pdl(c, gemm_sk_k, dim3(pl.P), dim3(SK_THREADS), smem, *g.w_map, *g.x_maps, p);
+  launch_pdl(c, gemm_sk_k<SK_EPI_PIECES>, dim3(pl.P), dim3(SK_THREADS), smem, *g.w_map, *g.x_maps, p, SkSampleArgs{});
   c->launches++;
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) {
     snprintf(c->err, sizeof(c->err), "launch gemm_sk: %s", cudaGetErrorString(e));
+    c->sticky = DARTS_ERR_CUDA;
+    return DARTS_ERR_CUDA;
+  }
+  return DARTS_OK;
+}
+
+// LM head of a decode step with the sampling epilogue (whole tiles, 256-row blocks); sample_finalize_k merges 4 entries per vocab tile.
+bool sk_sample_supported(const darts_ctx *c, int rows_ub) { return rows_ub > 0 && c->m.d_model % BK == 0 && c->m.vocab % 4 == 0; }
+
+darts_status launch_gemm_sk_sample(darts_ctx *c, const CUtensorMap *w_map, const XMaps *x_maps, int N, int K, int rows_ub, const int32_t *n_rows_dev) {
+  if (rows_ub <= 0) return DARTS_OK;
+  static_assert(sizeof(SkBars) <= SK_TILE_OFF, "transpose tiles overlap the barriers");
+  SkParams p{};
+  p.N = N; p.nkb = K / BK; p.n_wtiles = (N + BMW - 1) / BMW; p.rows_ub = rows_ub; p.n_rows_dev = n_rows_dev; p.unit_tile = 1;
+  SkSampleArgs sa{};
+  sa.top2 = (float4 *)c->top2; sa.lse = (float2 *)c->lse; sa.logits_dump = (c->rt.flags & DARTS_FLAG_DUMP_LOGITS) ? c->logits : nullptr;
+  sa.row_list = c->row_list; sa.row_prompt = c->row_prompt; sa.row_sample = c->row_sample; sa.row_len = c->row_len;
+  sa.temperature = c->temperature; sa.k0 = (uint32_t)(c->seed & 0xffffffffu); sa.k1 = (uint32_t)(c->seed >> 32);
+  const int smem = SK_SAMPLE_RING + SK_TILE_OFF + SK_TILE_BYTES + 1024;
+  static bool attr = false;
+  if (!attr) {
+    CUDA_TRY(c, cudaFuncSetAttribute(gemm_sk_k<SK_EPI_SAMPLE>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    attr = true;
+  }
+  const int n_sms = c->n_sms > 0 ? c->n_sms : 148;
+  launch_pdl(c, gemm_sk_k<SK_EPI_SAMPLE>, dim3(std::min(n_sms, p.n_wtiles)), dim3(SK_SAMPLE_THREADS), (size_t)smem, *w_map, *x_maps, p, sa);
+  c->launches++;
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) {
+    snprintf(c->err, sizeof(c->err), "launch gemm_sk (sampling): %s", cudaGetErrorString(e));
     c->sticky = DARTS_ERR_CUDA;
     return DARTS_ERR_CUDA;
   }
