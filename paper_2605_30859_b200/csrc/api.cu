@@ -234,10 +234,8 @@ SkGemm sk_gemm(darts_ctx *c, const XMaps *x, const CUtensorMap *w, int N, int K,
 darts_status forward_layers_tc(darts_ctx *c, int rows_ub, const int32_t *n_rows_dev) {
   const darts_model_desc &m = c->m;
   const int d = m.d_model, qd = m.n_q_heads * m.head_dim, F = m.ffn, L = m.n_layers;
-  TRY(launch_embed(c, c->slot_tok, 0, rows_ub, n_rows_dev));
-  TRY(launch_rope_table(c, rows_ub, n_rows_dev));
   TRY(launch_moe_begin_pass(c));
-  TRY(launch_rmsnorm(c, c->h, c->attn_norm[0], c->xn, rows_ub, n_rows_dev));
+  TRY(launch_embed_norm_rope(c, c->slot_tok, c->attn_norm[0], rows_ub, n_rows_dev));     // embedding, first RMSNorm, RoPE table: one launch
   // DARTS_SKIP (profiling aid): bit k drops the k-th kernel class of every layer so that the change of the step time gives that class's
   // LIVE cost (launch-list times are serialised and cold); results are garbage in that mode.
   const unsigned sk = c->skip_mask;

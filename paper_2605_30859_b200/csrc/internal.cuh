@@ -198,6 +198,7 @@ __device__ __forceinline__ float warp_max(float v) {
 // ---- launchers implemented across the .cu files (all asynchronous on ctx->stream) ----------------
 // n_rows_dev: device pointer to the live row count (kernels ignore slots >= *n_rows_dev); rows_ub: host upper bound.
 darts_status launch_embed(darts_ctx *c, const int32_t *tok_of_slot_src, int mode, int rows_ub, const int32_t *n_rows_dev);
+darts_status launch_embed_norm_rope(darts_ctx *c, const int32_t *slot_tok, const void *w, int rows_ub, const int32_t *n_rows_dev);
 darts_status launch_rmsnorm(darts_ctx *c, const float *h, const void *w, void *out, int rows_ub, const int32_t *n_rows_dev);
 darts_status launch_gemm(darts_ctx *c, const void *X, const void *W, float *C, int N, int K, int rows_ub,
                          const int32_t *n_rows_dev, bool accumulate, bool w_is_f32 = false);

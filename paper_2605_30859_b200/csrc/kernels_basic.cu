@@ -67,6 +67,49 @@ darts_status launch_rmsnorm(darts_ctx *c, const float *h, const void *w, void *o
   return post_launch(c, "rmsnorm");
 }
 
+// ---------------------------------------------------------------- embed + first RMSNorm + RoPE table in one launch (tensor-core path)
+// Same arithmetic as embed_k, rmsnorm_k and rope_table_k one after the other (same thread -> element mapping, same reduction
+// order); three step-boundary launches become one.
+template <typename T>
+__global__ void __launch_bounds__(256) embed_norm_rope_k(const T *__restrict__ E, const int32_t *__restrict__ slot_tok, float *__restrict__ h,
+                                                         const T *__restrict__ w, T *__restrict__ out, int d, float eps,
+                                                         const int32_t *__restrict__ slot_pos, float2 *__restrict__ cs, int half, double theta,
+                                                         const int32_t *n_rows_dev, int rows_ub) {
+  pdl_trigger();
+  int slot = blockIdx.x;
+  if (slot >= live_rows(n_rows_dev, rows_ub)) return;
+  const T *src = E + (size_t)slot_tok[slot] * d;
+  float *x = h + (size_t)slot * d;
+  float ss = 0.f;
+  for (int k = threadIdx.x; k < d; k += blockDim.x) { float v = to_f<T>(src[k]); x[k] = v; ss += v * v; }
+  __shared__ float red[32];
+  ss = warp_sum(ss);
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = ss;
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    float v = threadIdx.x < (blockDim.x >> 5) ? red[threadIdx.x] : 0.f;
+    v = warp_sum(v);
+    if (threadIdx.x == 0) red[0] = v;
+  }
+  __syncthreads();
+  float r = 1.0f / sqrtf(red[0] / d + eps);
+  for (int k = threadIdx.x; k < d; k += blockDim.x) out[(size_t)slot * d + k] = from_f<T>(to_f<T>(src[k]) * r * to_f<T>(w[k]));
+  for (int p = threadIdx.x; p < half; p += blockDim.x) {
+    double inv_freq = pow(theta, -(double)p / (double)half);
+    double s, co;
+    sincos((double)slot_pos[slot] * inv_freq, &s, &co);
+    cs[(size_t)slot * half + p] = make_float2((float)co, (float)s);
+  }
+}
+
+darts_status launch_embed_norm_rope(darts_ctx *c, const int32_t *slot_tok, const void *w, int rows_ub, const int32_t *n_rows_dev) {
+  if (rows_ub <= 0) return DARTS_OK;
+  DISPATCH_T(c, embed_norm_rope_k<T><<<rows_ub, 256, 0, c->stream>>>((const T *)c->embed, slot_tok, c->h, (const T *)w, (T *)c->xn, c->m.d_model,
+                                                                     c->m.rms_eps, c->slot_pos, c->slot_cs, c->m.head_dim / 2,
+                                                                     (double)c->m.rope_theta, n_rows_dev, rows_ub));
+  return post_launch(c, "embed_norm_rope");
+}
+
 // ---------------------------------------------------------------- SiLU(gate) * up
 template <typename T>
 __global__ void silu_mul_k(const float *__restrict__ gu, T *__restrict__ act, int F, const int32_t *n_rows_dev, int rows_ub) {

@@ -119,7 +119,7 @@ __global__ void __launch_bounds__(256) sample_k(DevState *st, const float *__res
 
 // LM-head tensor-core path: the GEMM epilogue left one (best, second, argbest) per (vocab tile, slot); merge the tiles
 // (max with lowest-id tie-break is order-independent) and apply the stop rules.
-__global__ void __launch_bounds__(128) sample_finalize_k(DevState *st, const float4 *__restrict__ top2, const float2 *__restrict__ lse,
+__global__ void __launch_bounds__(512) sample_finalize_k(DevState *st, const float4 *__restrict__ top2, const float2 *__restrict__ lse,
                                                          int n_tiles, int rows_ub,
                                                          const int32_t *__restrict__ row_list, int32_t *row_len, uint8_t *row_status,
                                                          const int32_t *__restrict__ row_forced, int32_t *row_last_tok, int32_t *row_slot,
@@ -131,9 +131,10 @@ __global__ void __launch_bounds__(128) sample_finalize_k(DevState *st, const flo
   int s = row_len[row];
   Top2 t{-INFINITY, -INFINITY, 0x7fffffff, 0.f};
   Lse l{-INFINITY, 0.f};
-  for (int k = threadIdx.x; k < n_tiles; k += blockDim.x) {
-    float4 v = top2[(size_t)k * rows_ub + slot];
-    float2 w = lse[(size_t)k * rows_ub + slot];
+#pragma unroll 4
+  for (int k = threadIdx.x; k < n_tiles; k += blockDim.x) {      // independent loads: unrolled so several are in flight per thread
+    float4 v = __ldcs(&top2[(size_t)k * rows_ub + slot]);
+    float2 w = __ldcs(&lse[(size_t)k * rows_ub + slot]);
     Top2 u{v.x, v.y, __float_as_int(v.z), v.w};
     t = top2_merge(t, u);
     l = lse_merge(l, Lse{w.x, w.y});
@@ -149,8 +150,8 @@ __global__ void __launch_bounds__(128) sample_finalize_k(DevState *st, const flo
     Lse lu{__shfl_xor_sync(0xffffffffu, l.m, o), __shfl_xor_sync(0xffffffffu, l.s, o)};
     l = lse_merge(l, lu);
   }
-  __shared__ Top2 red[4];
-  __shared__ Lse redl[4];
+  __shared__ Top2 red[16];
+  __shared__ Lse redl[16];
   if ((threadIdx.x & 31) == 0) { red[threadIdx.x >> 5] = t; redl[threadIdx.x >> 5] = l; }
   __syncthreads();
   if (threadIdx.x == 0) {
@@ -180,7 +181,7 @@ darts_status launch_sample(darts_ctx *c, const float *logits, int step0, int row
 
 darts_status launch_sample_finalize(darts_ctx *c, int n_tiles, int rows_ub) {
   if (rows_ub <= 0) return DARTS_OK;
-  sample_finalize_k<<<rows_ub, 128, 0, c->stream>>>(c->st, (const float4 *)c->top2, (const float2 *)c->lse, n_tiles, rows_ub, c->row_list, c->row_len,
+  sample_finalize_k<<<rows_ub, 512, 0, c->stream>>>(c->st, (const float4 *)c->top2, (const float2 *)c->lse, n_tiles, rows_ub, c->row_list, c->row_len,
                                                     c->row_status, c->row_forced, c->row_last_tok, c->row_slot, c->row_slot_step, c->tokens_out,
                                                     c->margin_out, c->logprob_out, c->rt.max_new, c->max_len, c->m.eos_id);
   c->launches++;
