@@ -34,6 +34,8 @@
  *   DARTS_SKIP=<bitmask>     profiling aid: drop one kernel class of every layer (results are garbage; see
  *                            profiles/r1_live_cost_by_kernel.md).  Never set it outside a timing experiment.
  *   DARTS_ADDNORM_REG_MAX=n  row bound under which the register-resident add + RMSNorm kernel is used (default 128)
+ *   DARTS_LM_SK_MAX_ROWS=n   decode LM head: persistent swap-AB kernel up to n rows, 128 x 128 tile kernel above (default: always the
+ *                            former; 0 selects the tile kernel — an A/B aid, both sample the same distribution from the same Philox stream)
  *
  * Layouts
  *   - Projections are [out_features, in_features] row-major in the model dtype (F32 or BF16).
