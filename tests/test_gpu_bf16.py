@@ -38,10 +38,12 @@ def run_stepwise(d, prompts, Kp, K, T, seed, forced, **kw):
 
 # std 0.02 is the configs' init recipe (tolerance: north_star's 2e-2).  std 0.08 is a stress case outside the recipe:
 # sharper softmaxes amplify the bf16 rounding of q, k, P and the activations, so it gets twice the tolerance.
-@pytest.mark.parametrize("qk_norm,std,tol", [(False, 0.02, LOGIT_TOL_BF16), (True, 0.02, LOGIT_TOL_BF16), (False, 0.08, 2 * LOGIT_TOL_BF16)])
-def test_small_bf16_model_matches_oracle(qk_norm, std, tol):
+# vocab 1000: the last 128-id tile of the LM head holds 104 ids and its last warp quadrant 8 (ragged tail of the sampling epilogue).
+@pytest.mark.parametrize("qk_norm,std,tol,vocab", [(False, 0.02, LOGIT_TOL_BF16, 1024), (True, 0.02, LOGIT_TOL_BF16, 1024),
+                                                   (False, 0.08, 2 * LOGIT_TOL_BF16, 1024), (False, 0.02, LOGIT_TOL_BF16, 1000)])
+def test_small_bf16_model_matches_oracle(qk_norm, std, tol, vocab):
     from paper_2605_30859_b200 import api
-    cfg = dict(SMALL, qk_norm=qk_norm)
+    cfg = dict(SMALL, qk_norm=qk_norm, vocab=vocab)
     seed, G, P, max_new, K, T = 5, 3, 70, 40, 2, 1.0
     rng = np.random.default_rng(seed)
     prompts = [rng.integers(0, cfg["vocab"] - 1, size=n).astype(np.int32) for n in (70, 33, 64)]
@@ -91,3 +93,28 @@ def test_bf16_rollout_loop_equals_stepwise_and_is_deterministic():
         assert np.array_equal(b[k], c[k]), k
     assert np.any(b["status"] == PRUNED)
     d.close()
+
+
+@pytest.mark.parametrize("vocab", [1024, 1000])
+def test_both_lm_head_kernels_sample_the_same_tokens(vocab, monkeypatch):
+    """The decode LM head runs on the persistent swap-AB kernel; DARTS_LM_SK_MAX_ROWS=0 (read at darts_create) selects the 128 x 128
+    tile kernel instead.  Same logits (same k order), same Philox stream, same y = z / T + g: the rollouts must be identical, the
+    log-probabilities equal up to the merge order of the per-tile log-sum-exps."""
+    cfg = dict(SMALL, vocab=vocab)
+    seed, G, P, max_new, K = 11, 4, 64, 40, 2
+    prompts = wl.make_prompts(G, P, cfg["vocab"], seed)
+    Kp = np.full(G, 5, dtype=np.int32)
+    forced = wl.make_forced_len(Kp, dict(kind="lognormal", mu=3.0, sigma=0.6, lo=2, hi=40), seed)
+    out = []
+    for env in (None, "0"):
+        if env is None:
+            monkeypatch.delenv("DARTS_LM_SK_MAX_ROWS", raising=False)
+        else:
+            monkeypatch.setenv("DARTS_LM_SK_MAX_ROWS", env)
+        d, _ = make_ctx(cfg, seed, G, 5, P, max_new, page=64)
+        out.append(d.rollout_host(prompts, Kp, K, max_new, 1.0, 3, forced_len=forced))
+        d.close()
+    a, b = out
+    for k in ("tokens", "len", "status", "sel", "sel_mask", "margin"):
+        assert np.array_equal(a[k], b[k]), k
+    assert np.max(np.abs(a["logprob"] - b["logprob"])) < 1e-5
