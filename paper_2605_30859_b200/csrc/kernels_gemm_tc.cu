@@ -42,22 +42,19 @@ struct GemmParams {
   uint32_t k0, k1;
 };
 
-// AR = activation rows a stage holds.  The MMA always reads BM = 128 rows: with AR < BM the rows beyond AR are whatever follows the slot
-// (later slots / the weight slots, never outside the allocation since the b array is >= 16 KB) and land in accumulator rows that no one
-// reads, exactly like the stale rows beyond `live` of a full-size slot.
-template <int BN, int STAGES, int AR = BM>
+template <int BN, int STAGES>
 struct GemmSmem {
-  alignas(1024) unsigned char a[STAGES][AR * BK * 2];
+  alignas(1024) unsigned char a[STAGES][A_STAGE_BYTES];
   alignas(1024) unsigned char b[STAGES][BN * BK * 2];
   unsigned long long full[STAGES], empty[STAGES], acc_full;
   uint32_t tmem_base;
 };
 
-template <int BN, int STAGES, int EPI, int AR = BM>
+template <int BN, int STAGES, int EPI>
 __global__ void __launch_bounds__(GEMM_THREADS) gemm_tc_k(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
                                                           GemmParams p) {
   extern __shared__ unsigned char smem_raw[];
-  using Smem = GemmSmem<BN, STAGES, AR>;
+  using Smem = GemmSmem<BN, STAGES>;
   Smem &sm = *reinterpret_cast<Smem *>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int split = blockIdx.z;
@@ -215,15 +212,15 @@ EncodeTiledFn encode_fn() {
   return fn;
 }
 
-template <int BN, int STAGES, int EPI, int AR = BM>
+template <int BN, int STAGES, int EPI>
 darts_status launch_cfg(darts_ctx *c, const CUtensorMap &a, const CUtensorMap &b, const GemmParams &p, dim3 grid) {
-  size_t smem = sizeof(GemmSmem<BN, STAGES, AR>) + 1024;
+  size_t smem = sizeof(GemmSmem<BN, STAGES>) + 1024;
   static bool attr = false;
   if (!attr) {
-    CUDA_TRY(c, cudaFuncSetAttribute(gemm_tc_k<BN, STAGES, EPI, AR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    CUDA_TRY(c, cudaFuncSetAttribute(gemm_tc_k<BN, STAGES, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     attr = true;
   }
-  gemm_tc_k<BN, STAGES, EPI, AR><<<grid, GEMM_THREADS, smem, c->stream>>>(a, b, p);
+  gemm_tc_k<BN, STAGES, EPI><<<grid, GEMM_THREADS, smem, c->stream>>>(a, b, p);
   c->launches++;
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) {
@@ -270,12 +267,10 @@ darts_status launch_gemm_tc(darts_ctx *c, const TcGemm &g) {
   p.top2 = (float4 *)c->top2; p.lse = (float2 *)c->lse; p.logits_dump = (c->rt.flags & DARTS_FLAG_DUMP_LOGITS) ? c->logits : nullptr;
   p.row_list = c->row_list; p.row_prompt = c->row_prompt; p.row_sample = c->row_sample; p.row_len = c->row_len;
   p.temperature = c->temperature; p.k0 = (uint32_t)(c->seed & 0xffffffffu); p.k1 = (uint32_t)(c->seed >> 32);
-  // two stages (65 KB): three CTAs per SM, so one CTA's sampling epilogue and pipeline ramp hide behind two others' loads.  Measured on the
+  // Sampling on this kernel is the A/B path (DARTS_LM_SK_MAX_ROWS); the decode LM head runs on gemm_sk_k<SK_EPI_SAMPLE>.
+  // Two stages (65 KB): three CTAs per SM, so one CTA's sampling epilogue and pipeline ramp hide behind two others' loads.  Measured on the
   // non-layer part of a c3 step (LM head + boundary kernels) at 16 / 288 / 512 rows: 0.47 / 1.03 / 1.37 ms with 3 stages (2 CTAs per SM),
-  // 0.43 / 0.91 / 1.17 ms with 2, 0.59 / 1.51 / 2.10 ms with 4 (1 CTA per SM).
-#ifndef DARTS_LM_SMALL_STAGES
-#define DARTS_LM_SMALL_STAGES 3
-#endif
-  if (g.rows_ub <= 32) return launch_cfg<128, DARTS_LM_SMALL_STAGES, EPI_SAMPLE, 32>(c, *g.a_map, *g.b_map, p, grid);
+  // 0.43 / 0.91 / 1.17 ms with 2, 0.59 / 1.51 / 2.10 ms with 4 (1 CTA per SM); a 32-row activation slot (more stages in the same
+  // shared memory) changed nothing: the tile kernel at few rows is bound by its 128-row MMA, not by bytes in flight.
   return launch_cfg<128, 2, EPI_SAMPLE>(c, *g.a_map, *g.b_map, p, grid);
 }
