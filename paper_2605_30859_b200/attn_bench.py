@@ -5,7 +5,8 @@ tail of a long rollout, where the pair is bound by its two kernel boundaries and
 
 Config-2 head geometry (32 q / 8 kv heads, head_dim 128, page 64), one 1024-token shared prefix per group, every row with the
 same suffix length.  Prints, per case, the time of ONE call between two CUDA events on the library's stream and the time per
-call of 20 back-to-back calls (the launch path amortised, the PDL chain as inside a decode step), with the KV bytes of the call.
+call of 20 back-to-back calls (the launch path amortised, the PDL chain as inside a decode step), the same 20 calls replayed from a
+CUDA graph (no host launch path: the GPU-side cost alone), with the KV bytes of the call.
 DARTS_SKIP=4 drops attn_main_k, 8 drops attn_merge_k (include/darts.h): what is left is the cost of the other kernel alone."""
 import os
 import sys
@@ -21,6 +22,8 @@ def main():
     tag = "skip=%s pdl=%s" % (os.environ.get("DARTS_SKIP", "0"), "off" if os.environ.get("DARTS_NO_PDL") else "on")
     page = 64
     kvb = 2 * 8 * 128 * 2
+    st = torch.cuda.Stream()
+    torch.cuda.set_stream(st)                       # graph capture needs a non-default stream; the library launches on this one
     for case in cases.split(","):
         G, Kp, suf = (int(v) for v in case.split(":"))
         x = wl.attention_inputs("c2", seed=1, device="cuda", G=G, Kp=Kp, suffix=dict(kind="lognormal", mu=0.0, sigma=0.1, lo=suf, hi=suf))
@@ -47,9 +50,24 @@ def main():
             b.record(d.stream)
         torch.cuda.synchronize()
         chained = float(np.median([a.elapsed_time(b) for a, b in ev[:20]])) * 1e3 / 20
+        # the same 20 calls replayed from a CUDA graph: no host launch path at all — what the GPU alone needs per pair
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=st):
+            for _ in range(20):
+                d.attention(x["q"], out)
+        g.replay()
+        torch.cuda.synchronize()
+        a, b = ev[0]
+        a.record(st)
+        for _ in range(5):
+            g.replay()
+        b.record(st)
+        torch.cuda.synchronize()
+        graph = a.elapsed_time(b) * 1e3 / 100
+        del g
         mb = (int(x["suffix_len"].sum()) + G * P) * kvb / 1e6
         print(f"{tag}: G={G} Kp={Kp} suffix={suf} ({mb:.1f} MB of KV): single {single:.1f} us, chained {chained:.1f} us per call "
-              f"({mb / chained:.2f} TB/s)", flush=True)
+              f"({mb / chained:.2f} TB/s), graph replay {graph:.1f} us per call ({mb / graph:.2f} TB/s)", flush=True)
         d.close()
         del x, d
 
