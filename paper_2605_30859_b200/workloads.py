@@ -2,7 +2,7 @@
 and the oracle; holds none of the method's arithmetic — only random draws and shapes).
 
 Recipe (DESIGN.md "Input recipe"):
-  weights   N(0, 0.02^2); norm weights 1; MoE router N(0, 1/d_model) so router logits of a
+  weights   N(0, 0.02^2); norm weights 1 (parity tests: 1 + N(0, 0.2^2), `norm_std`); MoE router N(0, 1/d_model) so router logits of a
             unit-RMS hidden are ~N(0,1) (BASELINE.json c5 "router logits N(0,1)")
   prompts   uniform ints in [0, V-2]  (eos_id = V-1 never appears in a prompt)
   forced    forced-EOS length of trajectory (i,j) = round(lognormal(mu, sigma)) clipped to
@@ -71,9 +71,19 @@ def _normal(shape, std, seed, tag, dtype, device):
     return x.to(dtype).contiguous()
 
 
-def make_model(cfg, seed=0, device="cpu", std=0.02):
+def _gamma(n, norm_std, seed, tag, dtype, device):
+    """RMSNorm weight: ones (the configs' recipe) or 1 + N(0, norm_std^2) with its own stream per tensor."""
+    if not norm_std:
+        return torch.ones(n, dtype=dtype, device=device)
+    return (1.0 + _normal((n,), norm_std, seed, tag, torch.float32, device)).to(dtype).contiguous()
+
+
+def make_model(cfg, seed=0, device="cpu", std=0.02, norm_std=0.0):
     """Random-init weights as torch tensors on `device` (the CUDA path borrows their pointers).
-    Layout: every projection is [out_features, in_features] row-major."""
+    Layout: every projection is [out_features, in_features] row-major.
+    norm_std > 0 draws every RMSNorm weight (attn / mlp / final / q / k, one stream per layer and tensor) from
+    1 + N(0, norm_std^2) instead of the recipe's ones: the parity tests use it so that a kernel that drops or
+    mis-indexes a norm weight cannot pass."""
     dt = torch.float32 if cfg["dtype"] == "f32" else torch.bfloat16
     d, Hq, Hkv, hd = cfg["d_model"], cfg["n_q_heads"], cfg["n_kv_heads"], cfg["head_dim"]
     V, E = cfg["vocab"], cfg["n_experts"]
@@ -81,15 +91,15 @@ def make_model(cfg, seed=0, device="cpu", std=0.02):
     if V:
         m["embed"] = _normal((V, d), std, seed, "embed", dt, device)
         m["lm_head"] = _normal((V, d), std, seed, "lm_head", dt, device)
-        m["final_norm"] = torch.ones(d, dtype=dt, device=device)
+        m["final_norm"] = _gamma(d, norm_std, seed, "final_norm", dt, device)
     for l in range(cfg["n_layers"]):
-        L = dict(attn_norm=torch.ones(d, dtype=dt, device=device),
-                 mlp_norm=torch.ones(d, dtype=dt, device=device),
+        L = dict(attn_norm=_gamma(d, norm_std, seed, f"attn_norm{l}", dt, device),
+                 mlp_norm=_gamma(d, norm_std, seed, f"mlp_norm{l}", dt, device),
                  wqkv=_normal(((Hq + 2 * Hkv) * hd, d), std, seed, f"wqkv{l}", dt, device),
                  wo=_normal((d, Hq * hd), std, seed, f"wo{l}", dt, device))
         if cfg.get("qk_norm"):
-            L["q_norm"] = torch.ones(hd, dtype=dt, device=device)
-            L["k_norm"] = torch.ones(hd, dtype=dt, device=device)
+            L["q_norm"] = _gamma(hd, norm_std, seed, f"q_norm{l}", dt, device)
+            L["k_norm"] = _gamma(hd, norm_std, seed, f"k_norm{l}", dt, device)
         if E == 0 and cfg["ffn"]:
             L["wgu"] = _normal((2 * cfg["ffn"], d), std, seed, f"wgu{l}", dt, device)
             L["wd"] = _normal((d, cfg["ffn"]), std, seed, f"wd{l}", dt, device)

@@ -14,8 +14,8 @@ def tiny_cfg(**kw):
     return cfg
 
 
-def tiny_model(seed=0, std=0.3, **kw):
-    return wl.host_model(wl.make_model(tiny_cfg(**kw), seed=seed, std=std))
+def tiny_model(seed=0, std=0.3, norm_std=0.0, **kw):
+    return wl.host_model(wl.make_model(tiny_cfg(**kw), seed=seed, std=std, norm_std=norm_std))
 
 
 def test_softmax_rows_sum_to_one_and_shift_invariant():
@@ -99,8 +99,12 @@ def torch_forward(model, tokens):
         a = F.rms_norm(h, (d,), t64(L["attn_norm"]), eps=cfg["rms_eps"])
         qkv = F.linear(a, t64(L["wqkv"]))
         q, k, v = qkv.split([Hq * hd, Hkv * hd, Hkv * hd], dim=-1)
-        q = t64(tr.rope(q.reshape(T, Hq, hd).numpy(), np.arange(T), cfg["rope_theta"])).permute(1, 0, 2)[None]
-        k = t64(tr.rope(k.reshape(T, Hkv, hd).numpy(), np.arange(T), cfg["rope_theta"])).permute(1, 0, 2)[None]
+        q, k = q.reshape(T, Hq, hd), k.reshape(T, Hkv, hd)
+        if cfg.get("qk_norm"):                              # per-head RMSNorm over head_dim BEFORE RoPE (R5)
+            q = F.rms_norm(q, (hd,), t64(L["q_norm"]), eps=cfg["rms_eps"])
+            k = F.rms_norm(k, (hd,), t64(L["k_norm"]), eps=cfg["rms_eps"])
+        q = t64(tr.rope(q.numpy(), np.arange(T), cfg["rope_theta"])).permute(1, 0, 2)[None]
+        k = t64(tr.rope(k.numpy(), np.arange(T), cfg["rope_theta"])).permute(1, 0, 2)[None]
         v = v.reshape(T, Hkv, hd).permute(1, 0, 2)[None]
         o = F.scaled_dot_product_attention(q, k, v, is_causal=True, enable_gqa=True)[0].permute(1, 0, 2).reshape(T, -1)
         h = h + F.linear(o, t64(L["wo"]))
@@ -111,9 +115,34 @@ def torch_forward(model, tokens):
 
 
 def test_forward_full_against_torch_library_decoder():
-    model = tiny_model(seed=5)
     tokens = np.array([3, 17, 0, 39, 22, 8, 8, 1, 30, 11])
-    assert np.allclose(tr.forward_full(model, tokens), torch_forward(model, tokens), atol=1e-11)
+    # unit norm weights (the configs' recipe), then random ones, then random ones with the per-head QK-norm
+    for kw in (dict(), dict(norm_std=0.3), dict(norm_std=0.3, qk_norm=True)):
+        model = tiny_model(seed=5, **kw)
+        assert np.allclose(tr.forward_full(model, tokens), torch_forward(model, tokens), atol=1e-11), kw
+
+
+def test_qk_norm_branch_against_torch_rms_norm_per_head_before_rope():
+    """Pins oracle.transformer.qkv_project's qk_norm branch (random q_norm / k_norm: with unit weights
+    rmsnorm and rope commute and neither the order nor the weight indexing would be checked)."""
+    model = tiny_model(seed=11, norm_std=0.5, qk_norm=True)
+    cfg, L = model["cfg"], model["layers"][1]
+    Hq, Hkv, hd = cfg["n_q_heads"], cfg["n_kv_heads"], cfg["head_dim"]
+    rng = np.random.default_rng(0)
+    a, pos = rng.normal(size=(3, cfg["d_model"])), np.array([0, 7, 19])
+    q, k, v = tr.qkv_project(L, cfg, a, pos)
+    qkv = torch.from_numpy(a) @ torch.from_numpy(np.asarray(L["wqkv"], dtype=np.float64)).T
+    tq, tk, tv = qkv.split([Hq * hd, Hkv * hd, Hkv * hd], dim=-1)
+    wq, wk = (torch.from_numpy(np.asarray(L[n], dtype=np.float64)) for n in ("q_norm", "k_norm"))
+    assert not np.allclose(wq.numpy(), wk.numpy()) and not np.allclose(wq.numpy(), 1.0)
+    nq = F.rms_norm(tq.reshape(3, Hq, hd), (hd,), wq, eps=cfg["rms_eps"]).numpy()
+    nk = F.rms_norm(tk.reshape(3, Hkv, hd), (hd,), wk, eps=cfg["rms_eps"]).numpy()
+    assert np.allclose(q, tr.rope(nq, pos, cfg["rope_theta"]), atol=1e-12)
+    assert np.allclose(k, tr.rope(nk, pos, cfg["rope_theta"]), atol=1e-12)
+    assert np.allclose(v, tv.reshape(3, Hkv, hd).numpy(), atol=1e-12)          # v: neither norm nor rotation
+    # the other order (rotate, then normalise) is a different function once the weights are not 1
+    wrong = F.rms_norm(torch.from_numpy(tr.rope(tq.reshape(3, Hq, hd).numpy(), pos, cfg["rope_theta"])), (hd,), wq, eps=cfg["rms_eps"]).numpy()
+    assert np.max(np.abs(wrong - q)) > 1e-3
 
 
 def test_incremental_decode_equals_full_causal_forward():
@@ -153,6 +182,35 @@ def test_moe_single_expert_equals_dense_and_gates_sum_to_one():
     assert len(set(ids.tolist())) == 3 and abs(np.sum(w) - 1.0) < 1e-14 and np.all(np.diff(w) <= 0)
     p = tr.softmax(np.asarray(m4["layers"][0]["wr"], dtype=np.float64) @ b)
     assert set(ids.tolist()) == set(np.argsort(p)[-3:].tolist())
+
+
+def test_moe_identical_experts_top3_equals_dense_and_scaled_experts_pin_the_gates():
+    """Pins the gate-weighted combine of oracle.transformer.mlp for top_k > 1.
+    (a) E identical experts, top-3: gates sum to 1, so the MoE block IS the dense MLP (a dropped gate gives 3x,
+        un-renormalised probabilities give sum(p_top) x).
+    (b) expert e's down-projection scaled by c_e: the block is dense(b) * sum_e w_e c_e with w from an independent
+        softmax / top-k, so each gate must meet its OWN expert."""
+    from scipy.special import softmax as sp_softmax
+    E, k = 5, 3
+    dense = tiny_model(seed=12, norm_std=0.2)
+    moe = tiny_model(seed=12, norm_std=0.2, n_experts=E, top_k=k, expert_ffn=48, ffn=0)
+    for Ld, Lm in zip(dense["layers"], moe["layers"]):
+        Lm["wqkv"], Lm["wo"] = Ld["wqkv"], Ld["wo"]
+        Lm["wgu_e"] = np.repeat(np.asarray(Ld["wgu"], dtype=np.float64)[None], E, axis=0)
+        Lm["wd_e"] = np.repeat(np.asarray(Ld["wd"], dtype=np.float64)[None], E, axis=0)
+    moe["embed"], moe["lm_head"] = dense["embed"], dense["lm_head"]
+    tokens = np.array([4, 4, 31, 7, 19])
+    assert np.allclose(tr.forward_full(moe, tokens), tr.forward_full(dense, tokens), atol=1e-11)
+    Ld, Lm, cfg = dense["layers"][0], dict(moe["layers"][0]), moe["cfg"]
+    c = np.array([1.0, -2.0, 0.5, 3.0, 7.0])
+    Lm["wd_e"] = c[:, None, None] * Lm["wd_e"]
+    b = np.random.default_rng(1).normal(size=(4, cfg["d_model"]))
+    base = tr.mlp(Ld, dense["cfg"], b)
+    p = sp_softmax(b @ np.asarray(Lm["wr"], dtype=np.float64).T, axis=-1)
+    for t in range(4):
+        top = np.argsort(p[t])[-k:]
+        scale = float(np.sum(p[t, top] * c[top]) / np.sum(p[t, top]))
+        assert np.allclose(tr.mlp(Lm, cfg, b[t:t + 1])[0], scale * base[t], atol=1e-11), t
 
 
 def test_moe_route_tie_prefers_lower_expert_id():
