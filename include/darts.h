@@ -147,6 +147,8 @@ typedef struct {
   int64_t n_row_steps;                 /* sum over steps of active rows (= n_generated_tokens) */
   int64_t peak_pages;                  /* high-water mark of pages in use */
   int64_t kernel_launches;             /* kernels this ctx launched since darts_create */
+  int64_t pages_allocated;             /* pages popped from the free stack since darts_prefill, prefix pages included
+                                        * (> n_pages: freed pages were handed out again) */
 } darts_counters;
 
 typedef struct darts_ctx darts_ctx;
@@ -218,6 +220,15 @@ darts_status darts_get_attention_times(darts_ctx *ctx, float *ms_host, int32_t c
 /* Parity hooks (valid with DARTS_FLAG_DUMP_LOGITS): fp32 logits of global row `row` from the most
  * recent step that row took part in (step 0: the prompt's prefill logits).  out: HOST [vocab]. */
 darts_status darts_debug_logits(darts_ctx *ctx, int32_t row, float *out_host);
+
+/* Parity hooks for the MoE router's discrete choice (R13; MoE context with DARTS_FLAG_DUMP_LOGITS):
+ * darts_debug_routing: expert ids, in selection order, that every layer's router chose for slots [slot_begin, slot_begin + n_slots)
+ *   of the MOST RECENT forward pass (a decode step: slot = position in the active row list; a prefill pass: slot = index of the
+ *   prompt token within the pass).  out: HOST [n_layers][n_slots][top_k].  Synchronises.
+ * darts_debug_row_slots: for every global row, the slot it occupied in the last decode step it took part in and that step's index
+ *   (-1: none yet).  HOST [n_rows] each.  Synchronises. */
+darts_status darts_debug_routing(darts_ctx *ctx, int32_t slot_begin, int32_t n_slots, int32_t *out_host);
+darts_status darts_debug_row_slots(darts_ctx *ctx, int32_t *slot_host, int32_t *step_host, int32_t n_rows);
 
 /* Teacher forcing for parity at bf16 (R12): overwrite the token the next decode step feeds
  * for global row `row`.  tokens: HOST [n_rows] (-1 = leave). */

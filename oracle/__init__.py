@@ -29,8 +29,11 @@ Parity pins (tests/test_oracle_*.py, run with -m "not gpu"):
   attention   torch float64 scaled_dot_product_attention; rows sum to 1;
               prefix-shared == unshared; split-KV + LSE merge == unsplit
   rope        relative-position invariance;  rmsnorm  scale invariance / unit RMS
-  transformer incremental decode == one full causal forward; zero weights ->
-              uniform logits; MoE(E=1, top-1) == dense MLP; gate weights sum to 1
+  transformer incremental decode == one full causal forward; == a torch library
+              decoder with random norm weights (incl. the per-head QK-norm); zero
+              weights -> uniform logits; MoE(E=1, top-1) == dense MLP; MoE(E
+              identical experts, top-3) == dense MLP and scaled experts pin each
+              gate to its own expert; qk_norm == torch rms_norm per head BEFORE rope
   selection   exhaustive enumeration on tiny pools vs. an independent brute-force
               statement of the rule; |sel| = K; EARLY == full-rollout-then-sort
   compaction  == stable partition

@@ -57,7 +57,11 @@ def _finish(out, G, K, offs):
 
 def rollout_stepwise(model, prompts, Kp, K, max_new, T, seed, forced_len=None, L_long=1,
                      M_up=None, mode=MODE_AUTO, eos_id=None, teacher=None, keep_logits=False,
-                     logit_filter=None):
+                     logit_filter=None, routing=None):
+    """routing (MoE, optional; R13 teacher-forced routing): dict with ("prefill", i) -> expert ids [L][P_i][top_k]
+    and (r, s) -> [L][top_k] for every decode step s >= 1 of row r; the result then carries route_regret[(r, s)], the largest regret
+    over the layers of that forward (step 0: over the layers and positions of the prompt's prefill) — see
+    oracle.transformer.ROUTE_OVERRIDE."""
     cfg = model["cfg"]
     eos_id = cfg["vocab"] - 1 if eos_id is None else eos_id
     M_up = 2 * K if M_up is None else M_up
@@ -65,9 +69,16 @@ def rollout_stepwise(model, prompts, Kp, K, max_new, T, seed, forced_len=None, L
 
     z0, kv0, gap0 = [], [], []
     router_gap = {}                                          # (r, s) -> smallest router gap seen (R13; MoE models only)
+    regret0, route_regret = [], {}
     for i in range(G):                                       # one prefill per prompt (:134)
         _tf.ROUTER_GAPS = [] if keep_logits else None
+        if routing is not None:
+            ids = np.asarray(routing[("prefill", i)])
+            _tf.ROUTE_OVERRIDE, _tf.ROUTE_REGRET = iter(ids.reshape(-1, ids.shape[-1])), []
         z, kv = prefill(model, prompts[i])
+        if routing is not None:
+            regret0.append(max(_tf.ROUTE_REGRET))
+            _tf.ROUTE_OVERRIDE = _tf.ROUTE_REGRET = None
         gap0.append(min(_tf.ROUTER_GAPS) if _tf.ROUTER_GAPS else np.inf)
         z0.append(z)
         kv0.append(kv)
@@ -94,9 +105,16 @@ def rollout_stepwise(model, prompts, Kp, K, max_new, T, seed, forced_len=None, L
             if s == 0:
                 z = z0[i]
                 gap = gap0[i]
+                if routing is not None:
+                    route_regret[(r, 0)] = regret0[i]
             else:
                 _tf.ROUTER_GAPS = [] if keep_logits else None
+                if routing is not None:
+                    _tf.ROUTE_OVERRIDE, _tf.ROUTE_REGRET = iter(np.asarray(routing[(r, s)])), []
                 z = decode_one(model, kv[r], tokens[r, s - 1], len(prompts[i]) + s - 1)
+                if routing is not None:
+                    route_regret[(r, s)] = max(_tf.ROUTE_REGRET)
+                    _tf.ROUTE_OVERRIDE = _tf.ROUTE_REGRET = None
                 gap = min(_tf.ROUTER_GAPS) if _tf.ROUTER_GAPS else np.inf
             if keep_logits and (logit_filter is None or logit_filter(r, s)):
                 logits[(r, s)] = z.copy()
@@ -122,7 +140,7 @@ def rollout_stepwise(model, prompts, Kp, K, max_new, T, seed, forced_len=None, L
 
     out = dict(tokens=tokens, len=length, status=status, sel=sel, sel_mask=mask,
                close_step=close_step, n_steps=s, margins=margins, logprobs=logprobs, oracle_tokens=otok,
-               logits=logits, router_gap=router_gap, n_active_hist=n_active_hist)
+               logits=logits, router_gap=router_gap, route_regret=route_regret, n_active_hist=n_active_hist)
     _tf.ROUTER_GAPS = None
     return _finish(out, G, K, offs)
 

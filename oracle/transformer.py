@@ -45,6 +45,21 @@ def f64(x):
     return np.asarray(x, dtype=np.float64)
 
 
+# Matched-rounding debug mode (SURVEY.md 8(c) "precision contract": "a second matched-rounding oracle mode that rounds to bf16 at
+# the GPU's documented rounding points").  ROUND = None (default): the un-rounded definition, nothing below changes a value.
+# ROUND = callable(name, array) -> array: applied where the bf16 CUDA path rounds an input of a tensor-core product
+# ("rounding points"): "xn" the normed hidden fed to QKV, "q" / "k" / "v" after RoPE (k, v as stored in the cache),
+# "p" the un-normalised attention probabilities exp(s - max) fed to P.V (the denominator sums the un-rounded ones), "ao" the
+# attention output fed to Wo, "xn2" the normed hidden fed to the MLP / the experts (the MoE router reads the un-rounded one),
+# "act" silu(g) * u fed to Wd, "xnf" the final normed hidden fed to the LM head.  It answers "how far is an ideal bf16 pipeline
+# from the definition on this model", which no kernel can beat; the parity tolerance is still stated against the definition.
+ROUND = None
+
+
+def _r(name, x):
+    return x if ROUND is None else ROUND(name, x)
+
+
 def rmsnorm(x, w, eps):
     x = f64(x)
     return x * f64(w) / np.sqrt(np.mean(x * x, axis=-1, keepdims=True) + eps)
@@ -83,8 +98,12 @@ def attention_one(q, K, V, n_kv_heads):
     for h in range(Hq):
         g = h // rep
         s = K[:, g, :] @ q[h] / np.sqrt(hd)                 # [T]
-        p = softmax(s)
-        out[h] = p @ V[:, g, :]
+        if ROUND is None:
+            p = softmax(s)
+            out[h] = p @ V[:, g, :]
+        else:                                               # matched rounding: rounded numerator, un-rounded denominator
+            e = np.exp(s - np.max(s))
+            out[h] = (ROUND("p", e) @ V[:, g, :]) / np.sum(e)
     return out
 
 
@@ -101,13 +120,21 @@ def qkv_project(layer, cfg, a, pos):
         k = rmsnorm(k, layer["k_norm"], cfg["rms_eps"])
     q = rope(q, pos, cfg["rope_theta"])
     k = rope(k, pos, cfg["rope_theta"])
-    return q, k, v
+    return _r("q", q), _r("k", k), _r("v", v)
 
 
 # DESIGN.md R13: when this is a list, every routing decision appends the probability gap between the
 # k-th and (k+1)-th expert (tests use it to set aside rows whose discrete expert choice is a near-tie).
 # Pure instrumentation: it does not change any value computed here.
 ROUTER_GAPS = None
+
+# DESIGN.md R13, teacher-forced routing (the analogue of teacher-forced tokens, R12): when ROUTE_OVERRIDE is an iterator,
+# every routing decision takes its expert ids from it (in call order: forward_full walks layers, then positions) instead of
+# from its own top-k; the gates are still this oracle's probabilities renormalised over those experts.  When ROUTE_REGRET is a
+# list, each such decision appends max p(own choice not taken) - min p(forced choice not own): 0 when the two sets agree, else how
+# far, in probability, the forced set is from being the top-k.  Both None: nothing changes.
+ROUTE_OVERRIDE = None
+ROUTE_REGRET = None
 
 
 def moe_route(layer, cfg, b):
@@ -118,33 +145,43 @@ def moe_route(layer, cfg, b):
     if ROUTER_GAPS is not None and cfg["top_k"] < len(p):
         ps = np.sort(p)[::-1]
         ROUTER_GAPS.append(float(ps[cfg["top_k"] - 1] - ps[cfg["top_k"]]))
+    if ROUTE_OVERRIDE is not None:
+        forced = np.asarray(next(ROUTE_OVERRIDE), dtype=np.int64)
+        assert forced.shape == order.shape and len(set(forced.tolist())) == len(forced) and forced.min() >= 0 and forced.max() < len(p)
+        if ROUTE_REGRET is not None:
+            own, frc = set(order.tolist()), set(forced.tolist())
+            ROUTE_REGRET.append(0.0 if own == frc else float(max(p[list(own - frc)]) - min(p[list(frc - own)])))
+        order = forced
     w = p[order] / np.sum(p[order])
     return order, w
 
 
 def mlp(layer, cfg, b):
     """b [T, d] -> m [T, d]."""
+    br = _r("xn2", b)                                        # == b unless the matched-rounding mode is on
     if cfg.get("n_experts", 0) == 0:
         F = cfg["ffn"]
-        gu = b @ f64(layer["wgu"]).T
-        return (silu(gu[:, :F]) * gu[:, F:]) @ f64(layer["wd"]).T
+        gu = br @ f64(layer["wgu"]).T
+        return _r("act", silu(gu[:, :F]) * gu[:, F:]) @ f64(layer["wd"]).T
     F = cfg["expert_ffn"]
     out = np.zeros_like(b)
     for t in range(b.shape[0]):
-        ids, w = moe_route(layer, cfg, b[t])
+        ids, w = moe_route(layer, cfg, b[t])                 # the router always sees the un-rounded hidden (DESIGN.md R13)
         for e, we in zip(ids, w):
-            gu = f64(layer["wgu_e"][e]) @ b[t]
-            out[t] += we * (f64(layer["wd_e"][e]) @ (silu(gu[:F]) * gu[F:]))
+            gu = f64(layer["wgu_e"][e]) @ br[t]
+            out[t] += we * (f64(layer["wd_e"][e]) @ _r("act", silu(gu[:F]) * gu[F:]))
     return out
 
 
 def logits_from_hidden(model, h):
     cfg = model["cfg"]
-    return rmsnorm(h, model["final_norm"], cfg["rms_eps"]) @ f64(model["lm_head"]).T
+    return _r("xnf", rmsnorm(h, model["final_norm"], cfg["rms_eps"])) @ f64(model["lm_head"]).T
 
 
-def forward_full(model, tokens, return_kv=False):
-    """THE DEFINITION: causal forward over tokens [T] -> logits [T, V] (and per-layer K,V)."""
+def forward_full(model, tokens, return_kv=False, last=None):
+    """THE DEFINITION: causal forward over tokens [T] -> logits [T, V] (and per-layer K,V).
+    last = n returns the logits of the last n positions only ([n, V]; the rows of the full result, nothing else
+    changes): a long teacher-forced history at vocab 151 936 would otherwise need T x V doubles."""
     cfg = model["cfg"]
     tokens = np.asarray(tokens, dtype=np.int64)
     T = tokens.shape[0]
@@ -152,16 +189,16 @@ def forward_full(model, tokens, return_kv=False):
     h = f64(model["embed"])[tokens]                          # [T, d]
     kv = []
     for layer in model["layers"]:
-        a = rmsnorm(h, layer["attn_norm"], cfg["rms_eps"])
+        a = _r("xn", rmsnorm(h, layer["attn_norm"], cfg["rms_eps"]))
         q, k, v = qkv_project(layer, cfg, a, pos)
         o = np.empty((T, cfg["n_q_heads"], cfg["head_dim"]))
         for t in range(T):                                   # causal: position t sees keys 0..t
             o[t] = attention_one(q[t], k[: t + 1], v[: t + 1], cfg["n_kv_heads"])
-        h = h + o.reshape(T, -1) @ f64(layer["wo"]).T
+        h = h + _r("ao", o.reshape(T, -1)) @ f64(layer["wo"]).T
         b = rmsnorm(h, layer["mlp_norm"], cfg["rms_eps"])
         h = h + mlp(layer, cfg, b)
         kv.append((k, v))
-    logits = logits_from_hidden(model, h)
+    logits = logits_from_hidden(model, h if last is None else h[T - last:])
     return (logits, kv) if return_kv else logits
 
 
@@ -178,13 +215,13 @@ def decode_one(model, kv, token, pos):
     cfg = model["cfg"]
     h = f64(model["embed"])[int(token)][None, :]             # [1, d]
     for l, layer in enumerate(model["layers"]):
-        a = rmsnorm(h, layer["attn_norm"], cfg["rms_eps"])
+        a = _r("xn", rmsnorm(h, layer["attn_norm"], cfg["rms_eps"]))
         q, k, v = qkv_project(layer, cfg, a, np.array([pos]))
         K = np.concatenate([kv[l][0], k], axis=0)
         V = np.concatenate([kv[l][1], v], axis=0)
         kv[l] = (K, V)
         o = attention_one(q[0], K, V, cfg["n_kv_heads"])
-        h = h + o.reshape(1, -1) @ f64(layer["wo"]).T
+        h = h + _r("ao", o.reshape(1, -1)) @ f64(layer["wo"]).T
         b = rmsnorm(h, layer["mlp_norm"], cfg["rms_eps"])
         h = h + mlp(layer, cfg, b)
     return logits_from_hidden(model, h)[0]

@@ -55,7 +55,7 @@ class Results(C.Structure):
 
 class Counters(C.Structure):
     _fields_ = [(n, C.c_int64) for n in ("n_steps", "n_generated_tokens", "n_kept_tokens", "n_near_ties", "n_row_steps",
-                                         "peak_pages", "kernel_launches")]
+                                         "peak_pages", "kernel_launches", "pages_allocated")]
 
 
 def _sig(name, *argtypes, restype=_i32):
@@ -83,6 +83,8 @@ darts_get_counters = _sig("darts_get_counters", _ctx, C.POINTER(Counters))
 darts_n_active = _sig("darts_n_active", _ctx, C.POINTER(_i32))
 darts_get_attention_times = _sig("darts_get_attention_times", _ctx, _vp, _i32, C.POINTER(_i32))
 darts_debug_logits = _sig("darts_debug_logits", _ctx, _i32, _vp)
+darts_debug_routing = _sig("darts_debug_routing", _ctx, _i32, _i32, _vp)
+darts_debug_row_slots = _sig("darts_debug_row_slots", _ctx, _vp, _vp, _i32)
 darts_debug_set_last_tokens = _sig("darts_debug_set_last_tokens", _ctx, _vp, _i32)
 darts_debug_gemm_bf16 = _sig("darts_debug_gemm_bf16", _ctx, _vp, _vp, _vp, _vp, _i32, _i32, _i32, _i32)
 darts_debug_gemm_scratch_floats = _sig("darts_debug_gemm_scratch_floats", _ctx, _i32, _i32, _i32, _i32, C.POINTER(C.c_size_t))
@@ -252,12 +254,16 @@ class Darts:
         cb = ChunkFn(tramp)
         self._check(darts_run_to_completion_streaming(self.ctx, chunk_steps, cb, None, None))
 
-    def rollout(self, prompts_dev, G, Kp, K, max_len, temperature, seed, forced_len_dev=None):
-        """north_star signature: device prompts [G,P] int32, scalar K'."""
+    def rollout(self, prompts_dev, G, Kp, K, max_len, temperature, seed, forced_len_dev=None, fetch=True):
+        """north_star signature: device prompts [G,P] int32, scalar K' (L_long = 1, M_up = 2K, mode AUTO); forced_len_dev [G,K'] int32
+        (cuda) or None.  fetch=True hands darts_rollout a darts_results and returns its buffers; False passes out = NULL."""
         assert prompts_dev.is_cuda and prompts_dev.dtype == torch.int32 and prompts_dev.is_contiguous()
-        self._check(darts_rollout(self.ctx, prompts_dev.data_ptr(), prompts_dev.shape[1], G, Kp, K, max_len, temperature, seed,
-                                  forced_len_dev.data_ptr() if forced_len_dev is not None else None, None))
+        assert forced_len_dev is None or (forced_len_dev.is_cuda and forced_len_dev.dtype == torch.int32 and tuple(forced_len_dev.shape) == (G, Kp))
         self.G, self.R, self.K = G, G * Kp, K
+        bufs, res = self._result_buffers() if fetch else (None, None)
+        self._check(darts_rollout(self.ctx, prompts_dev.data_ptr(), prompts_dev.shape[1], G, Kp, K, max_len, temperature, seed,
+                                  forced_len_dev.data_ptr() if forced_len_dev is not None else None, C.byref(res) if fetch else None))
+        return bufs
 
     def rollout_host(self, prompts, Kp, K, max_len, temperature, seed, forced_len=None, L_long=1, M_up=0, mode=MODE_AUTO,
                      out=None):
@@ -306,6 +312,18 @@ class Darts:
         out = np.empty(self.cfg["vocab"], np.float32)
         self._check(darts_debug_logits(self.ctx, row, _np_ptr(out)))
         return out
+
+    def debug_routing(self, slot_begin, n_slots):
+        """Expert ids [n_layers, n_slots, top_k] the routers chose for a slot range of the most recent pass (MoE + FLAG_DUMP_LOGITS)."""
+        out = np.empty((self.cfg["n_layers"], n_slots, self.cfg["top_k"]), np.int32)
+        self._check(darts_debug_routing(self.ctx, slot_begin, n_slots, _np_ptr(out)))
+        return out
+
+    def debug_row_slots(self):
+        """(slot, step) of every row's last decode step."""
+        slot, step = np.empty(self.R, np.int32), np.empty(self.R, np.int32)
+        self._check(darts_debug_row_slots(self.ctx, _np_ptr(slot), _np_ptr(step), self.R))
+        return slot, step
 
     def debug_set_last_tokens(self, tokens):
         t = np.ascontiguousarray(tokens, dtype=np.int32)

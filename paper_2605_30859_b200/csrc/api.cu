@@ -114,6 +114,7 @@ size_t carve(darts_ctx *c, void *base) {
       c->moe_w = k.take<float>(RK);
       c->moe_arrive_n = A / 4 + 1;
       c->moe_arrive = k.take<int32_t>(c->moe_arrive_n);         // router arrival counters, one per block of 4 slots; zero between launches
+      if (rt.flags & DARTS_FLAG_DUMP_LOGITS) c->moe_eid_dump = k.take<int32_t>((size_t)m.n_layers * RK);
     }
     if (c->tc_path) {
       // stream-K pieces [slots][rows][N]: whole-tile mode (1 slot) for the prefill-sized passes, up to 16 slots for decode rows
@@ -584,7 +585,7 @@ darts_status darts_get_counters(darts_ctx *c, darts_counters *o) {
   CUDA_TRY(c, cudaStreamSynchronize(c->stream));
   o->n_steps = st.step; o->n_generated_tokens = (int64_t)st.n_generated; o->n_kept_tokens = (int64_t)st.n_kept;
   o->n_near_ties = (int64_t)st.n_near_ties; o->n_row_steps = (int64_t)st.n_row_steps; o->peak_pages = st.peak_used;
-  o->kernel_launches = c->launches;
+  o->kernel_launches = c->launches; o->pages_allocated = (int64_t)st.n_pops;
   return DARTS_OK;
 }
 
@@ -744,6 +745,26 @@ darts_status darts_debug_logits(darts_ctx *c, int32_t row, float *out_host) {
     src = c->logits + (size_t)slot * c->m.vocab;
   }
   CUDA_TRY(c, cudaMemcpy(out_host, src, (size_t)c->m.vocab * 4, cudaMemcpyDeviceToHost));
+  return DARTS_OK;
+}
+
+darts_status darts_debug_routing(darts_ctx *c, int32_t slot_begin, int32_t n_slots, int32_t *out_host) {
+  if (!c || !out_host) return DARTS_ERR_INVALID_ARG;
+  if (!c->moe_eid_dump) FAIL(c, DARTS_ERR_BAD_STATE, "routing is kept only by a MoE context created with DARTS_FLAG_DUMP_LOGITS");
+  if (slot_begin < 0 || n_slots <= 0 || slot_begin + n_slots > c->act_rows) FAIL(c, DARTS_ERR_INVALID_ARG, "bad slot range");
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  const size_t k = c->m.top_k;
+  CUDA_TRY(c, cudaMemcpy2D(out_host, (size_t)n_slots * k * 4, c->moe_eid_dump + (size_t)slot_begin * k, (size_t)c->act_rows * k * 4, (size_t)n_slots * k * 4,
+                           (size_t)c->m.n_layers, cudaMemcpyDeviceToHost));
+  return DARTS_OK;
+}
+
+darts_status darts_debug_row_slots(darts_ctx *c, int32_t *slot_host, int32_t *step_host, int32_t n_rows) {
+  if (!c || !slot_host || !step_host) return DARTS_ERR_INVALID_ARG;
+  if (!c->prefilled || n_rows != c->R) FAIL(c, DARTS_ERR_INVALID_ARG, "n_rows must equal the rollout's row count");
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  CUDA_TRY(c, cudaMemcpy(slot_host, c->row_slot, (size_t)n_rows * 4, cudaMemcpyDeviceToHost));
+  CUDA_TRY(c, cudaMemcpy(step_host, c->row_slot_step, (size_t)n_rows * 4, cudaMemcpyDeviceToHost));
   return DARTS_OK;
 }
 

@@ -29,6 +29,7 @@ struct DevState {
   int32_t peak_used;
   int32_t n_open_groups;
   unsigned long long n_generated, n_near_ties, n_kept, n_row_steps;
+  unsigned long long n_pops;     // pages handed out since the prefill (prefix pages + every pop of the free stack)
 };
 
 // KV cache geometry.  One layer slab = [page][kv_head][K|V][token][head_dim]; the (K,V) tiles of one
@@ -104,6 +105,7 @@ struct darts_ctx {
   // MoE (kernels_moe.cu)
   int32_t *moe_eid, *moe_pos, *moe_off, *moe_cnt, *moe_tok, *moe_rb, *moe_nrb, *moe_arrive;
   size_t moe_arrive_n;   // moe_rb: row blocks {row0, nrows, expert, -}   // moe_cnt: [n_layers][E], zeroed once per forward pass
+  int32_t *moe_eid_dump;         // [n_layers][act_rows][top_k] expert ids of the last pass (DARTS_FLAG_DUMP_LOGITS only; parity hook)
   float *moe_w, *moe_logits, *moe_y;   // gates [rows*top_k]; router logits [rows][E]; generic path expert outputs [rows*top_k][d]
   void *xs;                      // expert-sorted copy of xn [max_rows * top_k][d]
   // tuned attention (kernels_attn_sm100.cu): per-step work list and split-KV partials

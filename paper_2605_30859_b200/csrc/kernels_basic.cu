@@ -289,6 +289,7 @@ __global__ void plan_decode_k(DevState *st, const int32_t *__restrict__ row_list
       pinned[2] = DARTS_ERR_KV_POOL_EXHAUSTED;
     } else {
       st->free_top = free_top - s_base;
+      st->n_pops += (unsigned long long)s_base;
     }
   }
 }

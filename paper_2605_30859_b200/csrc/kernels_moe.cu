@@ -38,7 +38,7 @@ darts_status post(darts_ctx *c, const char *what) {
 // grid (ceil(rows_ub / RROWS), ceil(E / REXP)), 256 threads, dynamic smem RROWS * d floats.  d % 4 == 0.
 // One warp per slot.  Ordering is taken on the logits (monotone in p, so identical to ordering by p in exact arithmetic).
 __device__ __forceinline__ void topk_row(const float *logits, int E, int top_k, int32_t *__restrict__ eid, float *__restrict__ gate,
-                                         int32_t *__restrict__ pos, int32_t *__restrict__ cnt, int slot, int lane) {
+                                         int32_t *__restrict__ pos, int32_t *__restrict__ cnt, int32_t *__restrict__ eid_dump, int slot, int lane) {
   float z[MAX_E_PER_LANE];
   float mx = -INFINITY;
 #pragma unroll
@@ -77,6 +77,7 @@ __device__ __forceinline__ void topk_row(const float *logits, int E, int top_k, 
   if (lane < top_k) {
     int a = slot * top_k + lane;
     eid[a] = my_e;
+    if (eid_dump) eid_dump[a] = my_e;                    // parity hook (darts_debug_routing): this layer's choices survive the pass
     gate[a] = my_p / psum;
     pos[a] = a;                                        // identity; moe_place_k overwrites it on the tensor-core path
     if (cnt) atomicAdd(&cnt[my_e], 1);
@@ -88,7 +89,7 @@ template <typename T>
 __global__ void __launch_bounds__(256) moe_router_k(const float *__restrict__ h, const T *__restrict__ wnorm, const float *__restrict__ wr,
                                                     float *logits, int d, int E, float eps, int top_k, int32_t *__restrict__ eid,
                                                     float *__restrict__ gate, int32_t *__restrict__ pos, int32_t *__restrict__ cnt,
-                                                    int32_t *arrive, const int32_t *n_rows_dev, int rows_ub) {
+                                                    int32_t *arrive, int32_t *eid_dump, const int32_t *n_rows_dev, int rows_ub) {
   pdl_trigger();
   pdl_wait();
   extern __shared__ float xs[];                       // [RROWS][d] normalised rows
@@ -144,7 +145,7 @@ __global__ void __launch_bounds__(256) moe_router_k(const float *__restrict__ h,
   if (!s_last) return;
   __threadfence();
   if (threadIdx.x == 0) arrive[blockIdx.x] = 0;       // ready for the next layer's launch
-  if (warp < RROWS && s0 + warp < n) topk_row(logits, E, top_k, eid, gate, pos, cnt, s0 + warp, lane);
+  if (warp < RROWS && s0 + warp < n) topk_row(logits, E, top_k, eid, gate, pos, cnt, eid_dump, s0 + warp, lane);
 }
 
 // One CTA per expert (tensor-core path).  off[e] = sum_{e'<e} cnt[e'];  the expert's assignments keep their slot
@@ -315,7 +316,8 @@ darts_status route(darts_ctx *c, int layer, int rows_ub, const int32_t *n_rows_d
     attr = true;
   }
   launch_pdl(c, moe_router_k<T>, grid, dim3(256), smem, c->h, (const T *)c->mlp_norm[layer], (const float *)c->wr[layer], c->moe_logits, m.d_model,
-             m.n_experts, m.rms_eps, m.top_k, c->moe_eid, c->moe_w, c->moe_pos, cnt, c->moe_arrive, n_rows_dev, rows_ub);
+             m.n_experts, m.rms_eps, m.top_k, c->moe_eid, c->moe_w, c->moe_pos, cnt, c->moe_arrive,
+             c->moe_eid_dump ? c->moe_eid_dump + (size_t)layer * c->act_rows * m.top_k : nullptr, n_rows_dev, rows_ub);
   return post(c, "moe_router");
 }
 

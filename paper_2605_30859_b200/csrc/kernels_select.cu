@@ -195,7 +195,7 @@ __global__ void init_rows_k(DevState *st, const int32_t *__restrict__ g_off, con
   if (t == 0) {
     st->n_active = R; st->n_rows = R; st->n_groups = G; st->free_top = nfree; st->err = 0; st->step = 0;
     st->peak_used = n_prefix_pages; st->n_open_groups = G;
-    st->n_generated = 0; st->n_near_ties = 0; st->n_kept = 0; st->n_row_steps = 0;
+    st->n_generated = 0; st->n_near_ties = 0; st->n_kept = 0; st->n_row_steps = 0; st->n_pops = (unsigned long long)n_prefix_pages;
     pinned[2] = 0;
   }
 }

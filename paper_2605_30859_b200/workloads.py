@@ -116,26 +116,27 @@ class HostWeights:
     """Lazy host view of a torch tensor for the oracle: converted to float64 only when used
     (np.asarray(w, dtype=float64) or w[index]) so a 4B-parameter model fits in host memory."""
 
-    def __init__(self, t):
-        self.t = t.detach().cpu()
+    def __init__(self, t, lazy=False):
+        # lazy: leave the tensor where it is (e.g. a 60 GB MoE model in HBM) and copy only what is indexed
+        self.t = t.detach() if lazy else t.detach().cpu()
         self.shape = tuple(self.t.shape)
 
     def __array__(self, dtype=None, copy=None):
-        return self.t.to(torch.float64).numpy()
+        return self.t.cpu().to(torch.float64).numpy()
 
     def __getitem__(self, idx):
         if isinstance(idx, np.ndarray):
-            idx = torch.from_numpy(idx.astype(np.int64))
-        return self.t[idx].to(torch.float64).numpy()
+            idx = torch.from_numpy(idx.astype(np.int64)).to(self.t.device)
+        return self.t[idx].cpu().to(torch.float64).numpy()
 
     def __len__(self):
         return self.shape[0]
 
 
-def host_model(m):
-    """The same weights as `make_model` returned, as host arrays the oracle can consume."""
+def host_model(m, lazy=False):
+    """The same weights as `make_model` returned, as host arrays the oracle can consume (lazy: device-backed views)."""
     def conv(v):
-        return HostWeights(v) if torch.is_tensor(v) else v
+        return HostWeights(v, lazy) if torch.is_tensor(v) else v
     out = dict(cfg=dict(m["cfg"]), layers=[{k: conv(v) for k, v in L.items()} for L in m["layers"]])
     for k in ("embed", "lm_head", "final_norm"):
         if k in m:

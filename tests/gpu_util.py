@@ -4,9 +4,9 @@ import numpy as np
 from paper_2605_30859_b200 import workloads as wl
 
 
-def make_ctx(cfg, seed, G, Kp_max, P, max_new, page=16, flags=0, n_pages=None, std=0.02):
+def make_ctx(cfg, seed, G, Kp_max, P, max_new, page=16, flags=0, n_pages=None, std=0.02, norm_std=0.0):
     from paper_2605_30859_b200 import api
-    model_cpu = wl.make_model(cfg, seed=seed, std=std)
+    model_cpu = wl.make_model(cfg, seed=seed, std=std, norm_std=norm_std)
     model_gpu = dict(cfg=model_cpu["cfg"], layers=[{k: v.cuda() for k, v in L.items()} for L in model_cpu["layers"]])
     for k in ("embed", "lm_head", "final_norm"):
         model_gpu[k] = model_cpu[k].cuda()

@@ -18,10 +18,18 @@ SMALL = dict(n_layers=2, d_model=256, n_q_heads=4, n_kv_heads=2, head_dim=128, f
              expert_ffn=0, qk_norm=False, rope_theta=1.0e6, rms_eps=1.0e-6, dtype="bf16")
 
 
-def run_stepwise(d, prompts, Kp, K, T, seed, forced, **kw):
-    """Drive the C-ABI step by step, keeping the fp32 logits of every (row, step)."""
+def run_stepwise(d, prompts, Kp, K, T, seed, forced, routing=False, **kw):
+    """Drive the C-ABI step by step, keeping the fp32 logits of every (row, step).  routing=True (MoE): also the expert ids every
+    layer's router chose, keyed the way oracle.rollout.rollout_stepwise(routing=...) takes them; returns (results, logits, routing)."""
     d.prefill(prompts, Kp, K, temperature=T, seed=seed, forced_len=forced, **kw)
     R = int(np.sum(Kp))
+    route = {}
+    if routing:
+        offs = np.concatenate([[0], np.cumsum([len(p) for p in prompts])])
+        assert offs[-1] <= 4096                                  # one prefill pass: slot = index of the prompt token
+        ids = d.debug_routing(0, int(offs[-1]))
+        for i in range(len(prompts)):
+            route[("prefill", i)] = ids[:, offs[i]:offs[i + 1], :].copy()
     glog = {(r, 0): d.debug_logits(r) for r in range(R)}
     d.select_and_compact()
     s = 0
@@ -29,11 +37,17 @@ def run_stepwise(d, prompts, Kp, K, T, seed, forced, **kw):
         s += 1
         d.decode_step()
         res = d.results()
+        if routing:
+            slot, step = d.debug_row_slots()
+            ids = d.debug_routing(0, int(slot[step == s].max()) + 1)
         for r in range(R):
             if res["len"][r] == s + 1:
                 glog[(r, s)] = d.debug_logits(r)
+                if routing:
+                    assert step[r] == s
+                    route[(r, s)] = ids[:, slot[r], :].copy()
         d.select_and_compact()
-    return d.results(), glog
+    return (d.results(), glog, route) if routing else (d.results(), glog)
 
 
 # std 0.02 is the configs' init recipe (tolerance: north_star's 2e-2).  std 0.08 is a stress case outside the recipe:

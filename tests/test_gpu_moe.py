@@ -17,40 +17,48 @@ MOE_BF16 = dict(n_layers=3, d_model=256, n_q_heads=4, n_kv_heads=2, head_dim=128
                 expert_ffn=128, qk_norm=False, rope_theta=1.0e6, rms_eps=1.0e-6, dtype="bf16")
 
 
-def _case(cfg, seed, page, tol, gap_tol, std):
+def _case(cfg, seed, page, tol, regret_tol, std, norm_std=0.0, max_swapped=0.2):
+    """Every (row, step) logit vector is compared: the oracle follows the GPU's expert choices (teacher-forced routing) and
+    reports how far each was from its own top-k; a choice may differ only by a near-tie (probability regret < regret_tol)."""
     from paper_2605_30859_b200 import api
     G, P, max_new, K, T = 3, 40, 24, 2, 1.0
     rng = np.random.default_rng(seed)
     prompts = [rng.integers(0, cfg["vocab"] - 1, size=n).astype(np.int32) for n in (40, 17, 33)]
     Kp = np.asarray([4, 5, 3], dtype=np.int32)
     forced = wl.make_forced_len(Kp, dict(kind="lognormal", mu=2.5, sigma=0.6, lo=2, hi=40), seed)
-    d, host = make_ctx(cfg, seed, G, 5, P, max_new, page=page, flags=api.FLAG_DUMP_LOGITS, std=std)
-    gpu, glog = run_stepwise(d, prompts, Kp, K, T, seed, forced)
-    orc = ro.rollout_stepwise(host, prompts, Kp, K, max_new, T, seed, forced_len=forced, teacher=gpu["tokens"], keep_logits=True)
+    d, host = make_ctx(cfg, seed, G, 5, P, max_new, page=page, flags=api.FLAG_DUMP_LOGITS, std=std, norm_std=norm_std)
+    gpu, glog, route = run_stepwise(d, prompts, Kp, K, T, seed, forced, routing=True)
+    orc = ro.rollout_stepwise(host, prompts, Kp, K, max_new, T, seed, forced_len=forced, teacher=gpu["tokens"], keep_logits=True, routing=route)
     for k in ("len", "status", "sel", "sel_mask", "close_step"):
         assert np.array_equal(gpu[k], orc[k]), k
-    assert set(glog.keys()) == set(orc["logits"].keys())
-    errs = {k: rel_inf(glog[k], orc["logits"][k]) for k in glog}
-    clear = [k for k in glog if orc["router_gap"][k] > gap_tol]
-    assert len(clear) >= len(glog) // 2, (len(clear), len(glog))
-    worst = max(errs[k] for k in clear)
+    assert set(glog.keys()) == set(orc["logits"].keys()) == set(orc["route_regret"].keys())
+    worst = max(rel_inf(glog[k], orc["logits"][k]) for k in glog)
     assert worst < tol, worst
+    regrets = np.asarray([orc["route_regret"][k] for k in glog])
+    assert regrets.max() < regret_tol, regrets.max()          # DESIGN.md R13: expert sets differ by near-ties only
+    swapped = int(np.sum(regrets > 0))
+    assert swapped <= max_swapped * len(glog), (swapped, len(glog))
+    for (r, s) in glog:
+        err = float(np.max(np.abs(glog[(r, s)] - orc["logits"][(r, s)]))) / T
+        if orc["margins"][r, s] > 2 * err + 1e-3:
+            forced_here = s + 1 == orc["len"][r] and gpu["tokens"][r, s] == cfg["vocab"] - 1
+            assert forced_here or orc["oracle_tokens"][r, s] == gpu["tokens"][r, s], (r, s)
     cnt = d.counters()
     assert cnt["n_generated_tokens"] == orc["n_generated_tokens"]
     d.close()
-    return len(glog) - len(clear), worst
+    return swapped, len(glog), float(regrets.max()), worst
 
 
 def test_moe_fp32_generic_path_matches_oracle():
-    near, worst = _case(MOE_F32, seed=1, page=16, tol=1e-4, gap_tol=1e-5, std=0.05)
-    print("fp32 MoE: near-tie routings set aside", near, "worst rel logit err", worst)
+    swapped, n, regret, worst = _case(MOE_F32, seed=1, page=16, tol=1e-4, regret_tol=1e-5, std=0.05, max_swapped=0.02)
+    print(f"fp32 MoE: {swapped}/{n} forwards with a near-tie expert swap (max regret {regret:.1e}), worst rel logit err {worst:.2e}")
 
 
 def test_moe_bf16_tensor_core_path_matches_oracle():
-    # the router sees the fp32 residual stream, whose bf16-induced error (~1e-2 relative) moves router probabilities by
-    # ~1e-3: decisions with a smaller gap are not comparable
-    near, worst = _case(MOE_BF16, seed=2, page=64, tol=2e-2, gap_tol=2e-3, std=0.05)
-    print("bf16 MoE: near-tie routings set aside", near, "worst rel logit err", worst)
+    # the router sees the fp32 residual stream, whose bf16-induced error (~1e-2 relative) moves router probabilities by up to
+    # ~1e-3 (DESIGN.md R13): the GPU's expert set may differ from the oracle's by experts that close, and by nothing else
+    swapped, n, regret, worst = _case(MOE_BF16, seed=2, page=64, tol=2e-2, regret_tol=1e-3, std=0.05)
+    print(f"bf16 MoE: {swapped}/{n} forwards with a near-tie expert swap (max regret {regret:.1e}), worst rel logit err {worst:.2e}")
 
 
 def test_moe_rollout_is_deterministic_and_loop_equals_stepwise():

@@ -35,12 +35,12 @@ def test_random_policies_match_oracle_bit_exact(seed, kind):
     prompts = [rng.integers(0, cfg["vocab"] - 1, size=int(rng.integers(1, P + 1))).astype(np.int32) for _ in range(G)]
     forced = np.zeros((G, int(Kp.max())), np.int32)
     for i in range(G):
-        kind = rng.integers(0, 4)
-        if kind == 0:      # long tail, some beyond the limit (TRUNC)
+        pat = rng.integers(0, 4)                              # (not `kind`: that is the test's dtype parameter, used below)
+        if pat == 0:      # long tail, some beyond the limit (TRUNC)
             forced[i, :Kp[i]] = np.clip(np.round(rng.lognormal(1.6, 0.9, size=Kp[i])), 1, 4 * max_new)
-        elif kind == 1:    # many equal lengths: tie-breaks by sample index
+        elif pat == 1:    # many equal lengths: tie-breaks by sample index
             forced[i, :Kp[i]] = rng.choice([2, 3, max_new], size=Kp[i])
-        elif kind == 2:    # nobody is forced: natural EOS or the length limit only
+        elif pat == 2:    # nobody is forced: natural EOS or the length limit only
             forced[i, :Kp[i]] = 0
         else:              # fewer than K valid rows
             forced[i, :Kp[i]] = np.where(rng.random(Kp[i]) < 0.3, rng.integers(1, max_new + 1, size=Kp[i]), 10 * max_new)

@@ -159,6 +159,14 @@ def test_incremental_decode_equals_full_causal_forward():
             assert np.allclose(z, full[t], atol=1e-10), (kw, t)
 
 
+def test_forward_full_last_n_is_a_slice_of_the_full_result():
+    model = tiny_model(seed=13, norm_std=0.2)
+    tokens = np.array([5, 1, 9, 33, 2, 2, 18])
+    full = tr.forward_full(model, tokens)
+    assert np.array_equal(tr.forward_full(model, tokens, last=2), full[-2:])
+    assert np.array_equal(tr.forward_full(model, tokens, last=7), full)
+
+
 def test_zero_weights_give_uniform_logits():
     model = tiny_model(seed=7)
     model["lm_head"] = np.zeros((40, 32))
@@ -211,6 +219,70 @@ def test_moe_identical_experts_top3_equals_dense_and_scaled_experts_pin_the_gate
         top = np.argsort(p[t])[-k:]
         scale = float(np.sum(p[t, top] * c[top]) / np.sum(p[t, top]))
         assert np.allclose(tr.mlp(Lm, cfg, b[t:t + 1])[0], scale * base[t], atol=1e-11), t
+
+
+def test_teacher_forced_routing_hook_is_neutral_on_own_choice_and_reports_the_regret():
+    """oracle.transformer.ROUTE_OVERRIDE / ROUTE_REGRET (R13): forcing the oracle's OWN expert ids changes nothing and
+    reports zero regret; forcing a swapped expert gives the gates of the forced set (independent softmax) and the probability
+    difference of the swapped pair."""
+    from scipy.special import softmax as sp_softmax
+    model = tiny_model(seed=14, norm_std=0.2, n_experts=6, top_k=2, expert_ffn=16, ffn=0)
+    tokens = np.array([3, 9, 27, 1])
+    full = tr.forward_full(model, tokens)
+    own = []
+    orig = tr.moe_route
+    try:
+        tr.moe_route = lambda L, c, b: (lambda r: (own.append(r[0].copy()), r)[1])(orig(L, c, b))
+        assert np.array_equal(tr.forward_full(model, tokens), full)
+    finally:
+        tr.moe_route = orig
+    assert len(own) == 2 * 4
+    tr.ROUTE_OVERRIDE, tr.ROUTE_REGRET = iter(own), []
+    try:
+        assert np.array_equal(tr.forward_full(model, tokens), full)
+        assert tr.ROUTE_REGRET == [0.0] * 8
+    finally:
+        tr.ROUTE_OVERRIDE = tr.ROUTE_REGRET = None
+    L, cfg = model["layers"][0], model["cfg"]
+    b = np.random.default_rng(2).normal(size=cfg["d_model"])
+    p = sp_softmax(np.asarray(L["wr"], dtype=np.float64) @ b)
+    rank = np.argsort(-p)
+    forced = np.array([rank[0], rank[2]])                    # second choice swapped for the third
+    tr.ROUTE_OVERRIDE, tr.ROUTE_REGRET = iter([forced]), []
+    try:
+        ids, w = tr.moe_route(L, cfg, b)
+        assert ids.tolist() == forced.tolist() and np.allclose(w, p[forced] / p[forced].sum(), atol=1e-15)
+        assert abs(tr.ROUTE_REGRET[0] - (p[rank[1]] - p[rank[2]])) < 1e-15
+    finally:
+        tr.ROUTE_OVERRIDE = tr.ROUTE_REGRET = None
+
+
+def test_matched_rounding_hook_is_neutral_when_off_visits_the_documented_points_and_stays_close():
+    """oracle.transformer.ROUND: an identity hook reproduces the definition (to rounding order: the matched attention divides after
+    P.V); every layer visits the documented rounding points; bf16 rounding moves the logits by O(2^-9), and incremental == full still
+    holds under it."""
+    for kw in (dict(), dict(qk_norm=True), dict(n_experts=4, top_k=2, expert_ffn=24, ffn=0)):
+        model = tiny_model(seed=15, norm_std=0.2, **kw)
+        tokens = np.array([5, 1, 9, 33, 2, 2, 18, 7])
+        full = tr.forward_full(model, tokens)
+        seen = []
+        bf16 = lambda name, x: torch.from_numpy(np.ascontiguousarray(x)).to(torch.bfloat16).to(torch.float64).numpy()
+        try:
+            tr.ROUND = lambda name, x: (seen.append(name), x)[1]
+            assert np.allclose(tr.forward_full(model, tokens), full, rtol=0, atol=1e-12), kw
+            per_layer = {"xn", "q", "k", "v", "p", "ao", "xn2", "act"}
+            assert set(seen) == per_layer | {"xnf"} and seen.count("xn") == 2 and seen.count("xnf") == 1
+            tr.ROUND = bf16
+            zr = tr.forward_full(model, tokens)
+            err = np.max(np.abs(zr - full)) / np.max(np.abs(full))
+            assert 1e-4 < err < 3e-2, err
+            z0, kv0 = tr.prefill(model, tokens[:5])
+            kv = [(a.copy(), b.copy()) for a, b in kv0]
+            assert np.allclose(z0, zr[4], atol=1e-10)
+            for t in range(5, len(tokens)):
+                assert np.allclose(tr.decode_one(model, kv, tokens[t], t), zr[t], atol=1e-10), (kw, t)
+        finally:
+            tr.ROUND = None
 
 
 def test_moe_route_tie_prefers_lower_expert_id():
