@@ -82,7 +82,9 @@ enum { DARTS_MODE_AUTO = 0, DARTS_MODE_DUAL_END = 1, DARTS_MODE_SHORTEST_EARLY_S
 enum {
   DARTS_FLAG_DUMP_LOGITS = 1,       /* keep fp32 logits of every row of the last step for darts_debug_logits */
   DARTS_FLAG_NO_PREFIX_SHARING = 2, /* A/B switch: attention re-reads the prefix once per row, not per group */
-  DARTS_FLAG_PROFILE_ATTENTION = 4  /* bracket layer 0's attention of every decode step with CUDA events (bench roofline) */
+  DARTS_FLAG_PROFILE_ATTENTION = 4, /* bracket layer 0's attention of every decode step with CUDA events (bench roofline) */
+  DARTS_FLAG_DUMP_HIDDEN = 8        /* keep the fp32 residual stream of every layer boundary of the last pass for darts_debug_hidden
+                                     * ((n_layers + 1) x rows x d_model floats of workspace; parity only) */
 };
 
 typedef struct {
@@ -230,6 +232,11 @@ darts_status darts_debug_logits(darts_ctx *ctx, int32_t row, float *out_host);
 darts_status darts_debug_routing(darts_ctx *ctx, int32_t slot_begin, int32_t n_slots, int32_t *out_host);
 darts_status darts_debug_row_slots(darts_ctx *ctx, int32_t *slot_host, int32_t *step_host, int32_t n_rows);
 
+/* Parity hook for layer-by-layer comparison at full depth (DARTS_FLAG_DUMP_HIDDEN): the fp32 residual stream ENTERING layer
+ * `layer` (layer == n_layers: leaving the last layer, i.e. the input of the final norm) for slots [slot_begin, slot_begin + n_slots)
+ * of the most recent forward pass (slot numbering as in darts_debug_routing).  out: HOST [n_slots][d_model].  Synchronises. */
+darts_status darts_debug_hidden(darts_ctx *ctx, int32_t layer, int32_t slot_begin, int32_t n_slots, float *out_host);
+
 /* Teacher forcing for parity at bf16 (R12): overwrite the token the next decode step feeds
  * for global row `row`.  tokens: HOST [n_rows] (-1 = leave). */
 darts_status darts_debug_set_last_tokens(darts_ctx *ctx, const int32_t *tokens_host, int32_t n_rows);
@@ -244,6 +251,13 @@ darts_status darts_debug_set_last_tokens(darts_ctx *ctx, const int32_t *tokens_h
 darts_status darts_debug_gemm_scratch_floats(darts_ctx *ctx, int32_t rows, int32_t N, int32_t K, int32_t split_k, size_t *out);
 darts_status darts_debug_gemm_bf16(darts_ctx *ctx, const void *X, const void *W, float *C, float *scratch, int32_t rows,
                                    int32_t N, int32_t K, int32_t split_k);
+
+/* Parity hook for the gate/up projection with its fused SwiGLU epilogue: act[rows][F] (bf16) =
+ * silu(X Wg^T) * (X Wu^T) with Wgu = [Wg ; Wu] stacked on rows, [2F][K] bf16, X [rows][K] bf16; fp32 accumulate, one rounding at the
+ * store.  scratch: darts_debug_gemm_scratch_floats(rows, 2F, K, 0) floats.  Needs F % 64 == 0, K % 64 == 0.  All pointers DEVICE;
+ * asynchronous on the ctx stream. */
+darts_status darts_debug_swiglu_bf16(darts_ctx *ctx, const void *X, const void *Wgu, void *act_out, float *scratch, int32_t rows, int32_t F,
+                                     int32_t K);
 
 /* ---- Adaptive redundancy allocation (§4.2.2; App. B Eq. 6-9 :384-411; App. C Alg. 1 :413-462) --------
  * Host-only helpers for the step upstream of the rollout: per-prompt length variances (darts_results.len_var) -> EMA ->

@@ -178,6 +178,21 @@ def logits_from_hidden(model, h):
     return _r("xnf", rmsnorm(h, model["final_norm"], cfg["rms_eps"])) @ f64(model["lm_head"]).T
 
 
+def layer_forward(layer, cfg, h, pos):
+    """One decoder layer over a whole causal sequence: h [T, d] entering the layer at positions pos [T] -> (h leaving it, k, v).
+    (The body of forward_full's loop, callable on its own so that a test can feed it a given residual stream layer by layer.)"""
+    T = h.shape[0]
+    a = _r("xn", rmsnorm(h, layer["attn_norm"], cfg["rms_eps"]))
+    q, k, v = qkv_project(layer, cfg, a, pos)
+    o = np.empty((T, cfg["n_q_heads"], cfg["head_dim"]))
+    for t in range(T):                                       # causal: position t sees keys 0..t
+        o[t] = attention_one(q[t], k[: t + 1], v[: t + 1], cfg["n_kv_heads"])
+    h = h + _r("ao", o.reshape(T, -1)) @ f64(layer["wo"]).T
+    b = rmsnorm(h, layer["mlp_norm"], cfg["rms_eps"])
+    h = h + mlp(layer, cfg, b)
+    return h, k, v
+
+
 def forward_full(model, tokens, return_kv=False, last=None):
     """THE DEFINITION: causal forward over tokens [T] -> logits [T, V] (and per-layer K,V).
     last = n returns the logits of the last n positions only ([n, V]; the rows of the full result, nothing else
@@ -189,14 +204,7 @@ def forward_full(model, tokens, return_kv=False, last=None):
     h = f64(model["embed"])[tokens]                          # [T, d]
     kv = []
     for layer in model["layers"]:
-        a = _r("xn", rmsnorm(h, layer["attn_norm"], cfg["rms_eps"]))
-        q, k, v = qkv_project(layer, cfg, a, pos)
-        o = np.empty((T, cfg["n_q_heads"], cfg["head_dim"]))
-        for t in range(T):                                   # causal: position t sees keys 0..t
-            o[t] = attention_one(q[t], k[: t + 1], v[: t + 1], cfg["n_kv_heads"])
-        h = h + _r("ao", o.reshape(T, -1)) @ f64(layer["wo"]).T
-        b = rmsnorm(h, layer["mlp_norm"], cfg["rms_eps"])
-        h = h + mlp(layer, cfg, b)
+        h, k, v = layer_forward(layer, cfg, h, pos)
         kv.append((k, v))
     logits = logits_from_hidden(model, h if last is None else h[T - last:])
     return (logits, kv) if return_kv else logits

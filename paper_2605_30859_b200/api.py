@@ -22,7 +22,7 @@ OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_KV_POOL_EXHAUSTED, ERR_WORKSPACE_TOO_S
 F32, BF16 = 0, 1
 ROW_ACTIVE, ROW_VALID, ROW_TRUNC, ROW_PRUNED = 0, 1, 2, 3
 MODE_AUTO, MODE_DUAL_END, MODE_SHORTEST_EARLY_STOP = 0, 1, 2
-FLAG_DUMP_LOGITS, FLAG_NO_PREFIX_SHARING, FLAG_PROFILE_ATTENTION = 1, 2, 4
+FLAG_DUMP_LOGITS, FLAG_NO_PREFIX_SHARING, FLAG_PROFILE_ATTENTION, FLAG_DUMP_HIDDEN = 1, 2, 4, 8
 
 _vp, _i32, _u32, _u64, _f32 = C.c_void_p, C.c_int32, C.c_uint32, C.c_uint64, C.c_float
 _pp = C.POINTER(C.c_void_p)
@@ -84,9 +84,11 @@ darts_n_active = _sig("darts_n_active", _ctx, C.POINTER(_i32))
 darts_get_attention_times = _sig("darts_get_attention_times", _ctx, _vp, _i32, C.POINTER(_i32))
 darts_debug_logits = _sig("darts_debug_logits", _ctx, _i32, _vp)
 darts_debug_routing = _sig("darts_debug_routing", _ctx, _i32, _i32, _vp)
+darts_debug_hidden = _sig("darts_debug_hidden", _ctx, _i32, _i32, _i32, _vp)
 darts_debug_row_slots = _sig("darts_debug_row_slots", _ctx, _vp, _vp, _i32)
 darts_debug_set_last_tokens = _sig("darts_debug_set_last_tokens", _ctx, _vp, _i32)
 darts_debug_gemm_bf16 = _sig("darts_debug_gemm_bf16", _ctx, _vp, _vp, _vp, _vp, _i32, _i32, _i32, _i32)
+darts_debug_swiglu_bf16 = _sig("darts_debug_swiglu_bf16", _ctx, _vp, _vp, _vp, _vp, _i32, _i32, _i32)
 darts_debug_gemm_scratch_floats = _sig("darts_debug_gemm_scratch_floats", _ctx, _i32, _i32, _i32, _i32, C.POINTER(C.c_size_t))
 darts_update_variance_ema = _sig("darts_update_variance_ema", _vp, _vp, _i32, _f32)
 darts_redundancy_budget = _sig("darts_redundancy_budget", C.c_double, C.c_double, C.c_double, _i32, _i32, C.POINTER(C.c_int64))
@@ -319,6 +321,13 @@ class Darts:
         self._check(darts_debug_routing(self.ctx, slot_begin, n_slots, _np_ptr(out)))
         return out
 
+    def debug_hidden(self, slot_begin, n_slots):
+        """fp32 residual stream [n_layers + 1, n_slots, d_model] at every layer boundary of the most recent pass (FLAG_DUMP_HIDDEN)."""
+        out = np.empty((self.cfg["n_layers"] + 1, n_slots, self.cfg["d_model"]), np.float32)
+        for b in range(self.cfg["n_layers"] + 1):
+            self._check(darts_debug_hidden(self.ctx, b, slot_begin, n_slots, _np_ptr(out[b])))
+        return out
+
     def debug_row_slots(self):
         """(slot, step) of every row's last decode step."""
         slot, step = np.empty(self.R, np.int32), np.empty(self.R, np.int32)
@@ -343,6 +352,18 @@ class Darts:
                                           rows, N, K, split_k))
         self._scratch = scratch
         return out if reduce else scratch
+
+    def debug_swiglu_bf16(self, X, Wgu):
+        """act = silu(X Wg^T) * (X Wu^T) on the gate/up GEMM with the fused epilogue (bf16 device tensors X [rows,K], Wgu [2F,K]); bf16 [rows,F]."""
+        rows, K = X.shape
+        F = Wgu.shape[0] // 2
+        need = C.c_size_t()
+        self._check(darts_debug_gemm_scratch_floats(self.ctx, rows, 2 * F, K, 0, C.byref(need)))
+        scratch = torch.empty(need.value, dtype=torch.float32, device="cuda")
+        out = torch.empty(rows, F, dtype=torch.bfloat16, device="cuda")
+        self._check(darts_debug_swiglu_bf16(self.ctx, X.data_ptr(), Wgu.data_ptr(), out.data_ptr(), scratch.data_ptr(), rows, F, K))
+        self._scratch = scratch
+        return out
 
     # ---- attention-only (config 2) -----------------------------------------------------------------
     def attn_load(self, G, P, Kp, k_prefix, v_prefix, suffix_len, k_suffix, v_suffix):

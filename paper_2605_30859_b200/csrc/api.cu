@@ -79,6 +79,8 @@ size_t carve(darts_ctx *c, void *base) {
   c->slot_npre = k.take<int32_t>(A);
   c->slot_nsuf = k.take<int32_t>(A);
   c->forced_stage = k.take<int32_t>(G * DARTS_MAX_KP);
+  c->sk_flags_n = 4096;                                      // tile arrival counters of the fused stream-K epilogues (also used by the debug GEMM hooks)
+  c->sk_flags = k.take<int32_t>(c->sk_flags_n);
   if (attention_sm100_supported(c)) {
     size_t npc_max = (size_t)ceil_div(rt.max_prompt_len, ATTN_CHUNK_TOKENS);
     size_t max_parts = R * (npc_max + 2) + (size_t)rt.n_pages / ATTN_CHUNK_PAGES + 16;
@@ -106,6 +108,7 @@ size_t carve(darts_ctx *c, void *base) {
     c->prompt_tokens = k.take<int32_t>(G * rt.max_prompt_len);
     c->slot_cs = k.take<float2>(A * (m.head_dim / 2));
     c->h = k.take<float>(A * m.d_model);
+    if (rt.flags & DARTS_FLAG_DUMP_HIDDEN) c->hid_dump = k.take<float>((size_t)(m.n_layers + 1) * A * m.d_model);
     if (m.n_experts) {
       size_t RK = A * m.top_k;
       c->moe_logits = k.take<float>(A * m.n_experts);
@@ -124,7 +127,12 @@ size_t carve(darts_ctx *c, void *base) {
       int shapes[4][2] = {{c->n_qkv, m.d_model}, {m.d_model, qd_}, {m.n_experts ? 0 : 2 * m.ffn, m.d_model}, {m.n_experts ? 0 : m.d_model, m.ffn}};
       for (auto &sh : shapes)
         if (sh[0] > 0) {
-          dec = std::max(dec, (size_t)sk_plan(sms, sh[0], sh[1], rt.max_rows, 0, false).slots * R * sh[0] * 4);
+          // a decode step re-plans with the host's current row bound: the slot count grows as the row blocks get fewer, so take
+          // the largest footprint over every row-block count the context can see (launch_gemm_sk re-checks at launch)
+          for (int rows = SK_ROWBLOCK; rows < rt.max_rows + SK_ROWBLOCK; rows += SK_ROWBLOCK) {
+            const size_t r = (size_t)std::min(rows, rt.max_rows);
+            dec = std::max(dec, (size_t)sk_plan(sms, sh[0], sh[1], (int)r, 0, false).slots * r * sh[0] * 4);
+          }
           dec = std::max(dec, (size_t)sk_plan(sms, sh[0], sh[1], (int)A, 0, true).slots * A * sh[0] * 4);
         }
       c->part_bytes = std::max<size_t>(std::max<size_t>(A * maxN * 4, dec), (size_t)64 << 20);
@@ -198,10 +206,19 @@ const void **dup_ptrs(const void *const *src, int n) {
 
 #define TRY(x) do { darts_status s__ = (x); if (s__ != DARTS_OK) return s__; } while (0)
 
+// Parity hook: keep the residual stream at a layer boundary (boundary b = input of layer b; b = n_layers: output of the last layer).
+darts_status dump_hidden(darts_ctx *c, int boundary, int rows_ub) {
+  if (!c->hid_dump) return DARTS_OK;
+  CUDA_TRY(c, cudaMemcpyAsync(c->hid_dump + (size_t)boundary * c->act_rows * c->m.d_model, c->h, (size_t)rows_ub * c->m.d_model * sizeof(float),
+                              cudaMemcpyDeviceToDevice, c->stream));
+  return DARTS_OK;
+}
+
 // One transformer pass over `rows` slots whose plan (slot_*) is already on the device.
 darts_status forward_layers(darts_ctx *c, int rows_ub, const int32_t *n_rows_dev) {
   const darts_model_desc &m = c->m;
   TRY(launch_embed(c, c->slot_tok, 0, rows_ub, n_rows_dev));
+  TRY(dump_hidden(c, 0, rows_ub));
   TRY(launch_rope_table(c, rows_ub, n_rows_dev));
   int qd = m.n_q_heads * m.head_dim;
   for (int l = 0; l < m.n_layers; ++l) {
@@ -218,6 +235,7 @@ darts_status forward_layers(darts_ctx *c, int rows_ub, const int32_t *n_rows_dev
     } else {
       TRY(launch_moe(c, l, rows_ub, n_rows_dev));
     }
+    TRY(dump_hidden(c, l + 1, rows_ub));
   }
   return DARTS_OK;
 }
@@ -237,6 +255,7 @@ darts_status forward_layers_tc(darts_ctx *c, int rows_ub, const int32_t *n_rows_
   const int d = m.d_model, qd = m.n_q_heads * m.head_dim, F = m.ffn, L = m.n_layers;
   TRY(launch_moe_begin_pass(c));
   TRY(launch_embed_norm_rope(c, c->slot_tok, c->attn_norm[0], rows_ub, n_rows_dev));     // embedding, first RMSNorm, RoPE table: one launch
+  TRY(dump_hidden(c, 0, rows_ub));
   // DARTS_SKIP (profiling aid): bit k drops the k-th kernel class of every layer so that the change of the step time gives that class's
   // LIVE cost (launch-list times are serialised and cold); results are garbage in that mode.
   const unsigned sk = c->skip_mask;
@@ -250,15 +269,22 @@ darts_status forward_layers_tc(darts_ctx *c, int rows_ub, const int32_t *n_rows_
     if (!(sk & 32)) TRY(launch_add_rmsnorm_sk(c, sk_view(g), c->mlp_norm[l], rows_ub, n_rows_dev));
     const void *next_norm = l + 1 < L ? c->attn_norm[l + 1] : c->final_norm;
     if (m.n_experts == 0) {
-      g = sk_gemm(c, &c->xm_xn, &c->tm_wgu[l], 2 * F, d, rows_ub, n_rows_dev);
-      if (!(sk & 64)) TRY(launch_gemm_sk(c, g));
-      if (!(sk & 128)) TRY(launch_silu_mul_sk(c, sk_view(g), rows_ub, n_rows_dev));
+      if (c->tm_wgu64) {                                      // SwiGLU in the GEMM's epilogue: act leaves the kernel in bf16
+        g = sk_gemm(c, &c->xm_xn, &c->tm_wgu64[l], 2 * F, d, rows_ub, n_rows_dev);
+        g.epi = SK_GEMM_SILU; g.act_out = c->act;
+        if (!(sk & 64)) TRY(launch_gemm_sk(c, g));
+      } else {
+        g = sk_gemm(c, &c->xm_xn, &c->tm_wgu[l], 2 * F, d, rows_ub, n_rows_dev);
+        if (!(sk & 64)) TRY(launch_gemm_sk(c, g));
+        if (!(sk & 128)) TRY(launch_silu_mul_sk(c, sk_view(g), rows_ub, n_rows_dev));
+      }
       g = sk_gemm(c, &c->xm_act, &c->tm_wd[l], d, F, rows_ub, n_rows_dev);
       if (!(sk & 256)) TRY(launch_gemm_sk(c, g));
       if (!(sk & 512)) TRY(launch_add_rmsnorm_sk(c, sk_view(g), next_norm, rows_ub, n_rows_dev));
     } else {
       TRY(launch_moe_tc(c, l, next_norm, rows_ub, n_rows_dev));
     }
+    TRY(dump_hidden(c, l + 1, rows_ub));
   }
   return DARTS_OK;
 }
@@ -275,13 +301,14 @@ darts_status make_maps(darts_ctx *c) {
   const darts_model_desc &m = c->m;
   const int d = m.d_model, qd = m.n_q_heads * m.head_dim, L = m.n_layers;
   c->tm_wqkv = new CUtensorMap[L]; c->tm_wo = new CUtensorMap[L];
-  if (m.n_experts == 0) { c->tm_wgu = new CUtensorMap[L]; c->tm_wd = new CUtensorMap[L]; }
+  if (m.n_experts == 0) { c->tm_wgu = new CUtensorMap[L]; c->tm_wd = new CUtensorMap[L]; if (m.ffn % 64 == 0) c->tm_wgu64 = new CUtensorMap[L]; }
   else { c->tm_wgu_e = new CUtensorMap[L]; c->tm_wd_e = new CUtensorMap[L]; }
   for (int l = 0; l < L; ++l) {
     TRY(tc_make_map(c, &c->tm_wqkv[l], c->wqkv[l], c->n_qkv, d, 128));
     TRY(tc_make_map(c, &c->tm_wo[l], c->wo[l], d, qd, 128));
     if (m.n_experts == 0) {
       TRY(tc_make_map(c, &c->tm_wgu[l], c->wgu[l], 2 * m.ffn, d, 128));
+      if (c->tm_wgu64) TRY(tc_make_map(c, &c->tm_wgu64[l], c->wgu[l], 2 * m.ffn, d, 64));
       TRY(tc_make_map(c, &c->tm_wd[l], c->wd[l], d, m.ffn, 128));
     } else {
       TRY(tc_make_map(c, &c->tm_wgu_e[l], c->wgu_e[l], (long long)m.n_experts * 2 * m.expert_ffn, d, 128));
@@ -466,6 +493,7 @@ darts_status darts_create(const darts_model_desc *m, const darts_weights *w, con
   CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev[1], cudaEventDisableTiming));
   CUDA_TRY(c, cudaMemsetAsync(c->st, 0, sizeof(DevState), c->stream));
   if (c->moe_arrive) CUDA_TRY(c, cudaMemsetAsync(c->moe_arrive, 0, c->moe_arrive_n * sizeof(int32_t), c->stream));
+  if (c->sk_flags) CUDA_TRY(c, cudaMemsetAsync(c->sk_flags, 0, c->sk_flags_n * sizeof(int32_t), c->stream));
   // The pool must hold finite values everywhere: a partially filled page is multiplied by zero probabilities.
   CUDA_TRY(c, cudaMemsetAsync(c->kv_pool, 0, (size_t)m->n_layers * c->kv_layer_elems * c->elt, c->stream));
   return DARTS_OK;
@@ -485,7 +513,7 @@ darts_status darts_destroy(darts_ctx *c) {
   }
   const void **arrs[] = {c->attn_norm, c->wqkv, c->q_norm, c->k_norm, c->wo, c->mlp_norm, c->wgu, c->wd, c->wr, c->wgu_e, c->wd_e};
   for (auto a : arrs) delete[] a;
-  CUtensorMap *maps[] = {c->tm_wqkv, c->tm_wo, c->tm_wgu, c->tm_wd, c->tm_wgu_e, c->tm_wd_e};
+  CUtensorMap *maps[] = {c->tm_wqkv, c->tm_wo, c->tm_wgu, c->tm_wd, c->tm_wgu_e, c->tm_wd_e, c->tm_wgu64};
   for (auto a : maps) delete[] a;
   delete c;
   return DARTS_OK;
@@ -759,6 +787,16 @@ darts_status darts_debug_routing(darts_ctx *c, int32_t slot_begin, int32_t n_slo
   return DARTS_OK;
 }
 
+darts_status darts_debug_hidden(darts_ctx *c, int32_t layer, int32_t slot_begin, int32_t n_slots, float *out_host) {
+  if (!c || !out_host) return DARTS_ERR_INVALID_ARG;
+  if (!c->hid_dump) FAIL(c, DARTS_ERR_BAD_STATE, "the residual stream is kept only by a context created with DARTS_FLAG_DUMP_HIDDEN");
+  if (layer < 0 || layer > c->m.n_layers || slot_begin < 0 || n_slots <= 0 || slot_begin + n_slots > c->act_rows) FAIL(c, DARTS_ERR_INVALID_ARG, "bad layer / slot range");
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  CUDA_TRY(c, cudaMemcpy(out_host, c->hid_dump + ((size_t)layer * c->act_rows + slot_begin) * c->m.d_model, (size_t)n_slots * c->m.d_model * sizeof(float),
+                         cudaMemcpyDeviceToHost));
+  return DARTS_OK;
+}
+
 darts_status darts_debug_row_slots(darts_ctx *c, int32_t *slot_host, int32_t *step_host, int32_t n_rows) {
   if (!c || !slot_host || !step_host) return DARTS_ERR_INVALID_ARG;
   if (!c->prefilled || n_rows != c->R) FAIL(c, DARTS_ERR_INVALID_ARG, "n_rows must equal the rollout's row count");
@@ -812,6 +850,22 @@ darts_status darts_debug_gemm_bf16(darts_ctx *c, const void *X, const void *W, f
   TRY(launch_gemm_tc(c, g));
   if (!C) return DARTS_OK;                                   // partials only (timing the GEMM kernel alone)
   return launch_sum_partials(c, scratch, C, split_k, (size_t)rows * N);
+}
+
+darts_status darts_debug_swiglu_bf16(darts_ctx *c, const void *X, const void *Wgu, void *act_out, float *scratch, int32_t rows, int32_t F, int32_t K) {
+  if (!c) return DARTS_ERR_INVALID_ARG;
+  if (c->sticky) return c->sticky;
+  if (!X || !Wgu || !act_out || !scratch || rows <= 0 || F <= 0 || K <= 0) FAIL(c, DARTS_ERR_INVALID_ARG, "NULL / non-positive argument");
+  if (F % 64 || !tc_shape_ok(2 * F, K)) FAIL(c, DARTS_ERR_UNSUPPORTED, "fused SwiGLU needs F %% 64 == 0, K %% 64 == 0");
+  CUtensorMap tw;
+  XMaps xm;
+  TRY(tc_make_xmaps(c, &xm, X, rows, K));
+  TRY(tc_make_map(c, &tw, Wgu, 2 * F, K, 64));
+  SkGemm g{};
+  g.epi = SK_GEMM_SILU; g.act_out = act_out;
+  g.w_map = &tw; g.x_maps = &xm; g.C = scratch; g.N = 2 * F; g.rows_ub = rows; g.slot_stride = (size_t)rows * 2 * F;
+  g.plan = sk_plan(c->n_sms, 2 * F, K, rows, 0, true);
+  return launch_gemm_sk(c, g);
 }
 
 darts_status darts_attn_load(darts_ctx *c, int32_t G, int32_t P, int32_t Kp, const void *k_prefix, const void *v_prefix,

@@ -122,12 +122,12 @@ class HostWeights:
         self.shape = tuple(self.t.shape)
 
     def __array__(self, dtype=None, copy=None):
-        return self.t.cpu().to(torch.float64).numpy()
+        return self.t.to(torch.float64).cpu().numpy()          # exact widening where the tensor lives, then one copy
 
     def __getitem__(self, idx):
         if isinstance(idx, np.ndarray):
             idx = torch.from_numpy(idx.astype(np.int64)).to(self.t.device)
-        return self.t[idx].cpu().to(torch.float64).numpy()
+        return self.t[idx].to(torch.float64).cpu().numpy()
 
     def __len__(self):
         return self.shape[0]
