@@ -252,13 +252,6 @@ darts_status darts_debug_gemm_scratch_floats(darts_ctx *ctx, int32_t rows, int32
 darts_status darts_debug_gemm_bf16(darts_ctx *ctx, const void *X, const void *W, float *C, float *scratch, int32_t rows,
                                    int32_t N, int32_t K, int32_t split_k);
 
-/* Parity hook for the gate/up projection with its fused SwiGLU epilogue: act[rows][F] (bf16) =
- * silu(X Wg^T) * (X Wu^T) with Wgu = [Wg ; Wu] stacked on rows, [2F][K] bf16, X [rows][K] bf16; fp32 accumulate, one rounding at the
- * store.  scratch: darts_debug_gemm_scratch_floats(rows, 2F, K, 0) floats.  Needs F % 64 == 0, K % 64 == 0.  All pointers DEVICE;
- * asynchronous on the ctx stream. */
-darts_status darts_debug_swiglu_bf16(darts_ctx *ctx, const void *X, const void *Wgu, void *act_out, float *scratch, int32_t rows, int32_t F,
-                                     int32_t K);
-
 /* ---- Adaptive redundancy allocation (§4.2.2; App. B Eq. 6-9 :384-411; App. C Alg. 1 :413-462) --------
  * Host-only helpers for the step upstream of the rollout: per-prompt length variances (darts_results.len_var) -> EMA ->
  * total budget -> greedy plan Kp[G] for the next darts_prefill.  All pointers HOST.  No context, no GPU work.

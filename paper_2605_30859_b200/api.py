@@ -88,7 +88,6 @@ darts_debug_hidden = _sig("darts_debug_hidden", _ctx, _i32, _i32, _i32, _vp)
 darts_debug_row_slots = _sig("darts_debug_row_slots", _ctx, _vp, _vp, _i32)
 darts_debug_set_last_tokens = _sig("darts_debug_set_last_tokens", _ctx, _vp, _i32)
 darts_debug_gemm_bf16 = _sig("darts_debug_gemm_bf16", _ctx, _vp, _vp, _vp, _vp, _i32, _i32, _i32, _i32)
-darts_debug_swiglu_bf16 = _sig("darts_debug_swiglu_bf16", _ctx, _vp, _vp, _vp, _vp, _i32, _i32, _i32)
 darts_debug_gemm_scratch_floats = _sig("darts_debug_gemm_scratch_floats", _ctx, _i32, _i32, _i32, _i32, C.POINTER(C.c_size_t))
 darts_update_variance_ema = _sig("darts_update_variance_ema", _vp, _vp, _i32, _f32)
 darts_redundancy_budget = _sig("darts_redundancy_budget", C.c_double, C.c_double, C.c_double, _i32, _i32, C.POINTER(C.c_int64))
@@ -352,18 +351,6 @@ class Darts:
                                           rows, N, K, split_k))
         self._scratch = scratch
         return out if reduce else scratch
-
-    def debug_swiglu_bf16(self, X, Wgu):
-        """act = silu(X Wg^T) * (X Wu^T) on the gate/up GEMM with the fused epilogue (bf16 device tensors X [rows,K], Wgu [2F,K]); bf16 [rows,F]."""
-        rows, K = X.shape
-        F = Wgu.shape[0] // 2
-        need = C.c_size_t()
-        self._check(darts_debug_gemm_scratch_floats(self.ctx, rows, 2 * F, K, 0, C.byref(need)))
-        scratch = torch.empty(need.value, dtype=torch.float32, device="cuda")
-        out = torch.empty(rows, F, dtype=torch.bfloat16, device="cuda")
-        self._check(darts_debug_swiglu_bf16(self.ctx, X.data_ptr(), Wgu.data_ptr(), out.data_ptr(), scratch.data_ptr(), rows, F, K))
-        self._scratch = scratch
-        return out
 
     # ---- attention-only (config 2) -----------------------------------------------------------------
     def attn_load(self, G, P, Kp, k_prefix, v_prefix, suffix_len, k_suffix, v_suffix):

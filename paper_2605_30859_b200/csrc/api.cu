@@ -79,8 +79,6 @@ size_t carve(darts_ctx *c, void *base) {
   c->slot_npre = k.take<int32_t>(A);
   c->slot_nsuf = k.take<int32_t>(A);
   c->forced_stage = k.take<int32_t>(G * DARTS_MAX_KP);
-  c->sk_flags_n = 4096;                                      // tile arrival counters of the fused stream-K epilogues (also used by the debug GEMM hooks)
-  c->sk_flags = k.take<int32_t>(c->sk_flags_n);
   if (attention_sm100_supported(c)) {
     size_t npc_max = (size_t)ceil_div(rt.max_prompt_len, ATTN_CHUNK_TOKENS);
     size_t max_parts = R * (npc_max + 2) + (size_t)rt.n_pages / ATTN_CHUNK_PAGES + 16;
@@ -269,15 +267,9 @@ darts_status forward_layers_tc(darts_ctx *c, int rows_ub, const int32_t *n_rows_
     if (!(sk & 32)) TRY(launch_add_rmsnorm_sk(c, sk_view(g), c->mlp_norm[l], rows_ub, n_rows_dev));
     const void *next_norm = l + 1 < L ? c->attn_norm[l + 1] : c->final_norm;
     if (m.n_experts == 0) {
-      if (c->tm_wgu64) {                                      // SwiGLU in the GEMM's epilogue: act leaves the kernel in bf16
-        g = sk_gemm(c, &c->xm_xn, &c->tm_wgu64[l], 2 * F, d, rows_ub, n_rows_dev);
-        g.epi = SK_GEMM_SILU; g.act_out = c->act;
-        if (!(sk & 64)) TRY(launch_gemm_sk(c, g));
-      } else {
-        g = sk_gemm(c, &c->xm_xn, &c->tm_wgu[l], 2 * F, d, rows_ub, n_rows_dev);
-        if (!(sk & 64)) TRY(launch_gemm_sk(c, g));
-        if (!(sk & 128)) TRY(launch_silu_mul_sk(c, sk_view(g), rows_ub, n_rows_dev));
-      }
+      g = sk_gemm(c, &c->xm_xn, &c->tm_wgu[l], 2 * F, d, rows_ub, n_rows_dev);
+      if (!(sk & 64)) TRY(launch_gemm_sk(c, g));
+      if (!(sk & 128)) TRY(launch_silu_mul_sk(c, sk_view(g), rows_ub, n_rows_dev));
       g = sk_gemm(c, &c->xm_act, &c->tm_wd[l], d, F, rows_ub, n_rows_dev);
       if (!(sk & 256)) TRY(launch_gemm_sk(c, g));
       if (!(sk & 512)) TRY(launch_add_rmsnorm_sk(c, sk_view(g), next_norm, rows_ub, n_rows_dev));
@@ -301,14 +293,13 @@ darts_status make_maps(darts_ctx *c) {
   const darts_model_desc &m = c->m;
   const int d = m.d_model, qd = m.n_q_heads * m.head_dim, L = m.n_layers;
   c->tm_wqkv = new CUtensorMap[L]; c->tm_wo = new CUtensorMap[L];
-  if (m.n_experts == 0) { c->tm_wgu = new CUtensorMap[L]; c->tm_wd = new CUtensorMap[L]; if (m.ffn % 64 == 0) c->tm_wgu64 = new CUtensorMap[L]; }
+  if (m.n_experts == 0) { c->tm_wgu = new CUtensorMap[L]; c->tm_wd = new CUtensorMap[L]; }
   else { c->tm_wgu_e = new CUtensorMap[L]; c->tm_wd_e = new CUtensorMap[L]; }
   for (int l = 0; l < L; ++l) {
     TRY(tc_make_map(c, &c->tm_wqkv[l], c->wqkv[l], c->n_qkv, d, 128));
     TRY(tc_make_map(c, &c->tm_wo[l], c->wo[l], d, qd, 128));
     if (m.n_experts == 0) {
       TRY(tc_make_map(c, &c->tm_wgu[l], c->wgu[l], 2 * m.ffn, d, 128));
-      if (c->tm_wgu64) TRY(tc_make_map(c, &c->tm_wgu64[l], c->wgu[l], 2 * m.ffn, d, 64));
       TRY(tc_make_map(c, &c->tm_wd[l], c->wd[l], d, m.ffn, 128));
     } else {
       TRY(tc_make_map(c, &c->tm_wgu_e[l], c->wgu_e[l], (long long)m.n_experts * 2 * m.expert_ffn, d, 128));
@@ -493,7 +484,6 @@ darts_status darts_create(const darts_model_desc *m, const darts_weights *w, con
   CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev[1], cudaEventDisableTiming));
   CUDA_TRY(c, cudaMemsetAsync(c->st, 0, sizeof(DevState), c->stream));
   if (c->moe_arrive) CUDA_TRY(c, cudaMemsetAsync(c->moe_arrive, 0, c->moe_arrive_n * sizeof(int32_t), c->stream));
-  if (c->sk_flags) CUDA_TRY(c, cudaMemsetAsync(c->sk_flags, 0, c->sk_flags_n * sizeof(int32_t), c->stream));
   // The pool must hold finite values everywhere: a partially filled page is multiplied by zero probabilities.
   CUDA_TRY(c, cudaMemsetAsync(c->kv_pool, 0, (size_t)m->n_layers * c->kv_layer_elems * c->elt, c->stream));
   return DARTS_OK;
@@ -513,7 +503,7 @@ darts_status darts_destroy(darts_ctx *c) {
   }
   const void **arrs[] = {c->attn_norm, c->wqkv, c->q_norm, c->k_norm, c->wo, c->mlp_norm, c->wgu, c->wd, c->wr, c->wgu_e, c->wd_e};
   for (auto a : arrs) delete[] a;
-  CUtensorMap *maps[] = {c->tm_wqkv, c->tm_wo, c->tm_wgu, c->tm_wd, c->tm_wgu_e, c->tm_wd_e, c->tm_wgu64};
+  CUtensorMap *maps[] = {c->tm_wqkv, c->tm_wo, c->tm_wgu, c->tm_wd, c->tm_wgu_e, c->tm_wd_e};
   for (auto a : maps) delete[] a;
   delete c;
   return DARTS_OK;
@@ -850,22 +840,6 @@ darts_status darts_debug_gemm_bf16(darts_ctx *c, const void *X, const void *W, f
   TRY(launch_gemm_tc(c, g));
   if (!C) return DARTS_OK;                                   // partials only (timing the GEMM kernel alone)
   return launch_sum_partials(c, scratch, C, split_k, (size_t)rows * N);
-}
-
-darts_status darts_debug_swiglu_bf16(darts_ctx *c, const void *X, const void *Wgu, void *act_out, float *scratch, int32_t rows, int32_t F, int32_t K) {
-  if (!c) return DARTS_ERR_INVALID_ARG;
-  if (c->sticky) return c->sticky;
-  if (!X || !Wgu || !act_out || !scratch || rows <= 0 || F <= 0 || K <= 0) FAIL(c, DARTS_ERR_INVALID_ARG, "NULL / non-positive argument");
-  if (F % 64 || !tc_shape_ok(2 * F, K)) FAIL(c, DARTS_ERR_UNSUPPORTED, "fused SwiGLU needs F %% 64 == 0, K %% 64 == 0");
-  CUtensorMap tw;
-  XMaps xm;
-  TRY(tc_make_xmaps(c, &xm, X, rows, K));
-  TRY(tc_make_map(c, &tw, Wgu, 2 * F, K, 64));
-  SkGemm g{};
-  g.epi = SK_GEMM_SILU; g.act_out = act_out;
-  g.w_map = &tw; g.x_maps = &xm; g.C = scratch; g.N = 2 * F; g.rows_ub = rows; g.slot_stride = (size_t)rows * 2 * F;
-  g.plan = sk_plan(c->n_sms, 2 * F, K, rows, 0, true);
-  return launch_gemm_sk(c, g);
 }
 
 darts_status darts_attn_load(darts_ctx *c, int32_t G, int32_t P, int32_t Kp, const void *k_prefix, const void *v_prefix,

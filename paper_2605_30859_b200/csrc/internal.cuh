@@ -98,12 +98,9 @@ struct darts_ctx {
   bool use_pdl;                  // launch the stream-K GEMMs as programmatic dependents (DARTS_NO_PDL=1 in the environment disables)
   float *part;                   // [S][rows][N] fp32 partials of the GEMM in flight
   size_t part_bytes;
-  int32_t *sk_flags;             // per-tile arrival counters of the fused stream-K epilogues (zero between launches)
-  size_t sk_flags_n;
   float *top2;                   // float4 [vocab tiles][max_rows]
   float *lse;                    // float2 [vocab tiles][max_rows]
   CUtensorMap *tm_wqkv, *tm_wo, *tm_wgu, *tm_wd, *tm_wgu_e, *tm_wd_e;   // host arrays [n_layers]
-  CUtensorMap *tm_wgu64;                                                 // wgu again with 64-row boxes (fused SwiGLU epilogue); NULL if ffn % 64
   CUtensorMap tm_lm, tm_xn, tm_ao, tm_act, tm_xs, tm_hl;                      // activations: 16-row boxes
   XMaps xm_xn, xm_ao, xm_act, xm_xs;                                            // the same matrices for the stream-K kernel
   // MoE (kernels_moe.cu)
@@ -242,10 +239,7 @@ bool tc_shape_ok(int N, int K);
 // stream-K weight-streaming GEMM (kernels_gemm_sk.cu)
 #define SK_ROWBLOCK 256            // activation rows per MMA N block
 struct SkPlan { int nkb, n_wtiles, P, unit_tile, slots, stage_bytes, n_stages, tm_cols, n_acc; };   // stage / TMEM fields: grouped mode only
-enum { SK_GEMM_PIECES = 0, SK_GEMM_SILU = 2 };   // epilogue of a stream-K launch
 struct SkGemm {
-  int epi;                            // SK_GEMM_*
-  void *act_out;                      // SK_GEMM_SILU: bf16 [rows][N / 2] = silu(gate) * up, w_map then holds 64-row boxes of [gate ; up]
   const CUtensorMap *w_map;           // weights [N (x groups)][K], 128-row boxes
   const XMaps *x_maps;
   float *C;                           // pieces [slot][rows][N]

@@ -17,12 +17,6 @@
 // Warp roles: warp 0 TMA producer, warp 1 MMA issuer (+ TMEM alloc), warps 2-5 epilogue (TMEM lane = weight row,
 // column = activation row; a warp's 32 lanes store 32 consecutive output columns of one row: coalesced 128 B).
 // Grouped mode (MoE): row blocks come from a device list {row0, nrows, weight row base}, units are whole tiles.
-// Fused SwiGLU mode (SK_EPI_SILU, the gate/up projection): a weight tile is 64 gate rows + the 64 up rows of the SAME ffn indices (two
-// 64-row TMA boxes into one 128-row stage), so a tile's accumulator holds everything act = silu(g) * u needs.  Stream-K still cuts
-// tiles into pieces; the CTA that owns a tile's FIRST k-blocks (its "head", slot 0 — the last thing that CTA computes) waits for the
-// other pieces (written to their slots by CTAs that computed them FIRST in their own ranges: no cycle), adds them to its accumulator
-// in slot order — the order the separate consumer kernel used, so the bits are the same — applies silu(g) * u and stores bf16 act.
-// Lanes 0-63 of the accumulator are gate rows and 64-127 up rows: the up warps hand their values to the gate warps through shared memory.
 // Sampling mode (EPI_SAMPLE, the LM head of a decode step): whole (vocab tile, 256-row block) units; the
 // epilogue never stores the logits: each warp transposes its 32 ids x 32 rows blocks through shared memory so that a thread owns a
 // row, perturbs that row's 32 logits (z / T + Gumbel from Philox keyed by the row), keeps best / second / argbest and the
@@ -54,10 +48,6 @@ struct SkParams {
   int unit_tile;
   int stage_bytes, n_stages, tm_cols;            // tm_cols: columns of ONE accumulator (power of two >= 32)
   int n_acc;                                     // TMEM accumulators: 2 (epilogue overlaps the next piece) | 1 (one 512-column accumulator)
-  // fused epilogues (SK_EPI_SILU)
-  int32_t *flags;                                // per-tile arrival counters of the non-head pieces (zero between launches)
-  __nv_bfloat16 *act_out;                        // [rows][F]
-  int F;
 };
 
 struct SkSampleArgs {
@@ -68,8 +58,7 @@ struct SkSampleArgs {
   float temperature;
   uint32_t k0, k1;
 };
-enum { SK_EPI_PIECES = 0, SK_EPI_SAMPLE = 1, SK_EPI_SILU = 2 };
-constexpr int SK_XBUF_BYTES = 2 * 2 * 32 * 32 * 4;  // SILU: (warp pair) x (double buffer) x 32 rows x 32 ffn indices of up values
+enum { SK_EPI_PIECES = 0, SK_EPI_SAMPLE = 1 };
 constexpr int SK_TILE_OFF = 512;                 // behind the barriers: 32 x 33 fp32 transpose tiles, one per epilogue warp
 constexpr int SK_SAMPLE_EPI_WARPS = 8;           // two per TMEM lane quadrant (alternate 32-column chunks): one warp per scheduler cannot hide its own latencies
 constexpr int SK_TILE_BYTES = SK_SAMPLE_EPI_WARPS * 32 * 33 * 4;
@@ -82,7 +71,7 @@ struct SkBars {
 };
 
 struct Piece {
-  int wtile, row0, nrows, wbase, kb0, kb1, slot, tile, npieces;
+  int wtile, row0, nrows, wbase, kb0, kb1, slot;
 };
 
 // Walks the pieces of CTA `cta`; the three roles call it with identical arguments and so see the same sequence.
@@ -100,8 +89,6 @@ struct PieceIter {
     if (rb_list) { p.row0 = rb_list[4 * rb]; p.nrows = rb_list[4 * rb + 1]; p.wbase = rb_list[4 * rb + 2] * w_rows_per_group; }
     else { p.row0 = rb * rb_rows; p.nrows = min(rb_rows, live - p.row0); p.wbase = 0; }
     p.slot = unit_tile ? 0 : cta - sk_owner(tile * nkb, P, T);
-    p.tile = tile;
-    p.npieces = unit_tile ? 1 : sk_owner(tile * nkb + nkb - 1, P, T) - sk_owner(tile * nkb, P, T) + 1;
     u += unit_tile ? 1 : p.kb1 - p.kb0;
     return true;
   }
@@ -164,14 +151,6 @@ __global__ void __launch_bounds__(EPI == SK_EPI_SAMPLE ? SK_SAMPLE_THREADS : SK_
     // One row block: every weight byte is used once (evict-first).  Several row blocks re-read a weight tile a few k-blocks
     // later: keep it in L2 (evict-last), or the second pass goes back to HBM (measured: 2x DRAM reads on the gate/up GEMM).
     const uint64_t w_hint = (!p.rb_list && it0.n_rb > 1) ? HINT_EVICT_LAST : HINT_EVICT_FIRST;
-    auto load_w = [&](unsigned char *st, int kb, const Piece &pc, unsigned long long *bar_full) {
-      if constexpr (EPI == SK_EPI_SILU) {                 // 64 gate rows, then the 64 up rows of the same ffn indices (tmW: 64-row boxes)
-        tma_load_2d_hint(st, &tmW, kb * BK, pc.wtile * (BMW / 2), bar_full, w_hint);
-        tma_load_2d_hint(st + W_STAGE_BYTES / 2, &tmW, kb * BK, p.F + pc.wtile * (BMW / 2), bar_full, w_hint);
-      } else {
-        tma_load_2d_hint(st, &tmW, kb * BK, pc.wbase + pc.wtile * BMW, bar_full, w_hint);
-      }
-    };
     int n_pre = 0;
     if (!p.rb_list) {
       PieceIter it = it0;
@@ -182,7 +161,7 @@ __global__ void __launch_bounds__(EPI == SK_EPI_SAMPLE ? SK_SAMPLE_THREADS : SK_
           if (lane == 0) {
             unsigned char *st = stage_base + (size_t)n_pre * p.stage_bytes;
             mbar_expect_tx(&bar.full[n_pre], W_STAGE_BYTES + n16 * BOX_BYTES);
-            load_w(st, kb, pc, &bar.full[n_pre]);
+            tma_load_2d_hint(st, &tmW, kb * BK, pc.wbase + pc.wtile * BMW, &bar.full[n_pre], w_hint);
           }
       }
     }
@@ -193,6 +172,7 @@ __global__ void __launch_bounds__(EPI == SK_EPI_SAMPLE ? SK_SAMPLE_THREADS : SK_
     while (it.next(pc)) {
       const int n16 = (pc.nrows + BOX_ROWS - 1) / BOX_ROWS;
       const int tx = W_STAGE_BYTES + n16 * BOX_BYTES;
+      const int wrow = pc.wbase + pc.wtile * BMW;
       // sub-block A = rows [0, 256) on lanes 0-4, sub-block B = rows [256, 512) on lanes 8-12 (only with rb_rows = 512)
       const int sub = lane >> 3, bit = lane & 7;
       const int n16s = sub == 0 ? min(n16, 16) : n16 - min(n16, 16);
@@ -204,7 +184,7 @@ __global__ void __launch_bounds__(EPI == SK_EPI_SAMPLE ? SK_SAMPLE_THREADS : SK_
           mbar_wait(&bar.empty[stage], phase ^ 1);
           if (lane == 0) {
             mbar_expect_tx(&bar.full[stage], tx);
-            load_w(st, kb, pc, &bar.full[stage]);
+            tma_load_2d_hint(st, &tmW, kb * BK, wrow, &bar.full[stage], w_hint);
           }
           __syncwarp();
         }
@@ -318,92 +298,6 @@ __global__ void __launch_bounds__(EPI == SK_EPI_SAMPLE ? SK_SAMPLE_THREADS : SK_
         if (lane == 0) mbar_arrive(&bar.acc_empty[buf]);
         ++piece;
       }
-    } else if constexpr (EPI == SK_EPI_SILU) {
-      // Pieces live in TILE order: column of (wtile, accumulator lane) = wtile * 128 + lane (private to this kernel).
-      float *xbuf = reinterpret_cast<float *>(stage_base + RING + SK_TILE_OFF) + (q & 1) * (2 * 32 * 32);
-      const int pair_bar = 2 + (q & 1);                    // named barrier of the (gate warp q, up warp q + 2) pair
-      const bool is_up = q >= 2;
-      const size_t ldp = (size_t)p.n_wtiles * BMW;
-      PieceIter it = it0;
-      Piece pc;
-      int piece = 0, par = 0;
-      while (it.next(pc)) {
-        const int buf = piece % p.n_acc, use = piece / p.n_acc;
-        mbar_wait(&bar.acc_full[buf], use & 1);
-        tc_fence_after();
-        const uint32_t src = tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)(buf * p.tm_cols);
-        const size_t col = (size_t)pc.wtile * BMW + q * 32 + lane;
-        if (pc.slot != 0) {
-          // not the head: park the partial in this piece's slot and tell the head
-          float *dst = p.C + (size_t)pc.slot * p.slot_stride + (size_t)pc.row0 * ldp + col;
-#pragma unroll 1
-          for (int c = 0; c < pc.nrows; c += 32) {
-            uint32_t v[32];
-            tmem_ld32(src + c, v);
-            tmem_ld_wait();
-            float *o = dst + (size_t)c * ldp;
-#pragma unroll
-            for (int j = 0; j < 32; ++j, o += ldp)
-              if (c + j < pc.nrows) *o = __uint_as_float(v[j]);
-          }
-          tc_fence_before();
-          __syncwarp();
-          if (lane == 0) {
-            mbar_arrive(&bar.acc_empty[buf]);
-            __threadfence();                                 // the warp's stores (ordered before this by the warp barrier) become visible first
-            atomicAdd(&p.flags[pc.tile], 1);
-          }
-        } else {
-          if (pc.npieces > 1) {                              // wait for the 4 epilogue warps of each of the other pieces
-            if (lane == 0) {
-              const int want = 4 * (pc.npieces - 1);
-              for (uint32_t spins = 0; *reinterpret_cast<volatile int32_t *>(&p.flags[pc.tile]) < want; ++spins)
-                if (spins > (1u << 28)) __trap();
-              __threadfence();
-            }
-            __syncwarp();
-          }
-          const float *part = p.C + (size_t)pc.row0 * ldp + col;
-#pragma unroll 1
-          for (int c = 0; c < pc.nrows; c += 32, par ^= 1) {
-            uint32_t v[32];
-            tmem_ld32(src + c, v);
-            tmem_ld_wait();
-            float x[32];
-#pragma unroll
-            for (int j = 0; j < 32; ++j) x[j] = __uint_as_float(v[j]);
-            for (int s = 1; s < pc.npieces; ++s) {           // slot order: head + piece 1 + piece 2 + ...
-              const float *ps = part + (size_t)s * p.slot_stride + (size_t)c * ldp;
-#pragma unroll
-              for (int j = 0; j < 32; ++j)
-                if (c + j < pc.nrows) x[j] += __ldcg(ps + (size_t)j * ldp);
-            }
-            float *xb = xbuf + par * (32 * 32);
-            if (is_up) {
-#pragma unroll
-              for (int j = 0; j < 32; ++j) xb[j * 32 + lane] = x[j];
-            }
-            asm volatile("bar.sync %0, 64;" ::"r"(pair_bar) : "memory");
-            if (!is_up) {
-              const int f = pc.wtile * (BMW / 2) + q * 32 + lane;         // ffn index of this lane
-              __nv_bfloat16 *o = p.act_out + (size_t)(pc.row0 + c) * p.F + f;
-#pragma unroll
-              for (int j = 0; j < 32; ++j, o += p.F) {
-                const float g = x[j], u = xb[j * 32 + lane];
-                if (c + j < pc.nrows) *o = __float2bfloat16_rn(g / (1.0f + expf(-g)) * u);
-              }
-            }
-          }
-          tc_fence_before();
-          __syncwarp();
-          if (lane == 0) mbar_arrive(&bar.acc_empty[buf]);
-          if (pc.npieces > 1) {                              // all four warps are past the wait: clear the counter for the next launch
-            asm volatile("bar.sync 1, 128;" ::: "memory");
-            if (q == 0 && lane == 0) p.flags[pc.tile] = 0;
-          }
-        }
-        ++piece;
-      }
     } else {
       PieceIter it = it0;
       Piece pc;
@@ -474,7 +368,9 @@ SkPlan sk_plan(int n_sms, int N, int K, int rows_ub, int n_rb_ub_grouped, bool r
     pl.P = (int)std::min<long long>(n_sms, tiles_ub);
     pl.slots = 1;
   } else {
-    const int T_min = pl.n_wtiles * pl.nkb * (rows_exact ? n_rb_ub : 1);   // fewest units a launch can see
+    // fewest units a launch can see: one row block when the live count is only bounded; the exact count's blocks otherwise
+    // (257..384 rows are ONE 512-row block, sk_rb_rows: counting two there under-sized the slot count)
+    const int T_min = pl.n_wtiles * pl.nkb * (rows_exact ? (rows_ub + sk_rb_rows(rows_ub) - 1) / sk_rb_rows(rows_ub) : 1);
     pl.P = std::max(1, std::min(n_sms, T_min / 4));                        // >= 4 k-blocks (64 KB of weights) per CTA
     for (;;) {
       const int per = T_min / pl.P;                                        // every CTA range holds >= per units
@@ -495,7 +391,7 @@ SkPlan sk_plan(int n_sms, int N, int K, int rows_ub, int n_rb_ub_grouped, bool r
 darts_status launch_gemm_sk(darts_ctx *c, const SkGemm &g) {
   if (g.rows_ub <= 0) return DARTS_OK;
   const SkPlan &pl = g.plan;
-  if (!pl.unit_tile && (size_t)pl.slots * g.slot_stride * sizeof(float) > c->part_bytes && g.C == c->part)
+  if (g.C == c->part && !pl.unit_tile && (size_t)pl.slots * g.slot_stride * sizeof(float) > c->part_bytes)
     FAIL(c, DARTS_ERR_WORKSPACE_TOO_SMALL, "stream-K piece buffer: %d slots x %zu floats > %zu bytes", pl.slots, g.slot_stride, c->part_bytes);
   SkParams p{};
   p.C = g.C; p.slot_stride = g.slot_stride; p.N = g.N; p.nkb = pl.nkb; p.n_wtiles = pl.n_wtiles; p.rows_ub = g.rows_ub; p.n_rows_dev = g.n_rows_dev;
@@ -505,16 +401,8 @@ darts_status launch_gemm_sk(darts_ctx *c, const SkGemm &g) {
   static bool attr = false;
   if (!attr) {
     CUDA_TRY(c, cudaFuncSetAttribute(gemm_sk_k<SK_EPI_PIECES>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET + (int)sizeof(SkBars) + 2048));
-    CUDA_TRY(c, cudaFuncSetAttribute(gemm_sk_k<SK_EPI_SILU>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET + SK_TILE_OFF + SK_XBUF_BYTES + 1024));
     attr = true;
   }
-  if (g.epi == SK_GEMM_SILU) {
-    // fused SwiGLU: g.w_map holds 64-row boxes of [gate ; up] (N = 2F rows), the output is act [rows][F] in bf16
-    if (g.rb_list || g.N % BMW || !g.act_out || !c->sk_flags) FAIL(c, DARTS_ERR_UNSUPPORTED, "fused SwiGLU GEMM needs a dense launch with ffn %% 64 == 0");
-    if (!pl.unit_tile && (size_t)pl.n_wtiles * ((g.rows_ub + SK_ROWBLOCK - 1) / SK_ROWBLOCK) > c->sk_flags_n) FAIL(c, DARTS_ERR_WORKSPACE_TOO_SMALL, "stream-K flag array too small");
-    p.flags = c->sk_flags; p.act_out = (__nv_bfloat16 *)g.act_out; p.F = g.N / 2;
-    launch_pdl(c, gemm_sk_k<SK_EPI_SILU>, dim3(pl.P), dim3(SK_THREADS), (size_t)(SMEM_BUDGET + SK_TILE_OFF + SK_XBUF_BYTES + 1024), *g.w_map, *g.x_maps, p, SkSampleArgs{});
-  } else
   launch_pdl(c, gemm_sk_k<SK_EPI_PIECES>, dim3(pl.P), dim3(SK_THREADS), smem, *g.w_map, *g.x_maps, p, SkSampleArgs{});
   c->launches++;
   cudaError_t e = cudaGetLastError();
