@@ -26,6 +26,8 @@ import numpy as np
 
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
+T_START = time.perf_counter()
+EXTRA_EST_S = {"c4": 260, "c5": 290}     # one 16 384-step rollout + building the model (c5: 61 GB of random weights)
 
 KV_BYTES_PER_TOKEN_LAYER = {"c2": 2 * 8 * 128 * 2}
 
@@ -168,8 +170,10 @@ def oracle_attention_sample(x_full_seed=0, n_rows=32):
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE attn_main_k launch from an `ncu --set full` capture (profiles/), with the
 # algorithmic bytes of that same launch beside it (launches differ in size over a rollout; `achieved` is the rollout average)
 NCU_ATTENTION_TRAFFIC = {"c3": dict(dram_bytes=1.2947e9, algorithmic_bytes=1.2322e9, ratio=1.051,
-                                    launch="decode step 1001: 289 rows, mean suffix 1003 tokens, 19 open groups",
-                                    source="profiles/r1_gemm_sk.md (ncu --set full, bench.py --profile-step 1000)")}
+                                    launch="decode step 1001 of the seed-0 rollout: 289 rows, mean suffix 1003 tokens, 19 open groups",
+                                    source="profiles/r1_launches_c3_step1000.md (ncu --set full, bench.py --profile-step 1000)")}
+# the same for ONE launch of the config-2 microbench (seed 0: 3 131 237 suffix tokens + 128 x 1024 prefix tokens = 13.396 GB algorithmic)
+NCU_ATTENTION_C2 = dict(ncu_dram_bytes=13.95e9, ncu_traffic_over_algorithmic=1.041, ncu_source="profiles/r1_attention_c2.md")
 KV_POOL_CAP_BYTES = {"c3": 64e9, "c4": 100e9, "c5": 36e9}
 
 
@@ -253,6 +257,150 @@ def oracle_rollout_sample(name, model_gpu, cfg, P, n_tokens=1, seed=0):
     return n_tokens / dt, dt, os.cpu_count()
 
 
+def rollout_bench(name, warmup, steps, e2e_steps, args, rank, world, peaks, keep_model):
+    """`warmup` untimed rollouts, `steps` device-timed rollouts (inputs resident in HBM) and `e2e_steps` rollouts through darts_rollout_host
+    (host buffers in, host results out; the same inputs and seeds as the device phase).  Returns the bench line's keys for this workload."""
+    import torch
+    from paper_2605_30859_b200 import api, workloads as wl
+    d, model, c, cfg, G, max_new = build_rollout(name, seed=0, max_new=args.max_new, G=args.G, n_layers=args.layers)
+    K, P = c["K"], c["P"]
+    mode = api.MODE_SHORTEST_EARLY_STOP if args.mode == "early" else api.MODE_AUTO
+    kvb = 2 * cfg["n_kv_heads"] * cfg["head_dim"] * 2
+    n_runs = warmup + steps                               # the e2e phase re-runs the device phase's inputs and seeds: same work, comparable numbers
+    host_in = [wl.rollout_inputs(name, seed=1000 * rank + it, G=G, max_new=max_new) for it in range(n_runs)]
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    gen_tokens, kept_tokens, dev_ms, e2e_ms, e2e_tokens, attn_ms, attn_bytes, steps_count, near, step_bytes = [], [], [], [], [], [], [], [], [], []
+    launches = 0
+    it = 0
+    for phase, n in (("warmup", warmup), ("device", steps), ("e2e", e2e_steps)):
+        if phase != "warmup":
+            barrier(world)
+        if phase == "e2e":
+            it = warmup
+        for _ in range(n):
+            xin = host_in[it]; it += 1
+            if phase == "e2e":
+                p_pin, f_pin = pin(xin["prompts"]), pin(xin["forced_len"])
+                t0 = time.perf_counter()
+                out = d.rollout_host(p_pin.numpy(), xin["Kp"], K, max_new, 1.0, 7 + it, forced_len=f_pin.numpy(), mode=mode)
+                e2e_ms.append((time.perf_counter() - t0) * 1e3)
+                e2e_tokens.append(int(out["len"].sum()))
+            else:
+                toks = torch.from_numpy(np.ascontiguousarray(xin["prompts"])).cuda()
+                f_dev = torch.from_numpy(np.ascontiguousarray(xin["forced_len"])).cuda()
+                l0 = d.counters()["kernel_launches"]
+                torch.cuda.synchronize()
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(d.stream)
+                d.prefill_device(toks, P, xin["Kp"], K, temperature=1.0, seed=7 + it, forced_len_dev=f_dev, mode=mode, max_len=max_new)
+                d.run_to_completion()
+                b.record(d.stream)
+                torch.cuda.synchronize()
+                if phase == "device":
+                    dev_ms.append(a.elapsed_time(b))
+                    cnt = d.counters()
+                    launches += cnt["kernel_launches"] - l0
+                    gen_tokens.append(cnt["n_generated_tokens"]); kept_tokens.append(cnt["n_kept_tokens"])
+                    steps_count.append(cnt["n_steps"]); near.append(cnt["n_near_ties"])
+                    res = d.results()
+                    step_bytes.append(rollout_algo_step_bytes(cfg, res["len"], xin["Kp"], P))
+                    tot, per_step = rollout_algo_attention_bytes(res["len"], xin["Kp"], P, kvb)
+                    t_ms = d.attention_times()
+                    m = min(len(t_ms), len(per_step))
+                    attn_ms.append(float(np.sum(t_ms[:m])))
+                    attn_bytes.append(float(np.sum(per_step[:m])))
+        if phase != "warmup":
+            barrier(world)
+    value, tot_ms, tot_tok = aggregate(world, np.sum(dev_ms), np.sum(gen_tokens))
+    e2e_value, tot_e2e_ms, tot_e2e_tok = aggregate(world, max(np.sum(e2e_ms), 1e-9), np.sum(e2e_tokens)) if e2e_steps else (None, 0.0, 0)
+    ach = float(np.sum(attn_bytes)) / (float(np.sum(attn_ms)) * 1e-3) / 1e9 if np.sum(attn_ms) > 0 else 0.0
+    R = int(host_in[0]["Kp"].sum())
+    h2d = int(host_in[0]["prompts"].nbytes + host_in[0]["forced_len"].nbytes + host_in[0]["Kp"].nbytes)
+    d2h = int(R * max_new * 12 + R * 5 + G * (K * 4 + 4 * 4))     # tokens, margins, log-probs; len, status; sel, mask, close step, mean, var
+    attn_share = float(np.sum(attn_ms)) * cfg["n_layers"] / max(float(np.sum(dev_ms)), 1e-9)
+    rule = {"c3": "K'=16 >= 2K: shortest-only + early stop", "c4": "K' in {8,12,16}: early stop only for K'=16 prompts, dual-end otherwise",
+            "c5": "K'=12 < 2K: dual-end, no early stop"}[name] if args.mode == "auto" else "forced shortest-only + early stop (variant, DESIGN.md R17)"
+    out = dict(metric="rollout generated tokens/s on 1 B200 (K'-of-K early stop)", value=value, unit="tokens/s",
+               ms_per_step=tot_ms / max(1, steps),
+               config=dict(workload=f"{name}: {cfg['n_layers']} layers d={cfg['d_model']} bf16, G={G} prompts of {P}, K'={c['Kp']}, keep {K}, "
+                                    f"max_new={max_new}, forced-EOS {c['forced']['kind']}, rule: {rule}",
+                           l2="per-step working set (weights + KV, > 8 GB) >> 126 MB L2, no flush",
+                           decode_steps_per_rollout=int(np.mean(steps_count)), generated_tokens_per_rollout=int(np.mean(gen_tokens)),
+                           kept_tokens_per_rollout=int(np.mean(kept_tokens)), near_ties_per_rollout=int(np.mean(near)),
+                           ms_per_decode_step=float(np.sum(dev_ms) / max(1, np.sum(steps_count))),
+                           kv_pool_pages=int(d.rt.n_pages), kv_pages_allocated_last_rollout=int(d.counters()["pages_allocated"]),
+                           kv_peak_pages_last_rollout=int(d.counters()["peak_pages"])),
+               roofline=dict(bound="hbm", achieved=ach, peak=peaks["hbm"], unit="GB/s", frac=ach / peaks["hbm"],
+                             traffic=NCU_ATTENTION_TRAFFIC.get(name, {}).get("dram_bytes"), traffic_detail=NCU_ATTENTION_TRAFFIC.get(name),
+                             traffic_note="a rollout's ~2000 x 36 launches differ in size: `achieved` is their byte-weighted average, measured live; `traffic` is "
+                                          "ncu's DRAM bytes of ONE of those launches (traffic_detail names it and gives that launch's algorithmic bytes)",
+                             kernel="attn_main_k+attn_merge_k (layer 0 of every decode step, CUDA events on the library's stream inside the rollout)",
+                             share_of_step=attn_share, peak_source=peaks["source"]),
+               gpu_launches=int(launches))
+    step_gbps = float(np.sum(step_bytes)) / (float(np.sum(dev_ms)) * 1e-3) / 1e9
+    out["decode_path_roofline"] = dict(bound="hbm", achieved=step_gbps, peak=peaks["hbm"], unit="GB/s", frac=step_gbps / peaks["hbm"],
+                                       what="algorithmic bytes of ALL kernels of the rollout (active weights once per step, suffix KV per row, "
+                                            "prefix KV once per open group, KV appends) / device time of the rollout incl. prefill")
+    if e2e_steps:
+        out["e2e"] = dict(value=e2e_value if tot_e2e_tok > 0 else None, unit="tokens/s", h2d_bytes_per_step=h2d,
+                          d2h_bytes_per_step=d2h, ms_per_step=tot_e2e_ms / max(1, e2e_steps), api="darts_rollout_host (pinned host buffers in, host results out)")
+    if args.max_new or args.G or args.layers:
+        out["config"]["INVALID"] = "debug flags shrink the workload"
+    d.close()
+    out["cpu_model"] = None
+    if keep_model:
+        out["cpu_model"] = dict(cfg=model["cfg"], layers=[{k: v.cpu() for k, v in L.items()} for L in model["layers"]],
+                                **{k: model[k].cpu() for k in ("embed", "lm_head", "final_norm")})
+    out["cfg"] = cfg
+    del model
+    torch.cuda.empty_cache()
+    return out
+
+
+def gemm_tensor_bench(peaks, rows_list=(256, 512)):
+    """The projection GEMMs of config 3 alone through the C-ABI hook (stream-K tcgen05 kernel, fp32 pieces left in place): CUDA-graph replay
+    on the library's stream so the Python call path does not bound the time, weights rotated through copies that together exceed the L2,
+    CUDA events around three replays.  TFLOP/s = 2 rows N K / time, against the measured bf16 burst peak (kernels timed alone)."""
+    import torch
+    from paper_2605_30859_b200 import api, workloads as wl
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        d = api.Darts(dict(cfg=dict(wl.CONFIGS["c2"]["model"])), page_size=64, n_pages=64, max_rows=8, max_prompts=2, max_prompt_len=64, max_new=64, stream=st)
+    out = {}
+    for gname, N, K in (("qkv", 6144, 2560), ("o", 2560, 4096), ("gate_up", 19456, 2560), ("down", 2560, 9728)):
+        ncopy = max(2, int(400e6 // (N * K * 2)) + 1)
+        Ws = [(torch.randn(N, K, device="cuda") * 0.02).to(torch.bfloat16) for _ in range(ncopy)]
+        for rows in rows_list:
+            X = torch.randn(rows, K, device="cuda").to(torch.bfloat16)
+            scratch = torch.empty(24 * rows * N, dtype=torch.float32, device="cuda")
+            n = 2 * ncopy
+            torch.cuda.synchronize()
+            with torch.cuda.stream(st):
+                for i in range(2):
+                    d.debug_gemm_bf16(X, Ws[i % ncopy], split_k=0, scratch=scratch, reduce=False)
+            torch.cuda.synchronize()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=st):
+                for i in range(n):
+                    d.debug_gemm_bf16(X, Ws[i % ncopy], split_k=0, scratch=scratch, reduce=False)
+            g.replay()
+            torch.cuda.synchronize()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            for _ in range(3):
+                g.replay()
+            b.record()
+            torch.cuda.synchronize()
+            us = a.elapsed_time(b) * 1e3 / (3 * n)
+            tf = 2.0 * rows * N * K / us / 1e6
+            out[f"{gname}_{rows}"] = dict(N=N, K=K, rows=rows, us=us, tflops=tf, frac_of_bf16_burst_peak=tf / peaks["bf16"], weight_GBps=N * K * 2 / us / 1e3)
+            del g
+        del Ws
+    d.close()
+    out["peak"] = dict(bf16_tflops_burst=peaks["bf16"], source=peaks["source"], launches=int(sum(1 for _ in out)))
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -265,6 +413,8 @@ def main():
     ap.add_argument("--G", type=int, default=None, help="debug only")
     ap.add_argument("--layers", type=int, default=None, help="debug only")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extra", action="store_true", help="skip the extra_workloads leg (configs 4 and 5, one timed rollout each)")
+    ap.add_argument("--budget-s", type=float, default=1450.0, help="wall-clock budget of the whole command; an extra workload that would not fit is skipped and says so")
     ap.add_argument("--profile-step", type=int, default=None,
                     help="profiling aid (prints no bench line): run the workload's rollout step by step up to this decode step, then bracket "
                          "two more steps with cudaProfilerStart/Stop (use with `ncu --profile-from-start off`)")
@@ -302,97 +452,30 @@ def main():
                     gpu_launches=res["launches"])
     else:
         name = args.workload
-        d, model, c, cfg, G, max_new = build_rollout(name, seed=0, max_new=args.max_new, G=args.G, n_layers=args.layers)
-        K, P = c["K"], c["P"]
-        mode = api.MODE_SHORTEST_EARLY_STOP if args.mode == "early" else api.MODE_AUTO
-        kvb = 2 * cfg["n_kv_heads"] * cfg["head_dim"] * 2
-        n_runs = args.warmup + args.steps                     # the e2e phase re-runs the device phase's inputs and seeds: same work, comparable numbers
-        host_in = [wl.rollout_inputs(name, seed=1000 * rank + it, G=G, max_new=max_new) for it in range(n_runs)]
-        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
-        gen_tokens, kept_tokens, dev_ms, e2e_ms, e2e_tokens, attn_ms, attn_bytes, steps_count, near, step_bytes = [], [], [], [], [], [], [], [], [], []
-        launches = 0
-        it = 0
-        for phase, n in (("warmup", args.warmup), ("device", args.steps), ("e2e", args.steps)):
-            if phase != "warmup":
-                barrier(world)
-            if phase == "e2e":
-                it = args.warmup
-            for _ in range(n):
-                xin = host_in[it]; it += 1
-                if phase == "e2e":
-                    p_pin, f_pin = pin(xin["prompts"]), pin(xin["forced_len"])
-                    t0 = time.perf_counter()
-                    out = d.rollout_host(p_pin.numpy(), xin["Kp"], K, max_new, 1.0, 7 + it, forced_len=f_pin.numpy(), mode=mode)
-                    e2e_ms.append((time.perf_counter() - t0) * 1e3)
-                    e2e_tokens.append(int(out["len"].sum()))
-                else:
-                    toks = torch.from_numpy(np.ascontiguousarray(xin["prompts"])).cuda()
-                    f_dev = torch.from_numpy(np.ascontiguousarray(xin["forced_len"])).cuda()
-                    l0 = d.counters()["kernel_launches"]
-                    torch.cuda.synchronize()
-                    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                    a.record(d.stream)
-                    d.prefill_device(toks, P, xin["Kp"], K, temperature=1.0, seed=7 + it, forced_len_dev=f_dev, mode=mode, max_len=max_new)
-                    d.run_to_completion()
-                    b.record(d.stream)
-                    torch.cuda.synchronize()
-                    if phase == "device":
-                        dev_ms.append(a.elapsed_time(b))
-                        cnt = d.counters()
-                        launches += cnt["kernel_launches"] - l0
-                        gen_tokens.append(cnt["n_generated_tokens"]); kept_tokens.append(cnt["n_kept_tokens"])
-                        steps_count.append(cnt["n_steps"]); near.append(cnt["n_near_ties"])
-                        res = d.results()
-                        step_bytes.append(rollout_algo_step_bytes(cfg, res["len"], xin["Kp"], P))
-                        tot, per_step = rollout_algo_attention_bytes(res["len"], xin["Kp"], P, kvb)
-                        t_ms = d.attention_times()
-                        m = min(len(t_ms), len(per_step))
-                        attn_ms.append(float(np.sum(t_ms[:m])))
-                        attn_bytes.append(float(np.sum(per_step[:m])))
-            if phase != "warmup":
-                barrier(world)
-        value, tot_ms, tot_tok = aggregate(world, np.sum(dev_ms), np.sum(gen_tokens))
-        e2e_value, tot_e2e_ms, tot_e2e_tok = aggregate(world, max(np.sum(e2e_ms), 1e-9), np.sum(e2e_tokens))
-        ach = float(np.sum(attn_bytes)) / (float(np.sum(attn_ms)) * 1e-3) / 1e9 if np.sum(attn_ms) > 0 else 0.0
-        R = int(host_in[0]["Kp"].sum())
-        h2d = int(host_in[0]["prompts"].nbytes + host_in[0]["forced_len"].nbytes + host_in[0]["Kp"].nbytes)
-        d2h = int(R * max_new * 12 + R * 5 + G * (K * 4 + 4 * 4))     # tokens, margins, log-probs; len, status; sel, mask, close step, mean, var
-        attn_share = float(np.sum(attn_ms)) * cfg["n_layers"] / max(float(np.sum(dev_ms)), 1e-9)
-        rule = {"c3": "K'=16 >= 2K: shortest-only + early stop", "c4": "K' in {8,12,16}: early stop only for K'=16 prompts, dual-end otherwise",
-                "c5": "K'=12 < 2K: dual-end, no early stop"}[name] if args.mode == "auto" else "forced shortest-only + early stop (variant, DESIGN.md R17)"
-        line.update(metric="rollout generated tokens/s on 1 B200 (K'-of-K early stop)", value=value, unit="tokens/s",
-                    ms_per_step=tot_ms / max(1, args.steps),
-                    config=dict(workload=f"{name}: {cfg['n_layers']} layers d={cfg['d_model']} bf16, G={G} prompts of {P}, K'={c['Kp']}, keep {K}, "
-                                         f"max_new={max_new}, forced-EOS {c['forced']['kind']}, rule: {rule}",
-                                l2="per-step working set (weights + KV, > 8 GB) >> 126 MB L2, no flush",
-                                decode_steps_per_rollout=int(np.mean(steps_count)), generated_tokens_per_rollout=int(np.mean(gen_tokens)),
-                                kept_tokens_per_rollout=int(np.mean(kept_tokens)), near_ties_per_rollout=int(np.mean(near)),
-                                ms_per_decode_step=float(np.sum(dev_ms) / max(1, np.sum(steps_count)))),
-                    roofline=dict(bound="hbm", achieved=ach, peak=peaks["hbm"], unit="GB/s", frac=ach / peaks["hbm"],
-                                  traffic=NCU_ATTENTION_TRAFFIC.get(name, {}).get("dram_bytes"), traffic_detail=NCU_ATTENTION_TRAFFIC.get(name),
-                                  kernel="attn_main_k+attn_merge_k (layer 0 of every decode step, CUDA events on the library's stream inside the rollout)",
-                                  share_of_step=attn_share, peak_source=peaks["source"]),
-                    gpu_launches=int(launches))
-        step_gbps = float(np.sum(step_bytes)) / (float(np.sum(dev_ms)) * 1e-3) / 1e9
-        line["decode_path_roofline"] = dict(bound="hbm", achieved=step_gbps, peak=peaks["hbm"], unit="GB/s", frac=step_gbps / peaks["hbm"],
-                                            what="algorithmic bytes of ALL kernels of the rollout (active weights once per step, suffix KV per row, "
-                                                 "prefix KV once per open group, KV appends) / device time of the rollout incl. prefill")
-        line["e2e"] = dict(value=e2e_value if tot_e2e_tok > 0 else None, unit="tokens/s", h2d_bytes_per_step=h2d,
-                           d2h_bytes_per_step=d2h, ms_per_step=tot_e2e_ms / max(1, args.steps), api="darts_rollout_host (pinned host buffers in, host results out)")
-        if args.max_new or args.G or args.layers:
-            line["config"]["INVALID"] = "debug flags shrink the workload"
-        d.close()
-        if rank == 0 and not args.no_cpu_baseline:
-            cpu_model = dict(cfg=model["cfg"], layers=[{k: v.cpu() for k, v in L.items()} for L in model["layers"]],
-                             **{k: model[k].cpu() for k in ("embed", "lm_head", "final_norm")})
-        del model
-        torch.cuda.empty_cache()
-        # attention microbench (config 2) alongside: the dominant kernel timed alone on BASELINE.json configs[1]
+        P = wl.CONFIGS[name]["P"]
+        res = rollout_bench(name, args.warmup, args.steps, args.steps, args, rank, world, peaks, keep_model=rank == 0 and not args.no_cpu_baseline)
+        cpu_model, cfg = res.pop("cpu_model"), res.pop("cfg")
+        line.update(res)
         if rank == 0:
+            # the dominant kernel timed alone on BASELINE.json configs[1], and the projections alone at 512 rows
             res2, _ = attention_microbench(10, 3)
             a2 = res2["algo_bytes"] / (res2["ms"] * 1e-3) / 1e9
             line["attention_c2"] = dict(ms=res2["ms"], achieved_GBps=a2, frac_of_measured_peak=a2 / peaks["hbm"], rows=res2["rows"],
-                                        ncu_traffic_over_algorithmic=1.075, ncu_source="profiles/r1_attention_c2.md")
+                                        algorithmic_bytes=res2["algo_bytes"], **NCU_ATTENTION_C2)
+            line["gemm_tensor"] = gemm_tensor_bench(peaks)
+        # BASELINE.json configs[3] and [4] in the same driver-run line: ONE timed rollout each (16 384 lock-step iterations, minutes), only
+        # while the whole command stays clear of the driver's step limit
+        if world == 1 and not (args.max_new or args.G or args.layers) and name == "c3" and not args.no_extra:
+            line["extra_workloads"] = {}
+            for extra in ("c4", "c5"):
+                spent = time.perf_counter() - T_START
+                if spent + EXTRA_EST_S[extra] > args.budget_s:
+                    line["extra_workloads"][extra] = dict(skipped=f"{spent:.0f} s spent, needs ~{EXTRA_EST_S[extra]} s, budget {args.budget_s} s (driver step limit 1800 s)")
+                    continue
+                r = rollout_bench(extra, 0, 1, 0, args, rank, world, peaks, keep_model=False)
+                line["extra_workloads"][extra] = dict(value=r["value"], unit="tokens/s", ms_per_rollout=r["ms_per_step"], warmup_rollouts=0, timed_rollouts=1,
+                                                      config=r["config"], attention_roofline_frac=r["roofline"]["frac"], attention_share_of_step=r["roofline"]["share_of_step"],
+                                                      decode_path_roofline_frac=r["decode_path_roofline"]["frac"], gpu_launches=r["gpu_launches"])
 
     if rank == 0:
         line["clocks"] = sampler.stop()

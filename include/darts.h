@@ -204,6 +204,23 @@ typedef void (*darts_chunk_fn)(void *user, int32_t step_begin, int32_t step_end,
                                const float *logprob_host);
 darts_status darts_run_to_completion_streaming(darts_ctx *ctx, int32_t chunk_steps, darts_chunk_fn fn, void *user, darts_results *out);
 
+/* Token-level streaming, CONSUMER side (§4.3.2: chunks "are dispatched to the training engine ... it launches the
+ * forward computation"; App. E :481-489: an incremental forward over a per-trajectory KV cache).  A context of its own — the consumer's
+ * copy of the model, its own KV pool — scores streamed chunks with a teacher-forced forward: the tokens of a chunk are run through ONE
+ * causal pass over [shared prompt pages || the row's own pages] (chunked prefill on the decode path's kernels: weights are streamed once
+ * per chunk, not once per token), their K/V are appended, and each given token gets its log-probability under softmax(z / T) of the
+ * logits at the position before it (T == 0: softmax(z)).  With the rollout's weights and temperature the values reproduce
+ * darts_results.logprob wherever the rollout kept the token it drew (a forced EOS is scored as the EOS it is).
+ *   darts_score_begin: prompts as in darts_prefill (DEVICE tokens, HOST offsets and Kp); one causal pass per prompt, no sampling.
+ *   darts_score_chunk: tokens_host HOST [n_rows][step_end - step_begin] exactly as darts_chunk_fn delivers them (-1 from a row's end on);
+ *     chunks must arrive in step order; logprob_out_host HOST, same shape, 0 where tokens is -1.  Synchronises.
+ * Errors: DARTS_ERR_BAD_STATE (no darts_score_begin, chunk out of order), DARTS_ERR_KV_POOL_EXHAUSTED, DARTS_ERR_WORKSPACE_TOO_SMALL
+ * (a chunk longer than max_rows - 1 steps).  The step / rollout calls return DARTS_ERR_BAD_STATE on a scoring context until the next
+ * darts_prefill. */
+darts_status darts_score_begin(darts_ctx *ctx, const int32_t *prompt_tokens, const int32_t *prompt_offsets_host, int32_t G,
+                               const int32_t *Kp_host, float temperature);
+darts_status darts_score_chunk(darts_ctx *ctx, int32_t step_begin, int32_t step_end, const int32_t *tokens_host, float *logprob_out_host);
+
 /* End-to-end convenience with HOST inputs (bench `e2e`): copies prompts / forced_len host->device,
  * runs the rollout, copies results device->host. */
 darts_status darts_rollout_host(darts_ctx *ctx, const int32_t *prompts_host, int32_t prompt_len, int32_t G,
@@ -236,6 +253,12 @@ darts_status darts_debug_row_slots(darts_ctx *ctx, int32_t *slot_host, int32_t *
  * `layer` (layer == n_layers: leaving the last layer, i.e. the input of the final norm) for slots [slot_begin, slot_begin + n_slots)
  * of the most recent forward pass (slot numbering as in darts_debug_routing).  out: HOST [n_slots][d_model].  Synchronises. */
 darts_status darts_debug_hidden(darts_ctx *ctx, int32_t layer, int32_t slot_begin, int32_t n_slots, float *out_host);
+
+/* Profiling hook for PTL(b, ctx) sweeps (SURVEY.md 8(f) row f3; PAPER.md:163-169 Eq. 4, :372-382 App. A): give every ACTIVE row a
+ * generated length of new_len (1 <= new_len < max_len) without decoding the steps in between.  Page tables are extended from the free
+ * stack; the K/V of the skipped positions is whatever the pool holds (zeros after darts_create), so the tokens decoded afterwards are
+ * meaningless — the step TIME at that context is what the hook is for.  Asynchronous on the ctx stream. */
+darts_status darts_debug_fast_forward(darts_ctx *ctx, int32_t new_len);
 
 /* Teacher forcing for parity at bf16 (R12): overwrite the token the next decode step feeds
  * for global row `row`.  tokens: HOST [n_rows] (-1 = leave). */

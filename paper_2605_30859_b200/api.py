@@ -78,6 +78,8 @@ ChunkFn = C.CFUNCTYPE(None, C.c_void_p, _i32, _i32, _i32, C.POINTER(C.c_int32), 
 darts_run_to_completion_streaming = _sig("darts_run_to_completion_streaming", _ctx, _i32, ChunkFn, C.c_void_p, C.POINTER(Results))
 darts_rollout_host = _sig("darts_rollout_host", _ctx, _vp, _i32, _i32, _vp, _vp, C.POINTER(Policy), _i32, _f32, _u64,
                           C.POINTER(Results))
+darts_score_begin = _sig("darts_score_begin", _ctx, _vp, _vp, _i32, _vp, _f32)
+darts_score_chunk = _sig("darts_score_chunk", _ctx, _i32, _i32, _vp, _vp)
 darts_get_results = _sig("darts_get_results", _ctx, C.POINTER(Results))
 darts_get_counters = _sig("darts_get_counters", _ctx, C.POINTER(Counters))
 darts_n_active = _sig("darts_n_active", _ctx, C.POINTER(_i32))
@@ -86,6 +88,7 @@ darts_debug_logits = _sig("darts_debug_logits", _ctx, _i32, _vp)
 darts_debug_routing = _sig("darts_debug_routing", _ctx, _i32, _i32, _vp)
 darts_debug_hidden = _sig("darts_debug_hidden", _ctx, _i32, _i32, _i32, _vp)
 darts_debug_row_slots = _sig("darts_debug_row_slots", _ctx, _vp, _vp, _i32)
+darts_debug_fast_forward = _sig("darts_debug_fast_forward", _ctx, _i32)
 darts_debug_set_last_tokens = _sig("darts_debug_set_last_tokens", _ctx, _vp, _i32)
 darts_debug_gemm_bf16 = _sig("darts_debug_gemm_bf16", _ctx, _vp, _vp, _vp, _vp, _i32, _i32, _i32, _i32)
 darts_debug_gemm_scratch_floats = _sig("darts_debug_gemm_scratch_floats", _ctx, _i32, _i32, _i32, _i32, C.POINTER(C.c_size_t))
@@ -255,6 +258,24 @@ class Darts:
         cb = ChunkFn(tramp)
         self._check(darts_run_to_completion_streaming(self.ctx, chunk_steps, cb, None, None))
 
+    # ---- consumer side of token-level streaming ------------------------------------------------------
+    def score_begin(self, prompts, Kp, temperature=1.0):
+        """Prefill the prompts (list of int arrays or [G,P]) for chunk scoring: no sampling, rows = sum Kp."""
+        plist = [np.asarray(p, dtype=np.int32) for p in prompts]
+        offs = np.concatenate([[0], np.cumsum([len(p) for p in plist])]).astype(np.int32)
+        toks = torch.from_numpy(np.concatenate(plist)).cuda()
+        Kp = np.ascontiguousarray(Kp, dtype=np.int32)
+        self._check(darts_score_begin(self.ctx, toks.data_ptr(), _np_ptr(offs), len(plist), _np_ptr(Kp), temperature))
+        self.G, self.R = len(plist), int(Kp.sum())
+
+    def score_chunk(self, step_begin, step_end, tokens):
+        """tokens int32 [n_rows, step_end - step_begin] (-1 from a row's end on) -> float32 log-probabilities, same shape."""
+        t = np.ascontiguousarray(tokens, dtype=np.int32)
+        assert t.shape == (self.R, step_end - step_begin)
+        out = np.empty(t.shape, np.float32)
+        self._check(darts_score_chunk(self.ctx, step_begin, step_end, _np_ptr(t), _np_ptr(out)))
+        return out
+
     def rollout(self, prompts_dev, G, Kp, K, max_len, temperature, seed, forced_len_dev=None, fetch=True):
         """north_star signature: device prompts [G,P] int32, scalar K' (L_long = 1, M_up = 2K, mode AUTO); forced_len_dev [G,K'] int32
         (cuda) or None.  fetch=True hands darts_rollout a darts_results and returns its buffers; False passes out = NULL."""
@@ -332,6 +353,10 @@ class Darts:
         slot, step = np.empty(self.R, np.int32), np.empty(self.R, np.int32)
         self._check(darts_debug_row_slots(self.ctx, _np_ptr(slot), _np_ptr(step), self.R))
         return slot, step
+
+    def debug_fast_forward(self, new_len):
+        """Profiling hook: every active row gets a generated length of new_len (KV of the skipped positions is not computed)."""
+        self._check(darts_debug_fast_forward(self.ctx, new_len))
 
     def debug_set_last_tokens(self, tokens):
         t = np.ascontiguousarray(tokens, dtype=np.int32)

@@ -153,6 +153,11 @@ size_t carve(darts_ctx *c, void *base) {
       else c->gu32 = k.take<float>(A * 2 * F);
       c->logits = k.take<float>(R * m.vocab);
     }
+    c->score_tgt = k.take<int32_t>(R);
+    c->score_idx = k.take<int32_t>(2 * R);
+    c->score_lp = k.take<float>(R);
+    c->score_pend = k.take<char>(R * m.d_model * c->elt);
+    c->pend0 = k.take<char>(G * m.d_model * c->elt);
     c->z0 = k.take<float>(G * m.vocab);
     c->hlast = k.take<float>(G * m.d_model);
     c->xn = k.take<char>(A * m.d_model * c->elt);
@@ -330,7 +335,8 @@ void refresh_ub(darts_ctx *c) {
 }
 
 darts_status prefill_impl(darts_ctx *c, const int32_t *prompt_tokens_dev, bool tokens_in_place, const int32_t *offs, int32_t G,
-                          const int32_t *Kp, const int32_t *forced_len_dev, const darts_policy *pol, float temperature, uint64_t seed) {
+                          const int32_t *Kp, const int32_t *forced_len_dev, const darts_policy *pol, float temperature, uint64_t seed,
+                          bool sample_step0 = true) {
   if (c->sticky) return c->sticky;
   if (!c->has_weights) FAIL(c, DARTS_ERR_BAD_STATE, "context was created without weights (attention-only)");
   if (!offs || !Kp || !pol || G <= 0 || (!tokens_in_place && !prompt_tokens_dev)) FAIL(c, DARTS_ERR_INVALID_ARG, "NULL argument or G <= 0");
@@ -387,12 +393,15 @@ darts_status prefill_impl(darts_ctx *c, const int32_t *prompt_tokens_dev, bool t
       TRY(forward_layers(c, ntok, nullptr));
       TRY(launch_gather_last(c, tb, ntok, g0, g1));
       TRY(launch_rmsnorm(c, c->hlast, c->final_norm, c->xn, g1 - g0, nullptr));
+      CUDA_TRY(c, cudaMemcpyAsync((char *)c->pend0 + (size_t)g0 * c->m.d_model * c->elt, c->xn, (size_t)(g1 - g0) * c->m.d_model * c->elt,
+                                  cudaMemcpyDeviceToDevice, s));                   // kept for darts_score_begin (scores every row's token 0)
       TRY(launch_gemm(c, c->xn, c->lm_head, c->z0 + (size_t)g0 * c->m.vocab, c->m.vocab, c->m.d_model, g1 - g0, nullptr, false));
     }
     g0 = g1;
   }
-  TRY(launch_sample(c, c->z0, 1, R));                                            // step 0: Kp[i] draws from the shared z0[i]
+  if (sample_step0) TRY(launch_sample(c, c->z0, 1, R));                          // step 0: Kp[i] draws from the shared z0[i]
   c->prefilled = true;
+  c->score_mode = false;
   return DARTS_OK;
 }
 
@@ -521,7 +530,7 @@ darts_status darts_prefill(darts_ctx *c, const int32_t *prompt_tokens, const int
 darts_status darts_decode_step(darts_ctx *c) {
   if (!c) return DARTS_ERR_INVALID_ARG;
   if (c->sticky) return c->sticky;
-  if (!c->prefilled) FAIL(c, DARTS_ERR_BAD_STATE, "darts_decode_step before darts_prefill");
+  if (!c->prefilled || c->score_mode) FAIL(c, DARTS_ERR_BAD_STATE, "darts_decode_step before darts_prefill (or on a scoring context)");
   refresh_ub(c);
   int ub = c->host_active_ub;
   if (ub <= 0) return DARTS_OK;
@@ -554,7 +563,7 @@ darts_status darts_decode_step(darts_ctx *c) {
 darts_status darts_select_and_compact(darts_ctx *c, int32_t *n_active_out) {
   if (!c) return DARTS_ERR_INVALID_ARG;
   if (c->sticky) return c->sticky;
-  if (!c->prefilled) FAIL(c, DARTS_ERR_BAD_STATE, "darts_select_and_compact before darts_prefill");
+  if (!c->prefilled || c->score_mode) FAIL(c, DARTS_ERR_BAD_STATE, "darts_select_and_compact before darts_prefill (or on a scoring context)");
   TRY(launch_select(c));
   return launch_compact(c, n_active_out);
 }
@@ -744,6 +753,137 @@ darts_status darts_rollout_host(darts_ctx *c, const int32_t *prompts_host, int32
   return rollout_common(c, nullptr, true, prompt_len, G, Kp_host, forced_dev, policy, max_len, temperature, seed, out);
 }
 
+// ---- consumer half of token-level streaming (§4.3.2; App. E :481-489) --------------------------
+darts_status darts_score_begin(darts_ctx *c, const int32_t *prompt_tokens, const int32_t *prompt_offsets_host, int32_t G, const int32_t *Kp_host,
+                               float temperature) {
+  if (!c) return DARTS_ERR_INVALID_ARG;
+  if ((c->m.d_model * c->elt) % 16) FAIL(c, DARTS_ERR_UNSUPPORTED, "scoring needs 16-byte hidden rows");
+  c->max_len = c->rt.max_new;
+  darts_policy pol{1, 0, 0, DARTS_MODE_DUAL_END};              // no rule runs on a scoring context; the fields only have to be valid
+  TRY(prefill_impl(c, prompt_tokens, false, prompt_offsets_host, G, Kp_host, nullptr, &pol, temperature, 0, false));
+  const int R = c->R, page = c->rt.page_size;
+  std::vector<int32_t> prompt_of(R);
+  int n_prefix = 0, r = 0;
+  for (int i = 0; i < G; ++i) {
+    n_prefix += ceil_div(prompt_offsets_host[i + 1] - prompt_offsets_host[i], page);
+    for (int j = 0; j < Kp_host[i]; ++j) prompt_of[r++] = i;
+  }
+  c->sc_len.assign(R, 0);
+  c->sc_pages.assign((size_t)R * c->max_suffix_pages, -1);
+  c->sc_free.clear();
+  for (int p = c->rt.n_pages - 1; p >= n_prefix; --p) c->sc_free.push_back(p);      // back of the vector = lowest id = next page handed out
+  CUDA_TRY(c, cudaMemcpyAsync(c->score_idx, prompt_of.data(), (size_t)R * 4, cudaMemcpyHostToDevice, c->stream));
+  TRY(launch_score_init_pend(c, R));
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));                                   // prompt_of is a local
+  c->score_mode = true;
+  return DARTS_OK;
+}
+
+// One pass: rows [r0, r1), each forwarding its m[r] leading valid tokens of the chunk.  Slots are row-major, step-minor.
+static darts_status score_pass(darts_ctx *c, int r0, int r1, int s0, int n, const int32_t *tokens, const std::vector<int> &m, float *lp_out) {
+  const int page = c->rt.page_size, msp = c->max_suffix_pages;
+  std::vector<int32_t> g_plen(c->G), g_off(c->G + 1);
+  CUDA_TRY(c, cudaMemcpy(g_plen.data(), c->g_plen, (size_t)c->G * 4, cudaMemcpyDeviceToHost));
+  CUDA_TRY(c, cudaMemcpy(g_off.data(), c->g_off, (size_t)(c->G + 1) * 4, cudaMemcpyDeviceToHost));
+  std::vector<int32_t> s_row, s_tok, s_pos, s_pg, s_off, s_pr, s_npre, s_nsuf, tgt, idx_rows, idx_last;
+  int i = 0;
+  for (int r = r0; r < r1; ++r) {
+    if (m[r] == 0) continue;
+    while (g_off[i + 1] <= r) ++i;
+    for (int k = 0; k < m[r]; ++k) {
+      const int s = s0 + k;                                   // suffix index of this token = its step
+      if (s % page == 0) {
+        if (c->sc_free.empty()) { c->sticky = DARTS_ERR_KV_POOL_EXHAUSTED; FAIL(c, DARTS_ERR_KV_POOL_EXHAUSTED, "scoring context ran out of KV pages"); }
+        c->sc_pages[(size_t)r * msp + s / page] = c->sc_free.back();
+        c->sc_free.pop_back();
+      }
+      s_row.push_back(r); s_tok.push_back(tokens[(size_t)r * n + k]); s_pos.push_back(g_plen[i] + s);
+      s_pg.push_back(c->sc_pages[(size_t)r * msp + s / page]); s_off.push_back(s % page);
+      s_pr.push_back(i); s_npre.push_back(g_plen[i]); s_nsuf.push_back(s + 1);
+      tgt.push_back(k + 1 < m[r] ? tokens[(size_t)r * n + k + 1] : -1);              // this slot's logits score the row's NEXT token of the chunk
+    }
+    idx_rows.push_back(r);
+    idx_last.push_back((int32_t)s_row.size() - 1);
+    CUDA_TRY(c, cudaMemcpyAsync(c->row_pages + (size_t)r * msp, &c->sc_pages[(size_t)r * msp], (size_t)msp * 4, cudaMemcpyHostToDevice, c->stream));
+  }
+  const int S = (int)s_row.size(), n_pend = (int)idx_rows.size();
+  if (S == 0) return DARTS_OK;
+  for (int r : idx_rows) tgt.push_back(tokens[(size_t)r * n]);                       // the pending hidden scores the chunk's first token
+  cudaStream_t st = c->stream;
+  auto up = [&](int32_t *dst, const std::vector<int32_t> &v) { return cudaMemcpyAsync(dst, v.data(), v.size() * 4, cudaMemcpyHostToDevice, st); };
+  CUDA_TRY(c, up(c->slot_row, s_row)); CUDA_TRY(c, up(c->slot_tok, s_tok)); CUDA_TRY(c, up(c->slot_pos, s_pos));
+  CUDA_TRY(c, up(c->slot_dst_page, s_pg)); CUDA_TRY(c, up(c->slot_dst_off, s_off)); CUDA_TRY(c, up(c->slot_prompt, s_pr));
+  CUDA_TRY(c, up(c->slot_npre, s_npre)); CUDA_TRY(c, up(c->slot_nsuf, s_nsuf)); CUDA_TRY(c, up(c->score_tgt, tgt));
+  CUDA_TRY(c, up(c->score_idx, idx_rows)); CUDA_TRY(c, up(c->score_idx + c->rt.max_rows, idx_last));
+  c->attn_plan_valid = attention_sm100_supported(c);
+  if (c->attn_plan_valid) TRY(launch_attention_plan_sm100(c, S, nullptr));
+  const int rows_lm = S + n_pend;
+  if (c->tc_path) {
+    TRY(forward_layers_tc(c, S, nullptr));                                          // leaves xn = rmsnorm(h_L) * final_norm for the S slots
+    TRY(launch_score_gather(c, S, n_pend));
+    if (!sk_sample_supported(c, rows_lm)) FAIL(c, DARTS_ERR_UNSUPPORTED, "scoring needs d_model %% 64 == 0 and vocab %% 4 == 0 on the tensor-core path");
+    TRY(launch_gemm_sk_sample(c, &c->tm_lm, &c->xm_xn, c->m.vocab, c->m.d_model, rows_lm, nullptr, c->score_tgt));
+    TRY(launch_score_finalize(c, 4 * ceil_div(c->m.vocab, 128), rows_lm));
+  } else {
+    TRY(forward_layers(c, S, nullptr));
+    TRY(launch_rmsnorm(c, c->h, c->final_norm, c->xn, S, nullptr));
+    TRY(launch_score_gather(c, S, n_pend));
+    TRY(launch_gemm(c, c->xn, c->lm_head, c->logits, c->m.vocab, c->m.d_model, rows_lm, nullptr, false));
+    TRY(launch_score_logits(c, rows_lm));
+  }
+  TRY(launch_score_scatter(c, n_pend));
+  std::vector<float> lp(rows_lm);
+  CUDA_TRY(c, cudaMemcpyAsync(lp.data(), c->score_lp, (size_t)rows_lm * 4, cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(c, cudaStreamSynchronize(st));                                            // the host vectors above stay alive until here
+  int slot = 0;
+  for (int q = 0; q < n_pend; ++q) {
+    const int r = idx_rows[q];
+    lp_out[(size_t)r * n] = lp[S + q];
+    for (int k = 1; k < m[r]; ++k) lp_out[(size_t)r * n + k] = lp[slot + k - 1];
+    slot += m[r];
+    c->sc_len[r] += m[r];
+  }
+  return DARTS_OK;
+}
+
+darts_status darts_score_chunk(darts_ctx *c, int32_t step_begin, int32_t step_end, const int32_t *tokens_host, float *logprob_out_host) {
+  if (!c) return DARTS_ERR_INVALID_ARG;
+  if (c->sticky) return c->sticky;
+  if (!c->score_mode) FAIL(c, DARTS_ERR_BAD_STATE, "darts_score_chunk before darts_score_begin");
+  if (!tokens_host || !logprob_out_host || step_begin < 0 || step_end <= step_begin || step_end > c->rt.max_new)
+    FAIL(c, DARTS_ERR_INVALID_ARG, "bad chunk [%d, %d) (max_new %d) or NULL buffers", step_begin, step_end, c->rt.max_new);
+  const int R = c->R, n = step_end - step_begin, V = c->m.vocab;
+  std::vector<int> m(R, 0);
+  for (int r = 0; r < R; ++r) {
+    int k = 0;
+    while (k < n && tokens_host[(size_t)r * n + k] >= 0) {
+      if (tokens_host[(size_t)r * n + k] >= V) FAIL(c, DARTS_ERR_INVALID_ARG, "token %d of row %d outside the vocabulary", tokens_host[(size_t)r * n + k], r);
+      ++k;
+    }
+    m[r] = k;
+    if (k > 0 && c->sc_len[r] != step_begin) FAIL(c, DARTS_ERR_BAD_STATE, "row %d has %d tokens scored, chunk starts at step %d (chunks must arrive in order)", r, c->sc_len[r], step_begin);
+    for (int q = 0; q < n; ++q) logprob_out_host[(size_t)r * n + q] = 0.f;
+  }
+  // passes: slots + pending rows share the LM-head matrix (<= max_rows rows); the split-KV work list is bounded as well
+  const int npc_max = ceil_div(c->rt.max_prompt_len, ATTN_CHUNK_TOKENS);
+  int r0 = 0;
+  while (r0 < R) {
+    int r1 = r0, rows_lm = 0;
+    long long parts = 0;
+    while (r1 < R) {
+      long long p = 0;
+      for (int k = 0; k < m[r1]; ++k) p += npc_max + ceil_div(step_begin + k + 1, ATTN_CHUNK_TOKENS);
+      const int add = m[r1] ? m[r1] + 1 : 0;
+      if (rows_lm + add > c->rt.max_rows || (c->attn_max_items > 0 && parts + p > c->attn_max_items)) break;
+      rows_lm += add; parts += p; ++r1;
+    }
+    if (r1 == r0) FAIL(c, DARTS_ERR_WORKSPACE_TOO_SMALL, "a chunk of %d steps does not fit a pass (max_rows %d): use shorter chunks", n, c->rt.max_rows);
+    TRY(score_pass(c, r0, r1, step_begin, n, tokens_host, m, logprob_out_host));
+    r0 = r1;
+  }
+  return DARTS_OK;
+}
+
 darts_status darts_debug_logits(darts_ctx *c, int32_t row, float *out_host) {
   if (!c || !out_host) return DARTS_ERR_INVALID_ARG;
   if (!c->prefilled || row < 0 || row >= c->R) FAIL(c, DARTS_ERR_INVALID_ARG, "bad row %d", row);
@@ -794,6 +934,14 @@ darts_status darts_debug_row_slots(darts_ctx *c, int32_t *slot_host, int32_t *st
   CUDA_TRY(c, cudaMemcpy(slot_host, c->row_slot, (size_t)n_rows * 4, cudaMemcpyDeviceToHost));
   CUDA_TRY(c, cudaMemcpy(step_host, c->row_slot_step, (size_t)n_rows * 4, cudaMemcpyDeviceToHost));
   return DARTS_OK;
+}
+
+darts_status darts_debug_fast_forward(darts_ctx *c, int32_t new_len) {
+  if (!c) return DARTS_ERR_INVALID_ARG;
+  if (c->sticky) return c->sticky;
+  if (!c->prefilled || c->score_mode) FAIL(c, DARTS_ERR_BAD_STATE, "darts_debug_fast_forward needs a prefilled rollout context");
+  if (new_len < 1 || new_len >= c->max_len) FAIL(c, DARTS_ERR_INVALID_ARG, "new_len %d outside [1, max_len = %d)", new_len, c->max_len);
+  return launch_fast_forward(c, new_len);
 }
 
 darts_status darts_debug_set_last_tokens(darts_ctx *c, const int32_t *tokens_host, int32_t n_rows) {

@@ -141,6 +141,13 @@ struct darts_ctx {
   int32_t *chunk_stage[2];
   size_t chunk_stage_bytes;
   cudaEvent_t ev_copy_ready[2], ev_copy_done[2];
+  // chunk scoring (darts_score_begin / darts_score_chunk): a context used as the CONSUMER of streamed token chunks.  Pages are handed
+  // out by the host (the call takes host tokens and returns host log-probabilities anyway); device side: targets, results, pending rows.
+  bool score_mode;
+  std::vector<int32_t> sc_len, sc_free, sc_pages;   // tokens forwarded per row; free page ids (stack); host mirror of row_pages
+  int32_t *score_tgt, *score_idx;                   // [max_rows] target id per LM-head row; [2 * max_rows] gather / scatter indices
+  float *score_lp;                                  // [max_rows] log-probability per LM-head row
+  void *score_pend, *pend0;                         // [max_rows][d] / [max_prompts][d] final-normed hidden awaiting its next token (model dtype)
   char err[512];
   darts_status sticky;
 };
@@ -214,6 +221,7 @@ darts_status launch_moe_tc(darts_ctx *c, int layer, const void *next_norm, int r
 darts_status launch_moe_begin_pass(darts_ctx *c);
 darts_status launch_sample(darts_ctx *c, const float *logits, int step0, int rows_ub);
 darts_status launch_plan_decode(darts_ctx *c, int rows_ub);
+darts_status launch_fast_forward(darts_ctx *c, int new_len);
 darts_status launch_plan_prefill(darts_ctx *c, int tok_begin, int n_tok, int g_begin, int g_end);
 darts_status launch_gather_last(darts_ctx *c, int tok_begin, int n_tok, int g_begin, int g_end);
 darts_status launch_select(darts_ctx *c);
@@ -272,7 +280,14 @@ SkPlan sk_plan(int n_sms, int N, int K, int rows_ub, int n_rb_ub_grouped, bool r
 darts_status launch_gemm_sk(darts_ctx *c, const SkGemm &g);
 darts_status launch_sk_reduce(darts_ctx *c, const SkView &v, float *out, int rows);
 bool sk_sample_supported(const darts_ctx *c, int rows_ub);
-darts_status launch_gemm_sk_sample(darts_ctx *c, const CUtensorMap *w_map, const XMaps *x_maps, int N, int K, int rows_ub, const int32_t *n_rows_dev);
+darts_status launch_gemm_sk_sample(darts_ctx *c, const CUtensorMap *w_map, const XMaps *x_maps, int N, int K, int rows_ub, const int32_t *n_rows_dev,
+                                   const int32_t *target = nullptr);
+// chunk scoring (kernels_score.cu)
+darts_status launch_score_init_pend(darts_ctx *c, int R);
+darts_status launch_score_gather(darts_ctx *c, int S, int n_pend);
+darts_status launch_score_scatter(darts_ctx *c, int n_pend);
+darts_status launch_score_finalize(darts_ctx *c, int n_tiles, int rows);
+darts_status launch_score_logits(darts_ctx *c, int rows);
 inline SkView sk_view(const SkGemm &g) { return SkView{g.C, g.slot_stride, g.N, g.plan.nkb, g.plan.n_wtiles, g.plan.P, g.plan.unit_tile}; }
 darts_status launch_add_rmsnorm_sk(darts_ctx *c, const SkView &v, const void *w, int rows_ub, const int32_t *n_rows_dev);
 darts_status launch_silu_mul_sk(darts_ctx *c, const SkView &v, int rows_ub, const int32_t *n_rows_dev);

@@ -294,6 +294,33 @@ __global__ void plan_decode_k(DevState *st, const int32_t *__restrict__ row_list
   }
 }
 
+// Profiling hook (PTL(b, ctx) sweeps): give every active row a generated length of new_len without decoding the
+// steps in between — page tables are extended from the free stack, the cache content of the skipped positions is whatever the pool holds
+// (finite: the pool is zeroed at darts_create), which changes no timing.  One thread: a tool's hook, not a step of the path.
+__global__ void fast_forward_k(DevState *st, const int32_t *__restrict__ row_list, int32_t *row_len, int32_t *row_pages,
+                               const int32_t *__restrict__ free_pages, int page, int msp, int new_len, int32_t *pinned) {
+  if (threadIdx.x || blockIdx.x) return;
+  int top = st->free_top;
+  for (int s = 0; s < st->n_active; ++s) {
+    const int row = row_list[s];
+    const int t_old = row_len[row] - 1, t_new = new_len - 1;
+    if (t_new <= t_old) continue;
+    for (int p = (t_old + page - 1) / page; p < (t_new + page - 1) / page; ++p) {
+      if (top <= 0) { st->err = DARTS_ERR_KV_POOL_EXHAUSTED; st->n_active = 0; pinned[2] = DARTS_ERR_KV_POOL_EXHAUSTED; return; }
+      row_pages[(size_t)row * msp + p] = free_pages[--top];
+    }
+    row_len[row] = new_len;
+  }
+  st->n_pops += (unsigned long long)(st->free_top - top);
+  st->free_top = top;
+}
+
+darts_status launch_fast_forward(darts_ctx *c, int new_len) {
+  fast_forward_k<<<1, 32, 0, c->stream>>>(c->st, c->row_list, c->row_len, c->row_pages, c->free_pages, c->rt.page_size, c->max_suffix_pages, new_len,
+                                          c->pinned_dev);
+  return post_launch(c, "fast_forward");
+}
+
 darts_status launch_plan_decode(darts_ctx *c, int) {
   plan_decode_k<<<1, 1024, 0, c->stream>>>(c->st, c->row_list, c->row_len, c->row_prompt, c->row_last_tok, c->row_pages, c->g_plen,
                                            c->free_pages, c->slot_row, c->slot_tok, c->slot_pos, c->slot_dst_page, c->slot_dst_off,

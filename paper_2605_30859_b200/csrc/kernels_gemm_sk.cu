@@ -57,6 +57,8 @@ struct SkSampleArgs {
   const int32_t *row_list, *row_prompt, *row_sample, *row_len;
   float temperature;
   uint32_t k0, k1;
+  const int32_t *target;                         // scoring (darts_score_chunk): [rows_ub] vocabulary id whose z / T is wanted per row (-1: none);
+                                                 // no noise is drawn, the entry's "best" is the target's z / T, the log-sum-exp is unchanged
 };
 enum { SK_EPI_PIECES = 0, SK_EPI_SAMPLE = 1 };
 constexpr int SK_TILE_OFF = 512;                 // behind the barriers: 32 x 33 fp32 transpose tiles, one per epilogue warp
@@ -260,27 +262,32 @@ __global__ void __launch_bounds__(EPI == SK_EPI_SAMPLE ? SK_SAMPLE_THREADS : SK_
           for (int j = 0; j < 32; ++j) tile[lane * 33 + j] = __uint_as_float(v[j]);       // bank (lane + j) % 32: conflict-free
           __syncwarp();
           const bool row_ok = c + lane < pc.nrows;
-          int pi = 0, pj = 0, ps = 0;
-          if (row_ok) {
+          int pi = 0, pj = 0, ps = 0, tgt = -1;
+          if (row_ok && !sa.target) {
             const int row = sa.row_list[pc.row0 + c + lane];
             pi = sa.row_prompt[row]; pj = sa.row_sample[row]; ps = sa.row_len[row];
           }
+          if (row_ok && sa.target) tgt = sa.target[pc.row0 + c + lane];
           float b1 = -INFINITY, b2 = -INFINITY, z1 = 0.f, lm = -INFINITY, ls = 0.f;
           int i1 = 0x7fffffff;
 #pragma unroll
           for (int k = 0; k < 32; k += 4) {
             const int vid = nb + k;                          // multiple of 4: one Philox block serves 4 vocabulary ids
             if (vid < p.N) {                                 // warp-uniform (N % 4 == 0)
-              uint32_t x[4];
-              if (T != 0.f) philox4x32_10((uint32_t)(vid >> 2), (uint32_t)ps, (uint32_t)pj, (uint32_t)pi, sa.k0, sa.k1, x);
+              uint32_t x[4] = {0u, 0u, 0u, 0u};
+              if (T != 0.f && !sa.target) philox4x32_10((uint32_t)(vid >> 2), (uint32_t)ps, (uint32_t)pj, (uint32_t)pi, sa.k0, sa.k1, x);
               float zt[4];
 #pragma unroll
               for (int e = 0; e < 4; ++e) {
                 const float z = tile[(k + e) * 33 + lane];   // consecutive lanes, consecutive words
                 zt[e] = T != 0.f ? z / T : z;
-                const float y = T != 0.f ? zt[e] + gumbel_from_bits(x[e]) : z;
-                if (y > b1) { b2 = b1; b1 = y; i1 = vid + e; z1 = zt[e]; }          // ids ascend: strict > keeps the lowest id on ties
-                else if (y > b2) b2 = y;
+                if (sa.target) {                             // warp-uniform: scoring a GIVEN token
+                  if (vid + e == tgt) { b1 = zt[e]; z1 = zt[e]; i1 = tgt; }
+                } else {
+                  const float y = T != 0.f ? zt[e] + gumbel_from_bits(x[e]) : z;
+                  if (y > b1) { b2 = b1; b1 = y; i1 = vid + e; z1 = zt[e]; }        // ids ascend: strict > keeps the lowest id on ties
+                  else if (y > b2) b2 = y;
+                }
               }
               const float mn = fmaxf(fmaxf(lm, fmaxf(zt[0], zt[1])), fmaxf(zt[2], zt[3]));
               ls = ls * __expf(lm - mn) + ((__expf(zt[0] - mn) + __expf(zt[1] - mn)) + (__expf(zt[2] - mn) + __expf(zt[3] - mn)));
@@ -417,13 +424,15 @@ darts_status launch_gemm_sk(darts_ctx *c, const SkGemm &g) {
 // LM head of a decode step with the sampling epilogue (whole tiles, 256-row blocks); sample_finalize_k merges 4 entries per vocab tile.
 bool sk_sample_supported(const darts_ctx *c, int rows_ub) { return rows_ub > 0 && c->m.d_model % BK == 0 && c->m.vocab % 4 == 0; }
 
-darts_status launch_gemm_sk_sample(darts_ctx *c, const CUtensorMap *w_map, const XMaps *x_maps, int N, int K, int rows_ub, const int32_t *n_rows_dev) {
+darts_status launch_gemm_sk_sample(darts_ctx *c, const CUtensorMap *w_map, const XMaps *x_maps, int N, int K, int rows_ub, const int32_t *n_rows_dev,
+                                   const int32_t *target) {
   if (rows_ub <= 0) return DARTS_OK;
   static_assert(sizeof(SkBars) <= SK_TILE_OFF, "transpose tiles overlap the barriers");
   SkParams p{};
   p.N = N; p.nkb = K / BK; p.n_wtiles = (N + BMW - 1) / BMW; p.rows_ub = rows_ub; p.n_rows_dev = n_rows_dev; p.unit_tile = 1;
   SkSampleArgs sa{};
-  sa.top2 = (float4 *)c->top2; sa.lse = (float2 *)c->lse; sa.logits_dump = (c->rt.flags & DARTS_FLAG_DUMP_LOGITS) ? c->logits : nullptr;
+  sa.top2 = (float4 *)c->top2; sa.lse = (float2 *)c->lse; sa.logits_dump = ((c->rt.flags & DARTS_FLAG_DUMP_LOGITS) && !target) ? c->logits : nullptr;
+  sa.target = target;
   sa.row_list = c->row_list; sa.row_prompt = c->row_prompt; sa.row_sample = c->row_sample; sa.row_len = c->row_len;
   sa.temperature = c->temperature; sa.k0 = (uint32_t)(c->seed & 0xffffffffu); sa.k1 = (uint32_t)(c->seed >> 32);
   const int smem = SK_SAMPLE_RING + SK_TILE_OFF + SK_TILE_BYTES + 1024;

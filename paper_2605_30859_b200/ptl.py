@@ -4,11 +4,15 @@ its 3-stage piecewise-linear fit, and the rollout time Eq. 4 predicts from it (S
   PAPER.md:163-169 §4.2.1, Eq. 4:  T = sum_m (l_(m) - l_(m-1)) * PTL(d_TP, M' - m + 1)   (lengths sorted ascending)
   PAPER.md:372-382 App. A:         PTL is profiled per batch size and fitted with a 3-stage piecewise-linear curve.
 
-    python -m paper_2605_30859_b200.ptl --workload c3 [--rows 16,32,...] [--steps 24] [--P 512]
+    python -m paper_2605_30859_b200.ptl --workload c3 [--rows 16,32,...] [--ctx 0,1024,4096,8000] [--steps 24] [--P 512] [--predict]
 
 Measurement only (CUDA events around darts_decode_step + darts_select_and_compact through the C-ABI); the fit is an
-ordinary least-squares search over two breakpoints.  d_TP = 1 (one GPU).  Context is P + a few tokens, so the curve
-isolates the batch-size dependence (weights + launch floor); the KV term grows with context and is reported by bench.py.
+ordinary least-squares search over two breakpoints.  d_TP = 1 (one GPU).
+The paper's PTL has one argument, the active batch size (Eq. 4); on this GPU a decode step also reads every active row's own KV,
+so the cost has a second axis, the generated length t:  step(b, t) = PTL(b) + c_kv * b * t  (the attention term is linear in the
+sum of the rows' contexts).  --ctx sweeps t with darts_debug_fast_forward (the rows jump to a generated length of t; only the step
+TIME at that context is used), c_kv is the least-squares slope of step(b, t) - step(b, 0) over b * t, and --predict evaluates
+Eq. 4 with that term on one rollout of the workload.  eq6_k() turns the fit into Eq. 6's k.
 """
 import argparse
 import json
@@ -42,7 +46,29 @@ def eq4_rollout_time(lengths, ptl):
     return T
 
 
-def measure(workload="c3", rows=(16, 32, 64, 128, 192, 256, 384, 512), steps=24, P=None, seed=0, layers=None):
+def fit_ctx_slope(points):
+    """c_kv (ms per row-token) of step(b, t) = PTL(b) + c_kv b t: least squares through the origin of the excess over the t = 0 point of
+    the same b.  points: dicts with rows, ctx, ms_median.  Returns (c_kv, worst relative residual of the two-term model)."""
+    base = {p["rows"]: p["ms_median"] for p in points if p["ctx"] == 0}
+    x = np.array([p["rows"] * p["ctx"] for p in points if p["ctx"] > 0], float)
+    y = np.array([p["ms_median"] - base[p["rows"]] for p in points if p["ctx"] > 0], float)
+    if len(x) == 0:
+        return 0.0, 0.0
+    c = float(x @ y / (x @ x))
+    full = np.array([p["ms_median"] for p in points if p["ctx"] > 0], float)
+    return c, float(np.max(np.abs(y - c * x) / full))
+
+
+def eq6_k(b, t, c_kv, mean_len, b_at):
+    """Eq. 6's k ("derived from the measured PTL"): the rollout time one more trajectory costs at a batch of b_at rows — it
+    lengthens mean_len lock-step iterations by the PTL slope there, and its own KV is read once per iteration it lives
+    (sum_{s < mean_len} c_kv s = c_kv mean_len^2 / 2).  ms per trajectory."""
+    db = max(1.0, 0.05 * b_at)
+    slope = (np.interp(b_at + db, b, t) - np.interp(b_at - db, b, t)) / (2 * db)
+    return float(mean_len * slope + c_kv * mean_len ** 2 / 2.0)
+
+
+def measure(workload="c3", rows=(16, 32, 64, 128, 192, 256, 384, 512), steps=24, P=None, seed=0, layers=None, ctxs=(0,)):
     import torch
     from . import api, workloads as wl
     c = wl.CONFIGS[workload]
@@ -52,10 +78,12 @@ def measure(workload="c3", rows=(16, 32, 64, 128, 192, 256, 384, 512), steps=24,
     P = c["P"] if P is None else P
     model = wl.make_model(cfg, seed=seed, device="cuda")
     Rmax = max(rows)
-    page = 64
+    page = cfg.get("page", 64 if cfg["dtype"] == "bf16" else 16)
     Kp = 16
-    d = api.Darts(model, page_size=page, n_pages=(Rmax // Kp + 1) * (P // page + 1) + Rmax * 2 + 64, max_rows=Rmax, max_prompts=Rmax // Kp + 1,
-                  max_prompt_len=P, max_new=steps + 8, eos_id=-1)
+    ctxs = sorted(set(int(t) for t in ctxs))
+    max_new = max(ctxs) + (steps + 4) * len(ctxs) + 8
+    d = api.Darts(model, page_size=page, n_pages=(Rmax // Kp + 1) * (P // page + 1) + Rmax * (max_new // page + 2) + 64, max_rows=Rmax,
+                  max_prompts=Rmax // Kp + 1, max_prompt_len=P, max_new=max_new, eos_id=-1)
     out = []
     for R in rows:
         G = max(1, R // Kp)
@@ -63,24 +91,30 @@ def measure(workload="c3", rows=(16, 32, 64, 128, 192, 256, 384, 512), steps=24,
         prompts = wl.make_prompts(G, P, cfg["vocab"], seed)
         d.prefill(list(prompts), kp, 1, temperature=1.0, seed=seed, forced_len=None, L_long=0, mode=api.MODE_DUAL_END)
         d.select_and_compact()
-        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
-        for a, b in ev:
-            a.record(d.stream)
-            d.decode_step()
-            d.select_and_compact()
-            b.record(d.stream)
-        torch.cuda.synchronize()
-        ms = np.array([a.elapsed_time(b) for a, b in ev][4:])
-        assert d.n_active() == int(kp.sum())
-        out.append(dict(rows=int(kp.sum()), ms_median=float(np.median(ms)), ms_min=float(ms.min()), ms_max=float(ms.max())))
+        done = 1
+        for t in ctxs:
+            if t > done:
+                d.debug_fast_forward(t)                          # every row now has t generated tokens (profiling hook: only the time matters)
+                done = t
+            ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+            for a, b in ev:
+                a.record(d.stream)
+                d.decode_step()
+                d.select_and_compact()
+                b.record(d.stream)
+            torch.cuda.synchronize()
+            done += steps
+            ms = np.array([a.elapsed_time(b) for a, b in ev][4:])
+            assert d.n_active() == int(kp.sum())
+            out.append(dict(rows=int(kp.sum()), ctx=int(t), ms_median=float(np.median(ms)), ms_min=float(ms.min()), ms_max=float(ms.max())))
     d.close()
     return out
 
 
-def predict_rollout(workload, b, t, seed=0, layers=None):
-    """Eq. 4 on this GPU: T = sum over lock-step iterations of PTL(active rows), with PTL interpolated from the measured
-    points (prefill not included), against the measured device time of the same rollout.  PTL(b) is measured at context = prompt
-    length; Eq. 4 has no context-length term, so the prediction misses the growth of the KV reads — the difference is reported."""
+def predict_rollout(workload, b, t, seed=0, layers=None, c_kv=0.0):
+    """Eq. 4 on this GPU: T = sum over lock-step iterations of PTL(active rows) [+ c_kv x active rows x step index: the
+    rows' own KV, see the module docstring], with PTL interpolated from the measured points (prefill not included), against the measured
+    device time of the same rollout."""
     import torch
     from . import api, workloads as wl
     c = wl.CONFIGS[workload]
@@ -112,8 +146,10 @@ def predict_rollout(workload, b, t, seed=0, layers=None):
     steps = int(lens.max())
     rows = [int((lens > s).sum()) for s in range(1, steps)]
     pred = float(sum(np.interp(r, b, t) for r in rows))      # Eq. 4 written per step: same sum as over sorted length differences
-    return dict(decode_steps=len(rows), measured_ms=ms[-1], eq4_ms=pred, ratio=ms[-1] / pred,
-                note="PTL(b) measured at context = prompt length; the excess is KV traffic growing with the generated length")
+    pred_ctx = pred + float(sum(c_kv * r * (s + 1) for s, r in enumerate(rows)))
+    return dict(decode_steps=len(rows), measured_ms=ms[-1], eq4_ms=pred, ratio=ms[-1] / pred, eq4_with_ctx_ms=pred_ctx,
+                ratio_with_ctx=ms[-1] / pred_ctx, c_kv_ms_per_row_token=c_kv, mean_len=float(lens.mean()),
+                note="eq4_ms: PTL(b) at context = prompt length only (the paper's form); eq4_with_ctx_ms adds c_kv * rows * generated length per step")
 
 
 def main():
@@ -123,17 +159,22 @@ def main():
     ap.add_argument("--steps", type=int, default=24)
     ap.add_argument("--P", type=int, default=None)
     ap.add_argument("--layers", type=int, default=None)
+    ap.add_argument("--ctx", default="0", help="generated lengths t at which every row count is timed (0 = right after the prefill)")
     ap.add_argument("--predict", action="store_true",
                     help="also run one rollout of the workload and compare its device time with Eq. 4 evaluated on the fitted PTL(b)")
     a = ap.parse_args()
-    pts = measure(a.workload, tuple(int(x) for x in a.rows.split(",")), a.steps, a.P, layers=a.layers)
-    b, t = [p["rows"] for p in pts], [p["ms_median"] for p in pts]
+    pts = measure(a.workload, tuple(int(x) for x in a.rows.split(",")), a.steps, a.P, layers=a.layers, ctxs=tuple(int(x) for x in a.ctx.split(",")))
+    base = [p for p in pts if p["ctx"] == min(q["ctx"] for q in pts)]
+    b, t = [p["rows"] for p in base], [p["ms_median"] for p in base]
     res = dict(workload=a.workload, points=pts)
     if len(b) >= 4:
         knots, vals, rmse = fit_piecewise3(b, t)
         res["fit"] = dict(knots=knots, ms_at_knots=vals, rmse_ms=rmse)
+    c_kv, resid = fit_ctx_slope(pts) if any(p["ctx"] > 0 for p in pts) and any(p["ctx"] == 0 for p in pts) else (0.0, 0.0)
+    res["ctx_fit"] = dict(c_kv_ms_per_row_token=c_kv, worst_rel_residual=resid)
     if a.predict:
-        res["eq4"] = predict_rollout(a.workload, b, t, layers=a.layers)
+        res["eq4"] = predict_rollout(a.workload, b, t, layers=a.layers, c_kv=c_kv)
+        res["eq6_k_ms_per_trajectory"] = eq6_k(b, t, c_kv, res["eq4"]["mean_len"], float(np.mean(b)))
     json.dump(res, sys.stdout)
     print()
 

@@ -35,3 +35,20 @@ def test_eq4_matches_a_step_by_step_simulation():
     for step in range(int(lens.max())):
         T += ptl(int((lens > step).sum()))
     assert abs(eq4_rollout_time(lens, ptl) - T) < 1e-9
+
+
+def test_ctx_slope_recovers_the_second_axis_and_eq6_k_is_its_marginal_cost():
+    """step(b, t) = PTL(b) + c_kv b t: the least-squares slope recovers c_kv from a synthetic table, and Eq. 6's k is the
+    time one more trajectory costs: mean_len x dPTL/db for the batch it widens + c_kv x mean_len^2 / 2 for its own KV."""
+    from paper_2605_30859_b200.ptl import eq6_k, fit_ctx_slope
+    ptl = lambda b: 3.0 + 0.01 * b
+    pts = [dict(rows=b, ctx=t, ms_median=ptl(b) + 2.5e-5 * b * t) for b in (16, 64, 256) for t in (0, 1024, 4096)]
+    c, resid = fit_ctx_slope(pts)
+    assert abs(c - 2.5e-5) < 1e-12 and resid < 1e-9
+    b = np.array([16.0, 64.0, 256.0])
+    k = eq6_k(b, ptl(b), c, mean_len=1000.0, b_at=100.0)
+    assert abs(k - (1000.0 * 0.01 + 2.5e-5 * 1000.0 ** 2 / 2)) < 1e-9
+    # brute force: total time of n lock-step trajectories of equal length L, one more trajectory added
+    L, n = 1000, 100
+    T = lambda m: sum(ptl(m) + c * m * s for s in range(L))
+    assert abs((T(n + 1) - T(n)) - k) / k < 0.01
