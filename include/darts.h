@@ -29,13 +29,9 @@
  *   - There is no CPU fallback and no other backend: on a device that is not sm_100 every entry
  *     point that needs the GPU returns DARTS_ERR_UNSUPPORTED.
  *
- * Environment (read at darts_create; diagnostics only, never needed for correct use)
- *   DARTS_NO_PDL=1           launch every kernel as an ordinary stream launch (no programmatic dependent launch)
- *   DARTS_SKIP=<bitmask>     profiling aid: drop one kernel class of every layer (results are garbage; see
- *                            profiles/r1_live_cost_by_kernel.md).  Never set it outside a timing experiment.
- *   DARTS_ADDNORM_REG_MAX=n  row bound under which the register-resident add + RMSNorm kernel is used (default 128)
- *   DARTS_LM_SK_MAX_ROWS=n   decode LM head: persistent swap-AB kernel up to n rows, 128 x 128 tile kernel above (default: always the
- *                            former; 0 selects the tile kernel — an A/B aid, both sample the same distribution from the same Philox stream)
+ * Environment: the library as built by build.py reads none.  A -DDARTS_PROFILING build (DARTS_NVCC_FLAGS=-DDARTS_PROFILING) reads, at
+ * darts_create, DARTS_NO_PDL=1 (ordinary stream launches instead of programmatic dependent launch) and DARTS_SKIP=<bitmask> (drop one
+ * kernel class of every layer: results are garbage, only the step time means anything; profiles/r1_live_cost_by_kernel.md).
  *
  * Layouts
  *   - Projections are [out_features, in_features] row-major in the model dtype (F32 or BF16).
@@ -83,6 +79,8 @@ enum {
   DARTS_FLAG_DUMP_LOGITS = 1,       /* keep fp32 logits of every row of the last step for darts_debug_logits */
   DARTS_FLAG_NO_PREFIX_SHARING = 2, /* A/B switch: attention re-reads the prefix once per row, not per group */
   DARTS_FLAG_PROFILE_ATTENTION = 4, /* bracket layer 0's attention of every decode step with CUDA events (bench roofline) */
+  DARTS_FLAG_LM_HEAD_TILES = 16,    /* A/B switch: decode LM head on the 128 x 128 tile kernel instead of the persistent swap-AB kernel (both
+                                     * sample the same distribution from the same Philox stream) */
   DARTS_FLAG_DUMP_HIDDEN = 8        /* keep the fp32 residual stream of every layer boundary of the last pass for darts_debug_hidden
                                      * ((n_layers + 1) x rows x d_model floats of workspace; parity only) */
 };
@@ -135,10 +133,14 @@ typedef struct {
   int32_t *sel;                        /* [G][K] selected sample indices j, rule order */
   uint32_t *sel_mask;                  /* [G] bitset of sel */
   int32_t *close_step;                 /* [G] step index at which the group closed */
-  float *len_mean, *len_var;           /* [G] mean / population variance of the pool's lengths (sigma_L^2) */
+  float *len_mean, *len_var;           /* [G] mean / population variance of the pool's lengths (sigma_L^2), over ALL Kp[i]
+                                        * rows at the moment the group closed: a PRUNED row enters with the length at which the early stop
+                                        * cut it (R25), so the value of an early-stopped group is a censored, i.e. deflated, sigma_L^2 —
+                                        * n_pruned tells the caller which groups those are (skip or correct their EMA update) */
   float *logprob;                      /* [n_rows][max_new] log softmax(z / T) of the token the sampler DREW at each step (T == 0: of
                                         * softmax(z)); where a forced stop replaced the draw by EOS the value is still the draw's.
                                         * 0 beyond len.  fp32, accumulated per 128-id vocab tile then merged. */
+  int32_t *n_pruned;                   /* [G] rows of the group halted by the early-stop signal (0 for a dual-end group) */
 } darts_results;
 
 typedef struct {

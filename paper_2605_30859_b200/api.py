@@ -22,7 +22,7 @@ OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_KV_POOL_EXHAUSTED, ERR_WORKSPACE_TOO_S
 F32, BF16 = 0, 1
 ROW_ACTIVE, ROW_VALID, ROW_TRUNC, ROW_PRUNED = 0, 1, 2, 3
 MODE_AUTO, MODE_DUAL_END, MODE_SHORTEST_EARLY_STOP = 0, 1, 2
-FLAG_DUMP_LOGITS, FLAG_NO_PREFIX_SHARING, FLAG_PROFILE_ATTENTION, FLAG_DUMP_HIDDEN = 1, 2, 4, 8
+FLAG_DUMP_LOGITS, FLAG_NO_PREFIX_SHARING, FLAG_PROFILE_ATTENTION, FLAG_DUMP_HIDDEN, FLAG_LM_HEAD_TILES = 1, 2, 4, 8, 16
 
 _vp, _i32, _u32, _u64, _f32 = C.c_void_p, C.c_int32, C.c_uint32, C.c_uint64, C.c_float
 _pp = C.POINTER(C.c_void_p)
@@ -50,7 +50,7 @@ class Policy(C.Structure):
 
 
 class Results(C.Structure):
-    _fields_ = [(n, _vp) for n in ("tokens", "len", "status", "margin", "sel", "sel_mask", "close_step", "len_mean", "len_var", "logprob")]
+    _fields_ = [(n, _vp) for n in ("tokens", "len", "status", "margin", "sel", "sel_mask", "close_step", "len_mean", "len_var", "logprob", "n_pruned")]
 
 
 class Counters(C.Structure):
@@ -307,7 +307,7 @@ class Darts:
         bufs = dict(tokens=np.empty((R, mn), np.int32), len=np.empty(R, np.int32), status=np.empty(R, np.uint8),
                     margin=np.empty((R, mn), np.float32), sel=np.empty((G, K), np.int32), sel_mask=np.empty(G, np.uint32),
                     close_step=np.empty(G, np.int32), len_mean=np.empty(G, np.float32), len_var=np.empty(G, np.float32),
-                    logprob=np.empty((R, mn), np.float32))
+                    logprob=np.empty((R, mn), np.float32), n_pruned=np.empty(G, np.int32))
         res = Results(**{k: _np_ptr(v) for k, v in bufs.items()})
         return bufs, res
 

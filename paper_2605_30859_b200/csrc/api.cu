@@ -65,6 +65,7 @@ size_t carve(darts_ctx *c, void *base) {
   c->g_closed = k.take<int32_t>(G);
   c->g_sel = k.take<int32_t>(G * DARTS_MAX_KP);
   c->g_close_step = k.take<int32_t>(G);
+  c->g_n_pruned = k.take<int32_t>(G);
   c->g_prefix_pages = k.take<int32_t>(G * c->max_prefix_pages);
   c->g_tok_off = k.take<int32_t>(G + 1);
   c->g_mask = k.take<uint32_t>(G);
@@ -259,25 +260,24 @@ darts_status forward_layers_tc(darts_ctx *c, int rows_ub, const int32_t *n_rows_
   TRY(launch_moe_begin_pass(c));
   TRY(launch_embed_norm_rope(c, c->slot_tok, c->attn_norm[0], rows_ub, n_rows_dev));     // embedding, first RMSNorm, RoPE table: one launch
   TRY(dump_hidden(c, 0, rows_ub));
-  // DARTS_SKIP (profiling aid): bit k drops the k-th kernel class of every layer so that the change of the step time gives that class's
-  // LIVE cost (launch-list times are serialised and cold); results are garbage in that mode.
-  const unsigned sk = c->skip_mask;
+  // -DDARTS_PROFILING builds: DARTS_SKIP bit k drops the k-th kernel class of every layer so that the change of the step time gives that
+  // class's LIVE cost (launch-list times are serialised and cold); results are garbage in that mode.  Default build: nothing is skipped.
   for (int l = 0; l < L; ++l) {
     SkGemm g = sk_gemm(c, &c->xm_xn, &c->tm_wqkv[l], c->n_qkv, d, rows_ub, n_rows_dev);
-    if (!(sk & 1)) TRY(launch_gemm_sk(c, g));
-    if (!(sk & 2)) TRY(launch_rope_append_sk(c, l, sk_view(g), rows_ub, n_rows_dev));
-    if ((sk & 12) != 12) TRY(launch_attention(c, l, c->q, c->ao, rows_ub, n_rows_dev));
+    if (!DARTS_SKIPPED(c, 1)) TRY(launch_gemm_sk(c, g));
+    if (!DARTS_SKIPPED(c, 2)) TRY(launch_rope_append_sk(c, l, sk_view(g), rows_ub, n_rows_dev));
+    if (!(DARTS_SKIPPED(c, 4) && DARTS_SKIPPED(c, 8))) TRY(launch_attention(c, l, c->q, c->ao, rows_ub, n_rows_dev));
     g = sk_gemm(c, &c->xm_ao, &c->tm_wo[l], d, qd, rows_ub, n_rows_dev);
-    if (!(sk & 16)) TRY(launch_gemm_sk(c, g));
-    if (!(sk & 32)) TRY(launch_add_rmsnorm_sk(c, sk_view(g), c->mlp_norm[l], rows_ub, n_rows_dev));
+    if (!DARTS_SKIPPED(c, 16)) TRY(launch_gemm_sk(c, g));
+    if (!DARTS_SKIPPED(c, 32)) TRY(launch_add_rmsnorm_sk(c, sk_view(g), c->mlp_norm[l], rows_ub, n_rows_dev));
     const void *next_norm = l + 1 < L ? c->attn_norm[l + 1] : c->final_norm;
     if (m.n_experts == 0) {
       g = sk_gemm(c, &c->xm_xn, &c->tm_wgu[l], 2 * F, d, rows_ub, n_rows_dev);
-      if (!(sk & 64)) TRY(launch_gemm_sk(c, g));
-      if (!(sk & 128)) TRY(launch_silu_mul_sk(c, sk_view(g), rows_ub, n_rows_dev));
+      if (!DARTS_SKIPPED(c, 64)) TRY(launch_gemm_sk(c, g));
+      if (!DARTS_SKIPPED(c, 128)) TRY(launch_silu_mul_sk(c, sk_view(g), rows_ub, n_rows_dev));
       g = sk_gemm(c, &c->xm_act, &c->tm_wd[l], d, F, rows_ub, n_rows_dev);
-      if (!(sk & 256)) TRY(launch_gemm_sk(c, g));
-      if (!(sk & 512)) TRY(launch_add_rmsnorm_sk(c, sk_view(g), next_norm, rows_ub, n_rows_dev));
+      if (!DARTS_SKIPPED(c, 256)) TRY(launch_gemm_sk(c, g));
+      if (!DARTS_SKIPPED(c, 512)) TRY(launch_add_rmsnorm_sk(c, sk_view(g), next_norm, rows_ub, n_rows_dev));
     } else {
       TRY(launch_moe_tc(c, l, next_norm, rows_ub, n_rows_dev));
     }
@@ -467,9 +467,14 @@ darts_status darts_create(const darts_model_desc *m, const darts_weights *w, con
   if (need > rt->workspace_bytes) FAIL(c, DARTS_ERR_WORKSPACE_TOO_SMALL, "workspace %zu < %zu bytes", rt->workspace_bytes, need);
   if (((uintptr_t)rt->workspace & 255) != 0) FAIL(c, DARTS_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
   c->has_weights = m->vocab > 0;
+  c->use_pdl = true;
+#ifdef DARTS_PROFILING
   c->use_pdl = getenv("DARTS_NO_PDL") == nullptr;
-  c->lm_sk_max_rows = getenv("DARTS_LM_SK_MAX_ROWS") ? atoi(getenv("DARTS_LM_SK_MAX_ROWS")) : (1 << 30);
   c->skip_mask = getenv("DARTS_SKIP") ? (unsigned)strtoul(getenv("DARTS_SKIP"), nullptr, 0) : 0u;
+#endif
+  if ((s = gemm_sk_configure(c)) != DARTS_OK || (s = gemm_tc_configure(c)) != DARTS_OK || (s = attn_sm100_configure(c)) != DARTS_OK ||
+      (s = moe_configure(c)) != DARTS_OK)
+    return s;
   if (c->has_weights) {
     int L = m->n_layers;
     c->embed = w->embed; c->final_norm = w->final_norm; c->lm_head = w->lm_head;
@@ -543,7 +548,7 @@ darts_status darts_decode_step(darts_ctx *c) {
   if (c->tc_path) {
     TRY(forward_layers_tc(c, ub, n));
     // logits never reach HBM (unless DUMP_LOGITS): swap-AB persistent kernel with the sampling epilogue, 4 entries per vocab tile
-    if (ub <= c->lm_sk_max_rows && sk_sample_supported(c, ub)) {
+    if (!(c->rt.flags & DARTS_FLAG_LM_HEAD_TILES) && sk_sample_supported(c, ub)) {
       TRY(launch_gemm_sk_sample(c, &c->tm_lm, &c->xm_xn, c->m.vocab, c->m.d_model, ub, n));
       TRY(launch_sample_finalize(c, 4 * ceil_div(c->m.vocab, 128), ub));
     } else {
@@ -602,6 +607,7 @@ darts_status darts_get_results(darts_ctx *c, darts_results *o) {
   if (o->close_step) CUDA_TRY(c, cudaMemcpy(o->close_step, c->g_close_step, G * 4, cudaMemcpyDeviceToHost));
   if (o->len_mean) CUDA_TRY(c, cudaMemcpy(o->len_mean, c->g_len_mean, G * 4, cudaMemcpyDeviceToHost));
   if (o->len_var) CUDA_TRY(c, cudaMemcpy(o->len_var, c->g_len_var, G * 4, cudaMemcpyDeviceToHost));
+  if (o->n_pruned) CUDA_TRY(c, cudaMemcpy(o->n_pruned, c->g_n_pruned, G * 4, cudaMemcpyDeviceToHost));
   return DARTS_OK;
 }
 

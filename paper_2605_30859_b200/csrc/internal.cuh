@@ -77,7 +77,7 @@ struct darts_ctx {
   int32_t *tokens_out;
   float *margin_out;
   float *logprob_out;            // [max_rows][max_new] log softmax(z/T) of the drawn token
-  int32_t *g_off, *g_Kp, *g_plen, *g_closed, *g_sel, *g_close_step, *g_prefix_pages, *g_tok_off;
+  int32_t *g_off, *g_Kp, *g_plen, *g_closed, *g_sel, *g_close_step, *g_prefix_pages, *g_tok_off, *g_n_pruned;
   uint32_t *g_mask;
   float *g_len_mean, *g_len_var;
   int32_t *prompt_tokens;        // private copy of the prompt tokens [sum P]
@@ -92,10 +92,8 @@ struct darts_ctx {
   int32_t attn_rows;
   // tensor-core path (bf16, kernels_gemm_tc.cu): split-K partial buffer, LM-head top-2 partials, tensor maps
   bool tc_path;                  // every GEMM of this model runs on tcgen05
-  unsigned skip_mask;            // profiling aid (env DARTS_SKIP, bit per kernel class of a layer): skipped launches leave stale data — timing only
-  int lm_sk_max_rows;            // decode LM head: swap-AB persistent kernel up to this many rows (host bound), 128x128 tile kernel above
-                                 // (default: always; DARTS_LM_SK_MAX_ROWS=0 in the environment selects the tile kernel, an A/B aid)
-  bool use_pdl;                  // launch the stream-K GEMMs as programmatic dependents (DARTS_NO_PDL=1 in the environment disables)
+  unsigned skip_mask;            // -DDARTS_PROFILING builds only (env DARTS_SKIP, bit per kernel class of a layer): skipped launches leave stale data — timing only
+  bool use_pdl;                  // launch the kernels of a step as programmatic dependents (-DDARTS_PROFILING builds: DARTS_NO_PDL=1 disables)
   float *part;                   // [S][rows][N] fp32 partials of the GEMM in flight
   size_t part_bytes;
   float *top2;                   // float4 [vocab tiles][max_rows]
@@ -151,6 +149,13 @@ struct darts_ctx {
   char err[512];
   darts_status sticky;
 };
+
+// Profiling aid, compiled out of the default build: the product never reads the environment.
+#ifdef DARTS_PROFILING
+#define DARTS_SKIPPED(c, bit) (((c)->skip_mask & (bit)) != 0)
+#else
+#define DARTS_SKIPPED(c, bit) false
+#endif
 
 #define CUDA_TRY(ctx, expr)                                                                   \
   do {                                                                                        \
@@ -298,4 +303,9 @@ darts_status launch_sum_partials(darts_ctx *c, const float *part, float *out, in
 darts_status launch_gather_rows_bf16(darts_ctx *c, const void *src, void *dst, int tok_begin, int g_begin, int g_end);
 darts_status launch_attention_plan_sm100(darts_ctx *c, int rows_ub, const int32_t *n_rows_dev, bool prefill = false);
 bool attention_sm100_supported(const darts_ctx *c);
+// per-context kernel set-up (function attributes), called by darts_create
+darts_status gemm_sk_configure(darts_ctx *c);
+darts_status gemm_tc_configure(darts_ctx *c);
+darts_status attn_sm100_configure(darts_ctx *c);
+darts_status moe_configure(darts_ctx *c);
 darts_status launch_attention_ref(darts_ctx *c, int layer, const void *q, void *out, int rows_ub, const int32_t *n_rows_dev);

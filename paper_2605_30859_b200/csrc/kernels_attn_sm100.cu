@@ -45,11 +45,20 @@ __device__ __forceinline__ void mbar_expect_tx(void *bar, int bytes) {
 __device__ __forceinline__ void mbar_arrive(void *bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
+// Bounded wait (as in sm100_ptx.cuh): a protocol bug traps, the launch fails with an error, nothing hangs.
 __device__ __forceinline__ void mbar_wait(void *bar, int parity) {
-  asm volatile(
-      "{\n.reg .pred p;\nWAIT_%=:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-      "@p bra DONE_%=;\nbra WAIT_%=;\nDONE_%=:\n}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+  for (uint32_t spins = 0;; ++spins) {
+    uint32_t ok;
+    asm volatile(
+        "{\n.reg .pred p;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n}"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+    if (ok) return;
+    if (spins > (1u << 26)) __trap();
+  }
 }
 __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, int bytes, void *bar) {
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
@@ -474,6 +483,11 @@ darts_status launch_attention_plan_sm100(darts_ctx *c, int rows_ub, const int32_
   return DARTS_OK;
 }
 
+darts_status attn_sm100_configure(darts_ctx *c) {
+  CUDA_TRY(c, cudaFuncSetAttribute(attn_main_k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)attn_sm100_smem_bytes()));
+  return DARTS_OK;
+}
+
 bool attention_sm100_supported(const darts_ctx *c) {
   int rep = c->m.n_q_heads / c->m.n_kv_heads;
   return c->m.dtype == DARTS_BF16 && c->m.head_dim == HD && c->rt.page_size == PAGE && (rep == 1 || rep == 2 || rep == 4 || rep == 8 || rep == 16);
@@ -483,12 +497,7 @@ darts_status launch_attention_sm100(darts_ctx *c, int layer, const void *q, void
   *taken = false;
   if (!attention_sm100_supported(c) || !c->attn_plan_valid) return DARTS_OK;
   *taken = true;
-  static bool attr_set = false;
   size_t smem = attn_sm100_smem_bytes();
-  if (!attr_set) {
-    CUDA_TRY(c, cudaFuncSetAttribute(attn_main_k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    attr_set = true;
-  }
   Params p;
   p.q = (const __nv_bfloat16 *)q;
   p.kv_layer = (const __nv_bfloat16 *)c->kv_pool + (size_t)layer * c->kv_layer_elems;
@@ -499,10 +508,10 @@ darts_status launch_attention_sm100(darts_ctx *c, int layer, const void *q, void
   p.page_elems = c->kv_page_elems; p.tile_elems = c->kv_tile_elems;
   p.c = 1.4426950408889634f / sqrtf((float)HD);
   int grid = c->n_sms * 2;
-  if (!(c->skip_mask & 4)) launch_pdl(c, attn_main_k, dim3(grid), dim3(THREADS), smem, p);
+  if (!DARTS_SKIPPED(c, 4)) launch_pdl(c, attn_main_k, dim3(grid), dim3(THREADS), smem, p);
   c->launches++;
   if (cudaGetLastError() != cudaSuccess) FAIL(c, DARTS_ERR_CUDA, "launch attn_main failed: %s", cudaGetErrorString(cudaGetLastError()));
-  if (!(c->skip_mask & 8)) launch_pdl(c, attn_merge_k, dim3(rows_ub, (p.Hq + 7) / 8), dim3(256), 0, c->part_ml, c->part_acc, c->part_base, c->part_cnt, (__nv_bfloat16 *)out, p.Hq, p.c, n_rows_dev, rows_ub);
+  if (!DARTS_SKIPPED(c, 8)) launch_pdl(c, attn_merge_k, dim3(rows_ub, (p.Hq + 7) / 8), dim3(256), 0, c->part_ml, c->part_acc, c->part_base, c->part_cnt, (__nv_bfloat16 *)out, p.Hq, p.c, n_rows_dev, rows_ub);
   c->launches++;
   if (cudaGetLastError() != cudaSuccess) FAIL(c, DARTS_ERR_CUDA, "launch attn_merge failed");
   return DARTS_OK;

@@ -298,7 +298,7 @@ darts_status launch_sum_partials(darts_ctx *c, const float *part, float *out, in
 darts_status launch_add_rmsnorm_sk(darts_ctx *c, const SkView &v, const void *w, int rows_ub, const int32_t *n_rows_dev) {
   if (rows_ub <= 0) return DARTS_OK;
   // the register-resident variant pays with occupancy (101-175 registers): it is for launches that cannot fill the SMs anyway
-  static const int reg_max = getenv("DARTS_ADDNORM_REG_MAX") ? atoi(getenv("DARTS_ADDNORM_REG_MAX")) : 128;
+  const int reg_max = 128;                                 // measured cross-over (round 1, ptl sweeps)
   int d = c->m.d_model, iters = rows_ub <= reg_max ? (d / 4 + 255) / 256 : 99;
   const __nv_bfloat16 *wn = (const __nv_bfloat16 *)w;
   __nv_bfloat16 *xn = (__nv_bfloat16 *)c->xn;

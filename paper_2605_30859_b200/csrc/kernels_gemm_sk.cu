@@ -395,6 +395,13 @@ SkPlan sk_plan(int n_sms, int N, int K, int rows_ub, int n_rb_ub_grouped, bool r
   return pl;
 }
 
+// Per-context set-up (darts_create): function attributes belong to the device / context the library was created on, not to the process.
+darts_status gemm_sk_configure(darts_ctx *c) {
+  CUDA_TRY(c, cudaFuncSetAttribute(gemm_sk_k<SK_EPI_PIECES>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET + (int)sizeof(SkBars) + 2048));
+  CUDA_TRY(c, cudaFuncSetAttribute(gemm_sk_k<SK_EPI_SAMPLE>, cudaFuncAttributeMaxDynamicSharedMemorySize, SK_SAMPLE_RING + SK_TILE_OFF + SK_TILE_BYTES + 1024));
+  return DARTS_OK;
+}
+
 darts_status launch_gemm_sk(darts_ctx *c, const SkGemm &g) {
   if (g.rows_ub <= 0) return DARTS_OK;
   const SkPlan &pl = g.plan;
@@ -405,11 +412,6 @@ darts_status launch_gemm_sk(darts_ctx *c, const SkGemm &g) {
   p.rb_list = g.rb_list; p.n_rb_dev = g.n_rb_dev; p.w_rows_per_group = g.w_rows_per_group; p.unit_tile = pl.unit_tile; p.stage_bytes = pl.stage_bytes; p.n_stages = pl.n_stages;
   p.tm_cols = pl.tm_cols; p.n_acc = pl.n_acc;
   size_t smem = SMEM_BUDGET + sizeof(SkBars) + 1024;
-  static bool attr = false;
-  if (!attr) {
-    CUDA_TRY(c, cudaFuncSetAttribute(gemm_sk_k<SK_EPI_PIECES>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET + (int)sizeof(SkBars) + 2048));
-    attr = true;
-  }
   launch_pdl(c, gemm_sk_k<SK_EPI_PIECES>, dim3(pl.P), dim3(SK_THREADS), smem, *g.w_map, *g.x_maps, p, SkSampleArgs{});
   c->launches++;
   cudaError_t e = cudaGetLastError();
@@ -436,11 +438,6 @@ darts_status launch_gemm_sk_sample(darts_ctx *c, const CUtensorMap *w_map, const
   sa.row_list = c->row_list; sa.row_prompt = c->row_prompt; sa.row_sample = c->row_sample; sa.row_len = c->row_len;
   sa.temperature = c->temperature; sa.k0 = (uint32_t)(c->seed & 0xffffffffu); sa.k1 = (uint32_t)(c->seed >> 32);
   const int smem = SK_SAMPLE_RING + SK_TILE_OFF + SK_TILE_BYTES + 1024;
-  static bool attr = false;
-  if (!attr) {
-    CUDA_TRY(c, cudaFuncSetAttribute(gemm_sk_k<SK_EPI_SAMPLE>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    attr = true;
-  }
   const int n_sms = c->n_sms > 0 ? c->n_sms : 148;
   launch_pdl(c, gemm_sk_k<SK_EPI_SAMPLE>, dim3(std::min(n_sms, p.n_wtiles)), dim3(SK_SAMPLE_THREADS), (size_t)smem, *w_map, *x_maps, p, sa);
   c->launches++;

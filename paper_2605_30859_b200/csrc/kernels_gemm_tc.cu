@@ -215,11 +215,6 @@ EncodeTiledFn encode_fn() {
 template <int BN, int STAGES, int EPI>
 darts_status launch_cfg(darts_ctx *c, const CUtensorMap &a, const CUtensorMap &b, const GemmParams &p, dim3 grid) {
   size_t smem = sizeof(GemmSmem<BN, STAGES>) + 1024;
-  static bool attr = false;
-  if (!attr) {
-    CUDA_TRY(c, cudaFuncSetAttribute(gemm_tc_k<BN, STAGES, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    attr = true;
-  }
   gemm_tc_k<BN, STAGES, EPI><<<grid, GEMM_THREADS, smem, c->stream>>>(a, b, p);
   c->launches++;
   cudaError_t e = cudaGetLastError();
@@ -256,6 +251,12 @@ darts_status tc_make_xmaps(darts_ctx *c, XMaps *out, const void *base, long long
   return DARTS_OK;
 }
 
+darts_status gemm_tc_configure(darts_ctx *c) {
+  CUDA_TRY(c, cudaFuncSetAttribute(gemm_tc_k<128, 3, EPI_STORE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GemmSmem<128, 3>) + 1024));
+  CUDA_TRY(c, cudaFuncSetAttribute(gemm_tc_k<128, 2, EPI_SAMPLE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GemmSmem<128, 2>) + 1024));
+  return DARTS_OK;
+}
+
 bool tc_shape_ok(int N, int K) { return K % BK == 0 && K >= BK && N % 4 == 0; }
 
 darts_status launch_gemm_tc(darts_ctx *c, const TcGemm &g) {
@@ -267,7 +268,7 @@ darts_status launch_gemm_tc(darts_ctx *c, const TcGemm &g) {
   p.top2 = (float4 *)c->top2; p.lse = (float2 *)c->lse; p.logits_dump = (c->rt.flags & DARTS_FLAG_DUMP_LOGITS) ? c->logits : nullptr;
   p.row_list = c->row_list; p.row_prompt = c->row_prompt; p.row_sample = c->row_sample; p.row_len = c->row_len;
   p.temperature = c->temperature; p.k0 = (uint32_t)(c->seed & 0xffffffffu); p.k1 = (uint32_t)(c->seed >> 32);
-  // Sampling on this kernel is the A/B path (DARTS_LM_SK_MAX_ROWS); the decode LM head runs on gemm_sk_k<SK_EPI_SAMPLE>.
+  // Sampling on this kernel is the A/B path (DARTS_FLAG_LM_HEAD_TILES); the decode LM head runs on gemm_sk_k<SK_EPI_SAMPLE>.
   // Two stages (65 KB): three CTAs per SM, so one CTA's sampling epilogue and pipeline ramp hide behind two others' loads.  Measured on the
   // non-layer part of a c3 step (LM head + boundary kernels) at 16 / 288 / 512 rows: 0.47 / 1.03 / 1.37 ms with 3 stages (2 CTAs per SM),
   // 0.43 / 0.91 / 1.17 ms with 2, 0.59 / 1.51 / 2.10 ms with 4 (1 CTA per SM); a 32-row activation slot (more stages in the same

@@ -310,11 +310,6 @@ darts_status route(darts_ctx *c, int layer, int rows_ub, const int32_t *n_rows_d
   const darts_model_desc &m = c->m;
   dim3 grid((rows_ub + RROWS - 1) / RROWS, (m.n_experts + REXP - 1) / REXP);
   size_t smem = (size_t)RROWS * m.d_model * sizeof(float);
-  static bool attr = false;
-  if (!attr && smem > 48 * 1024) {
-    CUDA_TRY(c, cudaFuncSetAttribute(moe_router_k<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    attr = true;
-  }
   launch_pdl(c, moe_router_k<T>, grid, dim3(256), smem, c->h, (const T *)c->mlp_norm[layer], (const float *)c->wr[layer], c->moe_logits, m.d_model,
              m.n_experts, m.rms_eps, m.top_k, c->moe_eid, c->moe_w, c->moe_pos, cnt, c->moe_arrive,
              c->moe_eid_dump ? c->moe_eid_dump + (size_t)layer * c->act_rows * m.top_k : nullptr, n_rows_dev, rows_ub);
@@ -322,6 +317,16 @@ darts_status route(darts_ctx *c, int layer, int rows_ub, const int32_t *n_rows_d
 }
 
 }  // namespace
+
+darts_status moe_configure(darts_ctx *c) {
+  if (!c->m.n_experts) return DARTS_OK;
+  const size_t smem = (size_t)RROWS * c->m.d_model * sizeof(float);
+  if (smem > 48 * 1024) {
+    CUDA_TRY(c, cudaFuncSetAttribute(moe_router_k<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    CUDA_TRY(c, cudaFuncSetAttribute(moe_router_k<__nv_bfloat16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  }
+  return DARTS_OK;
+}
 
 // Zero the per-layer expert counters of one forward pass (tensor-core path; one memset per pass).
 darts_status launch_moe_begin_pass(darts_ctx *c) {

@@ -24,7 +24,7 @@ __device__ __forceinline__ int rank_among(bool in_set, int len, bool desc) {
 
 // One warp per prompt; lane j = sample j (Kp <= 32).
 __global__ void select_k(DevState *st, const int32_t *__restrict__ g_off, const int32_t *__restrict__ g_Kp, int32_t *g_closed,
-                         int32_t *g_sel, uint32_t *g_mask, int32_t *g_close_step, float *g_len_mean, float *g_len_var,
+                         int32_t *g_sel, uint32_t *g_mask, int32_t *g_close_step, float *g_len_mean, float *g_len_var, int32_t *g_n_pruned,
                          const int32_t *__restrict__ row_len, uint8_t *row_status, int G, int K, int L_long, int M_up, int mode) {
   int g = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
   int lane = threadIdx.x & 31;
@@ -69,6 +69,7 @@ __global__ void select_k(DevState *st, const int32_t *__restrict__ g_off, const 
     chosen = in_short || longsel;
   }
   unsigned mask = __ballot_sync(0xffffffffu, chosen);
+  unsigned pruned_mask = __ballot_sync(0xffffffffu, has && stt == DARTS_ROW_PRUNED);
   float fl = has ? (float)len : 0.f;
   float mean = warp_sum(fl) / Kp;
   float dv = has ? (fl - mean) * (fl - mean) : 0.f;
@@ -82,6 +83,7 @@ __global__ void select_k(DevState *st, const int32_t *__restrict__ g_off, const 
     g_close_step[g] = st->step;
     g_len_mean[g] = mean;
     g_len_var[g] = var;
+    g_n_pruned[g] = __popc(pruned_mask);
     atomicAdd(&st->n_kept, (unsigned long long)kept);
   }
 }
@@ -237,7 +239,7 @@ __global__ void attn_load_k(T *kv_layer, const T *__restrict__ kp, const T *__re
 darts_status launch_select(darts_ctx *c) {
   int G = c->G;
   select_k<<<(G + 3) / 4, 128, 0, c->stream>>>(c->st, c->g_off, c->g_Kp, c->g_closed, c->g_sel, c->g_mask, c->g_close_step, c->g_len_mean,
-                                               c->g_len_var, c->row_len, c->row_status, G, c->pol.K, c->pol.L_long, c->pol.M_up, c->pol.mode);
+                                               c->g_len_var, c->g_n_pruned, c->row_len, c->row_status, G, c->pol.K, c->pol.L_long, c->pol.M_up, c->pol.mode);
   c->launches++;
   if (cudaGetLastError() != cudaSuccess) FAIL(c, DARTS_ERR_CUDA, "launch select failed");
   return DARTS_OK;

@@ -110,22 +110,19 @@ def test_bf16_rollout_loop_equals_stepwise_and_is_deterministic():
 
 
 @pytest.mark.parametrize("vocab,G,kp", [(1024, 4, 5), (1000, 4, 5), (1000, 17, 16), (1024, 33, 8)])   # 20 rows; 272 = 256 + 16 and 264 = 256 + 8 rows
-def test_both_lm_head_kernels_sample_the_same_tokens(vocab, G, kp, monkeypatch):
-    """The decode LM head runs on the persistent swap-AB kernel; DARTS_LM_SK_MAX_ROWS=0 (read at darts_create) selects the 128 x 128
-    tile kernel instead.  Same logits (same k order), same Philox stream, same y = z / T + g: the rollouts must be identical, the
-    log-probabilities equal up to the merge order of the per-tile log-sum-exps."""
+def test_both_lm_head_kernels_sample_the_same_tokens(vocab, G, kp):
+    """The decode LM head runs on the persistent swap-AB kernel; DARTS_FLAG_LM_HEAD_TILES selects the 128 x 128 tile kernel instead.
+    Same logits (same k order), same Philox stream, same y = z / T + g: the rollouts must be identical, the log-probabilities equal
+    up to the merge order of the per-tile log-sum-exps."""
+    from paper_2605_30859_b200 import api
     cfg = dict(SMALL, vocab=vocab)
     seed, P, max_new, K = 11, 64, 40, 2
     prompts = wl.make_prompts(G, P, cfg["vocab"], seed)
     Kp = np.full(G, kp, dtype=np.int32)
     forced = wl.make_forced_len(Kp, dict(kind="lognormal", mu=3.0, sigma=0.6, lo=2, hi=40), seed)
     out = []
-    for env in (None, "0"):
-        if env is None:
-            monkeypatch.delenv("DARTS_LM_SK_MAX_ROWS", raising=False)
-        else:
-            monkeypatch.setenv("DARTS_LM_SK_MAX_ROWS", env)
-        d, _ = make_ctx(cfg, seed, G, kp, P, max_new, page=64)
+    for flags in (0, api.FLAG_LM_HEAD_TILES):
+        d, _ = make_ctx(cfg, seed, G, kp, P, max_new, page=64, flags=flags)
         out.append(d.rollout_host(prompts, Kp, K, max_new, 1.0, 3, forced_len=forced))
         d.close()
     a, b = out

@@ -350,13 +350,14 @@ def test_darts_rollout_north_star_signature_matches_oracle(Kp, K, max_len):
     assert np.all(gpu["tokens"][:, max_len:] == -1)
     assert cnt["n_steps"] == orc["n_steps"] and cnt["n_generated_tokens"] == orc["n_generated_tokens"] and cnt["n_kept_tokens"] == orc["n_kept_tokens"]
     assert np.any(gpu["status"] == PRUNED) == (Kp >= 2 * K)
+    assert np.array_equal(gpu["n_pruned"], (orc["status"].reshape(G, Kp) == PRUNED).sum(axis=1))   # which groups' sigma_L^2 is censored (R25)
     if max_len == 24:                                        # dual-end pool (nobody is pruned) with a limit below the forced lengths' tail
         assert np.any(gpu["status"] == TRUNC)
     # out = NULL, results fetched afterwards, and the host-buffer entry point with the same policy spelled out: same bits
     assert d.rollout(pd, G, Kp, K, max_len, 0.8, seed, forced_len_dev=fd, fetch=False) is None
     again = d.results()
     host_api = d.rollout_host(prompts, kp, K, max_len, 0.8, seed, forced_len=forced, L_long=1 if K > 1 else 0, M_up=2 * K, mode=MODE_AUTO)
-    for k in ("tokens", "len", "status", "sel", "sel_mask", "close_step", "margin", "logprob", "len_mean", "len_var"):
+    for k in ("tokens", "len", "status", "sel", "sel_mask", "close_step", "margin", "logprob", "len_mean", "len_var", "n_pruned"):
         assert np.array_equal(gpu[k], again[k]), k
         assert np.array_equal(gpu[k], host_api[k]), k
     d.close()
