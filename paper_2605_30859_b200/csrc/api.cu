@@ -80,6 +80,7 @@ size_t carve(darts_ctx *c, void *base) {
   c->slot_npre = k.take<int32_t>(A);
   c->slot_nsuf = k.take<int32_t>(A);
   c->forced_stage = k.take<int32_t>(G * DARTS_MAX_KP);
+  c->sk_np = k.take<int32_t>(SK_NP_TABLE);
   if (attention_sm100_supported(c)) {
     size_t npc_max = (size_t)ceil_div(rt.max_prompt_len, ATTN_CHUNK_TOKENS);
     size_t max_parts = R * (npc_max + 2) + (size_t)rt.n_pages / ATTN_CHUNK_PAGES + 16;
@@ -248,7 +249,7 @@ darts_status forward_layers(darts_ctx *c, int rows_ub, const int32_t *n_rows_dev
 // kernels, the residual add fused with the next RMSNorm.  Leaves xn = rmsnorm(h_L) * final_norm for the LM head.
 SkGemm sk_gemm(darts_ctx *c, const XMaps *x, const CUtensorMap *w, int N, int K, int rows_ub, const int32_t *n_rows_dev) {
   SkGemm g{};
-  g.w_map = w; g.x_maps = x; g.C = c->part; g.N = N; g.rows_ub = rows_ub; g.n_rows_dev = n_rows_dev;
+  g.w_map = w; g.x_maps = x; g.C = c->part; g.N = N; g.rows_ub = rows_ub; g.n_rows_dev = n_rows_dev; g.np_table = c->sk_np;
   g.plan = sk_plan(c->n_sms, N, K, rows_ub, 0, n_rows_dev == nullptr);
   g.slot_stride = (size_t)rows_ub * N;
   return g;
@@ -981,7 +982,7 @@ darts_status darts_debug_gemm_bf16(darts_ctx *c, const void *X, const void *W, f
     TRY(tc_make_xmaps(c, &xm, X, rows, K));
     TRY(tc_make_map(c, &tb, W, N, K, 128));
     SkGemm g{};
-    g.w_map = &tb; g.x_maps = &xm; g.C = scratch; g.N = N; g.rows_ub = rows; g.slot_stride = (size_t)rows * N;
+    g.w_map = &tb; g.x_maps = &xm; g.C = scratch; g.N = N; g.rows_ub = rows; g.slot_stride = (size_t)rows * N; g.np_table = c->sk_np;
     g.plan = sk_plan(c->n_sms, N, K, rows, 0, true);
     TRY(launch_gemm_sk(c, g));
     if (!C) return DARTS_OK;

@@ -96,6 +96,7 @@ struct darts_ctx {
   bool use_pdl;                  // launch the kernels of a step as programmatic dependents (-DDARTS_PROFILING builds: DARTS_NO_PDL=1 disables)
   float *part;                   // [S][rows][N] fp32 partials of the GEMM in flight
   size_t part_bytes;
+  int32_t *sk_np;                // [SK_NP_TABLE] pieces per tile of the stream-K GEMM in flight (read by its consumer kernel)
   float *top2;                   // float4 [vocab tiles][max_rows]
   float *lse;                    // float2 [vocab tiles][max_rows]
   CUtensorMap *tm_wqkv, *tm_wo, *tm_wgu, *tm_wd, *tm_wgu_e, *tm_wd_e;   // host arrays [n_layers]
@@ -251,6 +252,7 @@ darts_status tc_make_xmaps(darts_ctx *c, XMaps *out, const void *base, long long
 bool tc_shape_ok(int N, int K);
 // stream-K weight-streaming GEMM (kernels_gemm_sk.cu)
 #define SK_ROWBLOCK 256            // activation rows per MMA N block
+#define SK_NP_TABLE 2048           // >= tiles of a split (non whole-tile) dense launch: n_wtiles * row blocks < 8 * SMs
 struct SkPlan { int nkb, n_wtiles, P, unit_tile, slots, stage_bytes, n_stages, tm_cols, n_acc; };   // stage / TMEM fields: grouped mode only
 struct SkGemm {
   const CUtensorMap *w_map;           // weights [N (x groups)][K], 128-row boxes
@@ -259,6 +261,7 @@ struct SkGemm {
   size_t slot_stride;
   int N, rows_ub;
   const int32_t *n_rows_dev;
+  int32_t *np_table;                  // dense stream-K: pieces per tile, written by each tile's head piece for the consumers (NULL: not kept)
   const int32_t *rb_list, *n_rb_dev;  // grouped: {row0, nrows, group id, -} per row block, count on the device
   int w_rows_per_group;               // grouped: weight row base of a block = group id * w_rows_per_group
   SkPlan plan;
@@ -268,6 +271,7 @@ struct SkView {
   const float *part;
   size_t slot_stride;
   int N, nkb, n_wtiles, P, unit_tile;
+  const int32_t *np_table;            // pieces per tile, written by the GEMM that produced `part` (NULL: closed form)
 };
 // Activation rows per row block of a DENSE launch, decided from the LIVE row count on the device (never from the host's stale upper
 // bound: the block size fixes where a tile's pieces are cut, i.e. the fp32 summation order, and that must not depend on timing).
@@ -277,8 +281,13 @@ __host__ __device__ __forceinline__ int sk_rb_rows(int live) { return (live > SK
 __host__ __device__ __forceinline__ int sk_owner(int u, int P, int T) { return ((u + 1) * P - 1) / T; }
 __host__ __device__ __forceinline__ int sk_npieces(const SkView &v, int n_rb, int rb_rows, int col, int row) {
   if (v.unit_tile) return 1;
+  int t = (col >> 7) * n_rb + (rb_rows == 2 * SK_ROWBLOCK ? row / (2 * SK_ROWBLOCK) : row / SK_ROWBLOCK);
+#ifdef __CUDA_ARCH__
+  // the producing GEMM left the count of every tile it touched (its head piece writes it): one L2 hit instead of four integer divisions
+  // per warp, which were ~45 % of the instructions of the piece-summing consumers
+  if (v.np_table) return __ldg(v.np_table + t);
+#endif
   int T = v.n_wtiles * n_rb * v.nkb;
-  int t = (col >> 7) * n_rb + row / rb_rows;
   return sk_owner(t * v.nkb + v.nkb - 1, v.P, T) - sk_owner(t * v.nkb, v.P, T) + 1;
 }
 SkPlan sk_plan(int n_sms, int N, int K, int rows_ub, int n_rb_ub_grouped, bool rows_exact);
@@ -293,7 +302,7 @@ darts_status launch_score_gather(darts_ctx *c, int S, int n_pend);
 darts_status launch_score_scatter(darts_ctx *c, int n_pend);
 darts_status launch_score_finalize(darts_ctx *c, int n_tiles, int rows);
 darts_status launch_score_logits(darts_ctx *c, int rows);
-inline SkView sk_view(const SkGemm &g) { return SkView{g.C, g.slot_stride, g.N, g.plan.nkb, g.plan.n_wtiles, g.plan.P, g.plan.unit_tile}; }
+inline SkView sk_view(const SkGemm &g) { return SkView{g.C, g.slot_stride, g.N, g.plan.nkb, g.plan.n_wtiles, g.plan.P, g.plan.unit_tile, g.np_table}; }
 darts_status launch_add_rmsnorm_sk(darts_ctx *c, const SkView &v, const void *w, int rows_ub, const int32_t *n_rows_dev);
 darts_status launch_silu_mul_sk(darts_ctx *c, const SkView &v, int rows_ub, const int32_t *n_rows_dev);
 darts_status launch_rope_append_sk(darts_ctx *c, int layer, const SkView &v, int rows_ub, const int32_t *n_rows_dev);

@@ -345,16 +345,39 @@ __global__ void attn_merge_k(const float *__restrict__ part_ml, const float *__r
   int lane = threadIdx.x & 31;
   int base = part_base[slot], cnt = part_cnt[slot];
   for (int h = blockIdx.y * (blockDim.x >> 5) + (threadIdx.x >> 5); h < Hq; h += gridDim.y * (blockDim.x >> 5)) {   // one head per warp
-    float M = -INFINITY;
-    for (int k = 0; k < cnt; ++k) M = fmaxf(M, part_ml[((size_t)(base + k) * Hq + h) * 2]);
-    float L = 0.f;
+    float M = -INFINITY, L = 0.f;
     float4 a = make_float4(0.f, 0.f, 0.f, 0.f);
-    for (int k = 0; k < cnt; ++k) {
-      size_t pi = (size_t)(base + k) * Hq + h;
-      float sc = exp2f((part_ml[pi * 2] - M) * c);
-      L += sc * part_ml[pi * 2 + 1];
-      float4 v = *reinterpret_cast<const float4 *>(part_acc + pi * HD + lane * 4);
-      a.x += sc * v.x; a.y += sc * v.y; a.z += sc * v.z; a.w += sc * v.w;
+    if (cnt <= 4) {
+      // the common case (prefix chunk + up to three suffix chunks): every load of the row is issued before the first use — one L2
+      // round trip instead of two dependent passes; the sums below run in chunk order as in the general loop
+      float2 ml[4];
+      float4 v[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k)
+        if (k < cnt) {
+          const size_t pi = (size_t)(base + k) * Hq + h;
+          ml[k] = *reinterpret_cast<const float2 *>(part_ml + pi * 2);
+          v[k] = *reinterpret_cast<const float4 *>(part_acc + pi * HD + lane * 4);
+        }
+#pragma unroll
+      for (int k = 0; k < 4; ++k)
+        if (k < cnt) M = fmaxf(M, ml[k].x);
+#pragma unroll
+      for (int k = 0; k < 4; ++k)
+        if (k < cnt) {
+          const float sc = exp2f((ml[k].x - M) * c);
+          L += sc * ml[k].y;
+          a.x += sc * v[k].x; a.y += sc * v[k].y; a.z += sc * v[k].z; a.w += sc * v[k].w;
+        }
+    } else {
+      for (int k = 0; k < cnt; ++k) M = fmaxf(M, part_ml[((size_t)(base + k) * Hq + h) * 2]);
+      for (int k = 0; k < cnt; ++k) {
+        size_t pi = (size_t)(base + k) * Hq + h;
+        float sc = exp2f((part_ml[pi * 2] - M) * c);
+        L += sc * part_ml[pi * 2 + 1];
+        float4 v = *reinterpret_cast<const float4 *>(part_acc + pi * HD + lane * 4);
+        a.x += sc * v.x; a.y += sc * v.y; a.z += sc * v.z; a.w += sc * v.w;
+      }
     }
     float inv = 1.0f / L;
     uint2 o;

@@ -202,7 +202,9 @@ __global__ void __launch_bounds__(256) silu_mul_sk_k(SkView v, __nv_bfloat16 *__
   const size_t row = (size_t)slot * 2 * F;
   float4 g, u;
   sk_sum4x2(v, sk_npieces(v, n_rb, rbr, k, slot), row + k, sk_npieces(v, n_rb, rbr, F + k, slot), row + F + k, g, u);
-  auto f = [](float gg, float uu) { return gg / (1.0f + expf(-gg)) * uu; };
+  // fast exp / division (a few ulp, against 2^-9 of the bf16 store that follows): the IEEE forms were ~160 of this kernel's ~210
+  // instructions per warp and the kernel is issue-bound (ncu: issue slots 53 % busy, L2 15 % — profiles/r2_consumers.md)
+  auto f = [](float gg, float uu) { return __fdividef(gg, 1.0f + __expf(-gg)) * uu; };
   *reinterpret_cast<uint2 *>(act + (size_t)slot * F + k) = pack4_bf16(f(g.x, u.x), f(g.y, u.y), f(g.z, u.z), f(g.w, u.w));
 }
 
@@ -235,13 +237,11 @@ __global__ void __launch_bounds__(128) rope_append_sk_k(SkView v, __nv_bfloat16 
     a1[0] = x1.x; a1[1] = x1.y; a1[2] = x1.z; a1[3] = x1.w;
     a2[0] = x2.x; a2[1] = x2.y; a2[2] = x2.z; a2[3] = x2.w;
   }
+  // p is a multiple of 4: the four elements of each half stay adjacent under the 16-byte-chunk swizzle of kv_elem -> one 8-byte store
   if (is_v) {
     if (act) {
-#pragma unroll
-      for (int e = 0; e < 4; ++e) {
-        kv_layer[kv_elem(geo, page, head - Hq - Hkv, 1, off, p + e)] = __float2bfloat16_rn(a1[e]);
-        kv_layer[kv_elem(geo, page, head - Hq - Hkv, 1, off, half + p + e)] = __float2bfloat16_rn(a2[e]);
-      }
+      *reinterpret_cast<uint2 *>(&kv_layer[kv_elem(geo, page, head - Hq - Hkv, 1, off, p)]) = pack4_bf16(a1[0], a1[1], a1[2], a1[3]);
+      *reinterpret_cast<uint2 *>(&kv_layer[kv_elem(geo, page, head - Hq - Hkv, 1, off, half + p)]) = pack4_bf16(a2[0], a2[1], a2[2], a2[3]);
     }
     return;
   }
@@ -258,16 +258,20 @@ __global__ void __launch_bounds__(128) rope_append_sk_k(SkView v, __nv_bfloat16 
     }
   }
   if (!act) return;
-  __nv_bfloat16 *qdst = q_out + (size_t)slot * Hq * hd + (size_t)head * hd;
+  const float4 *tp = reinterpret_cast<const float4 *>(cs + (size_t)slot * half + p);   // (cos, sin) of pairs p .. p+3: two 16-byte loads
+  const float4 t01 = tp[0], t23 = tp[1];
+  const float co[4] = {t01.x, t01.z, t23.x, t23.z}, si[4] = {t01.y, t01.w, t23.y, t23.w};
+  float y1[4], y2[4];
 #pragma unroll
-  for (int e = 0; e < 4; ++e) {
-    const float2 t = cs[(size_t)slot * half + p + e];
-    const __nv_bfloat16 y1 = __float2bfloat16_rn(a1[e] * t.x - a2[e] * t.y), y2 = __float2bfloat16_rn(a2[e] * t.x + a1[e] * t.y);
-    if (is_q) { qdst[p + e] = y1; qdst[half + p + e] = y2; }
-    else {
-      kv_layer[kv_elem(geo, page, head - Hq, 0, off, p + e)] = y1;
-      kv_layer[kv_elem(geo, page, head - Hq, 0, off, half + p + e)] = y2;
-    }
+  for (int e = 0; e < 4; ++e) { y1[e] = a1[e] * co[e] - a2[e] * si[e]; y2[e] = a2[e] * co[e] + a1[e] * si[e]; }
+  const uint2 o1 = pack4_bf16(y1[0], y1[1], y1[2], y1[3]), o2 = pack4_bf16(y2[0], y2[1], y2[2], y2[3]);
+  if (is_q) {
+    __nv_bfloat16 *qdst = q_out + (size_t)slot * Hq * hd + (size_t)head * hd;
+    *reinterpret_cast<uint2 *>(qdst + p) = o1;
+    *reinterpret_cast<uint2 *>(qdst + half + p) = o2;
+  } else {
+    *reinterpret_cast<uint2 *>(&kv_layer[kv_elem(geo, page, head - Hq, 0, off, p)]) = o1;
+    *reinterpret_cast<uint2 *>(&kv_layer[kv_elem(geo, page, head - Hq, 0, off, half + p)]) = o2;
   }
 }
 

@@ -48,6 +48,7 @@ struct SkParams {
   int unit_tile;
   int stage_bytes, n_stages, tm_cols;            // tm_cols: columns of ONE accumulator (power of two >= 32)
   int n_acc;                                     // TMEM accumulators: 2 (epilogue overlaps the next piece) | 1 (one 512-column accumulator)
+  int32_t *np_table;                             // dense split mode: [tile] = pieces of the tile, written by its head piece (nullable)
 };
 
 struct SkSampleArgs {
@@ -73,7 +74,7 @@ struct SkBars {
 };
 
 struct Piece {
-  int wtile, row0, nrows, wbase, kb0, kb1, slot;
+  int wtile, row0, nrows, wbase, kb0, kb1, slot, tile, npieces;
 };
 
 // Walks the pieces of CTA `cta`; the three roles call it with identical arguments and so see the same sequence.
@@ -91,6 +92,8 @@ struct PieceIter {
     if (rb_list) { p.row0 = rb_list[4 * rb]; p.nrows = rb_list[4 * rb + 1]; p.wbase = rb_list[4 * rb + 2] * w_rows_per_group; }
     else { p.row0 = rb * rb_rows; p.nrows = min(rb_rows, live - p.row0); p.wbase = 0; }
     p.slot = unit_tile ? 0 : cta - sk_owner(tile * nkb, P, T);
+    p.tile = tile;
+    p.npieces = unit_tile ? 1 : sk_owner(tile * nkb + nkb - 1, P, T) - sk_owner(tile * nkb, P, T) + 1;
     u += unit_tile ? 1 : p.kb1 - p.kb0;
     return true;
   }
@@ -315,6 +318,7 @@ __global__ void __launch_bounds__(EPI == SK_EPI_SAMPLE ? SK_SAMPLE_THREADS : SK_
         tc_fence_after();
         const int n = pc.wtile * BMW + q * 32 + lane;        // output column = weight row
         const bool n_ok = n < p.N;
+        if (p.np_table && !p.unit_tile && pc.slot == 0 && q == 0 && lane == 0 && pc.tile < SK_NP_TABLE) p.np_table[pc.tile] = pc.npieces;
         float *dst = p.C + (size_t)pc.slot * p.slot_stride + (size_t)pc.row0 * p.N + n;
         const uint32_t src = tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)(buf * p.tm_cols);
         const size_t ldc = (size_t)p.N;
@@ -411,6 +415,9 @@ darts_status launch_gemm_sk(darts_ctx *c, const SkGemm &g) {
   p.C = g.C; p.slot_stride = g.slot_stride; p.N = g.N; p.nkb = pl.nkb; p.n_wtiles = pl.n_wtiles; p.rows_ub = g.rows_ub; p.n_rows_dev = g.n_rows_dev;
   p.rb_list = g.rb_list; p.n_rb_dev = g.n_rb_dev; p.w_rows_per_group = g.w_rows_per_group; p.unit_tile = pl.unit_tile; p.stage_bytes = pl.stage_bytes; p.n_stages = pl.n_stages;
   p.tm_cols = pl.tm_cols; p.n_acc = pl.n_acc;
+  p.np_table = g.rb_list ? nullptr : g.np_table;
+  if (p.np_table && !pl.unit_tile && (long long)pl.n_wtiles * ((g.rows_ub + SK_ROWBLOCK - 1) / SK_ROWBLOCK) > SK_NP_TABLE)
+    FAIL(c, DARTS_ERR_UNSUPPORTED, "stream-K piece-count table too small for %d weight tiles x %d rows", pl.n_wtiles, g.rows_ub);
   size_t smem = SMEM_BUDGET + sizeof(SkBars) + 1024;
   launch_pdl(c, gemm_sk_k<SK_EPI_PIECES>, dim3(pl.P), dim3(SK_THREADS), smem, *g.w_map, *g.x_maps, p, SkSampleArgs{});
   c->launches++;

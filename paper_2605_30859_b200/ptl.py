@@ -68,7 +68,7 @@ def eq6_k(b, t, c_kv, mean_len, b_at):
     return float(mean_len * slope + c_kv * mean_len ** 2 / 2.0)
 
 
-def measure(workload="c3", rows=(16, 32, 64, 128, 192, 256, 384, 512), steps=24, P=None, seed=0, layers=None, ctxs=(0,)):
+def measure(workload="c3", rows=(16, 32, 64, 128, 192, 256, 384, 512), steps=24, P=None, seed=0, layers=None, ctxs=(0,), pool_bytes=100e9):
     import torch
     from . import api, workloads as wl
     c = wl.CONFIGS[workload]
@@ -82,7 +82,11 @@ def measure(workload="c3", rows=(16, 32, 64, 128, 192, 256, 384, 512), steps=24,
     Kp = 16
     ctxs = sorted(set(int(t) for t in ctxs))
     max_new = max(ctxs) + (steps + 4) * len(ctxs) + 8
-    d = api.Darts(model, page_size=page, n_pages=(Rmax // Kp + 1) * (P // page + 1) + Rmax * (max_new // page + 2) + 64, max_rows=Rmax,
+    # every (rows, t) pair whose KV fits the pool is timed; 512 rows x 8 K tokens (600 GB at c3) never occurs in a rollout and is skipped
+    kv_page_bytes = cfg["n_layers"] * 2 * cfg["n_kv_heads"] * page * cfg["head_dim"] * (2 if cfg["dtype"] == "bf16" else 4)
+    n_prefix = (Rmax // Kp + 1) * (P // page + 1)
+    n_pages = min(n_prefix + Rmax * (max_new // page + 2) + 64, int(pool_bytes // kv_page_bytes))
+    d = api.Darts(model, page_size=page, n_pages=n_pages, max_rows=Rmax,
                   max_prompts=Rmax // Kp + 1, max_prompt_len=P, max_new=max_new, eos_id=-1)
     out = []
     for R in rows:
@@ -93,6 +97,8 @@ def measure(workload="c3", rows=(16, 32, 64, 128, 192, 256, 384, 512), steps=24,
         d.select_and_compact()
         done = 1
         for t in ctxs:
+            if n_prefix + int(kp.sum()) * ((max(t, done) + steps + 4) // page + 2) > n_pages:
+                continue
             if t > done:
                 d.debug_fast_forward(t)                          # every row now has t generated tokens (profiling hook: only the time matters)
                 done = t

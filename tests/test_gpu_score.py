@@ -33,8 +33,9 @@ def _score_all(d, tokens, lens, n, max_new):
     return out
 
 
-def _oracle_given_logprobs(host, prompts, Kp, K, max_new, T, seed, forced, gpu):
-    orc = ro.rollout_stepwise(host, prompts, Kp, K, max_new, T, seed, forced_len=forced, teacher=gpu["tokens"], keep_logits=True)
+def _oracle_given_logprobs(host, prompts, Kp, K, max_new, T, seed, forced, gpu, mode=0):
+    orc = ro.rollout_stepwise(host, prompts, Kp, K, max_new, T, seed, forced_len=forced, teacher=gpu["tokens"], keep_logits=True, mode=mode)
+    assert np.array_equal(orc["len"], gpu["len"])
     lp = np.zeros((len(gpu["len"]), max_new))
     zmax = np.zeros((len(gpu["len"]), max_new))
     for (r, s), z in orc["logits"].items():
@@ -95,7 +96,7 @@ def test_bf16_chunk_scoring_matches_oracle_and_rollout(qk_norm):
     a.run_to_completion()
     gpu = a.results()
     a.close()
-    orc, lp_ref, zmax = _oracle_given_logprobs(host, prompts, Kp, K, max_new, T, seed, forced, gpu)
+    orc, lp_ref, zmax = _oracle_given_logprobs(host, prompts, Kp, K, max_new, T, seed, forced, gpu, mode=1)
     lens, R = gpu["len"], len(gpu["len"])
     assert lens.max() > 130
     valid = np.arange(max_new)[None, :] < lens[:, None]
