@@ -81,6 +81,8 @@ enum {
   DARTS_FLAG_PROFILE_ATTENTION = 4, /* bracket layer 0's attention of every decode step with CUDA events (bench roofline) */
   DARTS_FLAG_LM_HEAD_TILES = 16,    /* A/B switch: decode LM head on the 128 x 128 tile kernel instead of the persistent swap-AB kernel (both
                                      * sample the same distribution from the same Philox stream) */
+  DARTS_FLAG_CTA_PAIRS = 32,        /* dense projections on the CTA-pair (tcgen05 cta_group::2) stream-K kernel: two SMs share the activation block
+                                     * of one MMA of 256 weight rows (a third less L2 -> SM operand traffic from ~256 live rows on) */
   DARTS_FLAG_DUMP_HIDDEN = 8        /* keep the fp32 residual stream of every layer boundary of the last pass for darts_debug_hidden
                                      * ((n_layers + 1) x rows x d_model floats of workspace; parity only) */
 };

@@ -22,7 +22,7 @@ OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_KV_POOL_EXHAUSTED, ERR_WORKSPACE_TOO_S
 F32, BF16 = 0, 1
 ROW_ACTIVE, ROW_VALID, ROW_TRUNC, ROW_PRUNED = 0, 1, 2, 3
 MODE_AUTO, MODE_DUAL_END, MODE_SHORTEST_EARLY_STOP = 0, 1, 2
-FLAG_DUMP_LOGITS, FLAG_NO_PREFIX_SHARING, FLAG_PROFILE_ATTENTION, FLAG_DUMP_HIDDEN, FLAG_LM_HEAD_TILES = 1, 2, 4, 8, 16
+FLAG_DUMP_LOGITS, FLAG_NO_PREFIX_SHARING, FLAG_PROFILE_ATTENTION, FLAG_DUMP_HIDDEN, FLAG_LM_HEAD_TILES, FLAG_CTA_PAIRS = 1, 2, 4, 8, 16, 32
 
 _vp, _i32, _u32, _u64, _f32 = C.c_void_p, C.c_int32, C.c_uint32, C.c_uint64, C.c_float
 _pp = C.POINTER(C.c_void_p)

@@ -250,10 +250,13 @@ darts_status forward_layers(darts_ctx *c, int rows_ub, const int32_t *n_rows_dev
 SkGemm sk_gemm(darts_ctx *c, const XMaps *x, const CUtensorMap *w, int N, int K, int rows_ub, const int32_t *n_rows_dev) {
   SkGemm g{};
   g.w_map = w; g.x_maps = x; g.C = c->part; g.N = N; g.rows_ub = rows_ub; g.n_rows_dev = n_rows_dev; g.np_table = c->sk_np;
-  g.plan = sk_plan(c->n_sms, N, K, rows_ub, 0, n_rows_dev == nullptr);
+  g.pairs = c->use_pairs;
+  g.plan = g.pairs ? sk2_plan(c->n_sms, N, K, rows_ub, n_rows_dev == nullptr) : sk_plan(c->n_sms, N, K, rows_ub, 0, n_rows_dev == nullptr);
   g.slot_stride = (size_t)rows_ub * N;
   return g;
 }
+
+darts_status run_gemm_sk(darts_ctx *c, const SkGemm &g) { return g.pairs ? launch_gemm_sk2(c, g) : launch_gemm_sk(c, g); }
 
 darts_status forward_layers_tc(darts_ctx *c, int rows_ub, const int32_t *n_rows_dev) {
   const darts_model_desc &m = c->m;
@@ -265,19 +268,19 @@ darts_status forward_layers_tc(darts_ctx *c, int rows_ub, const int32_t *n_rows_
   // class's LIVE cost (launch-list times are serialised and cold); results are garbage in that mode.  Default build: nothing is skipped.
   for (int l = 0; l < L; ++l) {
     SkGemm g = sk_gemm(c, &c->xm_xn, &c->tm_wqkv[l], c->n_qkv, d, rows_ub, n_rows_dev);
-    if (!DARTS_SKIPPED(c, 1)) TRY(launch_gemm_sk(c, g));
+    if (!DARTS_SKIPPED(c, 1)) TRY(run_gemm_sk(c, g));
     if (!DARTS_SKIPPED(c, 2)) TRY(launch_rope_append_sk(c, l, sk_view(g), rows_ub, n_rows_dev));
     if (!(DARTS_SKIPPED(c, 4) && DARTS_SKIPPED(c, 8))) TRY(launch_attention(c, l, c->q, c->ao, rows_ub, n_rows_dev));
     g = sk_gemm(c, &c->xm_ao, &c->tm_wo[l], d, qd, rows_ub, n_rows_dev);
-    if (!DARTS_SKIPPED(c, 16)) TRY(launch_gemm_sk(c, g));
+    if (!DARTS_SKIPPED(c, 16)) TRY(run_gemm_sk(c, g));
     if (!DARTS_SKIPPED(c, 32)) TRY(launch_add_rmsnorm_sk(c, sk_view(g), c->mlp_norm[l], rows_ub, n_rows_dev));
     const void *next_norm = l + 1 < L ? c->attn_norm[l + 1] : c->final_norm;
     if (m.n_experts == 0) {
       g = sk_gemm(c, &c->xm_xn, &c->tm_wgu[l], 2 * F, d, rows_ub, n_rows_dev);
-      if (!DARTS_SKIPPED(c, 64)) TRY(launch_gemm_sk(c, g));
+      if (!DARTS_SKIPPED(c, 64)) TRY(run_gemm_sk(c, g));
       if (!DARTS_SKIPPED(c, 128)) TRY(launch_silu_mul_sk(c, sk_view(g), rows_ub, n_rows_dev));
       g = sk_gemm(c, &c->xm_act, &c->tm_wd[l], d, F, rows_ub, n_rows_dev);
-      if (!DARTS_SKIPPED(c, 256)) TRY(launch_gemm_sk(c, g));
+      if (!DARTS_SKIPPED(c, 256)) TRY(run_gemm_sk(c, g));
       if (!DARTS_SKIPPED(c, 512)) TRY(launch_add_rmsnorm_sk(c, sk_view(g), next_norm, rows_ub, n_rows_dev));
     } else {
       TRY(launch_moe_tc(c, l, next_norm, rows_ub, n_rows_dev));
@@ -473,7 +476,8 @@ darts_status darts_create(const darts_model_desc *m, const darts_weights *w, con
   c->use_pdl = getenv("DARTS_NO_PDL") == nullptr;
   c->skip_mask = getenv("DARTS_SKIP") ? (unsigned)strtoul(getenv("DARTS_SKIP"), nullptr, 0) : 0u;
 #endif
-  if ((s = gemm_sk_configure(c)) != DARTS_OK || (s = gemm_tc_configure(c)) != DARTS_OK || (s = attn_sm100_configure(c)) != DARTS_OK ||
+  c->use_pairs = (rt->flags & DARTS_FLAG_CTA_PAIRS) != 0;
+  if ((s = gemm_sk_configure(c)) != DARTS_OK || (s = gemm_sk2_configure(c)) != DARTS_OK || (s = gemm_tc_configure(c)) != DARTS_OK || (s = attn_sm100_configure(c)) != DARTS_OK ||
       (s = moe_configure(c)) != DARTS_OK)
     return s;
   if (c->has_weights) {
@@ -965,7 +969,7 @@ darts_status darts_debug_set_last_tokens(darts_ctx *c, const int32_t *tokens_hos
 darts_status darts_debug_gemm_scratch_floats(darts_ctx *c, int32_t rows, int32_t N, int32_t K, int32_t split_k, size_t *out) {
   if (!c || !out || rows <= 0 || N <= 0 || K <= 0 || split_k < 0) return DARTS_ERR_INVALID_ARG;
   if (!tc_shape_ok(N, K)) FAIL(c, DARTS_ERR_UNSUPPORTED, "tcgen05 GEMM needs K %% 64 == 0, N %% 4 == 0");
-  int slots = split_k > 0 ? split_k : sk_plan(c->n_sms, N, K, rows, 0, true).slots;
+  int slots = split_k > 0 ? split_k : (c->use_pairs ? sk2_plan(c->n_sms, N, K, rows, true) : sk_plan(c->n_sms, N, K, rows, 0, true)).slots;
   *out = (size_t)slots * rows * N;
   return DARTS_OK;
 }
@@ -983,8 +987,9 @@ darts_status darts_debug_gemm_bf16(darts_ctx *c, const void *X, const void *W, f
     TRY(tc_make_map(c, &tb, W, N, K, 128));
     SkGemm g{};
     g.w_map = &tb; g.x_maps = &xm; g.C = scratch; g.N = N; g.rows_ub = rows; g.slot_stride = (size_t)rows * N; g.np_table = c->sk_np;
-    g.plan = sk_plan(c->n_sms, N, K, rows, 0, true);
-    TRY(launch_gemm_sk(c, g));
+    g.pairs = c->use_pairs;
+    g.plan = g.pairs ? sk2_plan(c->n_sms, N, K, rows, true) : sk_plan(c->n_sms, N, K, rows, 0, true);
+    TRY(run_gemm_sk(c, g));
     if (!C) return DARTS_OK;
     return launch_sk_reduce(c, sk_view(g), C, rows);
   }

@@ -93,6 +93,7 @@ struct darts_ctx {
   // tensor-core path (bf16, kernels_gemm_tc.cu): split-K partial buffer, LM-head top-2 partials, tensor maps
   bool tc_path;                  // every GEMM of this model runs on tcgen05
   unsigned skip_mask;            // -DDARTS_PROFILING builds only (env DARTS_SKIP, bit per kernel class of a layer): skipped launches leave stale data — timing only
+  bool use_pairs;                // dense projections on the CTA-pair (cta_group::2) stream-K kernel (DARTS_FLAG_CTA_PAIRS)
   bool use_pdl;                  // launch the kernels of a step as programmatic dependents (-DDARTS_PROFILING builds: DARTS_NO_PDL=1 disables)
   float *part;                   // [S][rows][N] fp32 partials of the GEMM in flight
   size_t part_bytes;
@@ -252,6 +253,9 @@ darts_status tc_make_xmaps(darts_ctx *c, XMaps *out, const void *base, long long
 bool tc_shape_ok(int N, int K);
 // stream-K weight-streaming GEMM (kernels_gemm_sk.cu)
 #define SK_ROWBLOCK 256            // activation rows per MMA N block
+#ifndef SK_RB512_MAX
+#define SK_RB512_MAX 384           // largest live row count served as ONE 512-row block (two MMA N blocks sharing the weight tile)
+#endif
 #define SK_NP_TABLE 2048           // >= tiles of a split (non whole-tile) dense launch: n_wtiles * row blocks < 8 * SMs
 struct SkPlan { int nkb, n_wtiles, P, unit_tile, slots, stage_bytes, n_stages, tm_cols, n_acc; };   // stage / TMEM fields: grouped mode only
 struct SkGemm {
@@ -262,6 +266,7 @@ struct SkGemm {
   int N, rows_ub;
   const int32_t *n_rows_dev;
   int32_t *np_table;                  // dense stream-K: pieces per tile, written by each tile's head piece for the consumers (NULL: not kept)
+  bool pairs;                         // run on the CTA-pair kernel (plan from sk2_plan)
   const int32_t *rb_list, *n_rb_dev;  // grouped: {row0, nrows, group id, -} per row block, count on the device
   int w_rows_per_group;               // grouped: weight row base of a block = group id * w_rows_per_group
   SkPlan plan;
@@ -272,13 +277,15 @@ struct SkView {
   size_t slot_stride;
   int N, nkb, n_wtiles, P, unit_tile;
   const int32_t *np_table;            // pieces per tile, written by the GEMM that produced `part` (NULL: closed form)
+  int rb512;                          // 1: the producer used sk_rb_rows (one 512-row block for 257..384 live rows); 0: 256-row blocks always (CTA-pair kernel)
 };
 // Activation rows per row block of a DENSE launch, decided from the LIVE row count on the device (never from the host's stale upper
 // bound: the block size fixes where a tile's pieces are cut, i.e. the fp32 summation order, and that must not depend on timing).
 // 257..384 live rows: one 512-row block = two MMA N blocks per stage sharing the weight tile; otherwise 256-row blocks.
-__host__ __device__ __forceinline__ int sk_rb_rows(int live) { return (live > SK_ROWBLOCK && live <= 384) ? 2 * SK_ROWBLOCK : SK_ROWBLOCK; }
+__host__ __device__ __forceinline__ int sk_rb_rows(int live) { return (live > SK_ROWBLOCK && live <= SK_RB512_MAX) ? 2 * SK_ROWBLOCK : SK_ROWBLOCK; }
 // CTA that owns unit u when T units are cut into P ranges [c*T/P, (c+1)*T/P)
 __host__ __device__ __forceinline__ int sk_owner(int u, int P, int T) { return ((u + 1) * P - 1) / T; }
+__host__ __device__ __forceinline__ int sk_view_rb_rows(const SkView &v, int live) { return v.rb512 ? sk_rb_rows(live) : SK_ROWBLOCK; }
 __host__ __device__ __forceinline__ int sk_npieces(const SkView &v, int n_rb, int rb_rows, int col, int row) {
   if (v.unit_tile) return 1;
   int t = (col >> 7) * n_rb + (rb_rows == 2 * SK_ROWBLOCK ? row / (2 * SK_ROWBLOCK) : row / SK_ROWBLOCK);
@@ -302,7 +309,11 @@ darts_status launch_score_gather(darts_ctx *c, int S, int n_pend);
 darts_status launch_score_scatter(darts_ctx *c, int n_pend);
 darts_status launch_score_finalize(darts_ctx *c, int n_tiles, int rows);
 darts_status launch_score_logits(darts_ctx *c, int rows);
-inline SkView sk_view(const SkGemm &g) { return SkView{g.C, g.slot_stride, g.N, g.plan.nkb, g.plan.n_wtiles, g.plan.P, g.plan.unit_tile, g.np_table}; }
+inline SkView sk_view(const SkGemm &g) { return SkView{g.C, g.slot_stride, g.N, g.plan.nkb, g.plan.n_wtiles, g.plan.P, g.plan.unit_tile, g.np_table, g.pairs ? 0 : 1}; }
+// CTA-pair (cta_group::2) variant (kernels_gemm_sk2.cu)
+SkPlan sk2_plan(int n_sms, int N, int K, int rows_ub, bool rows_exact);
+darts_status launch_gemm_sk2(darts_ctx *c, const SkGemm &g);
+darts_status gemm_sk2_configure(darts_ctx *c);
 darts_status launch_add_rmsnorm_sk(darts_ctx *c, const SkView &v, const void *w, int rows_ub, const int32_t *n_rows_dev);
 darts_status launch_silu_mul_sk(darts_ctx *c, const SkView &v, int rows_ub, const int32_t *n_rows_dev);
 darts_status launch_rope_append_sk(darts_ctx *c, int layer, const SkView &v, int rows_ub, const int32_t *n_rows_dev);

@@ -87,7 +87,7 @@ __global__ void __launch_bounds__(256) add_rmsnorm_sk_k(float *__restrict__ h, S
   pdl_wait();
   const int slot = blockIdx.x, live = live_rows(n_rows_dev, rows_ub);
   if (slot >= live) return;
-  const int rbr = sk_rb_rows(live), n_rb = (live + rbr - 1) / rbr;
+  const int rbr = sk_view_rb_rows(v, live), n_rb = (live + rbr - 1) / rbr;
   float4 *hr = reinterpret_cast<float4 *>(h + (size_t)slot * d);
   float ss = 0.f;
   for (int k = threadIdx.x; k < d / 4; k += blockDim.x) {
@@ -127,7 +127,7 @@ __global__ void __launch_bounds__(256) add_rmsnorm_sk_reg_k(float *__restrict__ 
   pdl_wait();
   const int slot = blockIdx.x, live = live_rows(n_rows_dev, rows_ub);
   if (slot >= live) return;
-  const int rbr = sk_rb_rows(live), n_rb = (live + rbr - 1) / rbr;
+  const int rbr = sk_view_rb_rows(v, live), n_rb = (live + rbr - 1) / rbr;
   float4 *hr = reinterpret_cast<float4 *>(h + (size_t)slot * d);
   const size_t st = v.slot_stride / 4;
   float4 x[ITERS], acc[ITERS];
@@ -198,7 +198,7 @@ __global__ void __launch_bounds__(256) silu_mul_sk_k(SkView v, __nv_bfloat16 *__
   if (slot >= live) return;
   const int k = (blockIdx.x * blockDim.x + threadIdx.x) * 4;
   if (k >= F) return;
-  const int rbr = sk_rb_rows(live), n_rb = (live + rbr - 1) / rbr;
+  const int rbr = sk_view_rb_rows(v, live), n_rb = (live + rbr - 1) / rbr;
   const size_t row = (size_t)slot * 2 * F;
   float4 g, u;
   sk_sum4x2(v, sk_npieces(v, n_rb, rbr, k, slot), row + k, sk_npieces(v, n_rb, rbr, F + k, slot), row + F + k, g, u);
@@ -222,7 +222,7 @@ __global__ void __launch_bounds__(128) rope_append_sk_k(SkView v, __nv_bfloat16 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int head = blockIdx.x * 4 + warp;
   if (head >= Hq + 2 * Hkv) return;
-  const int rbr = sk_rb_rows(live), n_rb = (live + rbr - 1) / rbr;
+  const int rbr = sk_view_rb_rows(v, live), n_rb = (live + rbr - 1) / rbr;
   const int half = hd >> 1, col0 = head * hd;
   const size_t row = (size_t)slot * (Hq + 2 * Hkv) * hd + col0;
   const int page = slot_dst_page[slot], off = slot_dst_off[slot];

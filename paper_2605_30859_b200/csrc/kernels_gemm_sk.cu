@@ -356,7 +356,7 @@ __global__ void sk_reduce_k(SkView v, float *__restrict__ out, int rows) {
   size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= (size_t)rows * v.N) return;
   int r = (int)(i / v.N), n = (int)(i % v.N);
-  int rbr = sk_rb_rows(rows), n_rb = (rows + rbr - 1) / rbr;
+  int rbr = sk_view_rb_rows(v, rows), n_rb = (rows + rbr - 1) / rbr;
   int np = sk_npieces(v, n_rb, rbr, n, r);
   float a = v.part[i];
   for (int s = 1; s < np; ++s) a += v.part[(size_t)s * v.slot_stride + i];

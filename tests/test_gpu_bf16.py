@@ -53,9 +53,10 @@ def run_stepwise(d, prompts, Kp, K, T, seed, forced, routing=False, **kw):
 # std 0.02 is the configs' init recipe (tolerance: north_star's 2e-2).  std 0.08 is a stress case outside the recipe:
 # sharper softmaxes amplify the bf16 rounding of q, k, P and the activations, so it gets twice the tolerance.
 # vocab 1000: the last 128-id tile of the LM head holds 104 ids and its last warp quadrant 8 (ragged tail of the sampling epilogue).
-@pytest.mark.parametrize("qk_norm,std,tol,vocab", [(False, 0.02, LOGIT_TOL_BF16, 1024), (True, 0.02, LOGIT_TOL_BF16, 1024),
-                                                   (False, 0.08, 2 * LOGIT_TOL_BF16, 1024), (False, 0.02, LOGIT_TOL_BF16, 1000)])
-def test_small_bf16_model_matches_oracle(qk_norm, std, tol, vocab):
+@pytest.mark.parametrize("qk_norm,std,tol,vocab,pairs", [(False, 0.02, LOGIT_TOL_BF16, 1024, False), (True, 0.02, LOGIT_TOL_BF16, 1024, False),
+                                                         (False, 0.08, 2 * LOGIT_TOL_BF16, 1024, False), (False, 0.02, LOGIT_TOL_BF16, 1000, False),
+                                                         (True, 0.02, LOGIT_TOL_BF16, 1000, True)])      # projections on the CTA-pair kernel
+def test_small_bf16_model_matches_oracle(qk_norm, std, tol, vocab, pairs):
     from paper_2605_30859_b200 import api
     cfg = dict(SMALL, qk_norm=qk_norm, vocab=vocab)
     seed, G, P, max_new, K, T = 5, 3, 70, 40, 2, 1.0
@@ -63,7 +64,7 @@ def test_small_bf16_model_matches_oracle(qk_norm, std, tol, vocab):
     prompts = [rng.integers(0, cfg["vocab"] - 1, size=n).astype(np.int32) for n in (70, 33, 64)]
     Kp = np.asarray([4, 5, 3], dtype=np.int32)
     forced = wl.make_forced_len(Kp, dict(kind="lognormal", mu=2.8, sigma=0.7, lo=2, hi=60), seed)
-    d, host = make_ctx(cfg, seed, G, 5, P, max_new, page=64, flags=api.FLAG_DUMP_LOGITS, std=std)
+    d, host = make_ctx(cfg, seed, G, 5, P, max_new, page=64, flags=api.FLAG_DUMP_LOGITS | (api.FLAG_CTA_PAIRS if pairs else 0), std=std)
     gpu, glog = run_stepwise(d, prompts, Kp, K, T, seed, forced)
     orc = ro.rollout_stepwise(host, prompts, Kp, K, max_new, T, seed, forced_len=forced, teacher=gpu["tokens"], keep_logits=True)
     for k in ("len", "status", "sel", "sel_mask", "close_step"):

@@ -14,7 +14,7 @@ from tests.gpu_util import rel_inf
 pytestmark = pytest.mark.gpu
 
 
-def _case(name, prompts_sampled, P=None, steps=3):
+def _case(name, prompts_sampled, P=None, steps=3, flags=0):
     import torch
     from paper_2605_30859_b200 import api
     c = wl.CONFIGS[name]
@@ -28,7 +28,7 @@ def _case(name, prompts_sampled, P=None, steps=3):
     R = int(Kp.sum())
     offs = np.concatenate([[0], np.cumsum(Kp)])
     d = api.Darts(model, page_size=64, n_pages=G * ((P + 63) // 64) + R * 2 + 8, max_rows=R, max_prompts=G, max_prompt_len=P, max_new=64,
-                  flags=api.FLAG_DUMP_LOGITS)
+                  flags=api.FLAG_DUMP_LOGITS | flags)
     d.prefill(list(prompts), Kp, K, temperature=T, seed=seed, forced_len=None)
     rows_sampled = [int(offs[i] + (7 * i + 3) % Kp[i]) for i in prompts_sampled]
     moe = cfg["n_experts"] > 0
@@ -97,6 +97,12 @@ def _case(name, prompts_sampled, P=None, steps=3):
 
 def test_c3_width_sampled_rows_match_oracle():
     _case("c3", [0, 17, 31])
+
+
+def test_c3_width_on_the_cta_pair_kernel_matches_oracle():
+    # the four projections of every layer on the tcgen05 cta_group::2 stream-K kernel (512 rows = two 256-row blocks per weight-tile pair)
+    from paper_2605_30859_b200 import api
+    _case("c3", [5], steps=2, flags=api.FLAG_CTA_PAIRS)
 
 
 def test_c4_width_sampled_rows_match_oracle():

@@ -17,6 +17,15 @@ def ctx():
     d.close()
 
 
+@pytest.fixture(scope="module")
+def ctx_pairs():
+    from paper_2605_30859_b200 import api
+    d = api.Darts(dict(cfg=dict(wl.CONFIGS["c2"]["model"])), page_size=64, n_pages=64, max_rows=8, max_prompts=2, max_prompt_len=64, max_new=64,
+                  flags=api.FLAG_CTA_PAIRS)
+    yield d
+    d.close()
+
+
 def _mk(shape, seed, scale=1.0):
     g = torch.Generator(device="cuda").manual_seed(seed)
     return (torch.randn(*shape, generator=g, device="cuda") * scale).to(torch.bfloat16)
@@ -51,6 +60,21 @@ def test_gemm_matches_oracle(ctx, rows, N, K, S):
     # bf16 products are exact in fp32; only the fp32 accumulation order differs: ~K * 2^-24 relative to sum |x w|
     tol = 4 * K * 2.0 ** -24 * float(np.max(np.abs(X.float().cpu().numpy()) @ np.abs(W.float().cpu().numpy()).T))
     assert np.max(np.abs(got - ref)) <= tol, (np.max(np.abs(got - ref)), tol)
+
+
+@pytest.mark.parametrize("rows,N,K", [
+    (1, 128, 64), (16, 256, 256), (37, 132, 192), (200, 512, 1024), (256, 384, 512), (300, 1000, 2560), (512, 640, 512),
+    (289, 2560, 4096), (700, 640, 1024), (64, 6144, 2560), (130, 2560, 9728), (512, 19456, 2560), (2048, 19456, 256),
+])
+def test_cta_pair_gemm_matches_oracle(ctx_pairs, rows, N, K):
+    """The same shapes on the CTA-pair (tcgen05 cta_group::2) stream-K kernel: M = 256 weight rows per MMA, each CTA of the pair stages
+    its own weight tile and half of the activation rows; odd tile counts (N = 132, 1000, 640 ...) leave the pair's second tile empty."""
+    X, W = _mk((rows, K), rows + N), _mk((N, K), K + 3, 0.05)
+    got = ctx_pairs.debug_gemm_bf16(X, W, split_k=0).cpu().numpy().astype(np.float64)
+    ref = linear(X.float().cpu().numpy(), W.float().cpu().numpy())
+    tol = 4 * K * 2.0 ** -24 * float(np.max(np.abs(X.float().cpu().numpy()) @ np.abs(W.float().cpu().numpy()).T))
+    assert np.max(np.abs(got - ref)) <= tol, (np.max(np.abs(got - ref)), tol)
+    assert torch.equal(ctx_pairs.debug_gemm_bf16(X, W, split_k=0).cpu(), torch.from_numpy(got).float())
 
 
 @pytest.mark.parametrize("S", [4, 0])
