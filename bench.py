@@ -27,7 +27,7 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 T_START = time.perf_counter()
-EXTRA_EST_S = {"c4": 260, "c5": 290}     # one 16 384-step rollout + building the model (c5: 61 GB of random weights)
+EXTRA_EST_S = {"c4": 260, "c5": 290, "c5_early": 130}     # one rollout + building the model (c5: 61 GB of random weights)
 
 KV_BYTES_PER_TOKEN_LAYER = {"c2": 2 * 8 * 128 * 2}
 
@@ -169,11 +169,11 @@ def oracle_attention_sample(x_full_seed=0, n_rows=32):
 # ------------------------------------------------------------------------------------------------ full rollouts (c3 / c4 / c5)
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE attn_main_k launch from an `ncu --set full` capture (profiles/), with the
 # algorithmic bytes of that same launch beside it (launches differ in size over a rollout; `achieved` is the rollout average)
-NCU_ATTENTION_TRAFFIC = {"c3": dict(dram_bytes=1.2947e9, algorithmic_bytes=1.2322e9, ratio=1.051,
-                                    launch="decode step 1001 of the seed-0 rollout: 289 rows, mean suffix 1003 tokens, 19 open groups",
-                                    source="profiles/r1_launches_c3_step1000.md (ncu --set full, bench.py --profile-step 1000)")}
+NCU_ATTENTION_TRAFFIC = {"c3": dict(dram_bytes=1.2977e9, algorithmic_bytes=1.2277e9, ratio=1.057,
+                                    launch="decode step 1001 of the seed-0 rollout (the first warm-up rollout's inputs): 288 rows, mean suffix 1003 tokens, 19 open groups",
+                                    source="profiles/r2_launches_c3_step1000.md (ncu --set full -k attn_main_k, bench.py --profile-step 1000, round 2)")}
 # the same for ONE launch of the config-2 microbench (seed 0: 3 131 237 suffix tokens + 128 x 1024 prefix tokens = 13.396 GB algorithmic)
-NCU_ATTENTION_C2 = dict(ncu_dram_bytes=13.95e9, ncu_traffic_over_algorithmic=1.041, ncu_source="profiles/r1_attention_c2.md")
+NCU_ATTENTION_C2 = dict(ncu_dram_bytes=13.958e9, ncu_traffic_over_algorithmic=1.042, ncu_source="profiles/r2_attention_c2.md")
 KV_POOL_CAP_BYTES = {"c3": 64e9, "c4": 100e9, "c5": 36e9}
 
 
@@ -467,12 +467,15 @@ def main():
         # while the whole command stays clear of the driver's step limit
         if world == 1 and not (args.max_new or args.G or args.layers) and name == "c3" and not args.no_extra:
             line["extra_workloads"] = {}
-            for extra in ("c4", "c5"):
+            for extra in ("c4", "c5", "c5_early"):
                 spent = time.perf_counter() - T_START
                 if spent + EXTRA_EST_S[extra] > args.budget_s:
                     line["extra_workloads"][extra] = dict(skipped=f"{spent:.0f} s spent, needs ~{EXTRA_EST_S[extra]} s, budget {args.budget_s} s (driver step limit 1800 s)")
                     continue
-                r = rollout_bench(extra, 0, 1, 0, args, rank, world, peaks, keep_model=False)
+                # c5_early: config 5 with shortest-only + early stop FORCED (R17: under the paper's rule K' = 12 < 2K is dual-end and
+                # never stops early, while BASELINE.json's metric says "K'-of-K early stop"): a labelled variant, not the paper's rule
+                xargs = argparse.Namespace(**{**vars(args), "mode": "early"}) if extra == "c5_early" else args
+                r = rollout_bench(extra.split("_")[0], 0, 1, 0, xargs, rank, world, peaks, keep_model=False)
                 line["extra_workloads"][extra] = dict(value=r["value"], unit="tokens/s", ms_per_rollout=r["ms_per_step"], warmup_rollouts=0, timed_rollouts=1,
                                                       config=r["config"], attention_roofline_frac=r["roofline"]["frac"], attention_share_of_step=r["roofline"]["share_of_step"],
                                                       decode_path_roofline_frac=r["decode_path_roofline"]["frac"], gpu_launches=r["gpu_launches"])
