@@ -176,12 +176,25 @@ __global__ void __launch_bounds__(THREADS, 2) attn_main_k(Params p) {
         int first = it[0], page_begin = it[2], n_tok = it[3], is_pre = it[5];
         const int32_t *table = is_pre ? p.g_prefix_pages + (size_t)p.slot_prompt[first] * p.mpp : p.row_pages + (size_t)p.slot_row[first] * p.msp;
         int npg = (n_tok + PAGE - 1) / PAGE;
+        // A row's NEWEST page is on average half empty, and a whole tile pair is 32 KB: at 512 rows that is ~67 MB per layer of bytes nobody
+        // reads.  For a unit whose query rows fit one m-tile (the token-split path: a warp skips a 16-token group that lies wholly beyond the
+        // valid tokens, so un-copied shared memory is never touched) the last page is fetched as the valid part of K and of V, rounded up to
+        // 16 tokens — two smaller copies; only when that saves at least half of the tile.
+        const bool tok_split = it[1] * p.rep <= 16 && !p.causal;
         for (int pg = 0; pg < npg; ++pg) {
           mbar_wait(&sm.empty[stage], phase ^ 1);
           int page_id = table[page_begin + pg];
           const __nv_bfloat16 *src = p.kv_layer + (size_t)page_id * p.page_elems + (size_t)kvh * 2 * p.tile_elems;
-          mbar_expect_tx(&sm.full[stage], STAGE_BYTES);
-          bulk_g2s(sm.stage[stage], src, STAGE_BYTES, &sm.full[stage]);
+          const int v16 = (min(PAGE, n_tok - pg * PAGE) + 15) & ~15;
+          if (tok_split && v16 <= PAGE / 2) {
+            const int bytes = v16 * HD * 2;
+            mbar_expect_tx(&sm.full[stage], 2 * bytes);
+            bulk_g2s(sm.stage[stage], src, bytes, &sm.full[stage]);
+            bulk_g2s(sm.stage[stage] + PAGE * HD * 2, src + PAGE * HD, bytes, &sm.full[stage]);
+          } else {
+            mbar_expect_tx(&sm.full[stage], STAGE_BYTES);
+            bulk_g2s(sm.stage[stage], src, STAGE_BYTES, &sm.full[stage]);
+          }
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
       }

@@ -23,20 +23,32 @@ def check(cfg, prompts, Kp, K, max_new, T, seed, forced, page, margin_tol, **kw)
     d.prefill(prompts, Kp, K, temperature=T, seed=seed, forced_len=forced, **kw)
     d.run_to_completion()
     gpu = d.results()
-    orc = ro.rollout_stepwise(host, prompts, Kp, K, max_new, T, seed, forced_len=forced, teacher=gpu["tokens"], **kw)
+    bf16 = cfg["dtype"] == "bf16"
+    orc = ro.rollout_stepwise(host, prompts, Kp, K, max_new, T, seed, forced_len=forced, teacher=gpu["tokens"], keep_logits=bf16, **kw)
     for key in ("len", "status", "sel", "sel_mask", "close_step"):
         assert np.array_equal(gpu[key], orc[key]), key
+    near = total = 0
     for r in range(len(orc["len"])):
         for s in range(orc["len"][r]):
-            if orc["margins"][r, s] > margin_tol and not (s + 1 == orc["len"][r] and gpu["status"][r] == VALID):
-                assert orc["oracle_tokens"][r, s] == gpu["tokens"][r, s], (r, s)
+            # fp32: north_star's 1e-3.  bf16 (R12): a token may differ only where the oracle's margin is within twice the logit
+            # error the bf16 tolerance allows at this position, 2 x 2e-2 x |z|_inf / T (T = 0: greedy on z itself)
+            tol = 2 * 2e-2 * float(np.max(np.abs(orc["logits"][(r, s)]))) / (T if T else 1.0) + 1e-3 if bf16 else margin_tol
+            total += 1
+            if orc["margins"][r, s] > tol:
+                if not (s + 1 == orc["len"][r] and gpu["status"][r] == VALID):
+                    assert orc["oracle_tokens"][r, s] == gpu["tokens"][r, s], (r, s)
+            else:
+                near += 1
+    if total:
+        print(f"{cfg['dtype']}: {near}/{total} sampled tokens inside the near-tie band (not compared)")
+        assert near <= 0.25 * total, (near, total)
     cnt = d.counters()
     assert cnt["n_generated_tokens"] == orc["n_generated_tokens"] and cnt["n_kept_tokens"] == orc["n_kept_tokens"]
     d.close()
     return gpu
 
 
-@pytest.mark.parametrize("cfg,page,tol", [(F32, 16, 1e-3), (BF16, 64, 0.15)])
+@pytest.mark.parametrize("cfg,page,tol", [(F32, 16, 1e-3), (BF16, 64, None)])
 def test_greedy_temperature_zero(cfg, page, tol):
     rng = np.random.default_rng(1)
     prompts = [rng.integers(0, cfg["vocab"] - 1, size=n).astype(np.int32) for n in (9, 20)]
@@ -46,7 +58,7 @@ def test_greedy_temperature_zero(cfg, page, tol):
     assert np.array_equal(g["tokens"][0, :2], g["tokens"][1, :2])
 
 
-@pytest.mark.parametrize("cfg,page,tol", [(F32, 16, 1e-3), (BF16, 64, 0.15)])
+@pytest.mark.parametrize("cfg,page,tol", [(F32, 16, 1e-3), (BF16, 64, None)])
 def test_maximum_pool_of_32_samples(cfg, page, tol):
     rng = np.random.default_rng(2)
     prompts = [rng.integers(0, cfg["vocab"] - 1, size=33).astype(np.int32)]
@@ -62,7 +74,7 @@ def test_one_token_prompt_and_max_new_one():
     assert np.all(g["len"] == 1) and set(np.unique(g["status"]).tolist()) <= {VALID, TRUNC}
 
 
-@pytest.mark.parametrize("cfg,page,tol", [(F32, 16, 1e-3), (BF16, 64, 0.15)])
+@pytest.mark.parametrize("cfg,page,tol", [(F32, 16, 1e-3), (BF16, 64, None)])
 def test_all_rows_stop_at_their_first_token_and_all_rows_truncate(cfg, page, tol):
     rng = np.random.default_rng(4)
     prompts = [rng.integers(0, cfg["vocab"] - 1, size=n).astype(np.int32) for n in (6, 17, 11)]
