@@ -25,6 +25,9 @@ constexpr int STAGES = 3;
 constexpr int STAGE_BYTES = 2 * PAGE * HD * 2;   // K tile + V tile of one (page, head)
 constexpr int N_CONS = 4;                   // consumer warps
 constexpr int THREADS = (N_CONS + 1) * 32;
+#ifndef ATTN_PARTIAL_LAST_PAGE
+#define ATTN_PARTIAL_LAST_PAGE 1            // fetch only the valid part of a row's newest page (A/B switch: -DATTN_PARTIAL_LAST_PAGE=0)
+#endif
 constexpr int ITEM_INTS = 6;                // first_slot, n_slots, page_begin, n_tokens, chunk_k, is_prefix
 
 struct Smem {
@@ -180,7 +183,7 @@ __global__ void __launch_bounds__(THREADS, 2) attn_main_k(Params p) {
         // reads.  For a unit whose query rows fit one m-tile (the token-split path: a warp skips a 16-token group that lies wholly beyond the
         // valid tokens, so un-copied shared memory is never touched) the last page is fetched as the valid part of K and of V, rounded up to
         // 16 tokens — two smaller copies; only when that saves at least half of the tile.
-        const bool tok_split = it[1] * p.rep <= 16 && !p.causal;
+        const bool tok_split = ATTN_PARTIAL_LAST_PAGE && it[1] * p.rep <= 16 && !p.causal;
         for (int pg = 0; pg < npg; ++pg) {
           mbar_wait(&sm.empty[stage], phase ^ 1);
           int page_id = table[page_begin + pg];
