@@ -25,6 +25,9 @@ constexpr int STAGES = 3;
 constexpr int STAGE_BYTES = 2 * PAGE * HD * 2;   // K tile + V tile of one (page, head)
 constexpr int N_CONS = 4;                   // consumer warps
 constexpr int THREADS = (N_CONS + 1) * 32;
+#ifndef ATTN_TPATH
+#define ATTN_TPATH 1                        // units with <= 8 query rows: S^T = K Q^T (tokens on the MMA's m) (A/B switch: -DATTN_TPATH=0)
+#endif
 #ifndef ATTN_PARTIAL_LAST_PAGE
 #define ATTN_PARTIAL_LAST_PAGE 1            // fetch only the valid part of a row's newest page (A/B switch: -DATTN_PARTIAL_LAST_PAGE=0)
 #endif
@@ -78,6 +81,9 @@ __device__ __forceinline__ void mma16816(float (&c)[4], uint32_t a0, uint32_t a1
   asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
                : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
                : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+}
+__device__ __forceinline__ void movmatrix_t(uint32_t a, uint32_t &d) {
+  asm volatile("movmatrix.sync.aligned.m8n8.trans.b16 %0, %1;" : "=r"(d) : "r"(a));
 }
 __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
   __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
@@ -155,6 +161,29 @@ __device__ __forceinline__ void pv_16tok(uint32_t sV, int tokb, uint32_t a0, uin
   }
 }
 
+// One round of the cross-warp merge of a token-split unit: rows 4 rb .. 4 rb + 3, one consumer warp per row, 4 dims per lane.
+__device__ __forceinline__ void merge_round(Smem &sm, const Params &p, int rb, int n_rows, int first, int kvh, int chunk_k) {
+  int rr = threadIdx.x >> 5, d4 = (threadIdx.x & 31) * 4;     // 128 consumer threads: row rr, dims d4..d4+3
+  int r = rb * 4 + rr;
+  if (r < n_rows) {
+    float M = -INFINITY;
+#pragma unroll
+    for (int wv = 0; wv < N_CONS; ++wv) M = fmaxf(M, sm.ml[wv][r][0]);
+    float L = 0.f, a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
+#pragma unroll
+    for (int wv = 0; wv < N_CONS; ++wv) {
+      float sc = exp2f((sm.ml[wv][r][0] - M) * p.c);
+      float4 v = *reinterpret_cast<const float4 *>(&sm.scratch[wv][rr][d4]);
+      L += sc * sm.ml[wv][r][1];
+      a0 += sc * v.x; a1 += sc * v.y; a2 += sc * v.z; a3 += sc * v.w;
+    }
+    int slot = first + r / p.rep, head = kvh * p.rep + r % p.rep;
+    size_t pi = (size_t)(p.part_base[slot] + chunk_k) * p.Hq + head;
+    if ((threadIdx.x & 31) == 0) { p.part_ml[pi * 2] = M; p.part_ml[pi * 2 + 1] = L; }
+    *reinterpret_cast<float4 *>(p.part_acc + pi * HD + d4) = make_float4(a0, a1, a2, a3);
+  }
+}
+
 __global__ void __launch_bounds__(THREADS, 2) attn_main_k(Params p) {
   extern __shared__ unsigned char smem_raw[];
   Smem &sm = *reinterpret_cast<Smem *>(((uintptr_t)smem_raw + 127) & ~(uintptr_t)127);
@@ -213,6 +242,115 @@ __global__ void __launch_bounds__(THREADS, 2) attn_main_k(Params p) {
     int first = it[0], n_slots = it[1], n_tok = it[3], chunk_k = it[4];
     int n_rows = n_slots * p.rep;
     const int tok_begin = it[2] * PAGE;                            // first token of this item within its page table
+    if (ATTN_TPATH && n_rows <= 8) {
+      // ---- transposed token-split path (a decode row's own pages: n_rows = rep <= 8).  S^T = K . Q^T puts the warp's 16 tokens on the
+      // MMA's m dimension and the <= 8 query rows on n = 8: one MMA per k-step instead of two, and O^T (128 dims x 8 rows) is 32
+      // accumulators instead of 64.  C fragment of S^T: c0/c1 = token g, rows 2t/2t+1; c2/c3 = token g+8.
+      uint32_t Qb[8][2];
+      {
+        const __nv_bfloat16 *q = g < n_rows ? p.q + ((size_t)(first + g / p.rep) * p.Hq + kvh * p.rep + g % p.rep) * HD : nullptr;
+#pragma unroll
+        for (int ks = 0; ks < 8; ++ks) {
+          int d = 16 * ks + 2 * t;
+          Qb[ks][0] = q ? *reinterpret_cast<const uint32_t *>(q + d) : 0u;
+          Qb[ks][1] = q ? *reinterpret_cast<const uint32_t *>(q + d + 8) : 0u;
+        }
+      }
+      int limA = n_tok, limB = n_tok;                              // token limits of rows 2t and 2t+1
+      if (p.causal) {
+        int rA = 2 * t, rB = rA + 1;
+        limA = rA < n_rows ? min(n_tok, p.slot_npre[first + rA / p.rep] - tok_begin) : 0;
+        limB = rB < n_rows ? min(n_tok, p.slot_npre[first + rB / p.rep] - tok_begin) : 0;
+      }
+      float OT[8][4];
+#pragma unroll
+      for (int i = 0; i < 8; ++i) OT[i][0] = OT[i][1] = OT[i][2] = OT[i][3] = 0.f;
+      float mA = -INFINITY, mB = -INFINITY, lA = 0.f, lB = 0.f;
+      const int npg_t = (n_tok + PAGE - 1) / PAGE;
+      const int mat = lane >> 3, r8 = lane & 7;
+      for (int pg = 0; pg < npg_t; ++pg) {
+        mbar_wait(&sm.full[stage], phase);
+        const uint32_t sK = smem_u32(sm.stage[stage]), sV = sK + PAGE * HD * 2;
+        const int valid = min(PAGE, n_tok - pg * PAGE);
+        const int tok0 = warp * 16;
+        if (tok0 < valid) {
+          float c[4] = {0.f, 0.f, 0.f, 0.f};
+          {
+            const uint32_t rowaddr = sK + (tok0 + (mat & 1) * 8 + r8) * (HD * 2);
+#pragma unroll
+            for (int ks = 0; ks < 8; ++ks) {
+              uint32_t a0, a1, a2, a3;
+              ldsm4(rowaddr + (((2 * ks + (mat >> 1)) ^ r8) << 4), a0, a1, a2, a3);
+              mma16816(c, a0, a1, a2, a3, Qb[ks][0], Qb[ks][1]);
+            }
+          }
+          const int vA = limA - pg * PAGE, vB = limB - pg * PAGE, tkA = tok0 + g, tkB = tkA + 8;
+          if (tkA >= vA) c[0] = -INFINITY;
+          if (tkA >= vB) c[1] = -INFINITY;
+          if (tkB >= vA) c[2] = -INFINITY;
+          if (tkB >= vB) c[3] = -INFINITY;
+          float mxA = fmaxf(c[0], c[2]), mxB = fmaxf(c[1], c[3]);
+#pragma unroll
+          for (int o = 4; o <= 16; o <<= 1) {
+            mxA = fmaxf(mxA, __shfl_xor_sync(0xffffffffu, mxA, o));
+            mxB = fmaxf(mxB, __shfl_xor_sync(0xffffffffu, mxB, o));
+          }
+          const float mnA = fmaxf(mA, mxA), mnB = fmaxf(mB, mxB);
+          const float msA = mnA == -INFINITY ? 0.f : mnA, msB = mnB == -INFINITY ? 0.f : mnB;
+          const float corrA = exp2f((mA - msA) * p.c), corrB = exp2f((mB - msB) * p.c);
+          const float p0 = exp2f(fmaf(c[0], p.c, -msA * p.c)), p2 = exp2f(fmaf(c[2], p.c, -msA * p.c));
+          const float p1 = exp2f(fmaf(c[1], p.c, -msB * p.c)), p3 = exp2f(fmaf(c[3], p.c, -msB * p.c));
+          lA = lA * corrA + p0 + p2;
+          lB = lB * corrB + p1 + p3;
+          mA = mnA;
+          mB = mnB;
+#pragma unroll
+          for (int i = 0; i < 8; ++i) { OT[i][0] *= corrA; OT[i][2] *= corrA; OT[i][1] *= corrB; OT[i][3] *= corrB; }
+          // P^T (tokens x rows) -> the B operand (k = tokens, n = rows): transpose the two 8x8 blocks
+          uint32_t b0, b1;
+          movmatrix_t(pack_bf16(p0, p1), b0);
+          movmatrix_t(pack_bf16(p2, p3), b1);
+          {
+            const uint32_t rowaddr = sV + (tok0 + (mat >> 1) * 8 + r8) * (HD * 2);
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+              uint32_t a0, a1, a2, a3;
+              ldsm4t(rowaddr + (((2 * i + (mat & 1)) ^ r8) << 4), a0, a1, a2, a3);
+              mma16816(OT[i], a0, a1, a2, a3, b0, b1);
+            }
+          }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&sm.empty[stage]);
+        if (++stage == STAGES) { stage = 0; phase ^= 1; }
+      }
+#pragma unroll
+      for (int o = 4; o <= 16; o <<= 1) {
+        lA += __shfl_xor_sync(0xffffffffu, lA, o);
+        lB += __shfl_xor_sync(0xffffffffu, lB, o);
+      }
+      if (g == 0) {
+        sm.ml[warp][2 * t][0] = mA; sm.ml[warp][2 * t][1] = lA;
+        sm.ml[warp][2 * t + 1][0] = mB; sm.ml[warp][2 * t + 1][1] = lB;
+      }
+      const int rounds_t = (n_rows + 3) >> 2;
+      for (int rb = 0; rb < rounds_t; ++rb) {
+        if ((t >> 1) == rb) {                                      // rows 4 rb .. 4 rb + 3 are held by t = 2 rb, 2 rb + 1
+          const int lr = 2 * (t & 1);
+#pragma unroll
+          for (int i = 0; i < 8; ++i) {
+            sm.scratch[warp][lr][16 * i + g] = OT[i][0];
+            sm.scratch[warp][lr + 1][16 * i + g] = OT[i][1];
+            sm.scratch[warp][lr][16 * i + g + 8] = OT[i][2];
+            sm.scratch[warp][lr + 1][16 * i + g + 8] = OT[i][3];
+          }
+        }
+        cons_bar();
+        merge_round(sm, p, rb, n_rows, first, kvh, chunk_k);
+        cons_bar();
+      }
+      continue;
+    }
     bool rowsplit = n_rows > 16;
     int mt = rowsplit ? warp : 0;                                  // m-tile this warp works on
     bool warp_has_rows = mt * 16 < n_rows;
@@ -323,25 +461,7 @@ __global__ void __launch_bounds__(THREADS, 2) attn_main_k(Params p) {
             *reinterpret_cast<float2 *>(&sm.scratch[warp][g - glo][nt * 8 + 2 * t]) = rs == 0 ? make_float2(O[nt][0], O[nt][1]) : make_float2(O[nt][2], O[nt][3]);
         }
         cons_bar();
-        int rr = threadIdx.x >> 5, d4 = (threadIdx.x & 31) * 4;     // 128 consumer threads: row rr, dims d4..d4+3
-        int r = rb * 4 + rr;
-        if (r < n_rows) {
-          float M = -INFINITY;
-#pragma unroll
-          for (int wv = 0; wv < N_CONS; ++wv) M = fmaxf(M, sm.ml[wv][r][0]);
-          float L = 0.f, a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
-#pragma unroll
-          for (int wv = 0; wv < N_CONS; ++wv) {
-            float sc = exp2f((sm.ml[wv][r][0] - M) * p.c);
-            float4 v = *reinterpret_cast<const float4 *>(&sm.scratch[wv][rr][d4]);
-            L += sc * sm.ml[wv][r][1];
-            a0 += sc * v.x; a1 += sc * v.y; a2 += sc * v.z; a3 += sc * v.w;
-          }
-          int slot = first + r / p.rep, head = kvh * p.rep + r % p.rep;
-          size_t pi = (size_t)(p.part_base[slot] + chunk_k) * p.Hq + head;
-          if ((threadIdx.x & 31) == 0) { p.part_ml[pi * 2] = M; p.part_ml[pi * 2 + 1] = L; }
-          *reinterpret_cast<float4 *>(p.part_acc + pi * HD + d4) = make_float4(a0, a1, a2, a3);
-        }
+        merge_round(sm, p, rb, n_rows, first, kvh, chunk_k);
         cons_bar();
       }
     }
