@@ -36,7 +36,7 @@ constexpr int ITEM_INTS = 6;                // first_slot, n_slots, page_begin, 
 struct Smem {
   alignas(128) unsigned char stage[STAGES][STAGE_BYTES];
   float scratch[N_CONS][4][HD];             // cross-warp merge of TOKSPLIT items, 4 query rows per round
-  float ml[N_CONS][16][2];
+  float ml[2][N_CONS][16][2];               // (max, sum) of the warps' partials; two buffers, alternating per unit
   unsigned long long full[STAGES], empty[STAGES];
 };
 
@@ -98,7 +98,7 @@ struct Params {
   const int32_t *slot_prompt, *slot_row, *slot_npre, *g_prefix_pages, *row_pages, *part_base;
   int causal;                               // prefill pass: query row of slot s sees tokens < slot_npre[s] only
   float *part_ml, *part_acc;
-  int mpp, msp, Hq, Hkv, rep;
+  int mpp, msp, Hq, Hkv, rep, rep_shift;  // rep = Hq / Hkv = 1 << rep_shift (attention_sm100_supported)
   size_t page_elems, tile_elems;
   float c;                                  // softmax scale * log2(e)
 };
@@ -161,23 +161,176 @@ __device__ __forceinline__ void pv_16tok(uint32_t sV, int tokb, uint32_t a0, uin
   }
 }
 
+// A work item of the plan (ITEM_INTS ints, 8-byte aligned): first slot, slots, first page, tokens, partial index within the row, prefix?
+struct Hdr { int first, n_slots, page_begin, n_tok, chunk_k, is_pre; };
+__device__ __forceinline__ Hdr load_hdr(const Params &p, int n_pre, int item) {
+  const int2 *it = reinterpret_cast<const int2 *>(item < n_pre ? p.items_pre + (size_t)item * ITEM_INTS : p.items_suf + (size_t)(item - n_pre) * ITEM_INTS);
+  const int2 a = it[0], b = it[1], c = it[2];
+  return Hdr{a.x, a.y, b.x, b.y, c.x, c.y};
+}
+// B-operand fragments of Q^T for a unit of <= 8 query rows: lane (g, t) holds row g, dims 16 ks + 2 t (+1) and + 8
+__device__ __forceinline__ void load_qb(const Params &p, int first, int n_rows, int kvh, int lane, uint32_t (&Qb)[8][2]) {
+  const int g = lane >> 2, t = lane & 3;
+  const __nv_bfloat16 *q = g < n_rows ? p.q + ((size_t)(first + (g >> p.rep_shift)) * p.Hq + kvh * p.rep + (g & (p.rep - 1))) * HD : nullptr;
+#pragma unroll
+  for (int ks = 0; ks < 8; ++ks) {
+    const int d = 16 * ks + 2 * t;
+    Qb[ks][0] = q ? *reinterpret_cast<const uint32_t *>(q + d) : 0u;
+    Qb[ks][1] = q ? *reinterpret_cast<const uint32_t *>(q + d + 8) : 0u;
+  }
+}
+
+// One token-split unit of <= 8 query rows (a decode row's own pages: n_rows = rep), transposed: S^T = K . Q^T puts the warp's 16 tokens
+// on the MMA's m dimension and the query rows on n = 8 — one MMA per k-step instead of two, O^T (128 dims x 8 rows) in 32 accumulators
+// instead of 64.  C fragment of S^T: c0/c1 = token g, rows 2t/2t+1; c2/c3 = token g+8.  The four warps' partials meet in the unit's LAST
+// page stage — each warp overwrites its own 16 K rows (4 KB = 8 rows x 128 fp32), which nobody else reads — so the merge needs one CTA
+// barrier and no scratch of its own; the stage goes back to the producer after the merge.  pbase = part_base[first] (used when n_slots == 1).
+__device__ __forceinline__ void tpath_unit(Smem &sm, const Params &p, const Hdr &h, int kvh, int pbase, const uint32_t (&Qb)[8][2],
+                                           int &stage, int &phase, int &ubuf, int warp, int lane) {
+  const int g = lane >> 2, t = lane & 3;
+  const int n_rows = h.n_slots << p.rep_shift, n_tok = h.n_tok;
+  int limA = n_tok, limB = n_tok;                                  // token limits of rows 2t and 2t+1
+  if (p.causal) {
+    const int rA = 2 * t, rB = rA + 1, tok_begin = h.page_begin * PAGE;
+    limA = rA < n_rows ? min(n_tok, p.slot_npre[h.first + (rA >> p.rep_shift)] - tok_begin) : 0;
+    limB = rB < n_rows ? min(n_tok, p.slot_npre[h.first + (rB >> p.rep_shift)] - tok_begin) : 0;
+  }
+  float OT[8][4];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) OT[i][0] = OT[i][1] = OT[i][2] = OT[i][3] = 0.f;
+  float mA = -INFINITY, mB = -INFINITY, lA = 0.f, lB = 0.f;
+  const int npg = (n_tok + PAGE - 1) / PAGE;
+  const int mat = lane >> 3, r8 = lane & 7;
+  int last_stage = stage;
+  for (int pg = 0; pg < npg; ++pg) {
+    mbar_wait(&sm.full[stage], phase);
+    const uint32_t sK = smem_u32(sm.stage[stage]), sV = sK + PAGE * HD * 2;
+    const int valid = min(PAGE, n_tok - pg * PAGE);
+    const int tok0 = warp * 16;
+    if (tok0 < valid) {
+      float c[4] = {0.f, 0.f, 0.f, 0.f}, c2[4] = {0.f, 0.f, 0.f, 0.f};     // two accumulation chains over the k-steps
+      {
+        const uint32_t rowaddr = sK + (tok0 + (mat & 1) * 8 + r8) * (HD * 2);
+#pragma unroll
+        for (int ks = 0; ks < 8; ks += 2) {
+          uint32_t a0, a1, a2, a3, e0, e1, e2, e3;
+          ldsm4(rowaddr + (((2 * ks + (mat >> 1)) ^ r8) << 4), a0, a1, a2, a3);
+          ldsm4(rowaddr + (((2 * ks + 2 + (mat >> 1)) ^ r8) << 4), e0, e1, e2, e3);
+          mma16816(c, a0, a1, a2, a3, Qb[ks][0], Qb[ks][1]);
+          mma16816(c2, e0, e1, e2, e3, Qb[ks + 1][0], Qb[ks + 1][1]);
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) c[j] += c2[j];
+      }
+      const int vA = limA - pg * PAGE, vB = limB - pg * PAGE, tkA = tok0 + g, tkB = tkA + 8;
+      if (tkA >= vA) c[0] = -INFINITY;
+      if (tkA >= vB) c[1] = -INFINITY;
+      if (tkB >= vA) c[2] = -INFINITY;
+      if (tkB >= vB) c[3] = -INFINITY;
+      float mxA = fmaxf(c[0], c[2]), mxB = fmaxf(c[1], c[3]);
+#pragma unroll
+      for (int o = 4; o <= 16; o <<= 1) {
+        mxA = fmaxf(mxA, __shfl_xor_sync(0xffffffffu, mxA, o));
+        mxB = fmaxf(mxB, __shfl_xor_sync(0xffffffffu, mxB, o));
+      }
+      const float mnA = fmaxf(mA, mxA), mnB = fmaxf(mB, mxB);
+      const float msA = mnA == -INFINITY ? 0.f : mnA, msB = mnB == -INFINITY ? 0.f : mnB;
+      const float corrA = exp2f((mA - msA) * p.c), corrB = exp2f((mB - msB) * p.c);
+      const float p0 = exp2f(fmaf(c[0], p.c, -msA * p.c)), p2 = exp2f(fmaf(c[2], p.c, -msA * p.c));
+      const float p1 = exp2f(fmaf(c[1], p.c, -msB * p.c)), p3 = exp2f(fmaf(c[3], p.c, -msB * p.c));
+      lA = lA * corrA + p0 + p2;
+      lB = lB * corrB + p1 + p3;
+      mA = mnA;
+      mB = mnB;
+#pragma unroll
+      for (int i = 0; i < 8; ++i) { OT[i][0] *= corrA; OT[i][2] *= corrA; OT[i][1] *= corrB; OT[i][3] *= corrB; }
+      // P^T (tokens x rows) -> the B operand (k = tokens, n = rows): transpose the two 8x8 blocks
+      uint32_t b0, b1;
+      movmatrix_t(pack_bf16(p0, p1), b0);
+      movmatrix_t(pack_bf16(p2, p3), b1);
+      {
+        const uint32_t rowaddr = sV + (tok0 + (mat >> 1) * 8 + r8) * (HD * 2);
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+          uint32_t a0, a1, a2, a3;
+          ldsm4t(rowaddr + (((2 * i + (mat & 1)) ^ r8) << 4), a0, a1, a2, a3);
+          mma16816(OT[i], a0, a1, a2, a3, b0, b1);
+        }
+      }
+    }
+    __syncwarp();
+    if (pg + 1 < npg) {
+      if (lane == 0) mbar_arrive(&sm.empty[stage]);
+    } else {
+      last_stage = stage;                                          // kept until the merge below has read it
+    }
+    if (++stage == STAGES) { stage = 0; phase ^= 1; }
+  }
+#pragma unroll
+  for (int o = 4; o <= 16; o <<= 1) {
+    lA += __shfl_xor_sync(0xffffffffu, lA, o);
+    lB += __shfl_xor_sync(0xffffffffu, lB, o);
+  }
+  float (*ml)[16][2] = sm.ml[ubuf];
+  ubuf ^= 1;
+  if (g == 0) {
+    ml[warp][2 * t][0] = mA; ml[warp][2 * t][1] = lA;
+    ml[warp][2 * t + 1][0] = mB; ml[warp][2 * t + 1][1] = lB;
+  }
+  // partial of this warp: [row][128] fp32, the columns of rows 2t, 2t+1 rotated by 8 t (bank-conflict-free writes)
+  unsigned char *part = sm.stage[last_stage];
+  if (2 * t < n_rows) {
+    float *mine = reinterpret_cast<float *>(part + warp * 4096) + 2 * t * HD;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      const int c0 = (16 * i + g + 8 * t) & (HD - 1), c1 = (c0 + 8) & (HD - 1);
+      mine[c0] = OT[i][0]; mine[HD + c0] = OT[i][1];
+      mine[c1] = OT[i][2]; mine[HD + c1] = OT[i][3];
+    }
+  }
+  cons_bar();
+  for (int r = warp; r < n_rows; r += N_CONS) {
+    float M = -INFINITY;
+#pragma unroll
+    for (int wv = 0; wv < N_CONS; ++wv) M = fmaxf(M, ml[wv][r][0]);
+    float L = 0.f, a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
+    const int col = (lane * 4 + 8 * (r >> 1)) & (HD - 1);
+#pragma unroll
+    for (int wv = 0; wv < N_CONS; ++wv) {
+      const float sc = exp2f((ml[wv][r][0] - M) * p.c);
+      const float4 v = *reinterpret_cast<const float4 *>(reinterpret_cast<const float *>(part + wv * 4096) + r * HD + col);
+      L += sc * ml[wv][r][1];
+      a0 += sc * v.x; a1 += sc * v.y; a2 += sc * v.z; a3 += sc * v.w;
+    }
+    const int slot = h.first + (r >> p.rep_shift), head = kvh * p.rep + (r & (p.rep - 1));
+    const int pb = h.n_slots == 1 ? pbase : p.part_base[slot];
+    const size_t pi = (size_t)(pb + h.chunk_k) * p.Hq + head;
+    if (lane == 0) { p.part_ml[pi * 2] = M; p.part_ml[pi * 2 + 1] = L; }
+    *reinterpret_cast<float4 *>(p.part_acc + pi * HD + lane * 4) = make_float4(a0, a1, a2, a3);
+  }
+  // the stage's next user is the producer's bulk copy (async proxy): order this warp's generic accesses before it
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  __syncwarp();
+  if (lane == 0) mbar_arrive(&sm.empty[last_stage]);
+}
+
 // One round of the cross-warp merge of a token-split unit: rows 4 rb .. 4 rb + 3, one consumer warp per row, 4 dims per lane.
-__device__ __forceinline__ void merge_round(Smem &sm, const Params &p, int rb, int n_rows, int first, int kvh, int chunk_k) {
+__device__ __forceinline__ void merge_round(Smem &sm, const float (*ml)[16][2], const Params &p, int rb, int n_rows, int first, int kvh, int chunk_k) {
   int rr = threadIdx.x >> 5, d4 = (threadIdx.x & 31) * 4;     // 128 consumer threads: row rr, dims d4..d4+3
   int r = rb * 4 + rr;
   if (r < n_rows) {
     float M = -INFINITY;
 #pragma unroll
-    for (int wv = 0; wv < N_CONS; ++wv) M = fmaxf(M, sm.ml[wv][r][0]);
+    for (int wv = 0; wv < N_CONS; ++wv) M = fmaxf(M, ml[wv][r][0]);
     float L = 0.f, a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
 #pragma unroll
     for (int wv = 0; wv < N_CONS; ++wv) {
-      float sc = exp2f((sm.ml[wv][r][0] - M) * p.c);
+      float sc = exp2f((ml[wv][r][0] - M) * p.c);
       float4 v = *reinterpret_cast<const float4 *>(&sm.scratch[wv][rr][d4]);
-      L += sc * sm.ml[wv][r][1];
+      L += sc * ml[wv][r][1];
       a0 += sc * v.x; a1 += sc * v.y; a2 += sc * v.z; a3 += sc * v.w;
     }
-    int slot = first + r / p.rep, head = kvh * p.rep + r % p.rep;
+    int slot = first + (r >> p.rep_shift), head = kvh * p.rep + (r & (p.rep - 1));
     size_t pi = (size_t)(p.part_base[slot] + chunk_k) * p.Hq + head;
     if ((threadIdx.x & 31) == 0) { p.part_ml[pi * 2] = M; p.part_ml[pi * 2 + 1] = L; }
     *reinterpret_cast<float4 *>(p.part_acc + pi * HD + d4) = make_float4(a0, a1, a2, a3);
@@ -196,14 +349,16 @@ __global__ void __launch_bounds__(THREADS, 2) attn_main_k(Params p) {
   pdl_wait();                                    // q, the KV rows appended this step and the plan come from earlier kernels
   __syncthreads();
   int n_pre = p.n_items[0], n_suf = p.n_items[1];
-  long long total = (long long)(n_pre + n_suf) * p.Hkv;
+  const int total = (n_pre + n_suf) * p.Hkv;            // work units (item, kv head); attn_max_items * Hkv < 2^31
+  const int d_item = (int)gridDim.x / p.Hkv, d_kvh = (int)gridDim.x % p.Hkv;
   int stage = 0, phase = 0;
 
   if (warp == N_CONS) {
     // ------------------------------------------------------------------ producer: one lane streams the pages
     if (lane == 0) {
-      for (long long w = blockIdx.x; w < total; w += gridDim.x) {
-        int item = (int)(w / p.Hkv), kvh = (int)(w % p.Hkv);
+      int item = (int)blockIdx.x / p.Hkv, kvh = (int)blockIdx.x % p.Hkv;
+      for (int w = blockIdx.x; w < total; w += gridDim.x, item += d_item, kvh += d_kvh) {
+        if (kvh >= p.Hkv) { kvh -= p.Hkv; ++item; }
         const int32_t *it = item < n_pre ? p.items_pre + (size_t)item * ITEM_INTS : p.items_suf + (size_t)(item - n_pre) * ITEM_INTS;
         int first = it[0], page_begin = it[2], n_tok = it[3], is_pre = it[5];
         const int32_t *table = is_pre ? p.g_prefix_pages + (size_t)p.slot_prompt[first] * p.mpp : p.row_pages + (size_t)p.slot_row[first] * p.msp;
@@ -236,119 +391,23 @@ __global__ void __launch_bounds__(THREADS, 2) attn_main_k(Params p) {
 
   // -------------------------------------------------------------------- consumers
   int g = lane >> 2, t = lane & 3;
-  for (long long w = blockIdx.x; w < total; w += gridDim.x) {
-    int item = (int)(w / p.Hkv), kvh = (int)(w % p.Hkv);
-    const int32_t *it = item < n_pre ? p.items_pre + (size_t)item * ITEM_INTS : p.items_suf + (size_t)(item - n_pre) * ITEM_INTS;
-    int first = it[0], n_slots = it[1], n_tok = it[3], chunk_k = it[4];
+  int item = (int)blockIdx.x / p.Hkv, kvh = (int)blockIdx.x % p.Hkv;
+  int ubuf = 0;                                                    // which sm.ml buffer the next unit uses
+  // With rep <= 8 every suffix unit (one row's own pages) takes the transposed path: those run in a software-pipelined loop of their
+  // own below; this loop then serves the prefix units only.
+  const bool suffix_t = ATTN_TPATH && p.rep <= 8;
+  const int gen_end = suffix_t ? n_pre * p.Hkv : total;
+  int w = blockIdx.x;
+  for (; w < gen_end; w += gridDim.x, item += d_item, kvh += d_kvh) {
+    if (kvh >= p.Hkv) { kvh -= p.Hkv; ++item; }
+    const Hdr hd = load_hdr(p, n_pre, item);
+    int first = hd.first, n_slots = hd.n_slots, n_tok = hd.n_tok, chunk_k = hd.chunk_k;
     int n_rows = n_slots * p.rep;
-    const int tok_begin = it[2] * PAGE;                            // first token of this item within its page table
+    const int tok_begin = hd.page_begin * PAGE;                    // first token of this item within its page table
     if (ATTN_TPATH && n_rows <= 8) {
-      // ---- transposed token-split path (a decode row's own pages: n_rows = rep <= 8).  S^T = K . Q^T puts the warp's 16 tokens on the
-      // MMA's m dimension and the <= 8 query rows on n = 8: one MMA per k-step instead of two, and O^T (128 dims x 8 rows) is 32
-      // accumulators instead of 64.  C fragment of S^T: c0/c1 = token g, rows 2t/2t+1; c2/c3 = token g+8.
       uint32_t Qb[8][2];
-      {
-        const __nv_bfloat16 *q = g < n_rows ? p.q + ((size_t)(first + g / p.rep) * p.Hq + kvh * p.rep + g % p.rep) * HD : nullptr;
-#pragma unroll
-        for (int ks = 0; ks < 8; ++ks) {
-          int d = 16 * ks + 2 * t;
-          Qb[ks][0] = q ? *reinterpret_cast<const uint32_t *>(q + d) : 0u;
-          Qb[ks][1] = q ? *reinterpret_cast<const uint32_t *>(q + d + 8) : 0u;
-        }
-      }
-      int limA = n_tok, limB = n_tok;                              // token limits of rows 2t and 2t+1
-      if (p.causal) {
-        int rA = 2 * t, rB = rA + 1;
-        limA = rA < n_rows ? min(n_tok, p.slot_npre[first + rA / p.rep] - tok_begin) : 0;
-        limB = rB < n_rows ? min(n_tok, p.slot_npre[first + rB / p.rep] - tok_begin) : 0;
-      }
-      float OT[8][4];
-#pragma unroll
-      for (int i = 0; i < 8; ++i) OT[i][0] = OT[i][1] = OT[i][2] = OT[i][3] = 0.f;
-      float mA = -INFINITY, mB = -INFINITY, lA = 0.f, lB = 0.f;
-      const int npg_t = (n_tok + PAGE - 1) / PAGE;
-      const int mat = lane >> 3, r8 = lane & 7;
-      for (int pg = 0; pg < npg_t; ++pg) {
-        mbar_wait(&sm.full[stage], phase);
-        const uint32_t sK = smem_u32(sm.stage[stage]), sV = sK + PAGE * HD * 2;
-        const int valid = min(PAGE, n_tok - pg * PAGE);
-        const int tok0 = warp * 16;
-        if (tok0 < valid) {
-          float c[4] = {0.f, 0.f, 0.f, 0.f};
-          {
-            const uint32_t rowaddr = sK + (tok0 + (mat & 1) * 8 + r8) * (HD * 2);
-#pragma unroll
-            for (int ks = 0; ks < 8; ++ks) {
-              uint32_t a0, a1, a2, a3;
-              ldsm4(rowaddr + (((2 * ks + (mat >> 1)) ^ r8) << 4), a0, a1, a2, a3);
-              mma16816(c, a0, a1, a2, a3, Qb[ks][0], Qb[ks][1]);
-            }
-          }
-          const int vA = limA - pg * PAGE, vB = limB - pg * PAGE, tkA = tok0 + g, tkB = tkA + 8;
-          if (tkA >= vA) c[0] = -INFINITY;
-          if (tkA >= vB) c[1] = -INFINITY;
-          if (tkB >= vA) c[2] = -INFINITY;
-          if (tkB >= vB) c[3] = -INFINITY;
-          float mxA = fmaxf(c[0], c[2]), mxB = fmaxf(c[1], c[3]);
-#pragma unroll
-          for (int o = 4; o <= 16; o <<= 1) {
-            mxA = fmaxf(mxA, __shfl_xor_sync(0xffffffffu, mxA, o));
-            mxB = fmaxf(mxB, __shfl_xor_sync(0xffffffffu, mxB, o));
-          }
-          const float mnA = fmaxf(mA, mxA), mnB = fmaxf(mB, mxB);
-          const float msA = mnA == -INFINITY ? 0.f : mnA, msB = mnB == -INFINITY ? 0.f : mnB;
-          const float corrA = exp2f((mA - msA) * p.c), corrB = exp2f((mB - msB) * p.c);
-          const float p0 = exp2f(fmaf(c[0], p.c, -msA * p.c)), p2 = exp2f(fmaf(c[2], p.c, -msA * p.c));
-          const float p1 = exp2f(fmaf(c[1], p.c, -msB * p.c)), p3 = exp2f(fmaf(c[3], p.c, -msB * p.c));
-          lA = lA * corrA + p0 + p2;
-          lB = lB * corrB + p1 + p3;
-          mA = mnA;
-          mB = mnB;
-#pragma unroll
-          for (int i = 0; i < 8; ++i) { OT[i][0] *= corrA; OT[i][2] *= corrA; OT[i][1] *= corrB; OT[i][3] *= corrB; }
-          // P^T (tokens x rows) -> the B operand (k = tokens, n = rows): transpose the two 8x8 blocks
-          uint32_t b0, b1;
-          movmatrix_t(pack_bf16(p0, p1), b0);
-          movmatrix_t(pack_bf16(p2, p3), b1);
-          {
-            const uint32_t rowaddr = sV + (tok0 + (mat >> 1) * 8 + r8) * (HD * 2);
-#pragma unroll
-            for (int i = 0; i < 8; ++i) {
-              uint32_t a0, a1, a2, a3;
-              ldsm4t(rowaddr + (((2 * i + (mat & 1)) ^ r8) << 4), a0, a1, a2, a3);
-              mma16816(OT[i], a0, a1, a2, a3, b0, b1);
-            }
-          }
-        }
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&sm.empty[stage]);
-        if (++stage == STAGES) { stage = 0; phase ^= 1; }
-      }
-#pragma unroll
-      for (int o = 4; o <= 16; o <<= 1) {
-        lA += __shfl_xor_sync(0xffffffffu, lA, o);
-        lB += __shfl_xor_sync(0xffffffffu, lB, o);
-      }
-      if (g == 0) {
-        sm.ml[warp][2 * t][0] = mA; sm.ml[warp][2 * t][1] = lA;
-        sm.ml[warp][2 * t + 1][0] = mB; sm.ml[warp][2 * t + 1][1] = lB;
-      }
-      const int rounds_t = (n_rows + 3) >> 2;
-      for (int rb = 0; rb < rounds_t; ++rb) {
-        if ((t >> 1) == rb) {                                      // rows 4 rb .. 4 rb + 3 are held by t = 2 rb, 2 rb + 1
-          const int lr = 2 * (t & 1);
-#pragma unroll
-          for (int i = 0; i < 8; ++i) {
-            sm.scratch[warp][lr][16 * i + g] = OT[i][0];
-            sm.scratch[warp][lr + 1][16 * i + g] = OT[i][1];
-            sm.scratch[warp][lr][16 * i + g + 8] = OT[i][2];
-            sm.scratch[warp][lr + 1][16 * i + g + 8] = OT[i][3];
-          }
-        }
-        cons_bar();
-        merge_round(sm, p, rb, n_rows, first, kvh, chunk_k);
-        cons_bar();
-      }
+      load_qb(p, hd.first, n_rows, kvh, lane, Qb);
+      tpath_unit(sm, p, hd, kvh, p.part_base[hd.first], Qb, stage, phase, ubuf, warp, lane);
       continue;
     }
     bool rowsplit = n_rows > 16;
@@ -358,8 +417,8 @@ __global__ void __launch_bounds__(THREADS, 2) attn_main_k(Params p) {
     uint32_t Qa[8][4];
     {
       int r0 = mt * 16 + g, r1 = r0 + 8;
-      const __nv_bfloat16 *q0 = r0 < n_rows ? p.q + ((size_t)(first + r0 / p.rep) * p.Hq + kvh * p.rep + r0 % p.rep) * HD : nullptr;
-      const __nv_bfloat16 *q1 = r1 < n_rows ? p.q + ((size_t)(first + r1 / p.rep) * p.Hq + kvh * p.rep + r1 % p.rep) * HD : nullptr;
+      const __nv_bfloat16 *q0 = r0 < n_rows ? p.q + ((size_t)(first + (r0 >> p.rep_shift)) * p.Hq + kvh * p.rep + (r0 & (p.rep - 1))) * HD : nullptr;
+      const __nv_bfloat16 *q1 = r1 < n_rows ? p.q + ((size_t)(first + (r1 >> p.rep_shift)) * p.Hq + kvh * p.rep + (r1 & (p.rep - 1))) * HD : nullptr;
 #pragma unroll
       for (int ks = 0; ks < 8; ++ks) {
         int d = 16 * ks + 2 * t;
@@ -373,8 +432,8 @@ __global__ void __launch_bounds__(THREADS, 2) attn_main_k(Params p) {
     int lim0 = n_tok, lim1 = n_tok;
     if (p.causal) {
       int r0 = mt * 16 + g, r1 = r0 + 8;
-      lim0 = r0 < n_rows ? min(n_tok, p.slot_npre[first + r0 / p.rep] - tok_begin) : 0;
-      lim1 = r1 < n_rows ? min(n_tok, p.slot_npre[first + r1 / p.rep] - tok_begin) : 0;
+      lim0 = r0 < n_rows ? min(n_tok, p.slot_npre[first + (r0 >> p.rep_shift)] - tok_begin) : 0;
+      lim1 = r1 < n_rows ? min(n_tok, p.slot_npre[first + (r1 >> p.rep_shift)] - tok_begin) : 0;
     }
     float O[16][4];
 #pragma unroll
@@ -405,8 +464,23 @@ __global__ void __launch_bounds__(THREADS, 2) attn_main_k(Params p) {
         }
       } else if (warp_has_rows) {
         float S[8][4] = {};
+        {
+          // k-step outermost: the eight accumulators are independent MMA chains (one 16-token group at a time is two chains of eight
+          // dependent MMAs, and two warps per scheduler cannot hide their latency)
+          const int mat = lane >> 3, r = lane & 7;
+          const uint32_t rowaddr = sK + ((mat >> 1) * 8 + r) * (HD * 2);
 #pragma unroll
-        for (int np = 0; np < 4; ++np) qk_16tok(sK, np * 16, Qa, S[2 * np], S[2 * np + 1], lane);
+          for (int ks = 0; ks < 8; ++ks) {
+            const uint32_t off = ((2 * ks + (mat & 1)) ^ r) << 4;
+#pragma unroll
+            for (int np = 0; np < 4; ++np) {
+              uint32_t b0, b1, b2, b3;
+              ldsm4(rowaddr + np * 16 * (HD * 2) + off, b0, b1, b2, b3);
+              mma16816(S[2 * np], Qa[ks][0], Qa[ks][1], Qa[ks][2], Qa[ks][3], b0, b1);
+              mma16816(S[2 * np + 1], Qa[ks][0], Qa[ks][1], Qa[ks][2], Qa[ks][3], b2, b3);
+            }
+          }
+        }
         if (min(v0, v1) < PAGE) {
 #pragma unroll
           for (int nt = 0; nt < 8; ++nt) {
@@ -438,7 +512,7 @@ __global__ void __launch_bounds__(THREADS, 2) attn_main_k(Params p) {
       for (int rs = 0; rs < 2; ++rs) {
         int r = mt * 16 + g + 8 * rs;
         if (r < n_rows) {
-          int slot = first + r / p.rep, head = kvh * p.rep + r % p.rep;
+          int slot = first + (r >> p.rep_shift), head = kvh * p.rep + (r & (p.rep - 1));
           size_t pi = (size_t)(p.part_base[slot] + chunk_k) * p.Hq + head;
           if (t == 0) { p.part_ml[pi * 2] = m[rs]; p.part_ml[pi * 2 + 1] = l[rs]; }
 #pragma unroll
@@ -448,9 +522,11 @@ __global__ void __launch_bounds__(THREADS, 2) attn_main_k(Params p) {
       }
     } else {
       // the four warps hold partials over disjoint tokens of the same <= 16 rows: merge through shared memory
+      float (*ml)[16][2] = sm.ml[ubuf];
+      ubuf ^= 1;
       if (t == 0) {
-        sm.ml[warp][g][0] = m[0]; sm.ml[warp][g][1] = l[0];
-        sm.ml[warp][g + 8][0] = m[1]; sm.ml[warp][g + 8][1] = l[1];
+        ml[warp][g][0] = m[0]; ml[warp][g][1] = l[0];
+        ml[warp][g + 8][0] = m[1]; ml[warp][g + 8][1] = l[1];
       }
       int rounds = (n_rows + 3) >> 2;
       for (int rb = 0; rb < rounds; ++rb) {
@@ -461,10 +537,40 @@ __global__ void __launch_bounds__(THREADS, 2) attn_main_k(Params p) {
             *reinterpret_cast<float2 *>(&sm.scratch[warp][g - glo][nt * 8 + 2 * t]) = rs == 0 ? make_float2(O[nt][0], O[nt][1]) : make_float2(O[nt][2], O[nt][3]);
         }
         cons_bar();
-        merge_round(sm, p, rb, n_rows, first, kvh, chunk_k);
+        merge_round(sm, ml, p, rb, n_rows, first, kvh, chunk_k);
         cons_bar();
       }
     }
+  }
+  if (!suffix_t || w >= total) return;
+  // ---- suffix units, software-pipelined: a unit's header is loaded two units ahead, its Q fragments and partial index one unit ahead,
+  // so that no dependent global load is left at a unit's start (at short contexts a unit is one page: the chain was most of its time)
+  if (kvh >= p.Hkv) { kvh -= p.Hkv; ++item; }
+  Hdr h = load_hdr(p, n_pre, item);
+  int w1 = w + gridDim.x, item1 = item + d_item, kvh1 = kvh + d_kvh;
+  if (kvh1 >= p.Hkv) { kvh1 -= p.Hkv; ++item1; }
+  Hdr h1 = w1 < total ? load_hdr(p, n_pre, item1) : h;
+  uint32_t Qb[8][2];
+  load_qb(p, h.first, p.rep, kvh, lane, Qb);
+  int pb = p.part_base[h.first];
+  while (true) {
+    const bool has1 = w1 < total;
+    int w2 = w1 + gridDim.x, item2 = item1 + d_item, kvh2 = kvh1 + d_kvh;
+    if (kvh2 >= p.Hkv) { kvh2 -= p.Hkv; ++item2; }
+    uint32_t Qn[8][2];
+    int pbn = 0;
+    Hdr h2 = h1;
+    if (has1) {
+      load_qb(p, h1.first, p.rep, kvh1, lane, Qn);
+      pbn = p.part_base[h1.first];
+      if (w2 < total) h2 = load_hdr(p, n_pre, item2);
+    }
+    tpath_unit(sm, p, h, kvh, pb, Qb, stage, phase, ubuf, warp, lane);
+    if (!has1) break;
+    h = h1; kvh = kvh1; pb = pbn;
+#pragma unroll
+    for (int ks = 0; ks < 8; ++ks) { Qb[ks][0] = Qn[ks][0]; Qb[ks][1] = Qn[ks][1]; }
+    h1 = h2; w1 = w2; item1 = item2; kvh1 = kvh2;
   }
 }
 
@@ -664,6 +770,7 @@ darts_status launch_attention_sm100(darts_ctx *c, int layer, const void *q, void
   p.slot_prompt = c->slot_prompt; p.slot_row = c->slot_row; p.slot_npre = c->slot_npre; p.causal = c->attn_causal ? 1 : 0; p.g_prefix_pages = c->g_prefix_pages; p.row_pages = c->row_pages;
   p.part_base = c->part_base; p.part_ml = c->part_ml; p.part_acc = c->part_acc;
   p.mpp = c->max_prefix_pages; p.msp = c->max_suffix_pages; p.Hq = c->m.n_q_heads; p.Hkv = c->m.n_kv_heads; p.rep = p.Hq / p.Hkv;
+  p.rep_shift = 31 - __builtin_clz((unsigned)p.rep);
   p.page_elems = c->kv_page_elems; p.tile_elems = c->kv_tile_elems;
   p.c = 1.4426950408889634f / sqrtf((float)HD);
   int grid = c->n_sms * 2;
