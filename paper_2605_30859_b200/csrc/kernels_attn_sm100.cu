@@ -9,7 +9,10 @@
 // the (page, head) K+V tile pairs — 32 KB, contiguous in HBM by construction of the cache layout — into a
 // 3-stage shared-memory ring with cp.async.bulk (the TMA bulk-copy engine) + mbarrier transaction counts, and
 // four consumer warps run QK^T / PV on tensor cores (mma.sync m16n8k16 bf16, fp32 accumulate) with an online
-// softmax in fp32.  The cache is stored pre-swizzled (internal.cuh: kv_elem), so the linear copy lands in the
+// softmax in fp32.  Two inner loops: an item of more than 8 query rows (a prefix item) puts the query rows on the
+// MMA's m dimension (one 16-row m-tile per warp, every warp walks the whole page); an item of <= 8 query rows (a
+// row's own pages when Hq/Hkv <= 8) puts each warp's 16 tokens on m and the query rows on n = 8 (tpath_unit: half
+// the MMAs and accumulators), in a software-pipelined loop over the CTA's suffix units.  The cache is stored pre-swizzled (internal.cuh: kv_elem), so the linear copy lands in the
 // bank-conflict-free layout ldmatrix needs.  Every item writes one un-normalised partial (m, l, acc) per query
 // row; attn_merge_k combines a row's partials by log-sum-exp in chunk order.  The split depends only on a row's
 // own lengths (fixed 512-token chunks), so a row's arithmetic does not depend on which other rows are active,

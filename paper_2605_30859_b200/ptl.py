@@ -68,7 +68,10 @@ def eq6_k(b, t, c_kv, mean_len, b_at):
     return float(mean_len * slope + c_kv * mean_len ** 2 / 2.0)
 
 
-def measure(workload="c3", rows=(16, 32, 64, 128, 192, 256, 384, 512), steps=24, P=None, seed=0, layers=None, ctxs=(0,), pool_bytes=100e9):
+def measure(workload="c3", rows=(16, 32, 64, 128, 192, 256, 384, 512), steps=24, P=None, seed=0, layers=None, ctxs=(0,), pool_bytes=100e9,
+            attention=False):
+    """`attention`: also time the attention launches of layer 0 in every step (CUDA events inside the library, DARTS_FLAG_PROFILE_ATTENTION)
+    and report their median and the fraction of the measured HBM copy peak their algorithmic bytes reach."""
     import torch
     from . import api, workloads as wl
     c = wl.CONFIGS[workload]
@@ -87,7 +90,9 @@ def measure(workload="c3", rows=(16, 32, 64, 128, 192, 256, 384, 512), steps=24,
     n_prefix = (Rmax // Kp + 1) * (P // page + 1)
     n_pages = min(n_prefix + Rmax * (max_new // page + 2) + 64, int(pool_bytes // kv_page_bytes))
     d = api.Darts(model, page_size=page, n_pages=n_pages, max_rows=Rmax,
-                  max_prompts=Rmax // Kp + 1, max_prompt_len=P, max_new=max_new, eos_id=-1)
+                  max_prompts=Rmax // Kp + 1, max_prompt_len=P, max_new=max_new, eos_id=-1,
+                  flags=api.FLAG_PROFILE_ATTENTION if attention else 0)
+    kv_tok_bytes = 2 * cfg["n_kv_heads"] * cfg["head_dim"] * (2 if cfg["dtype"] == "bf16" else 4)     # K + V of one token in one layer
     out = []
     for R in rows:
         G = max(1, R // Kp)
@@ -113,6 +118,11 @@ def measure(workload="c3", rows=(16, 32, 64, 128, 192, 256, 384, 512), steps=24,
             ms = np.array([a.elapsed_time(b) for a, b in ev][4:])
             assert d.n_active() == int(kp.sum())
             out.append(dict(rows=int(kp.sum()), ctx=int(t), ms_median=float(np.median(ms)), ms_min=float(ms.min()), ms_max=float(ms.max())))
+            if attention:
+                a_ms = float(np.median(np.asarray(d.attention_times())[-(steps - 4):]))
+                # algorithmic bytes of one layer's attention in the middle of the timed steps: every row's own tokens + every prompt's prefix once
+                a_bytes = (int(kp.sum()) * (done - steps / 2) + G * P) * kv_tok_bytes
+                out[-1].update(attention_us=a_ms * 1e3, attention_GBps=a_bytes / (a_ms * 1e-3) / 1e9)
     d.close()
     return out
 
@@ -166,10 +176,12 @@ def main():
     ap.add_argument("--P", type=int, default=None)
     ap.add_argument("--layers", type=int, default=None)
     ap.add_argument("--ctx", default="0", help="generated lengths t at which every row count is timed (0 = right after the prefill)")
+    ap.add_argument("--attention", action="store_true", help="also report the attention launches of layer 0 per point (time, algorithmic GB/s)")
     ap.add_argument("--predict", action="store_true",
                     help="also run one rollout of the workload and compare its device time with Eq. 4 evaluated on the fitted PTL(b)")
     a = ap.parse_args()
-    pts = measure(a.workload, tuple(int(x) for x in a.rows.split(",")), a.steps, a.P, layers=a.layers, ctxs=tuple(int(x) for x in a.ctx.split(",")))
+    pts = measure(a.workload, tuple(int(x) for x in a.rows.split(",")), a.steps, a.P, layers=a.layers, ctxs=tuple(int(x) for x in a.ctx.split(",")),
+                  attention=a.attention)
     base = [p for p in pts if p["ctx"] == min(q["ctx"] for q in pts)]
     b, t = [p["rows"] for p in base], [p["ms_median"] for p in base]
     res = dict(workload=a.workload, points=pts)
