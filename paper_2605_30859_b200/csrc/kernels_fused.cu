@@ -116,80 +116,6 @@ __global__ void __launch_bounds__(256) add_rmsnorm_sk_k(float *__restrict__ h, S
   }
 }
 
-// Same operation with the slot's row held in registers (d / 4 <= ITERS * 256): every load of the row — the residual and up to four
-// pieces per element — is issued before the first add, and the row is read once (the two-pass version above re-reads h and walks
-// its elements one dependent round trip at a time, which is what a launch of 16 CTAs spends its 10 us on).
-template <int ITERS>
-__global__ void __launch_bounds__(256) add_rmsnorm_sk_reg_k(float *__restrict__ h, SkView v, const __nv_bfloat16 *__restrict__ w,
-                                                           __nv_bfloat16 *__restrict__ out, int d, float eps, const int32_t *n_rows_dev,
-                                                           int rows_ub) {
-  pdl_trigger();
-  pdl_wait();
-  const int slot = blockIdx.x, live = live_rows(n_rows_dev, rows_ub);
-  if (slot >= live) return;
-  const int rbr = sk_view_rb_rows(v, live), n_rb = (live + rbr - 1) / rbr;
-  float4 *hr = reinterpret_cast<float4 *>(h + (size_t)slot * d);
-  const size_t st = v.slot_stride / 4;
-  float4 x[ITERS], acc[ITERS];
-  int np[ITERS];
-  const float4 *pp[ITERS];
-  int npmax = 0;
-#pragma unroll
-  for (int it = 0; it < ITERS; ++it) {
-    const int k = threadIdx.x + it * 256;
-    const bool ok = k < d / 4;
-    np[it] = ok ? sk_npieces(v, n_rb, rbr, 4 * k, slot) : 0;
-    pp[it] = reinterpret_cast<const float4 *>(v.part + (size_t)slot * d) + (ok ? k : 0);
-    x[it] = ok ? hr[k] : make_float4(0.f, 0.f, 0.f, 0.f);
-    acc[it] = make_float4(0.f, 0.f, 0.f, 0.f);
-    npmax = max(npmax, np[it]);
-  }
-  for (int s0 = 0; s0 < npmax; s0 += 4) {
-    float4 y[ITERS][4];
-#pragma unroll
-    for (int it = 0; it < ITERS; ++it)
-#pragma unroll
-      for (int s = 0; s < 4; ++s)
-        if (s0 + s < np[it]) y[it][s] = __ldg(pp[it] + (size_t)(s0 + s) * st);
-#pragma unroll
-    for (int it = 0; it < ITERS; ++it)
-#pragma unroll
-      for (int s = 0; s < 4; ++s)
-        if (s0 + s < np[it]) { acc[it].x += y[it][s].x; acc[it].y += y[it][s].y; acc[it].z += y[it][s].z; acc[it].w += y[it][s].w; }
-  }
-  float ss = 0.f;
-#pragma unroll
-  for (int it = 0; it < ITERS; ++it) {
-    x[it].x += acc[it].x; x[it].y += acc[it].y; x[it].z += acc[it].z; x[it].w += acc[it].w;
-    const int k = threadIdx.x + it * 256;
-    if (k < d / 4) {
-      hr[k] = x[it];
-      ss += x[it].x * x[it].x + x[it].y * x[it].y + x[it].z * x[it].z + x[it].w * x[it].w;
-    }
-  }
-  __shared__ float red[32];
-  ss = warp_sum(ss);
-  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = ss;
-  __syncthreads();
-  if (threadIdx.x < 32) {
-    float t = threadIdx.x < (blockDim.x >> 5) ? red[threadIdx.x] : 0.f;
-    t = warp_sum(t);
-    if (threadIdx.x == 0) red[0] = t;
-  }
-  __syncthreads();
-  const float r = 1.0f / sqrtf(red[0] / d + eps);
-#pragma unroll
-  for (int it = 0; it < ITERS; ++it) {
-    const int k = threadIdx.x + it * 256;
-    if (k < d / 4) {
-      const __nv_bfloat162 *wp = reinterpret_cast<const __nv_bfloat162 *>(w + 4 * k);
-      float2 w0 = __bfloat1622float2(wp[0]), w1 = __bfloat1622float2(wp[1]);
-      *reinterpret_cast<uint2 *>(out + (size_t)slot * d + 4 * k) =
-          pack4_bf16(x[it].x * r * w0.x, x[it].y * r * w0.y, x[it].z * r * w1.x, x[it].w * r * w1.y);
-    }
-  }
-}
-
 // act[slot][k] = silu(g) * u with g = pieces(slot, k), u = pieces(slot, F + k)
 __global__ void __launch_bounds__(256) silu_mul_sk_k(SkView v, __nv_bfloat16 *__restrict__ act, int F, const int32_t *n_rows_dev, int rows_ub) {
   pdl_trigger();
@@ -275,6 +201,149 @@ __global__ void __launch_bounds__(128) rope_append_sk_k(SkView v, __nv_bfloat16 
   }
 }
 
+// ---- one-CTA-per-row forms (round 2, profiles/r2_consumers.md): every thread issues ALL the loads of its element — up to eight pieces —
+// before the first add.  The sums are still piece 0 + piece 1 + ... in slot order.
+
+// Up to NP pieces of one float4, all in flight together (np > NP: further rounds of NP)
+template <int NP>
+__device__ __forceinline__ float4 sk_sum4_wide(const float4 *p, size_t st, int np) {
+  float4 a = make_float4(0.f, 0.f, 0.f, 0.f);
+  for (int s0 = 0; s0 < np; s0 += NP) {
+    float4 y[NP];
+#pragma unroll
+    for (int s = 0; s < NP; ++s)
+      if (s0 + s < np) y[s] = __ldg(p + (size_t)(s0 + s) * st);
+#pragma unroll
+    for (int s = 0; s < NP; ++s)
+      if (s0 + s < np) { a.x += y[s].x; a.y += y[s].y; a.z += y[s].z; a.w += y[s].w; }
+  }
+  return a;
+}
+
+// h[slot] += pieces;  out = rmsnorm(h[slot]) * w.   One CTA per slot, ONE float4 per thread (blockDim >= d / 4, d <= 4096).
+__global__ void __launch_bounds__(1024) add_rmsnorm_sk_wide_k(float *__restrict__ h, SkView v, const __nv_bfloat16 *__restrict__ w,
+                                                             __nv_bfloat16 *__restrict__ out, int d, float eps, const int32_t *n_rows_dev,
+                                                             int rows_ub) {
+  pdl_trigger();
+  const int slot = blockIdx.x, k = threadIdx.x, live = live_rows(n_rows_dev, rows_ub);   // the row count is fixed for the step
+  const bool ok = k < d / 4;
+  float2 w0 = make_float2(0.f, 0.f), w1 = w0;
+  if (ok) {                                                  // weights do not depend on the previous kernel
+    const __nv_bfloat162 *wp = reinterpret_cast<const __nv_bfloat162 *>(w + 4 * k);
+    w0 = __bfloat1622float2(wp[0]);
+    w1 = __bfloat1622float2(wp[1]);
+  }
+  pdl_wait();
+  if (slot >= live) return;
+  const int rbr = sk_view_rb_rows(v, live), n_rb = (live + rbr - 1) / rbr;
+  float4 x = make_float4(0.f, 0.f, 0.f, 0.f);
+  float4 *hr = reinterpret_cast<float4 *>(h + (size_t)slot * d);
+  if (ok) {
+    x = hr[k];
+    const float4 a = sk_sum4_wide<8>(reinterpret_cast<const float4 *>(v.part + (size_t)slot * d) + k, v.slot_stride / 4,
+                                     sk_npieces(v, n_rb, rbr, 4 * k, slot));
+    x.x += a.x; x.y += a.y; x.z += a.z; x.w += a.w;
+    hr[k] = x;
+  }
+  // sum of squares in the ORDER of add_rmsnorm_sk_k (256 partial sums over k = t, t + 256, ..., then the warp tree, then the eight warps):
+  // the two kernels are chosen on the host's row bound, which may lag the live count, so they must agree to the bit
+  __shared__ float e[1024], red[32];
+  e[k] = x.x * x.x + x.y * x.y + x.z * x.z + x.w * x.w;
+  __syncthreads();
+  if (threadIdx.x < 256) {
+    float ss = 0.f;
+    for (int q = threadIdx.x; q < d / 4; q += 256) ss += e[q];
+    ss = warp_sum(ss);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = ss;
+  }
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    float t = threadIdx.x < 8 ? red[threadIdx.x] : 0.f;
+    t = warp_sum(t);
+    if (threadIdx.x == 0) red[0] = t;
+  }
+  __syncthreads();
+  const float r = 1.0f / sqrtf(red[0] / d + eps);
+  if (ok) *reinterpret_cast<uint2 *>(out + (size_t)slot * d + 4 * k) = pack4_bf16(x.x * r * w0.x, x.y * r * w0.y, x.z * r * w1.x, x.w * r * w1.y);
+}
+
+// (QK-norm) + RoPE + KV append, one CTA per slot: thread = (head, j) with j < hd / 8 owning elements 4j..4j+3 of both rotate-half halves
+// (hd in {64, 128, 256}: 8, 16 or 32 threads per head, a head never straddles a warp).
+__global__ void __launch_bounds__(768) rope_append_sk_row_k(SkView v, __nv_bfloat16 *__restrict__ q_out, __nv_bfloat16 *__restrict__ kv_layer,
+                                                            const int32_t *__restrict__ slot_dst_page, const int32_t *__restrict__ slot_dst_off,
+                                                            const float2 *__restrict__ cs, const __nv_bfloat16 *__restrict__ q_norm,
+                                                            const __nv_bfloat16 *__restrict__ k_norm, int Hq, int Hkv, int hd, int lph_shift, float eps,
+                                                            KvGeom geo, const int32_t *n_rows_dev, int rows_ub) {
+  pdl_trigger();
+  const int slot = blockIdx.x, live = live_rows(n_rows_dev, rows_ub);
+  const int head = threadIdx.x >> lph_shift, j = threadIdx.x & ((1 << lph_shift) - 1);
+  const int half = hd >> 1, col0 = head * hd, p = 4 * j;
+  const bool is_q = head < Hq, is_v = head >= Hq + Hkv;
+  if (slot >= live) return;                                // the row count and the append targets were fixed at the step boundary
+  const int page = slot_dst_page[slot], off = slot_dst_off[slot];
+  const bool act = head < Hq + 2 * Hkv && (is_q || page >= 0);
+  pdl_wait();
+  const int rbr = sk_view_rb_rows(v, live), n_rb = (live + rbr - 1) / rbr;
+  float4 x1 = make_float4(0.f, 0.f, 0.f, 0.f), x2 = x1, t01 = x1, t23 = x1;
+  if (act) {
+    const float4 *pp = reinterpret_cast<const float4 *>(v.part + (size_t)slot * (Hq + 2 * Hkv) * hd + col0 + p);
+    const int np1 = sk_npieces(v, n_rb, rbr, col0 + p, slot), np2 = sk_npieces(v, n_rb, rbr, col0 + half + p, slot);
+    if (!is_v) {
+      const float4 *tp = reinterpret_cast<const float4 *>(cs + (size_t)slot * half + p);   // (cos, sin) of pairs p .. p+3
+      t01 = tp[0];
+      t23 = tp[1];
+    }
+    const size_t st = v.slot_stride / 4;
+    float4 y1[4], y2[4];                                    // a QKV tile has 2-3 pieces (48 weight tiles on 148 CTAs): one round
+#pragma unroll
+    for (int s = 0; s < 4; ++s) {
+      if (s < np1) y1[s] = __ldg(pp + s * st);
+      if (s < np2) y2[s] = __ldg(pp + half / 4 + s * st);
+    }
+#pragma unroll
+    for (int s = 0; s < 4; ++s) {
+      if (s < np1) { x1.x += y1[s].x; x1.y += y1[s].y; x1.z += y1[s].z; x1.w += y1[s].w; }
+      if (s < np2) { x2.x += y2[s].x; x2.y += y2[s].y; x2.z += y2[s].z; x2.w += y2[s].w; }
+    }
+    if (np1 > 4) { const float4 a = sk_sum4_wide<4>(pp + 4 * st, st, np1 - 4); x1.x += a.x; x1.y += a.y; x1.z += a.z; x1.w += a.w; }
+    if (np2 > 4) { const float4 a = sk_sum4_wide<4>(pp + half / 4 + 4 * st, st, np2 - 4); x2.x += a.x; x2.y += a.y; x2.z += a.z; x2.w += a.w; }
+  }
+  float a1[4] = {x1.x, x1.y, x1.z, x1.w}, a2[4] = {x2.x, x2.y, x2.z, x2.w};
+  if (is_v) {
+    if (act) {
+      *reinterpret_cast<uint2 *>(&kv_layer[kv_elem(geo, page, head - Hq - Hkv, 1, off, p)]) = pack4_bf16(a1[0], a1[1], a1[2], a1[3]);
+      *reinterpret_cast<uint2 *>(&kv_layer[kv_elem(geo, page, head - Hq - Hkv, 1, off, half + p)]) = pack4_bf16(a2[0], a2[1], a2[2], a2[3]);
+    }
+  }
+  const bool rot = act && !is_v;
+  if (q_norm) {                                            // per-head RMSNorm over the head's 1 << lph_shift lanes (every lane of the warp takes the shuffles)
+    const __nv_bfloat16 *nw = is_q ? q_norm : k_norm;
+    float ss = 0.f;
+#pragma unroll
+    for (int e = 0; e < 4; ++e) ss += a1[e] * a1[e] + a2[e] * a2[e];
+    for (int o = (1 << lph_shift) >> 1; o > 0; o >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, o);
+    const float r = 1.0f / sqrtf(ss / hd + eps);
+    if (rot) {
+#pragma unroll
+      for (int e = 0; e < 4; ++e) { a1[e] *= r * __bfloat162float(nw[p + e]); a2[e] *= r * __bfloat162float(nw[half + p + e]); }
+    }
+  }
+  if (!rot) return;
+  const float co[4] = {t01.x, t01.z, t23.x, t23.z}, si[4] = {t01.y, t01.w, t23.y, t23.w};
+  float y1[4], y2[4];
+#pragma unroll
+  for (int e = 0; e < 4; ++e) { y1[e] = a1[e] * co[e] - a2[e] * si[e]; y2[e] = a2[e] * co[e] + a1[e] * si[e]; }
+  const uint2 o1 = pack4_bf16(y1[0], y1[1], y1[2], y1[3]), o2 = pack4_bf16(y2[0], y2[1], y2[2], y2[3]);
+  if (is_q) {
+    __nv_bfloat16 *qdst = q_out + (size_t)slot * Hq * hd + (size_t)head * hd;
+    *reinterpret_cast<uint2 *>(qdst + p) = o1;
+    *reinterpret_cast<uint2 *>(qdst + half + p) = o2;
+  } else {
+    *reinterpret_cast<uint2 *>(&kv_layer[kv_elem(geo, page, head - Hq, 0, off, p)]) = o1;
+    *reinterpret_cast<uint2 *>(&kv_layer[kv_elem(geo, page, head - Hq, 0, off, half + p)]) = o2;
+  }
+}
+
 darts_status post(darts_ctx *c, const char *what) {
   c->launches++;
   cudaError_t e = cudaGetLastError();
@@ -301,15 +370,12 @@ darts_status launch_sum_partials(darts_ctx *c, const float *part, float *out, in
 
 darts_status launch_add_rmsnorm_sk(darts_ctx *c, const SkView &v, const void *w, int rows_ub, const int32_t *n_rows_dev) {
   if (rows_ub <= 0) return DARTS_OK;
-  // the register-resident variant pays with occupancy (101-175 registers): it is for launches that cannot fill the SMs anyway
-  const int reg_max = 128;                                 // measured cross-over (round 1, ptl sweeps)
-  int d = c->m.d_model, iters = rows_ub <= reg_max ? (d / 4 + 255) / 256 : 99;
+  const int d = c->m.d_model;
   const __nv_bfloat16 *wn = (const __nv_bfloat16 *)w;
   __nv_bfloat16 *xn = (__nv_bfloat16 *)c->xn;
-  if (iters == 1) launch_pdl(c, add_rmsnorm_sk_reg_k<1>, dim3(rows_ub), dim3(256), 0, c->h, v, wn, xn, d, c->m.rms_eps, n_rows_dev, rows_ub);
-  else if (iters == 2) launch_pdl(c, add_rmsnorm_sk_reg_k<2>, dim3(rows_ub), dim3(256), 0, c->h, v, wn, xn, d, c->m.rms_eps, n_rows_dev, rows_ub);
-  else if (iters == 3) launch_pdl(c, add_rmsnorm_sk_reg_k<3>, dim3(rows_ub), dim3(256), 0, c->h, v, wn, xn, d, c->m.rms_eps, n_rows_dev, rows_ub);
-  else if (iters == 4) launch_pdl(c, add_rmsnorm_sk_reg_k<4>, dim3(rows_ub), dim3(256), 0, c->h, v, wn, xn, d, c->m.rms_eps, n_rows_dev, rows_ub);
+  // Up to 128 rows (measured cross-over: profiles/r2_consumers.md) one float4 per thread with every load of the row in flight at once; above,
+  // 256 threads walk the row (more rows resident per SM).  Same bits either way.
+  if (rows_ub <= 128 && d / 4 <= 1024 && d / 4 >= 256) launch_pdl(c, add_rmsnorm_sk_wide_k, dim3(rows_ub), dim3((d / 4 + 31) & ~31), 0, c->h, v, wn, xn, d, c->m.rms_eps, n_rows_dev, rows_ub);
   else launch_pdl(c, add_rmsnorm_sk_k, dim3(rows_ub), dim3(256), 0, c->h, v, wn, xn, d, c->m.rms_eps, n_rows_dev, rows_ub);
   return post(c, "add_rmsnorm_sk");
 }
@@ -317,19 +383,24 @@ darts_status launch_add_rmsnorm_sk(darts_ctx *c, const SkView &v, const void *w,
 darts_status launch_silu_mul_sk(darts_ctx *c, const SkView &v, int rows_ub, const int32_t *n_rows_dev) {
   if (rows_ub <= 0) return DARTS_OK;
   int F = c->m.ffn;
-  dim3 grid((F / 4 + 255) / 256, rows_ub);
-  launch_pdl(c, silu_mul_sk_k, grid, dim3(256), 0, v, (__nv_bfloat16 *)c->act, F, n_rows_dev, rows_ub);
+  launch_pdl(c, silu_mul_sk_k, dim3((F / 4 + 255) / 256, rows_ub), dim3(256), 0, v, (__nv_bfloat16 *)c->act, F, n_rows_dev, rows_ub);
   return post(c, "silu_mul_sk");
 }
 
 darts_status launch_rope_append_sk(darts_ctx *c, int layer, const SkView &v, int rows_ub, const int32_t *n_rows_dev) {
   if (rows_ub <= 0) return DARTS_OK;
   using T = __nv_bfloat16;
-  int nh = c->m.n_q_heads + 2 * c->m.n_kv_heads;
-  dim3 grid((nh + 3) / 4, rows_ub);
-  launch_pdl(c, rope_append_sk_k, grid, dim3(128), 0, v, (T *)c->q, (T *)c->kv_pool + (size_t)layer * c->kv_layer_elems, c->slot_dst_page, c->slot_dst_off,
-                                                c->slot_cs, c->m.qk_norm ? (const T *)c->q_norm[layer] : nullptr,
-                                                c->m.qk_norm ? (const T *)c->k_norm[layer] : nullptr, c->m.n_q_heads, c->m.n_kv_heads, c->m.head_dim,
-                                                c->m.rms_eps, c->geom(), n_rows_dev, rows_ub);
+  const int nh = c->m.n_q_heads + 2 * c->m.n_kv_heads, hd = c->m.head_dim;
+  T *kv = (T *)c->kv_pool + (size_t)layer * c->kv_layer_elems;
+  const T *qn = c->m.qk_norm ? (const T *)c->q_norm[layer] : nullptr, *kn = c->m.qk_norm ? (const T *)c->k_norm[layer] : nullptr;
+  const int lph = hd / 8;                                  // threads per head
+  if ((hd == 64 || hd == 128 || hd == 256) && nh * lph <= 768) {
+    const int lph_shift = hd == 64 ? 3 : hd == 128 ? 4 : 5;
+    launch_pdl(c, rope_append_sk_row_k, dim3(rows_ub), dim3((nh * lph + 31) & ~31), 0, v, (T *)c->q, kv, c->slot_dst_page, c->slot_dst_off, c->slot_cs, qn, kn,
+               c->m.n_q_heads, c->m.n_kv_heads, hd, lph_shift, c->m.rms_eps, c->geom(), n_rows_dev, rows_ub);
+  } else {
+    launch_pdl(c, rope_append_sk_k, dim3((nh + 3) / 4, rows_ub), dim3(128), 0, v, (T *)c->q, kv, c->slot_dst_page, c->slot_dst_off, c->slot_cs, qn, kn,
+               c->m.n_q_heads, c->m.n_kv_heads, hd, c->m.rms_eps, c->geom(), n_rows_dev, rows_ub);
+  }
   return post(c, "rope_append_sk");
 }
