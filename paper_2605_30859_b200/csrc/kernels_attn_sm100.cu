@@ -349,12 +349,22 @@ __global__ void __launch_bounds__(THREADS, 2) attn_main_k(Params p) {
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   pdl_trigger();
-  pdl_wait();                                    // q, the KV rows appended this step and the plan come from earlier kernels
-  __syncthreads();
+  // The plan (items, partial indices) and the page tables were written at the step boundary, by ordinary launches that everything in the
+  // layer chain comes after: they are read BEFORE the wait.  q and the KV rows appended this step come from the previous kernel.
   int n_pre = p.n_items[0], n_suf = p.n_items[1];
   const int total = (n_pre + n_suf) * p.Hkv;            // work units (item, kv head); attn_max_items * Hkv < 2^31
   const int d_item = (int)gridDim.x / p.Hkv, d_kvh = (int)gridDim.x % p.Hkv;
   int stage = 0, phase = 0;
+  Hdr h_first{};                                        // producer lane: its first unit's item, page table and first page id
+  const int32_t *table_first = nullptr;
+  int page_first = 0;
+  if (threadIdx.x == N_CONS * 32 && (int)blockIdx.x < total) {
+    h_first = load_hdr(p, n_pre, (int)blockIdx.x / p.Hkv);
+    table_first = h_first.is_pre ? p.g_prefix_pages + (size_t)p.slot_prompt[h_first.first] * p.mpp : p.row_pages + (size_t)p.slot_row[h_first.first] * p.msp;
+    page_first = table_first[h_first.page_begin];
+  }
+  pdl_wait();
+  __syncthreads();
 
   if (warp == N_CONS) {
     // ------------------------------------------------------------------ producer: one lane streams the pages
@@ -362,18 +372,20 @@ __global__ void __launch_bounds__(THREADS, 2) attn_main_k(Params p) {
       int item = (int)blockIdx.x / p.Hkv, kvh = (int)blockIdx.x % p.Hkv;
       for (int w = blockIdx.x; w < total; w += gridDim.x, item += d_item, kvh += d_kvh) {
         if (kvh >= p.Hkv) { kvh -= p.Hkv; ++item; }
-        const int32_t *it = item < n_pre ? p.items_pre + (size_t)item * ITEM_INTS : p.items_suf + (size_t)(item - n_pre) * ITEM_INTS;
-        int first = it[0], page_begin = it[2], n_tok = it[3], is_pre = it[5];
-        const int32_t *table = is_pre ? p.g_prefix_pages + (size_t)p.slot_prompt[first] * p.mpp : p.row_pages + (size_t)p.slot_row[first] * p.msp;
+        const bool first_unit = w == (int)blockIdx.x;
+        const Hdr h = first_unit ? h_first : load_hdr(p, n_pre, item);
+        const int first = h.first, page_begin = h.page_begin, n_tok = h.n_tok;
+        const int32_t *table = first_unit ? table_first
+                               : h.is_pre ? p.g_prefix_pages + (size_t)p.slot_prompt[first] * p.mpp : p.row_pages + (size_t)p.slot_row[first] * p.msp;
         int npg = (n_tok + PAGE - 1) / PAGE;
         // A row's NEWEST page is on average half empty, and a whole tile pair is 32 KB: at 512 rows that is ~67 MB per layer of bytes nobody
         // reads.  For a unit whose query rows fit one m-tile (the token-split path: a warp skips a 16-token group that lies wholly beyond the
         // valid tokens, so un-copied shared memory is never touched) the last page is fetched as the valid part of K and of V, rounded up to
         // 16 tokens — two smaller copies; only when that saves at least half of the tile.
-        const bool tok_split = ATTN_PARTIAL_LAST_PAGE && it[1] * p.rep <= 16 && !p.causal;
+        const bool tok_split = ATTN_PARTIAL_LAST_PAGE && h.n_slots * p.rep <= 16 && !p.causal;
         for (int pg = 0; pg < npg; ++pg) {
           mbar_wait(&sm.empty[stage], phase ^ 1);
-          int page_id = table[page_begin + pg];
+          const int page_id = first_unit && pg == 0 ? page_first : table[page_begin + pg];
           const __nv_bfloat16 *src = p.kv_layer + (size_t)page_id * p.page_elems + (size_t)kvh * 2 * p.tile_elems;
           const int v16 = (min(PAGE, n_tok - pg * PAGE) + 15) & ~15;
           if (tok_split && v16 <= PAGE / 2) {
@@ -583,12 +595,12 @@ __global__ void attn_merge_k(const float *__restrict__ part_ml, const float *__r
                              const int32_t *__restrict__ part_cnt, __nv_bfloat16 *__restrict__ out, int Hq, float c,
                              const int32_t *n_rows_dev, int rows_ub) {
   pdl_trigger();
-  pdl_wait();
   int slot = blockIdx.x;
-  int R = n_rows_dev ? min(*n_rows_dev, rows_ub) : rows_ub;
+  int R = n_rows_dev ? min(*n_rows_dev, rows_ub) : rows_ub;   // row count and plan: fixed at the step boundary, read before the wait
   if (slot >= R) return;
   int lane = threadIdx.x & 31;
   int base = part_base[slot], cnt = part_cnt[slot];
+  pdl_wait();
   for (int h = blockIdx.y * (blockDim.x >> 5) + (threadIdx.x >> 5); h < Hq; h += gridDim.y * (blockDim.x >> 5)) {   // one head per warp
     float M = -INFINITY, L = 0.f;
     float4 a = make_float4(0.f, 0.f, 0.f, 0.f);
