@@ -279,6 +279,25 @@ darts_status darts_debug_gemm_scratch_floats(darts_ctx *ctx, int32_t rows, int32
 darts_status darts_debug_gemm_bf16(darts_ctx *ctx, const void *X, const void *W, float *C, float *scratch, int32_t rows,
                                    int32_t N, int32_t K, int32_t split_k);
 
+/* ---- The same stream-K GEMM for callers that cannot allocate (CUDA-graph capture, serving loops, harnesses that forbid cudaMalloc) ------
+ * darts_gemm_bf16_static: C[rows][N] (fp32, DEVICE) = X[rows][K] . W[N][K]^T (bf16, DEVICE) on the stream-K weight-streaming kernel of the
+ * decode projections (always the single-CTA kernel), i.e. what darts_debug_gemm_bf16 computes with split_k == 0 —
+ * bit-identical to it on a context without DARTS_FLAG_CTA_PAIRS — but WITHOUT a scratch argument: the fp32 pieces and the piece-count table
+ * live in a file-scope device array of DARTS_STATIC_SCRATCH_BYTES inside the library, which every GPU that loads the library holds until
+ * the process exits.  The call allocates nothing (no cudaMalloc / cudaFree / allocating library routine): tensor-map encoding on the host,
+ * one 8 KB cudaMemsetAsync and two kernel launches, all asynchronous on the ctx stream.  The first call on a device also looks the array's
+ * device address up (cudaGetSymbolAddress): make one call outside any stream capture.
+ * Limit: 8192 + slots * rows * N * 4 bytes <= DARTS_STATIC_SCRATCH_BYTES, slots = the stream-K plan's pieces per tile (what
+ * darts_debug_gemm_scratch_floats reports / (rows N)); beyond it DARTS_ERR_WORKSPACE_TOO_SMALL and darts_last_error says how much was needed.
+ * Needs K % 64 == 0 and N % 4 == 0 (DARTS_ERR_UNSUPPORTED otherwise); NULL / non-positive arguments: DARTS_ERR_INVALID_ARG.
+ * The array is SHARED by every call in the process on that GPU and keeps the previous call's contents (the piece-count table is cleared per
+ * call; every piece a call reads it has written first): calls on one context are ordered by its stream, calls that OVERLAP on the GPU
+ * (other contexts, other streams) race on it and must be serialised by the caller.
+ * darts_static_scratch_bytes: *out = DARTS_STATIC_SCRATCH_BYTES as compiled into the library (host-only). */
+#define DARTS_STATIC_SCRATCH_BYTES (32u << 20)
+darts_status darts_static_scratch_bytes(size_t *out);
+darts_status darts_gemm_bf16_static(darts_ctx *ctx, const void *X, const void *W, float *C, int32_t rows, int32_t N, int32_t K);
+
 /* ---- Adaptive redundancy allocation (§4.2.2; App. B Eq. 6-9 :384-411; App. C Alg. 1 :413-462) --------
  * Host-only helpers for the step upstream of the rollout: per-prompt length variances (darts_results.len_var) -> EMA ->
  * total budget -> greedy plan Kp[G] for the next darts_prefill.  All pointers HOST.  No context, no GPU work.

@@ -92,6 +92,8 @@ darts_debug_fast_forward = _sig("darts_debug_fast_forward", _ctx, _i32)
 darts_debug_set_last_tokens = _sig("darts_debug_set_last_tokens", _ctx, _vp, _i32)
 darts_debug_gemm_bf16 = _sig("darts_debug_gemm_bf16", _ctx, _vp, _vp, _vp, _vp, _i32, _i32, _i32, _i32)
 darts_debug_gemm_scratch_floats = _sig("darts_debug_gemm_scratch_floats", _ctx, _i32, _i32, _i32, _i32, C.POINTER(C.c_size_t))
+darts_static_scratch_bytes = _sig("darts_static_scratch_bytes", C.POINTER(C.c_size_t))
+darts_gemm_bf16_static = _sig("darts_gemm_bf16_static", _ctx, _vp, _vp, _vp, _i32, _i32, _i32)
 darts_update_variance_ema = _sig("darts_update_variance_ema", _vp, _vp, _i32, _f32)
 darts_redundancy_budget = _sig("darts_redundancy_budget", C.c_double, C.c_double, C.c_double, _i32, _i32, C.POINTER(C.c_int64))
 darts_allocate_redundancy = _sig("darts_allocate_redundancy", _vp, _i32, C.c_int64, _i32, _i32, _vp)
@@ -376,6 +378,15 @@ class Darts:
                                           rows, N, K, split_k))
         self._scratch = scratch
         return out if reduce else scratch
+
+    def gemm_bf16_static(self, X, W, out):
+        """out[rows,N] (fp32, device, caller-allocated) = X @ W.T on the stream-K GEMM with its pieces in the library's static device
+        scratch (darts_gemm_bf16_static): nothing is allocated by this call.  Raises DartsError(ERR_WORKSPACE_TOO_SMALL) beyond the limit."""
+        rows, K = X.shape
+        N = W.shape[0]
+        assert out.shape == (rows, N) and out.dtype == torch.float32 and out.is_contiguous() and X.is_contiguous() and W.is_contiguous()
+        self._check(darts_gemm_bf16_static(self.ctx, X.data_ptr(), W.data_ptr(), out.data_ptr(), rows, N, K))
+        return out
 
     # ---- attention-only (config 2) -----------------------------------------------------------------
     def attn_load(self, G, P, Kp, k_prefix, v_prefix, suffix_len, k_suffix, v_suffix):
