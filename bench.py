@@ -169,11 +169,11 @@ def oracle_attention_sample(x_full_seed=0, n_rows=32):
 # ------------------------------------------------------------------------------------------------ full rollouts (c3 / c4 / c5)
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE attn_main_k launch from an `ncu --set full` capture (profiles/), with the
 # algorithmic bytes of that same launch beside it (launches differ in size over a rollout; `achieved` is the rollout average)
-NCU_ATTENTION_TRAFFIC = {"c3": dict(dram_bytes=1.2977e9, algorithmic_bytes=1.2277e9, ratio=1.057,
-                                    launch="decode step 1001 of the seed-0 rollout (the first warm-up rollout's inputs): 288 rows, mean suffix 1003 tokens, 19 open groups",
-                                    source="profiles/r2_launches_c3_step1000.md (ncu --set full -k attn_main_k, bench.py --profile-step 1000, round 2)")}
+NCU_ATTENTION_TRAFFIC = {"c3": dict(dram_bytes=1.2374e9, algorithmic_bytes=1.1927e9, ratio=1.037,
+                                    launch="decode step 1001 of the seed-0 rollout (the first warm-up rollout's inputs): 277 rows x 1001 suffix tokens, 25 open groups",
+                                    source="profiles/r2_launches_c3_step1000.md, re-capture on the final kernels (ncu --set full -k attn_main_k, bench.py --profile-step 1000)")}
 # the same for ONE launch of the config-2 microbench (seed 0: 3 131 237 suffix tokens + 128 x 1024 prefix tokens = 13.396 GB algorithmic)
-NCU_ATTENTION_C2 = dict(ncu_dram_bytes=13.958e9, ncu_traffic_over_algorithmic=1.042, ncu_source="profiles/r2_attention_c2.md")
+NCU_ATTENTION_C2 = dict(ncu_dram_bytes=13.717e9, ncu_traffic_over_algorithmic=1.024, ncu_source="profiles/r2_attention_c2.md (re-capture on the final kernels)")
 KV_POOL_CAP_BYTES = {"c3": 64e9, "c4": 100e9, "c5": 36e9}
 
 
@@ -524,8 +524,10 @@ def profile_steps(args):
     torch.cuda.profiler.stop()
     res = d.results()
     act = res["status"] == 0
+    group_of_row = np.repeat(np.arange(G), np.asarray(xin["Kp"]).reshape(-1))
     print(json.dumps(dict(profiled_steps=[args.profile_step + 1, args.profile_step + 2], active_rows=int(n0),
-                          mean_suffix_tokens=float(res["len"][act].mean()) if act.any() else 0.0, workload=name)))
+                          mean_suffix_tokens=float(res["len"][act].mean()) if act.any() else 0.0,
+                          active_rows_after=int(act.sum()), open_groups_after=int(len(np.unique(group_of_row[act]))), workload=name)))
     d.close()
 
 
