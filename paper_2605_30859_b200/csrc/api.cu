@@ -91,7 +91,6 @@ size_t carve(darts_ctx *c, void *base) {
     c->attn_nitems = k.take<int32_t>(4);
     c->part_base = k.take<int32_t>(A);
     c->part_cnt = k.take<int32_t>(A);
-    c->attn_done = k.take<int32_t>(A * m.n_kv_heads);
     c->part_ml = k.take<float>(max_parts * m.n_q_heads * 2);
     c->part_acc = k.take<float>(max_parts * m.n_q_heads * m.head_dim);
   }
@@ -504,7 +503,6 @@ darts_status darts_create(const darts_model_desc *m, const darts_weights *w, con
   CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev[1], cudaEventDisableTiming));
   CUDA_TRY(c, cudaMemsetAsync(c->st, 0, sizeof(DevState), c->stream));
   if (c->moe_arrive) CUDA_TRY(c, cudaMemsetAsync(c->moe_arrive, 0, c->moe_arrive_n * sizeof(int32_t), c->stream));
-  if (c->attn_done) CUDA_TRY(c, cudaMemsetAsync(c->attn_done, 0, (size_t)c->act_rows * m->n_kv_heads * sizeof(int32_t), c->stream));
   // The pool must hold finite values everywhere: a partially filled page is multiplied by zero probabilities.
   CUDA_TRY(c, cudaMemsetAsync(c->kv_pool, 0, (size_t)m->n_layers * c->kv_layer_elems * c->elt, c->stream));
   return DARTS_OK;

@@ -111,7 +111,6 @@ struct darts_ctx {
   void *xs;                      // expert-sorted copy of xn [max_rows * top_k][d]
   // tuned attention (kernels_attn_sm100.cu): per-step work list and split-KV partials
   int32_t *attn_items_pre, *attn_items_suf, *attn_nitems, *part_base, *part_cnt;
-  int32_t *attn_done;                  // [slot][kv head]: head-row partials stored so far in the running attention launch (fused merge); zero between launches
   float *part_ml, *part_acc;
   int attn_max_items;
   bool attn_plan_valid, attn_causal;   // attn_causal: the current plan is a prefill pass (row-wise causal masks)

@@ -31,9 +31,6 @@ constexpr int THREADS = (N_CONS + 1) * 32;
 #ifndef ATTN_TPATH
 #define ATTN_TPATH 1                        // units with <= 8 query rows: S^T = K Q^T (tokens on the MMA's m) (A/B switch: -DATTN_TPATH=0)
 #endif
-#ifndef ATTN_FUSED_MERGE
-#define ATTN_FUSED_MERGE 1                  // the warp that stores a (row, kv head)'s LAST partial merges them: no attn_merge_k launch (A/B: =0)
-#endif
 #ifndef ATTN_PARTIAL_LAST_PAGE
 #define ATTN_PARTIAL_LAST_PAGE 1            // fetch only the valid part of a row's newest page (A/B switch: -DATTN_PARTIAL_LAST_PAGE=0)
 #endif
@@ -104,9 +101,6 @@ struct Params {
   const int32_t *slot_prompt, *slot_row, *slot_npre, *g_prefix_pages, *row_pages, *part_base;
   int causal;                               // prefill pass: query row of slot s sees tokens < slot_npre[s] only
   float *part_ml, *part_acc;
-  const int32_t *part_cnt;                  // fused merge (ATTN_FUSED_MERGE): partials per slot, the arrival counters [slot][kv head], the output
-  int32_t *done;
-  __nv_bfloat16 *out;
   int mpp, msp, Hq, Hkv, rep, rep_shift;  // rep = Hq / Hkv = 1 << rep_shift (attention_sm100_supported)
   size_t page_elems, tile_elems;
   float c;                                  // softmax scale * log2(e)
@@ -167,89 +161,6 @@ __device__ __forceinline__ void pv_16tok(uint32_t sV, int tokb, uint32_t a0, uin
     ldsm4t(rowaddr + ((chunk ^ r) << 4), b0, b1, b2, b3);
     mma16816(O[2 * np], a0, a1, a2, a3, b0, b1);
     mma16816(O[2 * np + 1], a0, a1, a2, a3, b2, b3);
-  }
-}
-
-// out[slot][h] = sum_k w_k acc_k / sum_k w_k l_k,  w_k = 2^((m_k - M) c), over the row's partials in chunk order; one warp, lane = 4 dims.
-// CG: the partials were stored by other SMs during THIS launch — read them from L2 (this SM's L1 may hold last layer's values).
-template <bool CG>
-__device__ __forceinline__ void merge_head(const float *__restrict__ part_ml, const float *__restrict__ part_acc, int base, int cnt, int Hq, int h,
-                                           float c, int lane, __nv_bfloat16 *__restrict__ dst) {
-  auto ld2 = [](const float *q) { return CG ? __ldcg(reinterpret_cast<const float2 *>(q)) : *reinterpret_cast<const float2 *>(q); };
-  auto ld4 = [](const float *q) { return CG ? __ldcg(reinterpret_cast<const float4 *>(q)) : *reinterpret_cast<const float4 *>(q); };
-  float M = -INFINITY, L = 0.f;
-  float4 a = make_float4(0.f, 0.f, 0.f, 0.f);
-  if (cnt <= 4) {
-    // the common case (prefix chunk + up to three suffix chunks): every load of the row is issued before the first use — one L2
-    // round trip instead of two dependent passes; the sums below run in chunk order as in the general loop
-    float2 ml[4];
-    float4 v[4];
-#pragma unroll
-    for (int k = 0; k < 4; ++k)
-      if (k < cnt) {
-        const size_t pi = (size_t)(base + k) * Hq + h;
-        ml[k] = ld2(part_ml + pi * 2);
-        v[k] = ld4(part_acc + pi * HD + lane * 4);
-      }
-#pragma unroll
-    for (int k = 0; k < 4; ++k)
-      if (k < cnt) M = fmaxf(M, ml[k].x);
-#pragma unroll
-    for (int k = 0; k < 4; ++k)
-      if (k < cnt) {
-        const float sc = exp2f((ml[k].x - M) * c);
-        L += sc * ml[k].y;
-        a.x += sc * v[k].x; a.y += sc * v[k].y; a.z += sc * v[k].z; a.w += sc * v[k].w;
-      }
-  } else {
-    for (int k = 0; k < cnt; ++k) M = fmaxf(M, ld2(part_ml + ((size_t)(base + k) * Hq + h) * 2).x);
-    for (int k = 0; k < cnt; ++k) {
-      const size_t pi = (size_t)(base + k) * Hq + h;
-      const float2 ml = ld2(part_ml + pi * 2);
-      const float sc = exp2f((ml.x - M) * c);
-      L += sc * ml.y;
-      const float4 v = ld4(part_acc + pi * HD + lane * 4);
-      a.x += sc * v.x; a.y += sc * v.y; a.z += sc * v.z; a.w += sc * v.w;
-    }
-  }
-  const float inv = 1.0f / L;
-  uint2 o;
-  o.x = pack_bf16(a.x * inv, a.y * inv);
-  o.y = pack_bf16(a.z * inv, a.w * inv);
-  *reinterpret_cast<uint2 *>(dst + lane * 4) = o;
-}
-
-// the rep heads of one (slot, kv head); a real call, so that its registers do not weigh on the main loops of attn_main_k
-__device__ __noinline__ void merge_slot(const float *part_ml, const float *part_acc, int base, int cnt, int Hq, int h0, int rep, float c, int lane,
-                                        __nv_bfloat16 *dst) {
-  for (int hh = 0; hh < rep; ++hh) merge_head<true>(part_ml, part_acc, base, cnt, Hq, h0 + hh, c, lane, dst + (size_t)hh * HD);
-}
-
-// Fused merge.  Called by a whole warp after it has stored head-row partials: lane j < 32 names a slot it stored `my_heads` head rows of
-// (my_slot < 0: none).  Every (slot, kv head) receives part_cnt[slot] x rep head rows per launch; the warp whose count completes that sum
-// merges the rep heads (the same arithmetic, in the same chunk order, as attn_merge_k: identical bits whoever comes last) and puts the
-// counter back to zero for the next launch.  Release: each lane's stores are fenced before the warp's atomics; acquire: fence + L2 loads.
-__device__ __forceinline__ void count_and_merge(const Params &p, int kvh, int my_slot, int my_heads, int lane) {
-  __threadfence();
-  __syncwarp();
-  bool last = false;
-  int base = 0, cnt = 0;
-  if (my_slot >= 0) {
-    cnt = p.part_cnt[my_slot];
-    base = p.part_base[my_slot];
-    int *ctr = p.done + (size_t)my_slot * p.Hkv + kvh;
-    const int old = atomicAdd(ctr, my_heads);
-    last = old + my_heads == cnt * p.rep;
-    if (last) *ctr = 0;                                   // nobody else touches it before the next launch
-  }
-  unsigned win = __ballot_sync(0xffffffffu, last);
-  if (!win) return;
-  __threadfence();
-  while (win) {
-    const int j = __ffs(win) - 1;
-    win &= win - 1;
-    const int slot = __shfl_sync(0xffffffffu, my_slot, j), b = __shfl_sync(0xffffffffu, base, j), n = __shfl_sync(0xffffffffu, cnt, j);
-    merge_slot(p.part_ml, p.part_acc, b, n, p.Hq, kvh * p.rep, p.rep, p.c, lane, p.out + ((size_t)slot * p.Hq + kvh * p.rep) * HD);
   }
 }
 
@@ -404,10 +315,6 @@ __device__ __forceinline__ void tpath_unit(Smem &sm, const Params &p, const Hdr 
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   __syncwarp();
   if (lane == 0) mbar_arrive(&sm.empty[last_stage]);
-  if (ATTN_FUSED_MERGE) {
-    const int r = warp + N_CONS * lane;                             // lanes 0, 1: the rows this warp stored (warp, warp + 4)
-    count_and_merge(p, kvh, (lane < 2 && r < n_rows) ? h.first + (r >> p.rep_shift) : -1, 1, lane);
-  }
 }
 
 // One round of the cross-warp merge of a token-split unit: rows 4 rb .. 4 rb + 3, one consumer warp per row, 4 dims per lane.
@@ -628,10 +535,6 @@ __global__ void __launch_bounds__(THREADS, 2) attn_main_k(Params p) {
             *reinterpret_cast<float2 *>(p.part_acc + pi * HD + nt * 8 + 2 * t) = make_float2(O[nt][2 * rs], O[nt][2 * rs + 1]);
         }
       }
-      if (ATTN_FUSED_MERGE && warp_has_rows) {
-        const int row0 = mt * 16 + lane * p.rep;                    // lane j < 16 / rep: the j-th slot of this warp's m-tile (rep divides 16)
-        count_and_merge(p, kvh, (lane * p.rep < 16 && row0 < n_rows) ? first + (row0 >> p.rep_shift) : -1, p.rep, lane);
-      }
     } else {
       // the four warps hold partials over disjoint tokens of the same <= 16 rows: merge through shared memory
       float (*ml)[16][2] = sm.ml[ubuf];
@@ -651,10 +554,6 @@ __global__ void __launch_bounds__(THREADS, 2) attn_main_k(Params p) {
         cons_bar();
         merge_round(sm, ml, p, rb, n_rows, first, kvh, chunk_k);
         cons_bar();
-      }
-      if (ATTN_FUSED_MERGE) {
-        const int r = lane * 4 + warp;                              // lane i < rounds: the row this warp stored in round i
-        count_and_merge(p, kvh, (lane < rounds && r < n_rows) ? first + (r >> p.rep_shift) : -1, 1, lane);
       }
     }
   }
@@ -702,8 +601,47 @@ __global__ void attn_merge_k(const float *__restrict__ part_ml, const float *__r
   int lane = threadIdx.x & 31;
   int base = part_base[slot], cnt = part_cnt[slot];
   pdl_wait();
-  for (int h = blockIdx.y * (blockDim.x >> 5) + (threadIdx.x >> 5); h < Hq; h += gridDim.y * (blockDim.x >> 5))     // one head per warp
-    merge_head<false>(part_ml, part_acc, base, cnt, Hq, h, c, lane, out + ((size_t)slot * Hq + h) * HD);
+  for (int h = blockIdx.y * (blockDim.x >> 5) + (threadIdx.x >> 5); h < Hq; h += gridDim.y * (blockDim.x >> 5)) {   // one head per warp
+    float M = -INFINITY, L = 0.f;
+    float4 a = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (cnt <= 4) {
+      // the common case (prefix chunk + up to three suffix chunks): every load of the row is issued before the first use — one L2
+      // round trip instead of two dependent passes; the sums below run in chunk order as in the general loop
+      float2 ml[4];
+      float4 v[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k)
+        if (k < cnt) {
+          const size_t pi = (size_t)(base + k) * Hq + h;
+          ml[k] = *reinterpret_cast<const float2 *>(part_ml + pi * 2);
+          v[k] = *reinterpret_cast<const float4 *>(part_acc + pi * HD + lane * 4);
+        }
+#pragma unroll
+      for (int k = 0; k < 4; ++k)
+        if (k < cnt) M = fmaxf(M, ml[k].x);
+#pragma unroll
+      for (int k = 0; k < 4; ++k)
+        if (k < cnt) {
+          const float sc = exp2f((ml[k].x - M) * c);
+          L += sc * ml[k].y;
+          a.x += sc * v[k].x; a.y += sc * v[k].y; a.z += sc * v[k].z; a.w += sc * v[k].w;
+        }
+    } else {
+      for (int k = 0; k < cnt; ++k) M = fmaxf(M, part_ml[((size_t)(base + k) * Hq + h) * 2]);
+      for (int k = 0; k < cnt; ++k) {
+        size_t pi = (size_t)(base + k) * Hq + h;
+        float sc = exp2f((part_ml[pi * 2] - M) * c);
+        L += sc * part_ml[pi * 2 + 1];
+        float4 v = *reinterpret_cast<const float4 *>(part_acc + pi * HD + lane * 4);
+        a.x += sc * v.x; a.y += sc * v.y; a.z += sc * v.z; a.w += sc * v.w;
+      }
+    }
+    float inv = 1.0f / L;
+    uint2 o;
+    o.x = pack_bf16(a.x * inv, a.y * inv);
+    o.y = pack_bf16(a.z * inv, a.w * inv);
+    *reinterpret_cast<uint2 *>(out + ((size_t)slot * Hq + h) * HD + lane * 4) = o;
+  }
 }
 
 // ------------------------------------------------------------------------------------------------ plan (one CTA)
@@ -846,7 +784,6 @@ darts_status launch_attention_sm100(darts_ctx *c, int layer, const void *q, void
   p.items_pre = c->attn_items_pre; p.items_suf = c->attn_items_suf; p.n_items = c->attn_nitems;
   p.slot_prompt = c->slot_prompt; p.slot_row = c->slot_row; p.slot_npre = c->slot_npre; p.causal = c->attn_causal ? 1 : 0; p.g_prefix_pages = c->g_prefix_pages; p.row_pages = c->row_pages;
   p.part_base = c->part_base; p.part_ml = c->part_ml; p.part_acc = c->part_acc;
-  p.part_cnt = c->part_cnt; p.done = c->attn_done; p.out = (__nv_bfloat16 *)out;
   p.mpp = c->max_prefix_pages; p.msp = c->max_suffix_pages; p.Hq = c->m.n_q_heads; p.Hkv = c->m.n_kv_heads; p.rep = p.Hq / p.Hkv;
   p.rep_shift = 31 - __builtin_clz((unsigned)p.rep);
   p.page_elems = c->kv_page_elems; p.tile_elems = c->kv_tile_elems;
@@ -855,7 +792,6 @@ darts_status launch_attention_sm100(darts_ctx *c, int layer, const void *q, void
   if (!DARTS_SKIPPED(c, 4)) launch_pdl(c, attn_main_k, dim3(grid), dim3(THREADS), smem, p);
   c->launches++;
   if (cudaGetLastError() != cudaSuccess) FAIL(c, DARTS_ERR_CUDA, "launch attn_main failed: %s", cudaGetErrorString(cudaGetLastError()));
-  if (ATTN_FUSED_MERGE) return DARTS_OK;                   // merged inside attn_main_k by the warp that stores a row's last partial
   if (!DARTS_SKIPPED(c, 8)) launch_pdl(c, attn_merge_k, dim3(rows_ub, (p.Hq + 7) / 8), dim3(256), 0, c->part_ml, c->part_acc, c->part_base, c->part_cnt, (__nv_bfloat16 *)out, p.Hq, p.c, n_rows_dev, rows_ub);
   c->launches++;
   if (cudaGetLastError() != cudaSuccess) FAIL(c, DARTS_ERR_CUDA, "launch attn_merge failed");
