@@ -31,6 +31,9 @@ constexpr int THREADS = (N_CONS + 1) * 32;
 #ifndef ATTN_TPATH
 #define ATTN_TPATH 1                        // units with <= 8 query rows: S^T = K Q^T (tokens on the MMA's m) (A/B switch: -DATTN_TPATH=0)
 #endif
+#ifndef ATTN_CHUNK_MAJOR
+#define ATTN_CHUNK_MAJOR 1                 // plan: suffix items chunk-major when all rows have the same number of chunks (A/B switch: =0)
+#endif
 #ifndef ATTN_PARTIAL_LAST_PAGE
 #define ATTN_PARTIAL_LAST_PAGE 1            // fetch only the valid part of a row's newest page (A/B switch: -DATTN_PARTIAL_LAST_PAGE=0)
 #endif
@@ -675,13 +678,26 @@ __device__ __forceinline__ int scan1024(int v, int *total, int *smem) {
 __global__ void attn_plan_k(const int32_t *__restrict__ slot_prompt, const int32_t *__restrict__ slot_npre,
                             const int32_t *__restrict__ slot_nsuf, int32_t *items_pre, int32_t *items_suf, int32_t *n_items,
                             int32_t *part_base, int32_t *part_cnt, int rep, int no_share, int prefill, int max_items,
-                            const int32_t *n_rows_dev, int rows_ub) {
+                            const int32_t *n_rows_dev, int rows_ub, int cm_max_items) {
   __shared__ int sm[33];
   __shared__ int b_part, b_pre, b_suf;
   int n = n_rows_dev ? min(*n_rows_dev, rows_ub) : rows_ub;
   if (threadIdx.x == 0) { b_part = 0; b_pre = 0; b_suf = 0; }
   __syncthreads();
   int RB = 64 / rep;                                   // slots per ROWSPLIT item (64 query rows)
+  // In a rollout every live row has the same generated length (lock step), hence the same number of suffix chunks.  While a launch has
+  // only a few units per CTA (n x chunks <= cm_max_items: the thin tail of a rollout) the suffix items are written CHUNK-major (all rows'
+  // chunk 0, then chunk 1, ...), so that the last round of the kernel's strided unit assignment is made of the rows' short newest chunks
+  // instead of whole 512-token ones: -2 % per decode step at <= 64 rows.  With many units per CTA the row-major order wins by 1-2 % (a row's
+  // consecutive pages) and is kept.  The order of the items changes nothing else: every unit's arithmetic and partial index are its own.
+  // Rows of different lengths (chunk scoring, the attention-only entry) keep the row-major order.
+  int uniform_nsc = 0;
+  if (ATTN_CHUNK_MAJOR && !prefill && n > 0) {
+    const int nsc0 = (slot_nsuf[0] + CH_TOK - 1) / CH_TOK;
+    bool same = (long long)n * nsc0 <= cm_max_items;
+    for (int slot = threadIdx.x; slot < n; slot += blockDim.x) same &= (slot_nsuf[slot] + CH_TOK - 1) / CH_TOK == nsc0;
+    if (__syncthreads_and(same)) uniform_nsc = nsc0;
+  }
   for (int base = 0; base < n; base += blockDim.x) {
     int slot = base + threadIdx.x;
     int npc = 0, nsc = 0, gsize = 0, nblk = 0, npre_items = 0;
@@ -731,8 +747,8 @@ __global__ void attn_plan_k(const int32_t *__restrict__ slot_prompt, const int32
           it[4] = ck;
           it[5] = 1;
         }
-      idx = bs + es;
-      for (int ck = 0; ck < nsc; ++ck, ++idx) {
+      for (int ck = 0; ck < nsc; ++ck) {
+        idx = uniform_nsc ? ck * n + slot : bs + es + ck;
         if (idx >= max_items) continue;
         int32_t *it = items_suf + (size_t)idx * ITEM_INTS;
         it[0] = slot; it[1] = 1; it[2] = ck * CH_PAGES;
@@ -756,7 +772,7 @@ darts_status launch_attention_plan_sm100(darts_ctx *c, int rows_ub, const int32_
   int rep = c->m.n_q_heads / c->m.n_kv_heads;
   attn_plan_k<<<1, 1024, 0, c->stream>>>(c->slot_prompt, c->slot_npre, c->slot_nsuf, c->attn_items_pre, c->attn_items_suf, c->attn_nitems,
                                          c->part_base, c->part_cnt, rep, (c->rt.flags & DARTS_FLAG_NO_PREFIX_SHARING) ? 1 : 0, prefill ? 1 : 0,
-                                         c->attn_max_items, n_rows_dev, rows_ub);
+                                         c->attn_max_items, n_rows_dev, rows_ub, 8 * (2 * c->n_sms) / c->m.n_kv_heads);   // <= 8 suffix units per CTA
   c->attn_causal = prefill;
   c->launches++;
   if (cudaGetLastError() != cudaSuccess) FAIL(c, DARTS_ERR_CUDA, "launch attn_plan failed");
